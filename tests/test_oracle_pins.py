@@ -1,0 +1,322 @@
+"""Pins of the CPU oracle against things other than itself.
+
+Every check here compares oracle/etac_oracle.py with a closed form, a hand-derived value
+(tests/golden/*.txt), a brute-force pure-Python loop, or a library routine (scipy cdist,
+torch float64 linear/silu) -- never with the CUDA path."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import etac_oracle as O
+from paper_2604_20295_b200 import workloads as W
+from conftest import read_golden
+
+
+def pad_model(g1=16, g2=16, spacing=1.0, alpha=0.5, resid="none", weights=None, mode="passthrough"):
+    pos, nrm, edges = W.flat_pad(g1, g2, spacing)
+    mesh = W.assemble([(pos, nrm, edges)])
+    return O.OracleModel(mesh.pos, mesh.normal, mesh.patch_offset, np.float32([alpha]), weights, resid, mode)
+
+
+def one_sphere(centre, r):
+    ind = np.zeros((1, 1), dtype=W.INDENTER_DTYPE)
+    ind["type"] = W.IND_SPHERE
+    ind["param"][0, 0, 0] = r
+    ind["pose"][0, 0] = [*centre, 0, 0, 0, 1]
+    return ind
+
+
+# ---------------------------------------------------------------- P1
+def test_zero_contact_gives_zero():
+    wl = W.config2(seed=1, n_envs=3)
+    m = O.model_from_workload(wl)
+    ind = wl.indenters.copy()
+    ind["pose"][..., 0:3] += 500.0          # far away
+    r = O.step(m, indenters=ind)
+    assert not r["mask"].any() and not r["contact"].any()
+    assert np.all(r["U"] == 0.0) and np.all(r["analytic"] == 0.0)
+    ind["type"][:] = W.IND_NONE             # no indenter at all
+    r = O.step(m, indenters=ind)
+    assert np.all(r["U"] == 0.0) and not r["mask"].any()
+
+
+# ---------------------------------------------------------------- P2
+def test_linear_term_is_linear_and_superposes():
+    m = pad_model()
+    rng = np.random.default_rng(0)
+    d1 = np.zeros((1, 256), np.float32)
+    d2 = np.zeros((1, 256), np.float32)
+    d1[0, rng.choice(256, 9, replace=False)] = rng.uniform(0.1, 1, 9)
+    d2[0, rng.choice(256, 5, replace=False)] = rng.uniform(0.1, 1, 5)
+    a, b = 2.0, 0.5                          # exact in fp32
+    r1 = O.step(m, penetration=d1)["analytic"]
+    r2 = O.step(m, penetration=d2)["analytic"]
+    r12 = O.step(m, penetration=(a * d1 + b * d2).astype(np.float32))["analytic"]
+    np.testing.assert_allclose(r12, a * r1 + b * r2, rtol=0, atol=1e-13)
+
+
+# ---------------------------------------------------------------- P3
+def test_single_point_contact_closed_form_decay():
+    m = pad_model(21, 21)
+    c = 10 * 21 + 10
+    d = np.zeros((1, 441), np.float32)
+    d[0, c] = 0.75
+    r = O.step(m, penetration=d)
+    uz = r["analytic"][0, :, 2].reshape(21, 21)
+    assert np.all(r["analytic"][0, :, 0:2] == 0)
+    # e^{-alpha r} with alpha = 0.5: mathematical constants
+    expect = {(1, 0): 0.6065306597126334, (1, 1): 0.4930686913952398, (2, 0): 0.36787944117144233,
+              (5, 0): 0.0820849986238988, (10, 0): 0.006737946999085467, (3, 4): 0.0820849986238988}
+    for (dx, dy), k in expect.items():
+        assert uz[10 + dx, 10 + dy] == pytest.approx(-0.75 * k, abs=1e-14)
+    # radially symmetric and strictly decreasing with distance
+    for dx, dy in [(1, 2), (3, 4), (0, 5)]:
+        vals = {uz[10 + sx * a, 10 + sy * b] for a, b in [(dx, dy), (dy, dx)] for sx in (1, -1) for sy in (1, -1)}
+        assert max(vals) - min(vals) < 1e-15
+    rr = np.hypot(*(np.mgrid[0:21, 0:21] - 10)).ravel()
+    order = np.argsort(rr)
+    mag = -uz.ravel()[order]
+    assert np.all(np.diff(mag)[np.diff(rr[order]) > 1e-9] < 0)
+    # passthrough keeps u_hat on the active node
+    assert r["U"][0, c, 2] == pytest.approx(-0.75, abs=0)
+
+
+# ---------------------------------------------------------------- P4
+def test_bruteforce_triple_loop_and_libraries():
+    from scipy.spatial.distance import cdist
+    import torch
+    wl = W.config2(seed=3, n_envs=1)
+    sub = np.arange(0, 1024, 37)[:28]
+    mesh = wl.mesh
+    m = O.OracleModel(mesh.pos[sub], mesh.normal[sub], np.int32([0, 12, 28]), np.float32([0.5, 0.3]), None, "none")
+    rng = np.random.default_rng(5)
+    d = np.where(rng.random((1, 28)) < 0.3, rng.uniform(0.1, 1.0, (1, 28)), 0).astype(np.float32)
+    d[0, 0] = 0.5
+    d[0, 20] = 0.25
+    r = O.step(m, penetration=d)
+    P = m.pos.astype(np.float64)
+    Nn = m.normal.astype(np.float64)
+    ref = np.zeros((28, 3))
+    for lo, hi, al in [(0, 12, float(np.float32(0.5))), (12, 28, float(np.float32(0.3)))]:
+        for i in range(lo, hi):
+            for j in range(lo, hi):
+                if d[0, j] > 0:
+                    dist = math.sqrt(sum((P[i, c] - P[j, c]) ** 2 for c in range(3)))
+                    for c in range(3):
+                        ref[i, c] += math.exp(-al * dist) * (-float(d[0, j]) * Nn[j, c])
+    np.testing.assert_allclose(r["analytic"][0], ref, rtol=0, atol=1e-14)
+    # library: scipy cdist + torch float64 matmul on the dense zero-padded form K @ U_hat (R3)
+    K0 = np.exp(-float(np.float32(0.5)) * cdist(P[:12], P[:12]))
+    np.testing.assert_allclose(O.kernel_block(m, 0), K0, rtol=1e-14)
+    Uhat = -d[0, :12, None].astype(np.float64) * Nn[:12]
+    dense = (torch.from_numpy(K0) @ torch.from_numpy(Uhat)).numpy()
+    np.testing.assert_allclose(r["analytic"][0, :12], dense, rtol=0, atol=1e-14)
+    # block-diagonal: patch 1's contact does not leak into patch 0 (R9)
+    d2 = d.copy()
+    d2[0, 12:] = 0
+    np.testing.assert_array_equal(O.step(m, penetration=d2)["analytic"][0, :12], r["analytic"][0, :12])
+
+
+# ---------------------------------------------------------------- P5 / P6
+def test_kernel_structure_and_lattice_sums(golden_dir):
+    g = read_golden(os.path.join(golden_dir, "lattice_rowsums.txt"))
+    m = pad_model()
+    K = O.kernel_block(m, 0)
+    assert np.array_equal(K, K.T) and np.all(np.diag(K) == 1.0) and K.min() > 0 and K.max() <= 1.0
+    np.linalg.cholesky(K)                      # exponential kernel is positive definite
+    ev = np.linalg.eigvalsh(K)
+    assert ev[0] == pytest.approx(g["eig_min"][0], abs=5e-5) and ev[-1] == pytest.approx(g["eig_max"][0], abs=5e-4)
+    assert K[0].sum() == pytest.approx(g["corner_0_0"][0], abs=g["tol"][0])
+    assert K[7 * 16 + 7].sum() == pytest.approx(g["node_7_7"][0], abs=g["tol"][0])
+    # pure-Python restatement of the corner sum
+    s = sum(math.exp(-0.5 * math.hypot(a, b)) for a in range(16) for b in range(16))
+    assert K[0].sum() == pytest.approx(s, abs=1e-12)
+    assert K[7 * 16 + 7].sum() < 25.2465451858737 < 2 * math.pi / 0.25 + 0.2
+
+
+# ---------------------------------------------------------------- W1 / W2 / P7
+def test_worked_example_w1(golden_dir):
+    g = read_golden(os.path.join(golden_dir, "w1_collinear.txt"))
+    pos = np.float32([[0, 0, 0], [1, 0, 0], [2, 0, 0], [3, 0, 0]])
+    nrm = np.float32([[0, 0, 1]] * 4)
+    m = O.OracleModel(pos, nrm, np.int32([0, 4]), np.float32([0.5]), None, "none")
+    r = O.step(m, penetration=np.float32([[0.4, 0, 0, 0.2]]))
+    # fp32 inputs 0.4, 0.2 are not exact: tolerance covers their rounding (6e-9)
+    np.testing.assert_allclose(r["analytic"][0, :, 2], g["analytic_z"], rtol=0, atol=2e-8)
+    np.testing.assert_allclose(r["U"][0, :, 2], g["U_z"], rtol=0, atol=2e-8)
+    assert list(r["mask"][0]) == [True, False, False, True]
+
+
+def test_worked_example_w2_and_mask_semantics(golden_dir):
+    g = read_golden(os.path.join(golden_dir, "w2_pad_sphere.txt"))
+    m = pad_model()
+    r = O.step(m, indenters=one_sphere((7.3, 8.6, 2.2), 3.0))
+    ids = np.nonzero(r["mask"][0])[0]
+    assert list(ids) == [int(x) for x in g["active_ids"]]
+    tol = 5e-7        # centre coordinates 7.3/8.6/2.2 are fp32-rounded inputs
+    for n in (120, 121, 137):
+        assert r["delta"][0, n] == pytest.approx(g[f"delta_{n}"][0], abs=tol)
+    assert r["delta"][0].sum() == pytest.approx(g["delta_sum"][0], abs=13 * tol)
+    for n in (0, 89, 169, 255, 121):
+        assert r["analytic"][0, n, 2] == pytest.approx(g[f"analytic_z_{n}"][0], abs=20 * tol)
+    # P7: active rows keep u_hat, analytic on an active row double-counts
+    K = O.kernel_block(m, 0)
+    i = 121
+    others = [j for j in ids if j != i]
+    dbl = -r["delta"][0, i] - sum(K[i, j] * r["delta"][0, j] for j in others)
+    assert r["analytic"][0, i, 2] == pytest.approx(dbl, abs=1e-13)
+    assert r["U"][0, i, 2] == -r["delta"][0, i]
+    # contact radius sqrt(2 r d - d^2) for a sphere on a flat pad (P9)
+    d = 0.8
+    rc = math.sqrt(2 * 3.0 * d - d * d)
+    xy = m.pos[:, :2].astype(np.float64) - np.array([np.float32(7.3), np.float32(8.6)], dtype=np.float64)
+    assert np.array_equal(np.hypot(xy[:, 0], xy[:, 1]) < rc - 1e-6, r["mask"][0])
+
+
+# ---------------------------------------------------------------- P8
+def test_rigid_invariance_via_patch_pose():
+    wl = W.config2(seed=2, n_envs=2)
+    m = O.model_from_workload(wl, resid_arch="none")
+    base = O.step(m, indenters=wl.indenters)
+    rng = np.random.default_rng(11)
+    R = W.random_rotations(rng, 1)[0]
+    t = np.array([12.0, -7.0, 3.5])
+    ind = wl.indenters.copy()
+    pose = np.zeros((2, 1, 7), np.float32)
+    pose[..., 0:3] = t
+    pose[..., 3:7] = W.quat_from_matrix(R)
+    for e in range(2):
+        for k in range(ind.shape[1]):
+            c = ind["pose"][e, k, 0:3].astype(np.float64)
+            Rk = O.quat_to_rot(ind["pose"][e, k, 3:7].astype(np.float64))
+            ind["pose"][e, k, 0:3] = R @ c + t
+            ind["pose"][e, k, 3:7] = W.quat_from_matrix(R @ Rk)
+    moved = O.step(m, indenters=ind, patch_pose=pose)
+    far = np.abs(base["delta"]) > 1e-4
+    np.testing.assert_allclose(moved["delta"], base["delta"], rtol=0, atol=2e-5)
+    assert np.array_equal(moved["mask"][far], base["mask"][far])
+    np.testing.assert_allclose(moved["analytic"], base["analytic"], rtol=0, atol=2e-3)
+
+
+# ---------------------------------------------------------------- P9
+def test_sdf_spot_values_and_special_cases(golden_dir):
+    kinds = {"sphere": O.IND_SPHERE, "box": O.IND_BOX, "capsule": O.IND_CAPSULE}
+    n = 0
+    with open(os.path.join(golden_dir, "sdf_spot_values.txt")) as f:
+        for line in f:
+            line = line.split("#", 1)[0].split()
+            if not line:
+                continue
+            k, p, y, exp = kinds[line[0]], [float(x) for x in line[1:4]], [float(x) for x in line[4:7]], float(line[7])
+            got = O.sdf_local(k, p, *[np.array([v]) for v in y])[0]
+            assert got == pytest.approx(exp, abs=1e-14), line
+            n += 1
+    assert n == 12
+    rng = np.random.default_rng(3)
+    y = rng.normal(size=(3, 200)) * 4
+    # capsule with zero half-length is a sphere
+    np.testing.assert_allclose(O.sdf_local(O.IND_CAPSULE, [2.5, 0, 0], *y), O.sdf_local(O.IND_SPHERE, [2.5, 0, 0], *y), atol=1e-15)
+    # box with two huge half extents is a slab: |y2| - h
+    np.testing.assert_allclose(O.sdf_local(O.IND_BOX, [1e6, 1e6, 1.5], *y), np.abs(y[2]) - 1.5, atol=1e-9)
+    # 1-Lipschitz (exact distance fields): |phi(a)-phi(b)| <= |a-b|
+    a, b = rng.normal(size=(3, 500)) * 5, rng.normal(size=(3, 500)) * 5
+    for k, p in [(O.IND_SPHERE, [3, 0, 0]), (O.IND_BOX, [2, 3, 4]), (O.IND_CAPSULE, [2, 5, 0])]:
+        assert np.all(np.abs(O.sdf_local(k, p, *a) - O.sdf_local(k, p, *b)) <= np.linalg.norm(a - b, axis=0) + 1e-12)
+    # flat pad under a slab: delta equals the plane depth everywhere
+    m = pad_model()
+    ind = np.zeros((1, 1), dtype=W.INDENTER_DTYPE)
+    ind["type"], ind["param"][0, 0] = W.IND_BOX, [1e4, 1e4, 2.0]
+    ind["pose"][0, 0] = [0, 0, 1.75, 0, 0, 0, 1]
+    r = O.step(m, indenters=ind)
+    np.testing.assert_allclose(r["delta"][0], 0.25, atol=1e-12)
+    # quaternion -> rotation: 90 deg about z maps x to y; orthonormal; matches scipy
+    from scipy.spatial.transform import Rotation
+    q = np.array([0, 0, math.sin(math.pi / 4), math.cos(math.pi / 4)])
+    np.testing.assert_allclose(O.quat_to_rot(q) @ [1, 0, 0], [0, 1, 0], atol=1e-15)
+    qs = W.quat_from_matrix(W.random_rotations(rng, 20))
+    for qq in qs:
+        np.testing.assert_allclose(O.quat_to_rot(qq), Rotation.from_quat(qq).as_matrix(), atol=1e-14)
+
+
+# ---------------------------------------------------------------- P10
+def test_mlp_matches_torch_float64():
+    import torch
+    w = W.make_weights(9, seed=4, std=0.3)
+    rng = np.random.default_rng(2)
+    ul, p, n = rng.normal(size=(50, 3)), rng.normal(size=(50, 3)) * 5, rng.normal(size=(50, 3))
+    got = O.residual_pernode(w, ul, p, n)
+    t = {k: torch.from_numpy(v.astype(np.float64)) for k, v in w.items()}
+    x = torch.from_numpy(np.concatenate([ul, p, n], 1))
+    F = torch.nn.functional
+    ref = F.linear(F.silu(F.linear(F.silu(F.linear(x, t["W1"], t["b1"])), t["W2"], t["b2"])), t["W3"], t["b3"])
+    np.testing.assert_allclose(got, ref.numpy(), rtol=0, atol=1e-13)
+    # zero weights -> r = b3 ; zero everything -> U_passive = u_lin
+    z = {k: np.zeros_like(v) for k, v in w.items()}
+    z["b3"] = np.float32([0.1, -0.2, 0.3])
+    np.testing.assert_allclose(O.residual_pernode(z, ul, p, n), np.tile(z["b3"].astype(np.float64), (50, 1)))
+    m0 = pad_model(resid="pernode", weights={k: np.zeros_like(v) for k, v in w.items()})
+    r = O.step(m0, indenters=one_sphere((7.3, 8.6, 2.2), 3.0))
+    passive = ~r["mask"][0]
+    np.testing.assert_array_equal(r["U"][0][passive], r["analytic"][0][passive])
+    # input order [u_lin, p, n]: only W1[:,0:3] sees u_lin
+    w2 = {k: v.copy() for k, v in w.items()}
+    w2["W1"][:, 3:] = 0
+    a = O.residual_pernode(w2, ul, p, n)
+    b = O.residual_pernode(w2, ul, p * 0 + 1, n * 0 - 2)
+    np.testing.assert_allclose(a, b, atol=1e-15)
+
+
+# ---------------------------------------------------------------- P11
+def test_mode_reductions():
+    wl = W.config2(seed=5, n_envs=3)
+    full = O.step(O.model_from_workload(wl), indenters=wl.indenters)
+    lin = O.step(O.model_from_workload(wl, resid_arch="none"), indenters=wl.indenters)
+    passive = ~full["mask"]
+    np.testing.assert_array_equal(lin["U"][passive], lin["analytic"][passive])
+    np.testing.assert_array_equal(full["analytic"], lin["analytic"])
+    assert np.abs(full["U"] - lin["U"])[passive & full["contact"][:, [0]]].max() > 1e-4   # residual is there
+    # PENETRATION fed with the fp32 delta that INDENTERS emitted -> same masks, U within fp32 rounding
+    pen = O.step(O.model_from_workload(wl), penetration=full["delta32"])
+    assert np.array_equal(pen["mask"], full["mask"])
+    np.testing.assert_allclose(pen["U"], full["U"], rtol=0, atol=1e-5)
+    # propagate mode: no mask, active rows get u_lin + r too
+    prop = O.step(O.model_from_workload(wl, active_mode="propagate"), indenters=wl.indenters)
+    np.testing.assert_array_equal(prop["U"][passive], full["U"][passive])
+    act = full["mask"]
+    assert np.abs(prop["U"][act] - full["U"][act]).max() > 1e-3
+
+
+# ---------------------------------------------------------------- P12
+def test_pointnet_branch_is_permutation_equivariant():
+    rng = np.random.default_rng(8)
+    shp = {"E1": (64, 9), "e1": (64,), "E2": (64, 64), "e2": (64,), "G1": (64, 64), "g1": (64,),
+           "D1": (64, 128), "d1": (64,), "D2": (3, 64), "d2": (3,)}
+    w = {k: rng.normal(0, 0.2, s).astype(np.float32) for k, s in shp.items()}
+    n = 40
+    uh, p, nr = rng.normal(size=(n, 3)), rng.normal(size=(n, 3)), rng.normal(size=(n, 3))
+    perm = rng.permutation(n)
+    a = O.residual_pointnet(w, uh, p, nr)
+    b = O.residual_pointnet(w, uh[perm], p[perm], nr[perm])
+    np.testing.assert_allclose(a[perm], b, atol=1e-13)
+    assert a.shape == (n, 3)
+    # the global feature couples nodes: changing one node's input changes another node's output
+    uh2 = uh.copy()
+    uh2[0] += 5.0
+    assert np.abs(O.residual_pointnet(w, uh2, p, nr)[1:] - a[1:]).max() > 1e-6
+
+
+# ---------------------------------------------------------------- fp32 decision twin
+def test_fp32_twin_agrees_with_fp64_away_from_the_surface():
+    for wl in (W.config2(seed=7, n_envs=6), W.config3(seed=7, n_envs=4)):
+        m = O.model_from_workload(wl)
+        for e in range(wl.n_envs):
+            pp = None if wl.patch_pose is None else wl.patch_pose[e]
+            p64 = O.signed_distance(m, wl.indenters[e], pp, np.float64)
+            p32 = O.signed_distance(m, wl.indenters[e], pp, np.float32)
+            assert p32.dtype == np.float32
+            near = p64 < 100.0
+            assert np.abs(p32[near] - p64[near]).max() < 1e-4
+            far = np.abs(p64) > 1e-4
+            assert np.array_equal((p32 < 0)[far], (p64 < 0)[far])
