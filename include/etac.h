@@ -1,0 +1,166 @@
+/* etac.h -- C ABI of the B200-native ETac tactile hot path (arxiv/paper_2604_20295).
+ *
+ * One call per RL step turns rigid contact into elastomer surface displacement for a batch of
+ * E environments (Sec. III-A):
+ *   S1  contact detection + penalty displacement of the ACTIVE nodes
+ *   S2  decay-based linear propagation  u_i^j = exp(-alpha |p_j - p_i|) u^_j,
+ *       Omega U_a                                                             (Eq. 1)
+ *   S3  residual correction Phi (per-node MLP form of BASELINE.json)
+ *   S4  mask M_p + combine  U_p = Omega U_a + Phi_p                           (Eq. 2)
+ * Calibration of alpha / Phi (Eq. 3) is offline and out of scope: parameters are inputs.
+ *
+ * Conventions
+ *   - All functions return etac_status; nothing throws; no global state.
+ *   - "host" pointers are read during the call only (the ctx copies what it needs).
+ *     "device" pointers must be CUDA device memory on the ctx's device, owned by the caller and
+ *     kept alive until the stream reaches the end of the step.
+ *   - etac_step only enqueues work on the given CUDA stream: no host synchronisation, no
+ *     allocation, no host<->device copy of per-step data.  One in-flight stream per ctx;
+ *     different ctxs are independent.  Each step depends only on its arguments (the model is
+ *     quasi-static).
+ *   - Units are the caller's: alpha is in 1/(unit of node_pos).  The synthetic workloads use mm.
+ *   - Device-side data problems (NaN pose, non-unit quaternion) are not detected: the affected
+ *     environment's output is unspecified, other environments are unaffected.
+ *   - There is no CPU fallback: every entry point that computes needs a CUDA device of compute
+ *     capability 10.x and fails with ETAC_ERR_UNSUPPORTED / ETAC_ERR_CUDA otherwise.
+ */
+#ifndef ETAC_H_
+#define ETAC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ETAC_ABI_VERSION 1
+
+typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
+
+typedef enum {
+  ETAC_OK = 0,
+  ETAC_ERR_INVALID_ARG = 1, /* NULL / out-of-range / inconsistent argument; ctx unchanged */
+  ETAC_ERR_UNSUPPORTED = 2, /* valid request this build cannot serve (e.g. POINTNET residual) */
+  ETAC_ERR_ALLOC = 3,       /* host or device allocation failed */
+  ETAC_ERR_CUDA = 4,        /* a CUDA call failed; etac_last_error() has the CUDA message */
+  ETAC_ERR_CAPACITY = 5     /* n_envs > max_envs */
+} etac_status;
+
+/* Analytic indenters (north_star: "analytic indenter SDFs (sphere/box/capsule poses)").  The
+ * signed distance is exact (1-Lipschitz), negative inside.  PAPER.md:L77 detects contact with
+ * SDFs against object meshes; several indenters per environment are united by min. */
+typedef enum { ETAC_IND_NONE = 0, ETAC_IND_SPHERE = 1, ETAC_IND_BOX = 2, ETAC_IND_CAPSULE = 3 } etac_ind_type;
+
+typedef struct {
+  int32_t type;   /* etac_ind_type; NONE slots are skipped */
+  float param[3]; /* sphere {r,-,-}; box {hx,hy,hz} half extents; capsule {r, half length along local z, -} */
+  float pose[7];  /* {px,py,pz, qx,qy,qz,qw}: unit quaternion, Isaac-Gym order; world frame */
+  float _pad;
+} etac_indenter; /* 48 bytes */
+
+enum { ETAC_KERNEL_EXP_L2 = 0 };                                  /* Eq. (1): exp(-alpha*|p_j-p_i|_2) */
+enum { ETAC_RESID_NONE = 0, ETAC_RESID_PERNODE_MLP = 1, ETAC_RESID_POINTNET = 2 /* not built: UNSUPPORTED */ };
+enum { ETAC_PREC_FP32 = 0, ETAC_PREC_BF16 = 1 };                  /* BF16: 16-bit tensor-core operands, fp32 accumulate */
+enum { ETAC_ACTIVE_PASSTHROUGH = 0, ETAC_ACTIVE_PROPAGATE = 1 };  /* PASSTHROUGH: active rows keep u^ (mask M_p, L99) */
+enum { ETAC_IN_INDENTERS = 0, ETAC_IN_PENETRATION = 1 };
+
+typedef struct {
+  uint32_t struct_size;        /* = sizeof(etac_model_desc); ABI check */
+  int32_t n_nodes;             /* N >= 1 */
+  const float* node_pos;       /* host [N x 3], undeformed positions P, patch-local frame */
+  const float* node_normal;    /* host [N x 3], unit outward normals N */
+  int32_t n_patches;           /* P >= 1 when patch_offset != NULL; ignored otherwise */
+  const int32_t* patch_offset; /* host [P+1], 0 = off[0] < off[1] < ... < off[P] = N; nodes of a patch are
+                                  contiguous and K is zero across patches.  NULL: patches are the connected
+                                  components of the adjacency (must be contiguous index ranges), or one
+                                  patch if there is no adjacency either. */
+  const int32_t* adj_rowptr;   /* host [N+1] CSR mesh adjacency, optional (NULL) */
+  const int32_t* adj_col;      /* host [adj_rowptr[N]] */
+  int32_t kernel_type;         /* ETAC_KERNEL_EXP_L2 */
+  int32_t n_alpha;             /* 1 or P */
+  const float* alpha;          /* host [n_alpha], > 0 */
+  int32_t resid_arch;          /* ETAC_RESID_* */
+  int32_t resid_hidden;        /* 64 (only width built) */
+  const float *W1, *b1, *W2, *b2, *W3, *b3; /* host, Linear-layer layout [out x in]:
+                                  W1[64x9] (input order [u_lin(3), p(3), n(3)]) b1[64] W2[64x64] b2[64] W3[3x64] b3[3];
+                                  may be NULL when resid_arch == ETAC_RESID_NONE */
+  int32_t max_envs;            /* workspace sizing, >= 1 */
+  int32_t max_indenters;       /* M >= 0: indenter slots per environment */
+  int32_t precision;           /* ETAC_PREC_* */
+  int32_t active_mode;         /* ETAC_ACTIVE_* */
+  int32_t device;              /* CUDA ordinal */
+} etac_model_desc;
+
+/* Builds a context: validates, copies every host array, derives patches, builds the propagation
+ * matrix K (Eq. 1) per patch on the device, stages the MLP weights, allocates the per-step
+ * workspace for max_envs.  On failure *out is NULL.  The caller may free its arrays on return. */
+etac_status etac_create(const etac_model_desc* desc, etac_ctx** out);
+
+/* Frees everything the ctx owns after synchronising the device.  NULL is allowed. */
+etac_status etac_destroy(etac_ctx* ctx);
+
+typedef struct {
+  uint32_t struct_size;               /* = sizeof(etac_step_args) */
+  int32_t n_envs;                     /* 1..max_envs (0 is a no-op returning ETAC_OK) */
+  int32_t input_mode;                 /* ETAC_IN_* */
+  const etac_indenter* d_indenters;   /* device [E x max_indenters] (INDENTERS mode) */
+  const float* d_patch_pose;          /* device [E x P x 7] {t, q} of every patch in the indenters' world frame,
+                                         or NULL = identity */
+  const float* d_penetration;         /* device [E x N] (PENETRATION mode): delta; negatives clamp to 0 */
+  float* d_out;                       /* device [E x N x 3] fp32 displacement, REQUIRED, fully overwritten;
+                                         patch-local frame (u^ = -delta * n with the create-time normal) */
+  float* d_penetration_out;           /* optional device [E x N]: delta */
+  uint32_t* d_mask_out;               /* optional device [E x ceil(N/32)]: bit (i%32) of word i/32 = node i active */
+  float* d_analytic_out;              /* optional device [E x N x 3]: unmasked K.U^ on ALL rows
+                                         (the "linear decay only" term; test hook) */
+} etac_step_args;
+
+/* Enqueues S1-S4 for n_envs environments on cuda_stream (a cudaStream_t; NULL = default stream).
+ * Output for a patch none of whose nodes is in contact in that environment is exactly 0. */
+etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args);
+
+/* Options / introspection. */
+enum { ETAC_OPT_PATH = 1 };
+enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
+/* DENSE : tcgen05 tensor-core contraction K_p . U^ (needs ETAC_PREC_BF16);
+ * SPARSE: gather over the active nodes only (Omega U_a literally), fp32 SIMT;
+ * AUTO  : DENSE for BF16 contexts, SPARSE for FP32 contexts. */
+etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value);
+
+enum {
+  ETAC_INFO_N_NODES = 1,
+  ETAC_INFO_N_PATCHES = 2,
+  ETAC_INFO_MAX_ENVS = 3,
+  ETAC_INFO_DEVICE_BYTES = 4,       /* bytes of device memory the ctx owns */
+  ETAC_INFO_LAST_PATH = 5,          /* ETAC_PATH_* taken by the last step */
+  ETAC_INFO_LAST_LAUNCHES = 6,      /* kernels launched by the last step */
+  ETAC_INFO_LAST_CONTACT_PAIRS = 7, /* #(env,patch) pairs in contact in the last step; SYNCHRONISES the stream */
+  ETAC_INFO_SM_COUNT = 8
+};
+etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value);
+
+/* Message of the last failure on this ctx ("" if none); ctx-owned, valid until the next call.
+ * With ctx == NULL returns the message of the last failed etac_create on this thread. */
+const char* etac_last_error(const etac_ctx* ctx);
+
+/* Host-only helper (no CUDA): connected components of a CSR adjacency as contiguous patches.
+ * Writes off[0..*n_patches] (capacity cap entries).  ETAC_ERR_UNSUPPORTED if a component is not
+ * a contiguous index range, ETAC_ERR_CAPACITY if cap is too small. */
+etac_status etac_patches_from_adjacency(int32_t n_nodes, const int32_t* adj_rowptr, const int32_t* adj_col,
+                                        int32_t* off, int32_t cap, int32_t* n_patches);
+
+/* Library ABI version (ETAC_ABI_VERSION the .so was built with). */
+int32_t etac_abi_version(void);
+
+/* Timing helper for bench.py: times `iters` back-to-back etac_step calls on cuda_stream with CUDA
+ * events recorded on that stream and returns the mean milliseconds per step in *ms_per_step
+ * (host pointer).  If ms_kernels (host, [2]) is not NULL a second pass of `iters` steps records
+ * events between the kernels: ms_kernels[0] = S1 (sdf_penetration, incl. its two small memsets),
+ * ms_kernels[1] = fused S2+S3+S4 kernel, mean ms per launch.  Synchronises the stream on both sides. */
+etac_status etac_time_steps(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args, int32_t iters,
+                            float* ms_per_step, float* ms_kernels);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ETAC_H_ */

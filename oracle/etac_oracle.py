@@ -197,6 +197,7 @@ def step(model: OracleModel, indenters=None, patch_pose=None, penetration=None, 
     out["delta32"] = np.zeros((len(envs), N), dtype=np.float32)
     out["mask"] = np.zeros((len(envs), N), dtype=bool)
     out["contact"] = np.zeros((len(envs), Pn), dtype=bool)
+    out["patch_offset"] = np.asarray(model.patch_offset)
     for oi, e in enumerate(envs):
         # ---- O1
         if indenters is not None:

@@ -1,0 +1,496 @@
+// Host side of the C ABI declared in include/etac.h: validation, patch derivation, device
+// staging, workspace, tensor maps, and the per-step launch sequence  S1 -> (S2+S3+S4).
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <numeric>
+
+#include "etac_internal.h"
+
+using namespace etac;
+
+struct etac_ctx {
+  DevModel m{};
+  std::vector<void*> allocs;
+  size_t bytes = 0;
+  int device = 0, n_sm = 0, precision = 0, path_opt = ETAC_PATH_AUTO;
+  int last_path = ETAC_PATH_AUTO, last_launches = 0;
+  CUtensorMap tmA{}, tmB{};
+  bool have_tm = false;
+  cudaStream_t last_stream = nullptr;
+  std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+namespace {
+
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+    ok = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (prev >= 0) cudaSetDevice(prev);
+  }
+};
+
+etac_status fail(etac_ctx* c, etac_status st, const std::string& msg) {
+  if (c) c->err = msg; else g_create_err = msg;
+  return st;
+}
+std::string cuda_msg(const char* what, cudaError_t e) {
+  return std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
+}
+
+uint16_t f2bf(float f) {  // round-to-nearest-even
+  uint32_t u;
+  memcpy(&u, &f, 4);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+template <class T>
+cudaError_t dev_alloc(etac_ctx* c, T** p, size_t count, bool zero) {
+  void* q = nullptr;
+  const size_t bytes = std::max<size_t>(count * sizeof(T), 16);
+  cudaError_t e = cudaMalloc(&q, bytes);
+  if (e != cudaSuccess) return e;
+  c->allocs.push_back(q);
+  c->bytes += bytes;
+  if (zero) e = cudaMemset(q, 0, bytes);
+  *p = static_cast<T*>(q);
+  return e;
+}
+template <class T>
+cudaError_t dev_upload(etac_ctx* c, const T** p, const T* host, size_t count) {
+  T* q = nullptr;
+  cudaError_t e = dev_alloc(c, &q, count, false);
+  if (e != cudaSuccess) return e;
+  *p = q;
+  return cudaMemcpy(q, host, count * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 2-D bf16 tensor [rows x cols], row pitch ld elements; box [box_rows x 64 cols], 128-byte swizzle.
+bool make_tmap(CUtensorMap* tm, const void* base, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows,
+               std::string* why) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+  if (e != cudaSuccess || fn == nullptr || qres != cudaDriverEntryPointSuccess) {
+    *why = "cuTensorMapEncodeTiled entry point not available";
+    return false;
+  }
+  const cuuint64_t gdim[2] = {cols, rows};
+  const cuuint64_t gstride[1] = {ld * 2};
+  const cuuint32_t box[2] = {64, box_rows};
+  const cuuint32_t estr[2] = {1, 1};
+  CUresult r = reinterpret_cast<EncodeTiledFn>(fn)(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base),
+                                                   gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                                                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    *why = "cuTensorMapEncodeTiled failed with CUresult " + std::to_string((int)r);
+    return false;
+  }
+  return true;
+}
+
+int resolve_path(const etac_ctx* c) {
+  if (c->path_opt == ETAC_PATH_AUTO) return c->precision == ETAC_PREC_BF16 ? ETAC_PATH_DENSE : ETAC_PATH_SPARSE;
+  return c->path_opt;
+}
+
+// byte offset of element (n, k) in a K-major SWIZZLE_NONE UMMA operand with n_rows rows:
+// 8x8 core matrices (128 B), core matrices of one k-octet contiguous over the row groups.
+size_t wimg_off(int n, int k, int n_rows) {
+  return (size_t)(k / 8) * (n_rows / 8) * 128 + (size_t)(n / 8) * 128 + (size_t)(n % 8) * 16 + (size_t)(k % 8) * 2;
+}
+
+etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cudaEvent_t* ev) {
+  if (!ctx) return ETAC_ERR_INVALID_ARG;
+  if (!a || a->struct_size != sizeof(etac_step_args)) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_step_args");
+  if (a->n_envs < 0) return fail(ctx, ETAC_ERR_INVALID_ARG, "n_envs < 0");
+  if (a->n_envs > ctx->m.max_envs) return fail(ctx, ETAC_ERR_CAPACITY, "n_envs > max_envs");
+  if (a->input_mode != ETAC_IN_INDENTERS && a->input_mode != ETAC_IN_PENETRATION)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "bad input_mode");
+  if (!a->d_out) return fail(ctx, ETAC_ERR_INVALID_ARG, "d_out is required");
+  if (a->input_mode == ETAC_IN_INDENTERS && ctx->m.max_ind > 0 && !a->d_indenters)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "d_indenters is NULL");
+  if (a->input_mode == ETAC_IN_PENETRATION && !a->d_penetration)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "d_penetration is NULL");
+  const int path = resolve_path(ctx);
+  if (path == ETAC_PATH_DENSE && ctx->precision != ETAC_PREC_BF16)
+    return fail(ctx, ETAC_ERR_UNSUPPORTED, "ETAC_PATH_DENSE needs an ETAC_PREC_BF16 context");
+  ctx->last_path = path;
+  ctx->last_launches = 0;
+  ctx->last_stream = s;
+  if (a->n_envs == 0) return ETAC_OK;
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, ETAC_ERR_CUDA, "cudaSetDevice failed");
+
+  StepIO io{};
+  io.n_envs = a->n_envs, io.input_mode = a->input_mode;
+  io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
+  io.out = a->d_out, io.pen_out = a->d_penetration_out, io.mask_out = a->d_mask_out;
+  io.analytic_out = a->d_analytic_out;
+
+  cudaError_t e;
+  if (ev) cudaEventRecord(ev[0], s);
+  if (io.mask_out) {
+    const size_t words = (size_t)((ctx->m.n_nodes + 31) / 32) * a->n_envs;
+    if ((e = cudaMemsetAsync(io.mask_out, 0, words * 4, s)) != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset mask", e));
+  }
+  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess)
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset count", e));
+  if ((e = launch_sdf(ctx->m, io, path == ETAC_PATH_DENSE, s)) != cudaSuccess)
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
+  ++ctx->last_launches;
+  if (ev) cudaEventRecord(ev[1], s);
+  if (path == ETAC_PATH_DENSE) {
+    if ((e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, s)) != cudaSuccess)
+      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("dense_bf16_kernel", e));
+  } else {
+    if ((e = launch_gather_fp32(ctx->m, io, s)) != cudaSuccess)
+      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("gather_fp32_kernel", e));
+  }
+  ++ctx->last_launches;
+  if (ev) cudaEventRecord(ev[2], s);
+  return ETAC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t etac_abi_version(void) { return ETAC_ABI_VERSION; }
+
+const char* etac_last_error(const etac_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+etac_status etac_patches_from_adjacency(int32_t n, const int32_t* rowptr, const int32_t* col, int32_t* off,
+                                        int32_t cap, int32_t* n_patches) {
+  if (n < 1 || !rowptr || !off || !n_patches || cap < 2) return ETAC_ERR_INVALID_ARG;
+  if (rowptr[0] != 0) return ETAC_ERR_INVALID_ARG;
+  for (int i = 0; i < n; ++i)
+    if (rowptr[i + 1] < rowptr[i]) return ETAC_ERR_INVALID_ARG;
+  if (rowptr[n] > 0 && !col) return ETAC_ERR_INVALID_ARG;
+  std::vector<int32_t> parent(n);
+  std::iota(parent.begin(), parent.end(), 0);
+  auto find = [&](int x) {
+    while (parent[x] != x) x = parent[x] = parent[parent[x]];
+    return x;
+  };
+  for (int i = 0; i < n; ++i)
+    for (int k = rowptr[i]; k < rowptr[i + 1]; ++k) {
+      const int j = col[k];
+      if (j < 0 || j >= n) return ETAC_ERR_INVALID_ARG;
+      int a = find(i), b = find(j);
+      if (a != b) parent[std::max(a, b)] = std::min(a, b);  // representative = smallest index
+    }
+  int np = 0;
+  int cur = -1;
+  for (int i = 0; i < n; ++i) {
+    const int r = find(i);
+    if (r != cur) {
+      if (r != i) return ETAC_ERR_UNSUPPORTED;  // component re-entered: not a contiguous range
+      if (np + 1 >= cap) return ETAC_ERR_CAPACITY;
+      off[np++] = i;
+      cur = r;
+    }
+  }
+  off[np] = n;
+  *n_patches = np;
+  return ETAC_OK;
+}
+
+etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
+  if (!out) return fail(nullptr, ETAC_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  if (!d) return fail(nullptr, ETAC_ERR_INVALID_ARG, "desc is NULL");
+  if (d->struct_size != sizeof(etac_model_desc)) return fail(nullptr, ETAC_ERR_INVALID_ARG, "struct_size mismatch (ABI)");
+  if (d->n_nodes < 1 || !d->node_pos || !d->node_normal) return fail(nullptr, ETAC_ERR_INVALID_ARG, "mesh missing");
+  if (d->kernel_type != ETAC_KERNEL_EXP_L2) return fail(nullptr, ETAC_ERR_INVALID_ARG, "unknown kernel_type");
+  if (d->max_envs < 1 || d->max_indenters < 0) return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad max_envs / max_indenters");
+  if (d->precision != ETAC_PREC_FP32 && d->precision != ETAC_PREC_BF16) return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad precision");
+  if (d->active_mode != ETAC_ACTIVE_PASSTHROUGH && d->active_mode != ETAC_ACTIVE_PROPAGATE)
+    return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad active_mode");
+  if (d->resid_arch == ETAC_RESID_POINTNET) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "ETAC_RESID_POINTNET is not built");
+  if (d->resid_arch != ETAC_RESID_NONE && d->resid_arch != ETAC_RESID_PERNODE_MLP)
+    return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad resid_arch");
+  if (d->resid_arch == ETAC_RESID_PERNODE_MLP) {
+    if (d->resid_hidden != kHidden) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "only resid_hidden == 64 is built");
+    if (!d->W1 || !d->b1 || !d->W2 || !d->b2 || !d->W3 || !d->b3) return fail(nullptr, ETAC_ERR_INVALID_ARG, "MLP weights missing");
+  }
+  const int N = d->n_nodes;
+  // ---- patches
+  std::vector<int32_t> off;
+  if (d->patch_offset) {
+    if (d->n_patches < 1) return fail(nullptr, ETAC_ERR_INVALID_ARG, "n_patches < 1");
+    off.assign(d->patch_offset, d->patch_offset + d->n_patches + 1);
+    if (off.front() != 0 || off.back() != N) return fail(nullptr, ETAC_ERR_INVALID_ARG, "patch_offset must span [0, N]");
+    for (size_t p = 0; p + 1 < off.size(); ++p)
+      if (off[p + 1] <= off[p]) return fail(nullptr, ETAC_ERR_INVALID_ARG, "patch_offset must be strictly increasing");
+    if (d->adj_rowptr) {  // validate: no edge may cross a patch boundary
+      std::vector<int32_t> pid(N);
+      for (size_t p = 0; p + 1 < off.size(); ++p) std::fill(pid.begin() + off[p], pid.begin() + off[p + 1], (int32_t)p);
+      for (int i = 0; i < N; ++i)
+        for (int k = d->adj_rowptr[i]; k < d->adj_rowptr[i + 1]; ++k) {
+          const int j = d->adj_col ? d->adj_col[k] : -1;
+          if (j < 0 || j >= N) return fail(nullptr, ETAC_ERR_INVALID_ARG, "adjacency index out of range");
+          if (pid[j] != pid[i]) return fail(nullptr, ETAC_ERR_INVALID_ARG, "adjacency edge crosses a patch boundary");
+        }
+    }
+  } else if (d->adj_rowptr) {
+    off.resize((size_t)N + 1);
+    int32_t np = 0;
+    etac_status st = etac_patches_from_adjacency(N, d->adj_rowptr, d->adj_col, off.data(), N + 1, &np);
+    if (st != ETAC_OK) return fail(nullptr, st, "patches could not be derived from the adjacency");
+    off.resize((size_t)np + 1);
+  } else {
+    off = {0, N};
+  }
+  const int P = (int)off.size() - 1;
+  if (P > kMaxPatches) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "more than 1024 patches");
+  if (d->n_alpha != 1 && d->n_alpha != P) return fail(nullptr, ETAC_ERR_INVALID_ARG, "n_alpha must be 1 or P");
+  if (!d->alpha) return fail(nullptr, ETAC_ERR_INVALID_ARG, "alpha is NULL");
+  for (int k = 0; k < d->n_alpha; ++k)
+    if (!(d->alpha[k] > 0.0f) || !isfinite(d->alpha[k])) return fail(nullptr, ETAC_ERR_INVALID_ARG, "alpha must be > 0");
+
+  // ---- device
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    return fail(nullptr, ETAC_ERR_CUDA, "no CUDA device (this library has no CPU fallback)");
+  }
+  if (d->device < 0 || d->device >= ndev) return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad device ordinal");
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, d->device)) != cudaSuccess) return fail(nullptr, ETAC_ERR_CUDA, cuda_msg("cudaGetDeviceProperties", e));
+  if (prop.major != 10) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "needs a compute-capability 10.x (Blackwell, sm_100a) device");
+  DeviceGuard guard(d->device);
+  if (!guard.ok) return fail(nullptr, ETAC_ERR_CUDA, "cudaSetDevice failed");
+
+  etac_ctx* c = new (std::nothrow) etac_ctx();
+  if (!c) return fail(nullptr, ETAC_ERR_ALLOC, "host allocation failed");
+  c->device = d->device, c->n_sm = prop.multiProcessorCount, c->precision = d->precision;
+  DevModel& m = c->m;
+  m.n_nodes = N, m.n_patches = P, m.max_envs = d->max_envs, m.max_ind = d->max_indenters;
+  m.resid = d->resid_arch, m.active_mode = d->active_mode;
+
+  auto bail = [&](etac_status st, const std::string& msg) {
+    g_create_err = msg;
+    for (void* p : c->allocs) cudaFree(p);
+    delete c;
+    return st;
+  };
+#define CK(call, what)                                                                              \
+  do {                                                                                              \
+    cudaError_t e_ = (call);                                                                        \
+    if (e_ != cudaSuccess)                                                                          \
+      return bail(e_ == cudaErrorMemoryAllocation ? ETAC_ERR_ALLOC : ETAC_ERR_CUDA, cuda_msg(what, e_)); \
+  } while (0)
+
+  // mesh as float4 (coalesced 16-byte node loads)
+  std::vector<float4> pos4(N), nrm4(N);
+  for (int i = 0; i < N; ++i) {
+    pos4[i] = make_float4(d->node_pos[3 * i], d->node_pos[3 * i + 1], d->node_pos[3 * i + 2], 0.f);
+    nrm4[i] = make_float4(d->node_normal[3 * i], d->node_normal[3 * i + 1], d->node_normal[3 * i + 2], 0.f);
+  }
+  CK(dev_upload(c, &m.pos4, pos4.data(), N), "upload pos");
+  CK(dev_upload(c, &m.nrm4, nrm4.data(), N), "upload normal");
+
+  std::vector<PatchInfo> hp(P);
+  std::vector<ChunkInfo> chunks;
+  int64_t k32_total = 0;
+  int max_np = 0;
+  for (int p = 0; p < P; ++p) {
+    PatchInfo& pi = hp[p];
+    pi.off = off[p], pi.n = off[p + 1] - off[p];
+    pi.k32_off = k32_total;
+    k32_total += (int64_t)pi.n * pi.n;
+    pi.alpha = d->alpha[d->n_alpha == 1 ? 0 : p];
+    double c0 = 0, c1 = 0, c2 = 0;
+    for (int i = pi.off; i < pi.off + pi.n; ++i) c0 += pos4[i].x, c1 += pos4[i].y, c2 += pos4[i].z;
+    c0 /= pi.n, c1 /= pi.n, c2 /= pi.n;
+    pi.bc[0] = (float)c0, pi.bc[1] = (float)c1, pi.bc[2] = (float)c2;
+    double r2 = 0;
+    for (int i = pi.off; i < pi.off + pi.n; ++i) {
+      const double dx = pos4[i].x - pi.bc[0], dy = pos4[i].y - pi.bc[1], dz = pos4[i].z - pi.bc[2];
+      r2 = std::max(r2, dx * dx + dy * dy + dz * dz);
+    }
+    pi.brad = (float)(sqrt(r2) * (1.0 + 1e-5) + 1e-6);
+    max_np = std::max(max_np, pi.n);
+    for (int n0 = 0; n0 < pi.n; n0 += kGatherChunk)
+      chunks.push_back(ChunkInfo{p, pi.off + n0, std::min(kGatherChunk, pi.n - n0)});
+  }
+  m.n_chunks = (int)chunks.size();
+  m.kw = (max_np + 63) / 64 * 64;
+  m.ldu = (N + 63) / 64 * 64;
+  CK(dev_upload(c, &m.patch, hp.data(), P), "upload patches");
+  CK(dev_upload(c, &m.chunk, chunks.data(), chunks.size()), "upload chunks");
+
+  float* k32 = nullptr;
+  __nv_bfloat16* k16 = nullptr;
+  CK(dev_alloc(c, &k32, (size_t)k32_total, false), "alloc K fp32");
+  CK(dev_alloc(c, &k16, (size_t)N * m.kw, true), "alloc K bf16");
+  m.k32 = k32, m.k16 = k16;
+  CK(launch_build_k(m, k32, k16, 0), "build_k_kernel");
+
+  if (d->resid_arch == ETAC_RESID_PERNODE_MLP) {
+    // fp32 blob for the SIMT path
+    std::vector<float> wf(64 * 3 + 64 * 64 + 64 + 3 * 64 + 3);
+    float* q = wf.data();
+    for (int k = 0; k < 64; ++k)
+      for (int cc = 0; cc < 3; ++cc) *q++ = d->W1[k * 9 + cc];
+    memcpy(q, d->W2, 4096 * 4), q += 4096;
+    memcpy(q, d->b2, 64 * 4), q += 64;
+    memcpy(q, d->W3, 192 * 4), q += 192;
+    memcpy(q, d->b3, 3 * 4);
+    CK(dev_upload(c, &m.wf32, wf.data(), wf.size()), "upload weights");
+    const float *dW1 = nullptr, *db1 = nullptr;
+    CK(dev_upload(c, &dW1, d->W1, 64 * 9), "upload W1");
+    CK(dev_upload(c, &db1, d->b1, 64), "upload b1");
+    float* c1t = nullptr;
+    CK(dev_alloc(c, &c1t, (size_t)64 * N, false), "alloc c1");
+    m.c1t = c1t;
+    CK(launch_build_c1(m, dW1, db1, c1t, 0), "build_c1_kernel");
+    // bf16 shared-memory image for the tensor-core path.  The epilogue evaluates
+    // silu(x) = h + h*tanh(h) with h = x/2, so the 0.5 is folded into layers 1 and 2 (exact).
+    std::vector<uint8_t> img(kWImgBytes, 0);
+    auto put = [&](size_t base, int n, int k, int rows, float v) {
+      const uint16_t b = f2bf(v);
+      memcpy(&img[base + wimg_off(n, k, rows)], &b, 2);
+    };
+    for (int n = 0; n < 64; ++n) {
+      for (int k = 0; k < 9; ++k) put(0, n, k, 64, 0.5f * d->W1[n * 9 + k]);
+      put(0, n, 9, 64, 0.5f * d->b1[n]);
+      for (int k = 0; k < 64; ++k) put(kW1ImgBytes, n, k, 64, 0.5f * d->W2[n * 64 + k]);
+      put(kW1ImgBytes, n, 64, 64, 0.5f * d->b2[n]);
+    }
+    for (int n = 0; n < 3; ++n) {
+      for (int k = 0; k < 64; ++k) put(kW1ImgBytes + kW2ImgBytes, n, k, 16, d->W3[n * 64 + k]);
+      put(kW1ImgBytes + kW2ImgBytes, n, 64, 16, d->b3[n]);
+    }
+    CK(dev_upload(c, &m.wimg, img.data(), img.size()), "upload weight image");
+  }
+
+  // ---- per-step workspace
+  const size_t urows = (size_t)((d->max_envs + 31) / 32) * 96;
+  CK(dev_alloc(c, &m.delta, (size_t)d->max_envs * N, true), "alloc delta");
+  CK(dev_alloc(c, &m.count, (size_t)P, true), "alloc count");
+  CK(dev_alloc(c, &m.envlist, (size_t)P * d->max_envs, true), "alloc envlist");
+  CK(dev_alloc(c, &m.flags, (size_t)P * d->max_envs, true), "alloc flags");
+  if (d->precision == ETAC_PREC_BF16) {
+    CK(dev_alloc(c, &m.uhat_t, urows * m.ldu, true), "alloc uhat");
+    std::string why;
+    if (!make_tmap(&c->tmA, m.k16, (uint64_t)N, (uint64_t)m.kw, (uint64_t)m.kw, 128, &why) ||
+        !make_tmap(&c->tmB, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 96, &why))
+      return bail(ETAC_ERR_CUDA, why);
+    c->have_tm = true;
+    CK(dense_bf16_configure(), "cudaFuncSetAttribute(dense_bf16_kernel)");
+  }
+  CK(cudaDeviceSynchronize(), "create-time kernels");
+#undef CK
+  *out = c;
+  return ETAC_OK;
+}
+
+etac_status etac_destroy(etac_ctx* ctx) {
+  if (!ctx) return ETAC_OK;
+  etac_status st = ETAC_OK;
+  {
+    DeviceGuard guard(ctx->device);
+    if (cudaDeviceSynchronize() != cudaSuccess) st = ETAC_ERR_CUDA;
+    for (void* p : ctx->allocs) cudaFree(p);
+  }
+  delete ctx;
+  return st;
+}
+
+etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args) {
+  return step_impl(ctx, static_cast<cudaStream_t>(cuda_stream), args, nullptr);
+}
+
+etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
+  if (!ctx) return ETAC_ERR_INVALID_ARG;
+  if (key != ETAC_OPT_PATH) return fail(ctx, ETAC_ERR_INVALID_ARG, "unknown option");
+  if (value != ETAC_PATH_AUTO && value != ETAC_PATH_DENSE && value != ETAC_PATH_SPARSE)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_PATH value");
+  if (value == ETAC_PATH_DENSE && ctx->precision != ETAC_PREC_BF16)
+    return fail(ctx, ETAC_ERR_UNSUPPORTED, "ETAC_PATH_DENSE needs an ETAC_PREC_BF16 context");
+  ctx->path_opt = (int)value;
+  return ETAC_OK;
+}
+
+etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value) {
+  if (!ctx || !value) return ETAC_ERR_INVALID_ARG;
+  switch (key) {
+    case ETAC_INFO_N_NODES: *value = ctx->m.n_nodes; return ETAC_OK;
+    case ETAC_INFO_N_PATCHES: *value = ctx->m.n_patches; return ETAC_OK;
+    case ETAC_INFO_MAX_ENVS: *value = ctx->m.max_envs; return ETAC_OK;
+    case ETAC_INFO_DEVICE_BYTES: *value = (int64_t)ctx->bytes; return ETAC_OK;
+    case ETAC_INFO_LAST_PATH: *value = ctx->last_path; return ETAC_OK;
+    case ETAC_INFO_LAST_LAUNCHES: *value = ctx->last_launches; return ETAC_OK;
+    case ETAC_INFO_SM_COUNT: *value = ctx->n_sm; return ETAC_OK;
+    case ETAC_INFO_LAST_CONTACT_PAIRS: {
+      DeviceGuard guard(ctx->device);
+      std::vector<int32_t> cnt(ctx->m.n_patches);
+      if (cudaStreamSynchronize(ctx->last_stream) != cudaSuccess) return ETAC_ERR_CUDA;
+      if (cudaMemcpy(cnt.data(), ctx->m.count, cnt.size() * 4, cudaMemcpyDeviceToHost) != cudaSuccess) return ETAC_ERR_CUDA;
+      *value = std::accumulate(cnt.begin(), cnt.end(), (int64_t)0);
+      return ETAC_OK;
+    }
+    default: return ETAC_ERR_INVALID_ARG;
+  }
+}
+
+etac_status etac_time_steps(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args, int32_t iters,
+                            float* ms_per_step, float* ms_kernels) {
+  if (!ctx || !ms_per_step || iters < 1) return ETAC_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  DeviceGuard guard(ctx->device);
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, "cudaEventCreate");
+  etac_status st = ETAC_OK;
+  cudaStreamSynchronize(s);
+  cudaEventRecord(e0, s);
+  for (int i = 0; i < iters && st == ETAC_OK; ++i) st = step_impl(ctx, s, args, nullptr);
+  cudaEventRecord(e1, s);
+  cudaError_t e = cudaStreamSynchronize(s);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  *ms_per_step = ms / iters;
+  cudaEventDestroy(e0), cudaEventDestroy(e1);
+  if (st != ETAC_OK) return st;
+  if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("etac_time_steps", e));
+  if (ms_kernels) {
+    // second pass with events between the kernels: [0] = S1 (incl. its memsets), [1] = fused S2-S4
+    std::vector<cudaEvent_t> ev((size_t)iters * 3);
+    for (auto& x : ev) cudaEventCreate(&x);
+    for (int i = 0; i < iters && st == ETAC_OK; ++i) st = step_impl(ctx, s, args, &ev[(size_t)i * 3]);
+    e = cudaStreamSynchronize(s);
+    double a = 0, b = 0;
+    if (st == ETAC_OK && e == cudaSuccess)
+      for (int i = 0; i < iters; ++i) {
+        float t;
+        cudaEventElapsedTime(&t, ev[(size_t)i * 3], ev[(size_t)i * 3 + 1]), a += t;
+        cudaEventElapsedTime(&t, ev[(size_t)i * 3 + 1], ev[(size_t)i * 3 + 2]), b += t;
+      }
+    for (auto& x : ev) cudaEventDestroy(x);
+    ms_kernels[0] = (float)(a / iters), ms_kernels[1] = (float)(b / iters);
+    if (st != ETAC_OK) return st;
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("etac_time_steps", e));
+  }
+  return ETAC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,86 @@
+// Internal declarations shared by the host API (etac_api.cu) and the kernels.  Not installed.
+#pragma once
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/etac.h"
+
+namespace etac {
+
+constexpr int kHidden = 64;
+constexpr int kMaxPatches = 1024;
+
+// One sensor patch (contiguous node range; K is zero across patches, R9).
+struct PatchInfo {
+  int32_t off;        // first node
+  int32_t n;          // nodes in the patch
+  int64_t k32_off;    // element offset of K_p (fp32, [n x n] row-major) in k32
+  float alpha;
+  float bc[3];        // bounding-sphere centre (patch-local frame)
+  float brad;         // bounding-sphere radius
+};
+
+// Node chunk of <= kGatherChunk nodes of one patch, for the fp32 gather kernel's grid.
+struct ChunkInfo {
+  int32_t patch;
+  int32_t node0;  // first node (global index)
+  int32_t count;
+};
+constexpr int kGatherChunk = 128;
+
+// Shared-memory image of the MLP weights for the tensor-core path (bf16, UMMA K-major
+// SWIZZLE_NONE core-matrix layout; see k_dense_bf16.cu).
+constexpr int kW1ImgBytes = 64 * 16 * 2;   // N=64,  K=16   (9 inputs + bias column)
+constexpr int kW2ImgBytes = 64 * 80 * 2;   // N=64,  K=80   (64 + bias column, padded to 5 k-steps)
+constexpr int kW3ImgBytes = 16 * 80 * 2;   // N=16,  K=80   (3 outputs padded to 16)
+constexpr int kWImgBytes = kW1ImgBytes + kW2ImgBytes + kW3ImgBytes;
+
+struct DevModel {
+  int32_t n_nodes, n_patches, n_chunks;
+  int32_t kw;                 // padded column count of k16 (multiple of 64)
+  int32_t ldu;                // row pitch (elements) of uhat_t
+  int32_t max_envs, max_ind;
+  int32_t resid, active_mode;
+  const float4* pos4;         // [N] (x,y,z,0)
+  const float4* nrm4;         // [N]
+  const PatchInfo* patch;     // [P]
+  const ChunkInfo* chunk;     // [n_chunks]
+  const float* k32;           // per patch [n x n]
+  const __nv_bfloat16* k16;   // [N x kw], row i holds K_p[i - off_p][0..n_p) then zeros
+  const float* wf32;          // fp32 weights blob: W1u[64x3] | c1t[64 x N] is separate | W2[64x64] b2[64] W3[3x64] b3[3]
+  const float* c1t;           // [64 x N]: W1[:,3:9].[p;n] + b1, transposed for coalescing
+  const uint8_t* wimg;        // kWImgBytes
+  // per-step workspace
+  float* delta;               // [max_envs x N]
+  __nv_bfloat16* uhat_t;      // [3*max_envs (+pad) x ldu]: row slot*3+c, column = node j
+  int32_t* count;             // [P] contacting envs per patch (this step)
+  int32_t* envlist;           // [P x max_envs]
+  uint8_t* flags;             // [max_envs x P]
+};
+
+struct StepIO {
+  int32_t n_envs, input_mode;
+  const etac_indenter* ind;
+  const float* patch_pose;
+  const float* pen_in;
+  float* out;
+  float* pen_out;
+  uint32_t* mask_out;
+  float* analytic_out;
+};
+
+// kernel launchers (each returns cudaGetLastError())
+cudaError_t launch_build_k(const DevModel& m, float* k32, __nv_bfloat16* k16, cudaStream_t s);
+cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1, float* c1t, cudaStream_t s);
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, bool write_uhat, cudaStream_t s);
+cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
+cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
+                              int n_sm, cudaStream_t s);
+cudaError_t dense_bf16_configure();
+
+}  // namespace etac

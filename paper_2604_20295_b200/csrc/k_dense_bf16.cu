@@ -1,0 +1,291 @@
+// S2+S3+S4 fused, tensor-core path (sm_100a: TMA + tcgen05.mma + TMEM).
+//
+//   S2  u_lin = K_p . U^  as a dense bf16 contraction with fp32 accumulation in TMEM
+//       ("propagation matrix Omega ... computed as Omega U_a"; the zero rows of the
+//       zero-padded U^ contribute nothing, R3),
+//   S3  residual MLP 9 -> 64 -> 64 -> 3 (SiLU) on the accumulator tile, each layer one small
+//       tcgen05.mma whose A operand is written to TMEM by the epilogue warps and whose B operand
+//       (the weights, biases folded in as an extra K column) stays in shared memory,
+//   S4  mask M_p + combine (Eq. 2) and the store of U[e][i][0..2].
+//
+// Work item = (patch p, block of 128 nodes, tile of TE contacting environments of that patch).
+// The grid is persistent (2 CTAs per SM); every CTA walks items blockIdx.x, +gridDim.x, ...
+// 6 warps: 0 = TMA producer, 1 = MMA issuer (+ TMEM alloc), 2..5 = epilogue (thread = node).
+//
+// TMEM columns (fp32 lanes = nodes):   [0,96)  u_lin accumulator, column 3*env+c
+//                                      [96,160)  D: pre-activations of the current MLP layer
+//                                      [160,200) A2/A3: bf16 hidden activations (+ ones column)
+//                                      [200,208) A1: bf16 [u_lin(3), p(3), n(3), 1, 0..]
+#include "etac_internal.h"
+#include "sm100_prims.cuh"
+
+namespace etac {
+
+constexpr int BM = 128, BK = 64, TE = 32, BN = TE * 3, STAGES = 3;
+constexpr int A_STAGE = BM * BK * 2, B_STAGE = BN * BK * 2;
+constexpr int kDenseThreads = 192;
+constexpr uint32_t kTmemCols = 256;
+constexpr uint32_t COL_ACC = 0, COL_D = 96, COL_A2 = 160, COL_A1 = 200;
+
+struct __align__(8) DenseBars {
+  uint64_t full[STAGES], empty[STAGES];
+  uint64_t acc_full, acc_empty, a_ready, d_ready;
+  uint32_t tmem_base;
+  uint32_t pad;
+};
+
+__host__ __device__ constexpr size_t dense_smem_bytes(int n_patches) {
+  return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE + B_STAGE) + kWImgBytes + sizeof(DenseBars) +
+         (size_t)(n_patches + 1) * 4 + 16;
+}
+
+struct Item {
+  int p, mb, tile, cnt;
+};
+
+__device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, const DevModel& m, int w, int& pcur,
+                                            Item& it) {
+  if (w >= prefix[n_patches]) return false;
+  while (prefix[pcur + 1] <= w) ++pcur;
+  const int cnt = m.count[pcur];
+  const int tiles = (cnt + TE - 1) / TE;
+  const int r = w - prefix[pcur];
+  it.p = pcur;
+  it.mb = r / tiles;
+  it.tile = r - it.mb * tiles;
+  it.cnt = min(TE, cnt - it.tile * TE);
+  return true;
+}
+
+template <bool kResid>
+__global__ void __launch_bounds__(kDenseThreads, 2)
+    dense_bf16_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
+                      const __grid_constant__ CUtensorMap tmB) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* sA = smem;
+  uint8_t* sB = smem + STAGES * A_STAGE;
+  uint8_t* sW = sB + STAGES * B_STAGE;
+  DenseBars* bars = reinterpret_cast<DenseBars*>(sW + kWImgBytes);
+  int* prefix = reinterpret_cast<int*>(bars + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
+    mbar_init(&bars->acc_full, 1);
+    mbar_init(&bars->acc_empty, 4);
+    mbar_init(&bars->a_ready, 4);
+    mbar_init(&bars->d_ready, 1);
+    fence_barrier_init();
+    int acc = 0;
+    prefix[0] = 0;
+    for (int p = 0; p < m.n_patches; ++p) {
+      const int cnt = m.count[p];
+      acc += ((cnt + TE - 1) / TE) * ((m.patch[p].n + BM - 1) / BM);
+      prefix[p + 1] = acc;
+    }
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB);
+  }
+  if (warp == 1) tmem_alloc<kTmemCols>(&bars->tmem_base);
+  if constexpr (kResid) {
+    const uint4* src = reinterpret_cast<const uint4*>(m.wimg);
+    uint4* dst = reinterpret_cast<uint4*>(sW);
+    for (int k = threadIdx.x; k < kWImgBytes / 16; k += kDenseThreads) dst[k] = src[k];
+    fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor-core (async) proxy
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = bars->tmem_base;
+
+  if (warp == 0) {
+    // ------------------------------------------------------------------ TMA producer
+    if (lane == 0) {
+      int pcur = 0, stage = 0;
+      uint32_t ph = 0;
+      Item it;
+      for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+        const PatchInfo pi = m.patch[it.p];
+        const int nkb = (pi.n + BK - 1) / BK;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(&bars->empty[stage], ph ^ 1);
+          mbar_arrive_expect_tx(&bars->full[stage], A_STAGE + B_STAGE);
+          tma_load_2d(sA + stage * A_STAGE, &tmA, &bars->full[stage], kb * BK, pi.off + it.mb * BM);
+          tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], pi.off + kb * BK, it.tile * BN);
+          if (++stage == STAGES) stage = 0, ph ^= 1;
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------------ MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc_prop = make_idesc_bf16(BM, BN);
+      constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
+      constexpr uint32_t idesc_o = make_idesc_bf16(BM, 16);
+      const uint64_t dW1 = make_desc(smem_u32(sW), 1024, 128, kLayoutNone);
+      const uint64_t dW2 = make_desc(smem_u32(sW + kW1ImgBytes), 1024, 128, kLayoutNone);
+      const uint64_t dW3 = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 256, 128, kLayoutNone);
+      int pcur = 0, stage = 0;
+      uint32_t ph = 0, acc_ph = 0, a_ph = 0;
+      Item it;
+      for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+        const int nkb = (m.patch[it.p].n + BK - 1) / BK;
+        mbar_wait(&bars->acc_empty, acc_ph ^ 1);
+        acc_ph ^= 1;
+        tc_fence_after();
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(&bars->full[stage], ph);
+          tc_fence_after();
+          const uint64_t dA = make_desc(smem_u32(sA + stage * A_STAGE), 16, 1024, kLayoutSw128);
+          const uint64_t dB = make_desc(smem_u32(sB + stage * B_STAGE), 16, 1024, kLayoutSw128);
+#pragma unroll
+          for (int k = 0; k < BK / 16; ++k)
+            mma_ss(tmem + COL_ACC, dA + 2 * k, dB + 2 * k, idesc_prop, (kb | k) != 0);
+          tc_commit(&bars->empty[stage]);
+          if (++stage == STAGES) stage = 0, ph ^= 1;
+        }
+        tc_commit(&bars->acc_full);
+        if constexpr (kResid) {
+          for (int el = 0; el < it.cnt; ++el) {
+            mbar_wait(&bars->a_ready, a_ph), a_ph ^= 1;
+            tc_fence_after();
+            mma_ts(tmem + COL_D, tmem + COL_A1, dW1, idesc_h, 0);
+            tc_commit(&bars->d_ready);
+            mbar_wait(&bars->a_ready, a_ph), a_ph ^= 1;
+            tc_fence_after();
+#pragma unroll
+            for (int k = 0; k < 5; ++k)
+              mma_ts(tmem + COL_D, tmem + COL_A2 + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
+            tc_commit(&bars->d_ready);
+            mbar_wait(&bars->a_ready, a_ph), a_ph ^= 1;
+            tc_fence_after();
+#pragma unroll
+            for (int k = 0; k < 5; ++k)
+              mma_ts(tmem + COL_D, tmem + COL_A2 + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
+            tc_commit(&bars->d_ready);
+          }
+        }
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ epilogue (thread = node)
+    const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
+    const uint32_t trow = tmem + (lane_base << 16);
+    const int row = lane_base + lane;
+    if constexpr (kResid) {
+      // bias ("ones") column of A2/A3: bf16 element 64 = 1.0, elements 65..79 = 0; written once
+      const uint32_t ones[8] = {0x00003F80u, 0, 0, 0, 0, 0, 0, 0};
+      tmem_st8(trow + COL_A2 + 32, ones);
+      tc_wait_st();
+    }
+    int pcur = 0;
+    uint32_t acc_ph = 0, d_ph = 0;
+    Item it;
+    for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+      const PatchInfo pi = m.patch[it.p];
+      const int li = it.mb * BM + row;
+      const bool valid = li < pi.n;
+      const int g = pi.off + (valid ? li : 0);
+      const float4 nrm = m.nrm4[g];
+      uint32_t a1[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+      float px = 0.f;
+      if constexpr (kResid) {
+        const float4 pos = m.pos4[g];
+        px = pos.x;
+        a1[2] = pack_bf16(pos.y, pos.z);
+        a1[3] = pack_bf16(nrm.x, nrm.y);
+        a1[4] = pack_bf16(nrm.z, 1.0f);
+      }
+      const int* envs = m.envlist + (int64_t)it.p * m.max_envs + it.tile * TE;
+      mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
+      tc_fence_after();
+      for (int el = 0; el < it.cnt; ++el) {
+        const int env = envs[el];
+        const int64_t node = (int64_t)env * m.n_nodes + g;
+        const float dl = valid ? m.delta[node] : 0.0f;
+        uint32_t ur[4];
+        tmem_ld4(trow + COL_ACC + 3 * el, ur);
+        tc_wait_ld();
+        const float ux = __uint_as_float(ur[0]), uy = __uint_as_float(ur[1]), uz = __uint_as_float(ur[2]);
+        float ox = ux, oy = uy, oz = uz;
+        if constexpr (kResid) {
+          a1[0] = pack_bf16(ux, uy);
+          a1[1] = pack_bf16(uz, px);
+          tmem_st8(trow + COL_A1, a1);
+          tc_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bars->a_ready);
+#pragma unroll 1
+          for (int layer = 0; layer < 2; ++layer) {
+            mbar_wait(&bars->d_ready, d_ph), d_ph ^= 1;
+            tc_fence_after();
+            uint32_t h[32], packed[16];
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+              tmem_ld32(trow + COL_D + 32 * half, h);
+              tc_wait_ld();
+#pragma unroll
+              for (int k = 0; k < 16; ++k) {
+                // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
+                const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
+                packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
+              }
+              tmem_st16(trow + COL_A2 + 16 * half, packed);
+            }
+            tc_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars->a_ready);
+          }
+          mbar_wait(&bars->d_ready, d_ph), d_ph ^= 1;
+          tc_fence_after();
+          uint32_t rr[4];
+          tmem_ld4(trow + COL_D, rr);
+          tc_wait_ld();
+          ox += __uint_as_float(rr[0]), oy += __uint_as_float(rr[1]), oz += __uint_as_float(rr[2]);
+        }
+        if (valid) {
+          if (dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH) ox = -dl * nrm.x, oy = -dl * nrm.y, oz = -dl * nrm.z;
+          float* o = io.out + node * 3;
+          o[0] = ox, o[1] = oy, o[2] = oz;
+          if (io.analytic_out) {
+            float* a = io.analytic_out + node * 3;
+            a[0] = ux, a[1] = uy, a[2] = uz;
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&bars->acc_empty);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc<kTmemCols>(tmem);
+  }
+}
+
+cudaError_t dense_bf16_configure() {
+  const int bytes = (int)dense_smem_bytes(kMaxPatches);
+  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(dense_bf16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
+                              int n_sm, cudaStream_t s) {
+  const size_t smem = dense_smem_bytes(m.n_patches);
+  const int grid = 2 * n_sm;
+  if (m.resid != ETAC_RESID_NONE)
+    dense_bf16_kernel<true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  else
+    dense_bf16_kernel<false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  return cudaGetLastError();
+}
+
+}  // namespace etac

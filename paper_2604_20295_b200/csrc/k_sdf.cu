@@ -1,0 +1,198 @@
+// S1: contact detection and penalty displacement of the active nodes.
+//
+// One CTA per (environment, patch).  Every node of the patch is transformed into the world
+// frame of the indenters, the union SDF phi = min_k sdf_k is evaluated, active <=> phi < 0,
+// delta = -phi on active nodes.  The arithmetic of phi is single-rounded fp32 in a fixed order
+// (no FMA contraction -> __fmul_rn/__fadd_rn/__fsub_rn/__fsqrt_rn) so that the
+// contact decision is reproducible by an independent fp32 implementation.
+//
+// Outputs: delta workspace [E x N] (only where the patch was evaluated), per-(env,patch) contact
+// flag, per-patch compact list of contacting environments (slot = position in that list), and,
+// for the tensor-core path, the GEMM B operand U^ = -delta * n as bf16 rows uhat_t[slot*3+c][j].
+// A patch with no active node gets its rows of the output zero-filled here (R8), so
+// the contraction kernels only ever touch contacting (env, patch) pairs.
+#include "etac_internal.h"
+
+namespace etac {
+
+struct SInd {
+  int type;
+  float prm[3];
+  float t[3];
+  float R[9];
+};
+
+__device__ __forceinline__ void quat_to_rot(const float* q, float* R) {
+  const float x = q[0], y = q[1], z = q[2], w = q[3];
+  const float xx = __fmul_rn(x, x), yy = __fmul_rn(y, y), zz = __fmul_rn(z, z);
+  const float xy = __fmul_rn(x, y), xz = __fmul_rn(x, z), yz = __fmul_rn(y, z);
+  const float wx = __fmul_rn(w, x), wy = __fmul_rn(w, y), wz = __fmul_rn(w, z);
+  R[0] = __fsub_rn(1.0f, __fmul_rn(2.0f, __fadd_rn(yy, zz)));
+  R[1] = __fmul_rn(2.0f, __fsub_rn(xy, wz));
+  R[2] = __fmul_rn(2.0f, __fadd_rn(xz, wy));
+  R[3] = __fmul_rn(2.0f, __fadd_rn(xy, wz));
+  R[4] = __fsub_rn(1.0f, __fmul_rn(2.0f, __fadd_rn(xx, zz)));
+  R[5] = __fmul_rn(2.0f, __fsub_rn(yz, wx));
+  R[6] = __fmul_rn(2.0f, __fsub_rn(xz, wy));
+  R[7] = __fmul_rn(2.0f, __fadd_rn(yz, wx));
+  R[8] = __fsub_rn(1.0f, __fmul_rn(2.0f, __fadd_rn(xx, yy)));
+}
+
+__device__ __forceinline__ float len3(float a, float b, float c) {
+  return __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(a, a), __fmul_rn(b, b)), __fmul_rn(c, c)));
+}
+
+// Union signed distance at world point X.
+__device__ __forceinline__ float union_sdf(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2) {
+  float phi = __int_as_float(0x7f800000);
+  for (int k = 0; k < n_ind; ++k) {
+    const SInd& s = ind[k];
+    if (s.type == ETAC_IND_NONE) continue;
+    const float d0 = __fsub_rn(X0, s.t[0]), d1 = __fsub_rn(X1, s.t[1]), d2 = __fsub_rn(X2, s.t[2]);
+    // y = R^T d
+    const float y0 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[0], d0), __fmul_rn(s.R[3], d1)), __fmul_rn(s.R[6], d2));
+    const float y1 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[1], d0), __fmul_rn(s.R[4], d1)), __fmul_rn(s.R[7], d2));
+    const float y2 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[2], d0), __fmul_rn(s.R[5], d1)), __fmul_rn(s.R[8], d2));
+    float v;
+    if (s.type == ETAC_IND_SPHERE) {
+      v = __fsub_rn(len3(y0, y1, y2), s.prm[0]);
+    } else if (s.type == ETAC_IND_BOX) {
+      const float q0 = __fsub_rn(fabsf(y0), s.prm[0]);
+      const float q1 = __fsub_rn(fabsf(y1), s.prm[1]);
+      const float q2 = __fsub_rn(fabsf(y2), s.prm[2]);
+      const float outside = len3(fmaxf(q0, 0.0f), fmaxf(q1, 0.0f), fmaxf(q2, 0.0f));
+      const float inside = fminf(fmaxf(fmaxf(q0, q1), q2), 0.0f);
+      v = __fadd_rn(outside, inside);
+    } else {  // capsule along local z
+      const float L = s.prm[1];
+      const float cz = fminf(fmaxf(y2, -L), L);
+      v = __fsub_rn(len3(y0, y1, __fsub_rn(y2, cz)), s.prm[0]);
+    }
+    phi = fminf(phi, v);
+  }
+  return phi;
+}
+
+__device__ __forceinline__ void zero_fill(float* __restrict__ p, int count) {
+  // p is 4-byte aligned; vectorise the 16-byte aligned body
+  const int head = min(count, (int)(((16u - (uint32_t)((uintptr_t)p & 15u)) & 15u) >> 2));
+  if ((int)threadIdx.x < head) p[threadIdx.x] = 0.0f;
+  float4* body = reinterpret_cast<float4*>(p + head);
+  const int nvec = (count - head) >> 2;
+  for (int v = threadIdx.x; v < nvec; v += blockDim.x) body[v] = make_float4(0.f, 0.f, 0.f, 0.f);
+  const int tail0 = head + (nvec << 2);
+  if (tail0 + (int)threadIdx.x < count) p[tail0 + threadIdx.x] = 0.0f;
+}
+
+template <bool kIndenters>
+__global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int write_uhat) {
+  extern __shared__ uint8_t smem_raw[];
+  SInd* sind = reinterpret_cast<SInd*>(smem_raw);
+  __shared__ int s_slot;
+
+  const int e = blockIdx.x / m.n_patches;
+  const int p = blockIdx.x - e * m.n_patches;
+  const PatchInfo pi = m.patch[p];
+  const int64_t row0 = (int64_t)e * m.n_nodes + pi.off;
+  float* delta = m.delta + row0;
+
+  bool any = false;
+  bool evaluated = true;
+  if constexpr (kIndenters) {
+    for (int k = threadIdx.x; k < m.max_ind; k += blockDim.x) {
+      const etac_indenter in = io.ind[(int64_t)e * m.max_ind + k];
+      SInd s;
+      s.type = in.type;
+      s.prm[0] = in.param[0], s.prm[1] = in.param[1], s.prm[2] = in.param[2];
+      s.t[0] = in.pose[0], s.t[1] = in.pose[1], s.t[2] = in.pose[2];
+      quat_to_rot(in.pose + 3, s.R);
+      sind[k] = s;
+    }
+    float Rp[9], tp[3];
+    const bool posed = io.patch_pose != nullptr;
+    if (posed) {
+      const float* pp = io.patch_pose + ((int64_t)e * m.n_patches + p) * 7;
+      float q[4] = {pp[3], pp[4], pp[5], pp[6]};
+      tp[0] = pp[0], tp[1] = pp[1], tp[2] = pp[2];
+      quat_to_rot(q, Rp);
+    }
+    __syncthreads();
+    auto to_world = [&](float x, float y, float z, float& X0, float& X1, float& X2) {
+      if (posed) {
+        X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(Rp[0], x), __fmul_rn(Rp[1], y)), __fmul_rn(Rp[2], z)), tp[0]);
+        X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(Rp[3], x), __fmul_rn(Rp[4], y)), __fmul_rn(Rp[5], z)), tp[1]);
+        X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(Rp[6], x), __fmul_rn(Rp[7], y)), __fmul_rn(Rp[8], z)), tp[2]);
+      } else {
+        X0 = x, X1 = y, X2 = z;
+      }
+    };
+    // conservative bounding-sphere cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
+    float C0, C1, C2;
+    to_world(pi.bc[0], pi.bc[1], pi.bc[2], C0, C1, C2);
+    const float phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
+    evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
+    if (evaluated) {
+      for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
+        const float4 pos = m.pos4[pi.off + i];
+        float X0, X1, X2;
+        to_world(pos.x, pos.y, pos.z, X0, X1, X2);
+        const float phi = union_sdf(sind, m.max_ind, X0, X1, X2);
+        const float d = phi < 0.0f ? -phi : 0.0f;
+        delta[i] = d;
+        any |= d > 0.0f;
+      }
+    }
+  } else {
+    for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
+      const float d = fmaxf(io.pen_in[row0 + i], 0.0f);
+      delta[i] = d;
+      any |= d > 0.0f;
+    }
+  }
+  any = __syncthreads_or(any);
+
+  if (!any) {
+    if (threadIdx.x == 0) m.flags[(int64_t)e * m.n_patches + p] = 0;
+    zero_fill(io.out + row0 * 3, pi.n * 3);
+    if (io.analytic_out) zero_fill(io.analytic_out + row0 * 3, pi.n * 3);
+    if (io.pen_out) zero_fill(io.pen_out + row0, pi.n);
+    return;
+  }
+  if (threadIdx.x == 0) {
+    m.flags[(int64_t)e * m.n_patches + p] = 1;
+    const int slot = atomicAdd(&m.count[p], 1);
+    m.envlist[(int64_t)p * m.max_envs + slot] = e;
+    s_slot = slot;
+  }
+  __syncthreads();
+  const int slot = s_slot;
+  const int words = (m.n_nodes + 31) >> 5;
+  for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
+    const float d = delta[i];  // written by this same thread above
+    if (io.pen_out) io.pen_out[row0 + i] = d;
+    if (io.mask_out && d > 0.0f) {
+      const int g = pi.off + i;
+      atomicOr(&io.mask_out[(int64_t)e * words + (g >> 5)], 1u << (g & 31));
+    }
+    if (write_uhat) {
+      const float4 n = m.nrm4[pi.off + i];
+      __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.off + i;
+      u[0] = __float2bfloat16_rn(-d * n.x);
+      u[m.ldu] = __float2bfloat16_rn(-d * n.y);
+      u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * n.z);
+    }
+  }
+}
+
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, bool write_uhat, cudaStream_t s) {
+  const unsigned grid = (unsigned)io.n_envs * (unsigned)m.n_patches;
+  if (io.input_mode == ETAC_IN_INDENTERS) {
+    const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
+    sdf_penetration_kernel<true><<<grid, 256, smem, s>>>(m, io, write_uhat ? 1 : 0);
+  } else {
+    sdf_penetration_kernel<false><<<grid, 256, 0, s>>>(m, io, write_uhat ? 1 : 0);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace etac

@@ -1,0 +1,79 @@
+"""Shared helpers of the GPU parity tests: run a workload through the C ABI (via the thin
+binding) and through the CPU oracle on the same seeded inputs, and compare element by element.
+
+Tolerances (BASELINE.json north_star, written out in tests/test_parity_gpu.py):
+  masks bit-exact; fp32 path max|u_gpu-u_ref| <= 1e-4*max|u_ref|; bf16 path <= 2e-2*max|u_ref|."""
+import numpy as np
+
+from oracle import etac_oracle as O
+from paper_2604_20295_b200 import etac as T
+
+TOL = {"fp32": 1e-4, "bf16": 2e-2}
+
+
+def run_gpu(wl, *, precision=None, path=T.ETAC_PATH_AUTO, resid=True, active_mode=T.ETAC_ACTIVE_PASSTHROUGH,
+            penetration=None, max_envs=None, n_envs=None, steps=1):
+    import torch
+    n_envs = wl.n_envs if n_envs is None else n_envs
+    eng = T.Etac(wl, precision=precision, resid=resid, active_mode=active_mode, debug_outputs=True,
+                 max_envs=max_envs or max(n_envs, 1))
+    try:
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+        if penetration is not None:
+            dev = eng.upload(penetration=penetration)
+        else:
+            dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        # poison the outputs: every element must be overwritten by the step
+        eng.out.fill_(float("nan")), eng.analytic.fill_(float("nan")), eng.pen_out.fill_(float("nan"))
+        for _ in range(steps):
+            eng.step(n_envs, dev)
+        torch.cuda.synchronize()
+        res = {"U": eng.out[:n_envs].cpu().numpy(), "analytic": eng.analytic[:n_envs].cpu().numpy(),
+               "delta": eng.pen_out[:n_envs].cpu().numpy(), "mask": eng.mask_bool(n_envs),
+               "pairs": T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_CONTACT_PAIRS),
+               "path": T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_PATH),
+               "launches": T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_LAUNCHES)}
+    finally:
+        eng.close()
+    return res
+
+
+def run_oracle(wl, *, resid=True, active_mode="passthrough", penetration=None, envs=None):
+    m = O.model_from_workload(wl, resid_arch="pernode" if resid else "none", active_mode=active_mode)
+    if penetration is not None:
+        return O.step(m, penetration=penetration, envs=envs)
+    return O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose, envs=envs)
+
+
+def compare(gpu, ref, tol, envs=None, resid_tol=None, label=""):
+    """gpu: dict from run_gpu (all envs); ref: oracle dict for `envs` (default all)."""
+    sel = slice(None) if envs is None else np.asarray(list(envs))
+    U, A, D, M = gpu["U"][sel], gpu["analytic"][sel], gpu["delta"][sel], gpu["mask"][sel]
+    assert np.isfinite(U).all() and np.isfinite(A).all() and np.isfinite(D).all(), f"{label}: unwritten output"
+    # decisions: bit-exact (taken in fp32 on both sides)
+    assert np.array_equal(M, ref["mask"]), f"{label}: mask differs at {np.argwhere(M != ref['mask'])[:5]}"
+    assert np.array_equal(D, ref["delta32"]), f"{label}: delta not bit-exact vs the fp32 twin"
+    scale_d = max(1.0, float(np.abs(ref["delta"]).max()))
+    assert np.abs(D - ref["delta"]).max() <= 1e-5 * scale_d
+    umax = float(np.abs(ref["U"]).max())
+    amax = float(np.abs(ref["analytic"]).max())
+    err_u = float(np.abs(U - ref["U"]).max())
+    err_a = float(np.abs(A - ref["analytic"]).max())
+    stats = {"umax": umax, "err_u": err_u, "err_a": err_a, "rel_u": err_u / max(umax, 1e-30),
+             "rel_a": err_a / max(amax, 1e-30)}
+    assert err_u <= tol * umax, f"{label}: U err {err_u:.3e} > {tol}*{umax:.3e}"
+    assert err_a <= tol * amax, f"{label}: analytic err {err_a:.3e} > {tol}*{amax:.3e}"
+    # non-contacting (env, patch) pairs are exactly zero
+    zero_rows = ~np.repeat(ref["contact"], np.diff(ref["patch_offset"]), axis=1) if "patch_offset" in ref else None
+    if zero_rows is not None:
+        assert np.all(U[zero_rows] == 0.0) and np.all(A[zero_rows] == 0.0)
+    if resid_tol is not None:
+        # the residual alone: r = U - u_lin on passive nodes of contacting patches
+        passive = ~ref["mask"] & (np.abs(ref["U"]).sum(-1) > 0)
+        r_ref = (ref["U"] - ref["analytic"])[passive]
+        r_gpu = (U - A)[passive]
+        rmax = float(np.abs(r_ref).max())
+        err_r = float(np.abs(r_gpu - r_ref).max())
+        stats["rel_r"] = err_r / max(rmax, 1e-30)
+        assert err_r <= resid_tol * rmax, f"{label}: residual err {err_r:.3e} > {resid_tol}*{rmax:.3e}"
+    return stats

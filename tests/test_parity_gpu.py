@@ -1,0 +1,164 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerances are BASELINE.json's:
+   masks / contact decisions : bit-exact
+   fp32 path                 : max|u_gpu - u_ref| <= 1e-4 * max|u_ref|
+   bf16 tensor-core path     : max|u_gpu - u_ref| <= 2e-2 * max|u_ref|   (fp32 accumulation)
+The residual MLP is ~1 % of max|u| with the N(0, 0.02) weights of the configs, so it is also
+checked on its own (r = U - u_lin on passive nodes) and with larger weights."""
+import numpy as np
+import pytest
+
+from paper_2604_20295_b200 import etac as T
+from paper_2604_20295_b200 import workloads as W
+from parity_util import TOL, compare, run_gpu, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _report(name, st):
+    print(f"[parity] {name}: " + " ".join(f"{k}={v:.3e}" for k, v in st.items()))
+
+
+@pytest.mark.parametrize("seed,n_envs", [(0, 1), (1, 5)])
+def test_config1_fp32(seed, n_envs):
+    wl = W.config1(seed, n_envs)
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    assert gpu["path"] == T.ETAC_PATH_SPARSE and gpu["launches"] == 2
+    _report("cfg1", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="cfg1"))
+
+
+def test_config2_fp32():
+    wl = W.config2(0, 64)
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    _report("cfg2", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="cfg2"))
+    assert gpu["pairs"] == int(ref["contact"].sum())
+
+
+@pytest.mark.parametrize("n_envs", [40, 97])
+def test_config3_bf16_dense_small(n_envs):
+    wl = W.config3(1, n_envs)      # 40: one ragged env tile per patch; 97: several tiles + tail
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    assert gpu["path"] == T.ETAC_PATH_DENSE
+    _report(f"cfg3 E={n_envs}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="cfg3"))
+    assert gpu["pairs"] == int(ref["contact"].sum())
+
+
+def test_config3_sparse_path_matches_fp32_tolerance():
+    wl = W.config3(2, 24)
+    gpu = run_gpu(wl, path=T.ETAC_PATH_SPARSE)
+    _report("cfg3 sparse", compare(gpu, run_oracle(wl), TOL["fp32"], resid_tol=1e-4, label="cfg3-sparse"))
+
+
+def test_config4_bf16_dense_small():
+    wl = W.config4(0, 12)          # N = 8192: 64 node blocks x 128 k-blocks per env tile
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    _report("cfg4", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="cfg4"))
+
+
+def test_large_weights_bf16_mlp():
+    """With N(0, 0.3) weights the residual is comparable to u_lin: a wrong MLP cannot hide."""
+    wl = W.config3(3, 33)
+    wl.weights = W.make_weights(3, seed=9, std=0.3)
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    st = compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="large-w")
+    _report("large weights", st)
+    r = np.abs(ref["U"] - ref["analytic"])[~ref["mask"]].max()
+    assert r > 0.05 * st["umax"]
+
+
+def test_large_weights_fp32_mlp():
+    wl = W.config2(4, 16)
+    wl.weights = W.make_weights(2, seed=9, std=0.3)
+    _report("large weights fp32", compare(run_gpu(wl), run_oracle(wl), TOL["fp32"], resid_tol=1e-4, label="large-w32"))
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_penetration_input_mode(precision):
+    wl = W.config2(5, 9)
+    rng = np.random.default_rng(3)
+    pen = np.where(rng.random((9, 1024)) < 0.03, rng.uniform(-0.5, 1.5, (9, 1024)), 0).astype(np.float32)
+    pen[4] = 0.0                                   # one env without contact
+    pen[5] = -1.0                                  # negatives clamp to zero (R19)
+    gpu = run_gpu(wl, precision=precision, penetration=pen)
+    ref = run_oracle(wl, penetration=pen)
+    _report(f"penetration {precision}", compare(gpu, ref, TOL[precision], label="pen"))
+    assert np.all(gpu["U"][4] == 0) and np.all(gpu["U"][5] == 0)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_modes_no_residual_and_propagate(precision):
+    wl = W.config3(6, 17)
+    gpu = run_gpu(wl, precision=precision, resid=False)
+    ref = run_oracle(wl, resid=False)
+    compare(gpu, ref, TOL[precision], label="no-resid")
+    passive = ~ref["mask"]
+    assert np.array_equal(gpu["U"][passive], gpu["analytic"][passive])     # "linear decay only" (L137)
+    gpu = run_gpu(wl, precision=precision, active_mode=T.ETAC_ACTIVE_PROPAGATE)
+    compare(gpu, run_oracle(wl, active_mode="propagate"), TOL[precision], label="propagate")
+
+
+def test_zero_contact_and_edge_sizes():
+    wl = W.config2(7, 6)
+    wl.indenters["pose"][..., 0:3] += 500.0
+    for precision in ("fp32", "bf16"):
+        gpu = run_gpu(wl, precision=precision)
+        assert not gpu["mask"].any() and np.all(gpu["U"] == 0) and np.all(gpu["analytic"] == 0)
+        assert gpu["pairs"] == 0
+    wl = W.config2(7, 6)
+    # n_envs < max_envs, and the step is stateless: running twice gives the same answer
+    ref = run_oracle(wl, envs=range(3))
+    for precision in ("fp32", "bf16"):
+        gpu = run_gpu(wl, precision=precision, max_envs=64, n_envs=3, steps=2)
+        compare(gpu, ref, TOL[precision], label="partial")
+
+
+def test_ragged_patches_bf16_and_fp32():
+    """Patch sizes that are not multiples of the 128-node tile or the 64-wide k-block, patch
+    offsets not multiples of 32 (mask words shared by two patches), per-patch alpha."""
+    parts = [W.flat_pad(10, 20, 1.0), W.fib_cap(6.0, 72), W.half_cylinder(5.0, 12.0, 9, 15)]   # 200, 72, 135
+    mesh = W.assemble(parts)
+    rng = np.random.default_rng(12)
+    E = 37
+    pen = np.where(rng.random((E, mesh.n_nodes)) < 0.05, rng.uniform(0.05, 1.0, (E, mesh.n_nodes)), 0).astype(np.float32)
+    pen[3, :200] = 0
+    pen[9] = 0
+    wl = W.Workload("ragged", mesh, np.float32([0.5, 0.8, 0.3]), W.make_weights(7, 1, std=0.1), E, 0,
+                    np.zeros((E, 0), dtype=W.INDENTER_DTYPE), None, "bf16")
+    ref = run_oracle(wl, penetration=pen)
+    _report("ragged bf16", compare(run_gpu(wl, penetration=pen), ref, TOL["bf16"], resid_tol=5e-2, label="ragged"))
+    _report("ragged fp32", compare(run_gpu(wl, precision="fp32", penetration=pen), ref, TOL["fp32"], resid_tol=1e-4,
+                                   label="ragged32"))
+
+
+def test_patches_derived_from_adjacency_on_device():
+    wl = W.config3(8, 4)
+    import torch
+    ctx = T.etac_create(wl.mesh.pos, wl.mesh.normal, wl.alpha, adj_rowptr=wl.mesh.adj_rowptr,
+                        adj_col=wl.mesh.adj_col, weights=wl.weights, max_envs=4, precision=T.ETAC_PREC_BF16)
+    assert T.etac_get_info(ctx, T.ETAC_INFO_N_PATCHES) == 16 and T.etac_get_info(ctx, T.ETAC_INFO_N_NODES) == 5696
+    out = torch.empty((5, 5696, 3), device="cuda")
+    with pytest.raises(T.EtacError) as ei:
+        T.etac_step(ctx, None, T.make_step_args(5, out, indenters=out))
+    assert ei.value.status == T.ETAC_ERR_CAPACITY
+    with pytest.raises(T.EtacError) as ei:
+        T.etac_step(ctx, None, T.make_step_args(4, None, indenters=out))
+    assert ei.value.status == T.ETAC_ERR_INVALID_ARG
+    T.etac_step(ctx, None, T.make_step_args(0, out, indenters=out))       # no-op
+    T.etac_destroy(ctx)
+
+
+def test_full_size_config3_sampled():
+    """BASELINE.json's bench configuration (4096 envs, N = 5696, bf16) in the launch
+    configuration bench.py times; the oracle checks a sample of environments one by one."""
+    wl = W.config3(0, 4096)
+    gpu = run_gpu(wl)
+    envs = list(range(0, 4096, 171)) + [4095]
+    ref = run_oracle(wl, envs=envs)
+    _report("cfg3 full", compare(gpu, ref, TOL["bf16"], envs=envs, resid_tol=5e-2, label="cfg3-full"))
+    # properties that hold at any size: contact pairs = chosen patches; un-chosen patches are 0
+    assert gpu["pairs"] == int(wl.meta["chosen"].sum())
+    rows = ~np.repeat(wl.meta["chosen"], np.diff(wl.mesh.patch_offset), axis=1)
+    assert np.all(gpu["U"][rows] == 0.0)
+    act = gpu["mask"]
+    nrm = wl.mesh.normal[None]
+    np.testing.assert_array_equal(gpu["U"][act], (-gpu["delta"][..., None] * nrm)[act])   # P7 on every env
