@@ -384,7 +384,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   }
 
   // ---- per-step workspace
-  const size_t urows = (size_t)((d->max_envs + 31) / 32) * 96;
+  const size_t urows = (size_t)((d->max_envs + kDenseTE - 1) / kDenseTE) * kDenseBN;
   CK(dev_alloc(c, &m.delta, (size_t)d->max_envs * N, true), "alloc delta");
   CK(dev_alloc(c, &m.count, (size_t)P, true), "alloc count");
   CK(dev_alloc(c, &m.envlist, (size_t)P * d->max_envs, true), "alloc envlist");
@@ -393,7 +393,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
     CK(dev_alloc(c, &m.uhat_t, urows * m.ldu, true), "alloc uhat");
     std::string why;
     if (!make_tmap(&c->tmA, m.k16, (uint64_t)N, (uint64_t)m.kw, (uint64_t)m.kw, 128, &why) ||
-        !make_tmap(&c->tmB, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 96, &why))
+        !make_tmap(&c->tmB, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, kDenseBN, &why))
       return bail(ETAC_ERR_CUDA, why);
     c->have_tm = true;
     CK(dense_bf16_configure(), "cudaFuncSetAttribute(dense_bf16_kernel)");

@@ -33,6 +33,10 @@ struct ChunkInfo {
 };
 constexpr int kGatherChunk = 128;
 
+// tensor-core path tiling: environments per work item and the GEMM N extent (3 columns per env)
+constexpr int kDenseTE = 16;
+constexpr int kDenseBN = kDenseTE * 3;
+
 // Shared-memory image of the MLP weights for the tensor-core path (bf16, UMMA K-major
 // SWIZZLE_NONE core-matrix layout; see k_dense_bf16.cu).
 constexpr int kW1ImgBytes = 64 * 16 * 2;   // N=64,  K=16   (9 inputs + bias column)

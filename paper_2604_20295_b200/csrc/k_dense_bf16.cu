@@ -12,24 +12,29 @@
 // The grid is persistent (2 CTAs per SM); every CTA walks items blockIdx.x, +gridDim.x, ...
 // 6 warps: 0 = TMA producer, 1 = MMA issuer (+ TMEM alloc), 2..5 = epilogue (thread = node).
 //
-// TMEM columns (fp32 lanes = nodes):   [0,96)  u_lin accumulator, column 3*env+c
-//                                      [96,160)  D: pre-activations of the current MLP layer
-//                                      [160,200) A2/A3: bf16 hidden activations (+ ones column)
-//                                      [200,208) A1: bf16 [u_lin(3), p(3), n(3), 1, 0..]
+// The epilogue keeps TWO environments in flight per warp (slots 0/1, each with its own TMEM
+// D/A regions and mbarrier pair): while the tensor core runs layer L+1 of slot 0 the warp
+// evaluates the SiLUs of layer L of slot 1, which hides the MMA round trip.
+//
+// TMEM columns (fp32 lanes = nodes):   [0,48)   u_lin accumulator, column 3*env+c
+//   slot s at 48 + 104*s:              [+0,+64)   D: pre-activations of the current MLP layer
+//                                      [+64,+104) A: bf16 layer input; layer 1 uses words 0..7
+//                                                 [u_lin(3), p(3), n(3), 1, 0..], layers 2/3 use
+//                                                 64 activations + a ones column (word 32)
 #include "etac_internal.h"
 #include "sm100_prims.cuh"
 
 namespace etac {
 
-constexpr int BM = 128, BK = 64, TE = 32, BN = TE * 3, STAGES = 3;
+constexpr int BM = 128, BK = 64, TE = kDenseTE, BN = kDenseBN, STAGES = 4;
 constexpr int A_STAGE = BM * BK * 2, B_STAGE = BN * BK * 2;
 constexpr int kDenseThreads = 192;
 constexpr uint32_t kTmemCols = 256;
-constexpr uint32_t COL_ACC = 0, COL_D = 96, COL_A2 = 160, COL_A1 = 200;
+constexpr uint32_t COL_ACC = 0, COL_SLOT0 = 48, SLOT_STRIDE = 104, OFF_A = 64;
 
 struct __align__(8) DenseBars {
   uint64_t full[STAGES], empty[STAGES];
-  uint64_t acc_full, acc_empty, a_ready, d_ready;
+  uint64_t acc_full, acc_empty, a_ready[2], d_ready[2];
   uint32_t tmem_base;
   uint32_t pad;
 };
@@ -75,8 +80,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     for (int s = 0; s < STAGES; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
     mbar_init(&bars->acc_full, 1);
     mbar_init(&bars->acc_empty, 4);
-    mbar_init(&bars->a_ready, 4);
-    mbar_init(&bars->d_ready, 1);
+    for (int s = 0; s < 2; ++s) mbar_init(&bars->a_ready[s], 4), mbar_init(&bars->d_ready[s], 1);
     fence_barrier_init();
     int acc = 0;
     prefix[0] = 0;
@@ -148,23 +152,26 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         }
         tc_commit(&bars->acc_full);
         if constexpr (kResid) {
-          for (int el = 0; el < it.cnt; ++el) {
-            mbar_wait(&bars->a_ready, a_ph), a_ph ^= 1;
-            tc_fence_after();
-            mma_ts(tmem + COL_D, tmem + COL_A1, dW1, idesc_h, 0);
-            tc_commit(&bars->d_ready);
-            mbar_wait(&bars->a_ready, a_ph), a_ph ^= 1;
-            tc_fence_after();
+          for (int base = 0; base < it.cnt; base += 2) {
+            const int ns = min(2, it.cnt - base);
+#pragma unroll 1
+            for (int layer = 0; layer < 3; ++layer) {
+              for (int sl = 0; sl < ns; ++sl) {
+                const uint32_t tD = tmem + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
+                mbar_wait(&bars->a_ready[sl], (a_ph >> sl) & 1), a_ph ^= 1u << sl;
+                tc_fence_after();
+                if (layer == 0) {
+                  mma_ts(tD, tA, dW1, idesc_h, 0);
+                } else if (layer == 1) {
 #pragma unroll
-            for (int k = 0; k < 5; ++k)
-              mma_ts(tmem + COL_D, tmem + COL_A2 + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
-            tc_commit(&bars->d_ready);
-            mbar_wait(&bars->a_ready, a_ph), a_ph ^= 1;
-            tc_fence_after();
+                  for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
+                } else {
 #pragma unroll
-            for (int k = 0; k < 5; ++k)
-              mma_ts(tmem + COL_D, tmem + COL_A2 + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
-            tc_commit(&bars->d_ready);
+                  for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
+                }
+                tc_commit(&bars->d_ready[sl]);
+              }
+            }
           }
         }
       }
@@ -175,9 +182,10 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     const uint32_t trow = tmem + (lane_base << 16);
     const int row = lane_base + lane;
     if constexpr (kResid) {
-      // bias ("ones") column of A2/A3: bf16 element 64 = 1.0, elements 65..79 = 0; written once
+      // bias ("ones") column of the layer-2/3 input: bf16 element 64 = 1.0, 65..79 = 0; written once
       const uint32_t ones[8] = {0x00003F80u, 0, 0, 0, 0, 0, 0, 0};
-      tmem_st8(trow + COL_A2 + 32, ones);
+      tmem_st8(trow + COL_SLOT0 + OFF_A + 32, ones);
+      tmem_st8(trow + COL_SLOT0 + SLOT_STRIDE + OFF_A + 32, ones);
       tc_wait_st();
     }
     int pcur = 0;
@@ -201,59 +209,74 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       const int* envs = m.envlist + (int64_t)it.p * m.max_envs + it.tile * TE;
       mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
       tc_fence_after();
-      for (int el = 0; el < it.cnt; ++el) {
-        const int env = envs[el];
-        const int64_t node = (int64_t)env * m.n_nodes + g;
-        const float dl = valid ? m.delta[node] : 0.0f;
-        uint32_t ur[4];
-        tmem_ld4(trow + COL_ACC + 3 * el, ur);
-        tc_wait_ld();
-        const float ux = __uint_as_float(ur[0]), uy = __uint_as_float(ur[1]), uz = __uint_as_float(ur[2]);
-        float ox = ux, oy = uy, oz = uz;
-        if constexpr (kResid) {
-          a1[0] = pack_bf16(ux, uy);
-          a1[1] = pack_bf16(uz, px);
-          tmem_st8(trow + COL_A1, a1);
-          tc_wait_st();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&bars->a_ready);
-#pragma unroll 1
-          for (int layer = 0; layer < 2; ++layer) {
-            mbar_wait(&bars->d_ready, d_ph), d_ph ^= 1;
-            tc_fence_after();
-            uint32_t h[32], packed[16];
-#pragma unroll
-            for (int half = 0; half < 2; ++half) {
-              tmem_ld32(trow + COL_D + 32 * half, h);
-              tc_wait_ld();
-#pragma unroll
-              for (int k = 0; k < 16; ++k) {
-                // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
-                const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
-                packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
-              }
-              tmem_st16(trow + COL_A2 + 16 * half, packed);
-            }
+      for (int base = 0; base < it.cnt; base += 2) {
+        const int ns = min(2, it.cnt - base);
+        float u[2][3], dl[2];
+        int64_t node[2];
+        for (int sl = 0; sl < ns; ++sl) {
+          const int env = envs[base + sl];
+          node[sl] = (int64_t)env * m.n_nodes + g;
+          dl[sl] = valid ? m.delta[node[sl]] : 0.0f;
+          uint32_t ur[4];
+          tmem_ld4(trow + COL_ACC + 3 * (base + sl), ur);
+          tc_wait_ld();
+          u[sl][0] = __uint_as_float(ur[0]), u[sl][1] = __uint_as_float(ur[1]), u[sl][2] = __uint_as_float(ur[2]);
+          if constexpr (kResid) {
+            a1[0] = pack_bf16(u[sl][0], u[sl][1]);
+            a1[1] = pack_bf16(u[sl][2], px);
+            tmem_st8(trow + COL_SLOT0 + SLOT_STRIDE * sl + OFF_A, a1);
             tc_wait_st();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars->a_ready);
+            if (lane == 0) mbar_arrive(&bars->a_ready[sl]);
           }
-          mbar_wait(&bars->d_ready, d_ph), d_ph ^= 1;
-          tc_fence_after();
-          uint32_t rr[4];
-          tmem_ld4(trow + COL_D, rr);
-          tc_wait_ld();
-          ox += __uint_as_float(rr[0]), oy += __uint_as_float(rr[1]), oz += __uint_as_float(rr[2]);
         }
-        if (valid) {
-          if (dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH) ox = -dl * nrm.x, oy = -dl * nrm.y, oz = -dl * nrm.z;
-          float* o = io.out + node * 3;
-          o[0] = ox, o[1] = oy, o[2] = oz;
-          if (io.analytic_out) {
-            float* a = io.analytic_out + node * 3;
-            a[0] = ux, a[1] = uy, a[2] = uz;
+        if constexpr (kResid) {
+#pragma unroll 1
+          for (int layer = 0; layer < 2; ++layer) {
+            for (int sl = 0; sl < ns; ++sl) {
+              const uint32_t tD = trow + COL_SLOT0 + SLOT_STRIDE * sl;
+              mbar_wait(&bars->d_ready[sl], (d_ph >> sl) & 1), d_ph ^= 1u << sl;
+              tc_fence_after();
+              uint32_t h[32], packed[16];
+#pragma unroll
+              for (int half = 0; half < 2; ++half) {
+                tmem_ld32(tD + 32 * half, h);
+                tc_wait_ld();
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                  // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
+                  const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
+                  packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
+                }
+                tmem_st16(tD + OFF_A + 16 * half, packed);
+              }
+              tc_wait_st();
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive(&bars->a_ready[sl]);
+            }
+          }
+        }
+        for (int sl = 0; sl < ns; ++sl) {
+          float ox = u[sl][0], oy = u[sl][1], oz = u[sl][2];
+          if constexpr (kResid) {
+            mbar_wait(&bars->d_ready[sl], (d_ph >> sl) & 1), d_ph ^= 1u << sl;
+            tc_fence_after();
+            uint32_t rr[4];
+            tmem_ld4(trow + COL_SLOT0 + SLOT_STRIDE * sl, rr);
+            tc_wait_ld();
+            ox += __uint_as_float(rr[0]), oy += __uint_as_float(rr[1]), oz += __uint_as_float(rr[2]);
+          }
+          if (valid) {
+            if (dl[sl] > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH)
+              ox = -dl[sl] * nrm.x, oy = -dl[sl] * nrm.y, oz = -dl[sl] * nrm.z;
+            float* o = io.out + node[sl] * 3;
+            o[0] = ox, o[1] = oy, o[2] = oz;
+            if (io.analytic_out) {
+              float* a = io.analytic_out + node[sl] * 3;
+              a[0] = u[sl][0], a[1] = u[sl][1], a[2] = u[sl][2];
+            }
           }
         }
       }

@@ -1,6 +1,6 @@
 // S1: contact detection and penalty displacement of the active nodes.
 //
-// One CTA per (environment, patch).  Every node of the patch is transformed into the world
+// One CTA per environment.  Every node of a non-culled patch is transformed into the world
 // frame of the indenters, the union SDF phi = min_k sdf_k is evaluated, active <=> phi < 0,
 // delta = -phi on active nodes.  The arithmetic of phi is single-rounded fp32 in a fixed order
 // (no FMA contraction -> __fmul_rn/__fadd_rn/__fsub_rn/__fsqrt_rn) so that the
@@ -84,20 +84,26 @@ __device__ __forceinline__ void zero_fill(float* __restrict__ p, int count) {
   if (tail0 + (int)threadIdx.x < count) p[tail0 + threadIdx.x] = 0.0f;
 }
 
+constexpr int kPoseChunk = 32;
+struct SPose {
+  float R[9];
+  float t[3];
+  int evaluated;  // 0 = culled by the bounding-sphere test
+};
+
+// One CTA per environment.  Patch poses and the conservative bounding-sphere cull are computed
+// once per (env, patch) by one thread each (not per node), then the CTA walks the patches:
+// culled / contact-free patches are zero-filled, the others are evaluated node by node.
 template <bool kIndenters>
 __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int write_uhat) {
   extern __shared__ uint8_t smem_raw[];
   SInd* sind = reinterpret_cast<SInd*>(smem_raw);
+  __shared__ SPose s_pose[kPoseChunk];
   __shared__ int s_slot;
 
-  const int e = blockIdx.x / m.n_patches;
-  const int p = blockIdx.x - e * m.n_patches;
-  const PatchInfo pi = m.patch[p];
-  const int64_t row0 = (int64_t)e * m.n_nodes + pi.off;
-  float* delta = m.delta + row0;
-
-  bool any = false;
-  bool evaluated = true;
+  const int e = blockIdx.x;
+  const int words = (m.n_nodes + 31) >> 5;
+  const bool posed = io.patch_pose != nullptr;
   if constexpr (kIndenters) {
     for (int k = threadIdx.x; k < m.max_ind; k += blockDim.x) {
       const etac_indenter in = io.ind[(int64_t)e * m.max_ind + k];
@@ -108,84 +114,100 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       quat_to_rot(in.pose + 3, s.R);
       sind[k] = s;
     }
-    float Rp[9], tp[3];
-    const bool posed = io.patch_pose != nullptr;
-    if (posed) {
-      const float* pp = io.patch_pose + ((int64_t)e * m.n_patches + p) * 7;
-      float q[4] = {pp[3], pp[4], pp[5], pp[6]};
-      tp[0] = pp[0], tp[1] = pp[1], tp[2] = pp[2];
-      quat_to_rot(q, Rp);
+  }
+  for (int p0 = 0; p0 < m.n_patches; p0 += kPoseChunk) {
+    __syncthreads();  // sind ready / previous chunk's s_pose no longer read
+    if constexpr (kIndenters) {
+      const int p = p0 + threadIdx.x;
+      if (threadIdx.x < kPoseChunk && p < m.n_patches) {
+        const PatchInfo pi = m.patch[p];
+        SPose sp;
+        float C0 = pi.bc[0], C1 = pi.bc[1], C2 = pi.bc[2];
+        if (posed) {
+          const float* pp = io.patch_pose + ((int64_t)e * m.n_patches + p) * 7;
+          const float q[4] = {pp[3], pp[4], pp[5], pp[6]};
+          sp.t[0] = pp[0], sp.t[1] = pp[1], sp.t[2] = pp[2];
+          quat_to_rot(q, sp.R);
+          const float x = C0, y = C1, z = C2;
+          C0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[0], x), __fmul_rn(sp.R[1], y)), __fmul_rn(sp.R[2], z)), sp.t[0]);
+          C1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], x), __fmul_rn(sp.R[4], y)), __fmul_rn(sp.R[5], z)), sp.t[1]);
+          C2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], x), __fmul_rn(sp.R[7], y)), __fmul_rn(sp.R[8], z)), sp.t[2]);
+        }
+        // conservative bounding-sphere cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
+        const float phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
+        sp.evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
+        s_pose[threadIdx.x] = sp;
+      }
+      __syncthreads();
     }
-    __syncthreads();
-    auto to_world = [&](float x, float y, float z, float& X0, float& X1, float& X2) {
-      if (posed) {
-        X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(Rp[0], x), __fmul_rn(Rp[1], y)), __fmul_rn(Rp[2], z)), tp[0]);
-        X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(Rp[3], x), __fmul_rn(Rp[4], y)), __fmul_rn(Rp[5], z)), tp[1]);
-        X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(Rp[6], x), __fmul_rn(Rp[7], y)), __fmul_rn(Rp[8], z)), tp[2]);
+    const int pend = min(m.n_patches, p0 + kPoseChunk);
+    for (int p = p0; p < pend; ++p) {
+      const PatchInfo pi = m.patch[p];
+      const int64_t row0 = (int64_t)e * m.n_nodes + pi.off;
+      float* delta = m.delta + row0;
+      bool any = false;
+      if constexpr (kIndenters) {
+        const SPose& sp = s_pose[p - p0];
+        if (sp.evaluated) {
+          for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
+            const float4 pos = m.pos4[pi.off + i];
+            float X0 = pos.x, X1 = pos.y, X2 = pos.z;
+            if (posed) {
+              X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[0], pos.x), __fmul_rn(sp.R[1], pos.y)), __fmul_rn(sp.R[2], pos.z)), sp.t[0]);
+              X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
+              X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
+            }
+            const float phi = union_sdf(sind, m.max_ind, X0, X1, X2);
+            const float d = phi < 0.0f ? -phi : 0.0f;
+            delta[i] = d;
+            any |= d > 0.0f;
+          }
+        }
       } else {
-        X0 = x, X1 = y, X2 = z;
+        for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
+          const float d = fmaxf(io.pen_in[row0 + i], 0.0f);
+          delta[i] = d;
+          any |= d > 0.0f;
+        }
       }
-    };
-    // conservative bounding-sphere cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
-    float C0, C1, C2;
-    to_world(pi.bc[0], pi.bc[1], pi.bc[2], C0, C1, C2);
-    const float phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
-    evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
-    if (evaluated) {
+      any = __syncthreads_or(any);
+      if (!any) {
+        if (threadIdx.x == 0) m.flags[(int64_t)e * m.n_patches + p] = 0;
+        zero_fill(io.out + row0 * 3, pi.n * 3);
+        if (io.analytic_out) zero_fill(io.analytic_out + row0 * 3, pi.n * 3);
+        if (io.pen_out) zero_fill(io.pen_out + row0, pi.n);
+        continue;
+      }
+      if (threadIdx.x == 0) {
+        m.flags[(int64_t)e * m.n_patches + p] = 1;
+        const int slot = atomicAdd(&m.count[p], 1);
+        m.envlist[(int64_t)p * m.max_envs + slot] = e;
+        s_slot = slot;
+      }
+      __syncthreads();
+      const int slot = s_slot;
       for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
-        const float4 pos = m.pos4[pi.off + i];
-        float X0, X1, X2;
-        to_world(pos.x, pos.y, pos.z, X0, X1, X2);
-        const float phi = union_sdf(sind, m.max_ind, X0, X1, X2);
-        const float d = phi < 0.0f ? -phi : 0.0f;
-        delta[i] = d;
-        any |= d > 0.0f;
+        const float d = delta[i];  // written by this same thread above
+        if (io.pen_out) io.pen_out[row0 + i] = d;
+        if (io.mask_out && d > 0.0f) {
+          const int g = pi.off + i;
+          atomicOr(&io.mask_out[(int64_t)e * words + (g >> 5)], 1u << (g & 31));
+        }
+        if (write_uhat) {
+          const float4 n = m.nrm4[pi.off + i];
+          __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.off + i;
+          u[0] = __float2bfloat16_rn(-d * n.x);
+          u[m.ldu] = __float2bfloat16_rn(-d * n.y);
+          u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * n.z);
+        }
       }
-    }
-  } else {
-    for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
-      const float d = fmaxf(io.pen_in[row0 + i], 0.0f);
-      delta[i] = d;
-      any |= d > 0.0f;
-    }
-  }
-  any = __syncthreads_or(any);
-
-  if (!any) {
-    if (threadIdx.x == 0) m.flags[(int64_t)e * m.n_patches + p] = 0;
-    zero_fill(io.out + row0 * 3, pi.n * 3);
-    if (io.analytic_out) zero_fill(io.analytic_out + row0 * 3, pi.n * 3);
-    if (io.pen_out) zero_fill(io.pen_out + row0, pi.n);
-    return;
-  }
-  if (threadIdx.x == 0) {
-    m.flags[(int64_t)e * m.n_patches + p] = 1;
-    const int slot = atomicAdd(&m.count[p], 1);
-    m.envlist[(int64_t)p * m.max_envs + slot] = e;
-    s_slot = slot;
-  }
-  __syncthreads();
-  const int slot = s_slot;
-  const int words = (m.n_nodes + 31) >> 5;
-  for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
-    const float d = delta[i];  // written by this same thread above
-    if (io.pen_out) io.pen_out[row0 + i] = d;
-    if (io.mask_out && d > 0.0f) {
-      const int g = pi.off + i;
-      atomicOr(&io.mask_out[(int64_t)e * words + (g >> 5)], 1u << (g & 31));
-    }
-    if (write_uhat) {
-      const float4 n = m.nrm4[pi.off + i];
-      __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.off + i;
-      u[0] = __float2bfloat16_rn(-d * n.x);
-      u[m.ldu] = __float2bfloat16_rn(-d * n.y);
-      u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * n.z);
+      __syncthreads();  // s_slot is rewritten by the next contacting patch
     }
   }
 }
 
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, bool write_uhat, cudaStream_t s) {
-  const unsigned grid = (unsigned)io.n_envs * (unsigned)m.n_patches;
+  const unsigned grid = (unsigned)io.n_envs;
   if (io.input_mode == ETAC_IN_INDENTERS) {
     const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
     sdf_penetration_kernel<true><<<grid, 256, smem, s>>>(m, io, write_uhat ? 1 : 0);
