@@ -32,8 +32,8 @@ UNIT = "env-steps/s"
 N_INPUT_SETS = 4
 MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728
 # dram__bytes_read.sum + dram__bytes_write.sum of one dense_bf16_kernel launch, from the
-# `ncu --set full` capture summarised in profiles/ (None until captured).
-NCU_TRAFFIC_BYTES = None
+# `ncu --set full` capture summarised in profiles/r01_dense_ncu_full.md (79.3 MB read + 47.9 MB write).
+NCU_TRAFFIC_BYTES = 127.26e6
 
 
 def load_peaks():

@@ -18,6 +18,7 @@ HEADERS = ["etac_internal.h", "sm100_prims.cuh", os.path.join("..", "..", "inclu
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr", "-cudart", "static"]
+FLAGS += os.environ.get("ETAC_NVCC_EXTRA", "").split()      # experiments only (e.g. -DETAC_ABLATE=1)
 
 
 def _stale() -> bool:

@@ -10,11 +10,13 @@
 //
 // Work item = (patch p, block of 128 nodes, tile of TE contacting environments of that patch).
 // The grid is persistent (2 CTAs per SM); every CTA walks items blockIdx.x, +gridDim.x, ...
-// 6 warps: 0 = TMA producer, 1 = MMA issuer (+ TMEM alloc), 2..5 = epilogue (thread = node).
+// 12 warps: 0 = TMA producer, 1 = propagation-GEMM MMA issuer (+ TMEM alloc), 2..5 and 6..9 = two
+// epilogue warpgroups (thread = node), 10/11 = MLP MMA issuers of slot 0/1.
 //
-// The epilogue keeps TWO environments in flight per warp (slots 0/1, each with its own TMEM
-// D/A regions and mbarrier pair): while the tensor core runs layer L+1 of slot 0 the warp
-// evaluates the SiLUs of layer L of slot 1, which hides the MMA round trip.
+// TWO environments are in flight per CTA (slots 0/1, each with its own TMEM D/A regions, mbarrier
+// pair and epilogue warpgroup): while the tensor core runs a layer of slot 0, warpgroup 1
+// evaluates the SiLUs of slot 1 and vice versa; with 2 CTAs per SM every SM sub-partition has 4
+// epilogue warps to hide the MMA round trips and TMEM load latency behind the MUFU pipe.
 //
 // TMEM columns (fp32 lanes = nodes):   [0,48)   u_lin accumulator, column 3*env+c
 //   slot s at 48 + 104*s:              [+0,+64)   D: pre-activations of the current MLP layer
@@ -28,7 +30,7 @@ namespace etac {
 
 constexpr int BM = 128, BK = 64, TE = kDenseTE, BN = kDenseBN, STAGES = 4;
 constexpr int A_STAGE = BM * BK * 2, B_STAGE = BN * BK * 2;
-constexpr int kDenseThreads = 192;
+constexpr int kDenseThreads = 384;
 constexpr uint32_t kTmemCols = 256;
 constexpr uint32_t COL_ACC = 0, COL_SLOT0 = 48, SLOT_STRIDE = 104, OFF_A = 64;
 
@@ -43,6 +45,23 @@ __host__ __device__ constexpr size_t dense_smem_bytes(int n_patches) {
   return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE + B_STAGE) + kWImgBytes + sizeof(DenseBars) +
          (size_t)(n_patches + 1) * 4 + 16;
 }
+
+#ifdef ETAC_TRACE
+// timing experiment only: per-warp event log in shared memory (no global traffic while running)
+__device__ unsigned long long g_trace[12 * 400];
+__device__ unsigned int g_trace_n;
+__shared__ unsigned long long s_trace[12 * 400];
+__shared__ unsigned int s_trace_n[12];
+#define TR(tag)                                                                       \
+  do {                                                                                \
+    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {                                 \
+      unsigned int w_ = threadIdx.x >> 5, i_ = s_trace_n[w_];                         \
+      if (i_ < 400) s_trace[w_ * 400 + i_] = ((unsigned long long)(tag) << 48) | ((unsigned long long)w_ << 40) | (clock64() & 0xFFFFFFFFFFull), s_trace_n[w_] = i_ + 1; \
+    }                                                                                 \
+  } while (0)
+#else
+#define TR(tag)
+#endif
 
 struct Item {
   int p, mb, tile, cnt;
@@ -75,11 +94,14 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   int* prefix = reinterpret_cast<int*>(bars + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#ifdef ETAC_TRACE
+  if (threadIdx.x < 12) s_trace_n[threadIdx.x] = 0;
+#endif
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
     mbar_init(&bars->acc_full, 1);
-    mbar_init(&bars->acc_empty, 4);
+    mbar_init(&bars->acc_empty, 8);
     for (int s = 0; s < 2; ++s) mbar_init(&bars->a_ready[s], 4), mbar_init(&bars->d_ready[s], 1);
     fence_barrier_init();
     int acc = 0;
@@ -106,7 +128,8 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
 
   if (warp == 0) {
     // ------------------------------------------------------------------ TMA producer
-    if (lane == 0) {
+    // (the whole warp runs the loop so that every operand stays warp-uniform; one elected lane issues)
+    {
       int pcur = 0, stage = 0;
       uint32_t ph = 0;
       Item it;
@@ -115,16 +138,20 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         const int nkb = (pi.n + BK - 1) / BK;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(&bars->empty[stage], ph ^ 1);
-          mbar_arrive_expect_tx(&bars->full[stage], A_STAGE + B_STAGE);
-          tma_load_2d(sA + stage * A_STAGE, &tmA, &bars->full[stage], kb * BK, pi.off + it.mb * BM);
-          tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], pi.off + kb * BK, it.tile * BN);
+          if (elect_one()) {
+            mbar_arrive_expect_tx(&bars->full[stage], A_STAGE + B_STAGE);
+            tma_load_2d(sA + stage * A_STAGE, &tmA, &bars->full[stage], kb * BK, pi.off + it.mb * BM);
+            tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], pi.off + kb * BK, it.tile * BN);
+          }
+          __syncwarp();
           if (++stage == STAGES) stage = 0, ph ^= 1;
         }
       }
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
+    // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are issued by one elected lane.
+    {
       constexpr uint32_t idesc_prop = make_idesc_bf16(BM, BN);
       constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
       constexpr uint32_t idesc_o = make_idesc_bf16(BM, 16);
@@ -144,48 +171,86 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
           tc_fence_after();
           const uint64_t dA = make_desc(smem_u32(sA + stage * A_STAGE), 16, 1024, kLayoutSw128);
           const uint64_t dB = make_desc(smem_u32(sB + stage * B_STAGE), 16, 1024, kLayoutSw128);
+          if (elect_one()) {
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k)
-            mma_ss(tmem + COL_ACC, dA + 2 * k, dB + 2 * k, idesc_prop, (kb | k) != 0);
-          tc_commit(&bars->empty[stage]);
+            for (int k = 0; k < BK / 16; ++k)
+              mma_ss(tmem + COL_ACC, dA + 2 * k, dB + 2 * k, idesc_prop, (kb | k) != 0);
+            tc_commit(&bars->empty[stage]);
+            if (kb == nkb - 1) tc_commit(&bars->acc_full);
+          }
+          __syncwarp();
           if (++stage == STAGES) stage = 0, ph ^= 1;
         }
-        tc_commit(&bars->acc_full);
-        if constexpr (kResid) {
-          for (int base = 0; base < it.cnt; base += 2) {
-            const int ns = min(2, it.cnt - base);
+      }
+    }
+  } else if (warp >= 10) {
+    // ------------------------------------------------------------------ MLP MMA issuer of slot (warp - 10)
+    // One dedicated issuer warp per slot: a tcgen05.mma round trip is ~450 cycles during which the
+    // issuing warp makes no progress, so the two slots must not share an issuer.
+    if constexpr (kResid) {
+      const int sl = warp - 10;
+      constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
+      constexpr uint32_t idesc_o = make_idesc_bf16(BM, 16);
+      const uint64_t dW1 = make_desc(smem_u32(sW), 1024, 128, kLayoutNone);
+      const uint64_t dW2 = make_desc(smem_u32(sW + kW1ImgBytes), 1024, 128, kLayoutNone);
+      const uint64_t dW3 = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 256, 128, kLayoutNone);
+      const uint32_t tD = tmem + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
+      uint64_t* a_ready = &bars->a_ready[sl];
+      uint64_t* d_ready = &bars->d_ready[sl];
+      int pcur = 0;
+      uint32_t a_ph = 0;
+      Item it;
+      for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+        for (int el = sl; el < it.cnt; el += 2) {
 #pragma unroll 1
-            for (int layer = 0; layer < 3; ++layer) {
-              for (int sl = 0; sl < ns; ++sl) {
-                const uint32_t tD = tmem + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
-                mbar_wait(&bars->a_ready[sl], (a_ph >> sl) & 1), a_ph ^= 1u << sl;
-                tc_fence_after();
-                if (layer == 0) {
-                  mma_ts(tD, tA, dW1, idesc_h, 0);
-                } else if (layer == 1) {
+          for (int layer = 0; layer < 3; ++layer) {
+            mbar_wait(a_ready, a_ph), a_ph ^= 1;
+            TR(100 + sl * 10 + layer);
+            tc_fence_after();
+            if (elect_one()) {
+#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 4
+              if (layer == 99) {
+#else
+              if (layer == 0) {
+#endif
+                mma_ts(tD, tA, dW1, idesc_h, 0);
+#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 4
+              } else if (layer == 98) {
+#else
+              } else if (layer == 1) {
+#endif
 #pragma unroll
-                  for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
-                } else {
+                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
+#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 4
+              } else if (layer == 97) {
+#else
+              } else {
+#endif
 #pragma unroll
-                  for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
-                }
-                tc_commit(&bars->d_ready[sl]);
+                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
               }
+              tc_commit(d_ready);
             }
+            __syncwarp();
+            TR(200 + sl * 10 + layer);
           }
         }
       }
     }
   } else {
     // ------------------------------------------------------------------ epilogue (thread = node)
+    // Two warpgroups; warpgroup s owns TMEM slot s and takes the environments el = s, s+2, ...
+    const int sl = (warp - 2) >> 2;
     const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
     const uint32_t trow = tmem + (lane_base << 16);
+    const uint32_t tD = trow + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
     const int row = lane_base + lane;
+    uint64_t* a_ready = &bars->a_ready[sl];
+    uint64_t* d_ready = &bars->d_ready[sl];
     if constexpr (kResid) {
       // bias ("ones") column of the layer-2/3 input: bf16 element 64 = 1.0, 65..79 = 0; written once
       const uint32_t ones[8] = {0x00003F80u, 0, 0, 0, 0, 0, 0, 0};
-      tmem_st8(trow + COL_SLOT0 + OFF_A + 32, ones);
-      tmem_st8(trow + COL_SLOT0 + SLOT_STRIDE + OFF_A + 32, ones);
+      tmem_st8(tA + 32, ones);
       tc_wait_st();
     }
     int pcur = 0;
@@ -206,77 +271,86 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         a1[3] = pack_bf16(nrm.x, nrm.y);
         a1[4] = pack_bf16(nrm.z, 1.0f);
       }
-      const int* envs = m.envlist + (int64_t)it.p * m.max_envs + it.tile * TE;
+      // lane l prefetches the id of the item's l-th environment (broadcast by shuffle below)
+      const int my_env = lane < it.cnt ? m.envlist[(int64_t)it.p * m.max_envs + it.tile * TE + lane] : 0;
       mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
       tc_fence_after();
-      for (int base = 0; base < it.cnt; base += 2) {
-        const int ns = min(2, it.cnt - base);
-        float u[2][3], dl[2];
-        int64_t node[2];
-        for (int sl = 0; sl < ns; ++sl) {
-          const int env = envs[base + sl];
-          node[sl] = (int64_t)env * m.n_nodes + g;
-          dl[sl] = valid ? m.delta[node[sl]] : 0.0f;
-          uint32_t ur[4];
-          tmem_ld4(trow + COL_ACC + 3 * (base + sl), ur);
-          tc_wait_ld();
-          u[sl][0] = __uint_as_float(ur[0]), u[sl][1] = __uint_as_float(ur[1]), u[sl][2] = __uint_as_float(ur[2]);
-          if constexpr (kResid) {
-            a1[0] = pack_bf16(u[sl][0], u[sl][1]);
-            a1[1] = pack_bf16(u[sl][2], px);
-            tmem_st8(trow + COL_SLOT0 + SLOT_STRIDE * sl + OFF_A, a1);
+#ifdef ETAC_SKEW
+      // De-phase the two warpgroups: both leave the accumulator barrier together and would then
+      // alternate "both on the MUFU pipe" / "both waiting for the tensor core" in lock-step.
+      if (sl == 1) {
+        const long long t0 = clock64();
+        while (clock64() - t0 < ETAC_SKEW) {
+        }
+      }
+#endif
+      for (int el = sl; el < it.cnt; el += 2) {
+#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 3
+        const int env = it.tile * TE + el;
+        const int64_t node = (int64_t)env * m.n_nodes + g;
+        const float dl = 0.0f;
+#else
+        const int env = __shfl_sync(0xffffffffu, my_env, el);
+        const int64_t node = (int64_t)env * m.n_nodes + g;
+        const float dl = valid ? m.delta[node] : 0.0f;
+#endif
+        uint32_t ur[4];
+        tmem_ld4(trow + COL_ACC + 3 * el, ur);
+        tc_wait_ld();
+        const float ux = __uint_as_float(ur[0]), uy = __uint_as_float(ur[1]), uz = __uint_as_float(ur[2]);
+        float ox = ux, oy = uy, oz = uz;
+        if constexpr (kResid) {
+          a1[0] = pack_bf16(ux, uy);
+          a1[1] = pack_bf16(uz, px);
+          tmem_st8(tA, a1);
+          tc_wait_st();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(a_ready);
+          TR(1);
+#pragma unroll 1
+          for (int layer = 0; layer < 2; ++layer) {
+            mbar_wait(d_ready, d_ph), d_ph ^= 1;
+            TR(2 + layer * 2);
+            tc_fence_after();
+            uint32_t h[32], packed[16];
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+              tmem_ld32(tD + 32 * half, h);
+              tc_wait_ld();
+#pragma unroll
+              for (int k = 0; k < 16; ++k) {
+                // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
+                const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
+                packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
+              }
+              tmem_st16(tA + 16 * half, packed);
+            }
             tc_wait_st();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars->a_ready[sl]);
+            if (lane == 0) mbar_arrive(a_ready);
+            TR(3 + layer * 2);
           }
+          mbar_wait(d_ready, d_ph), d_ph ^= 1;
+          TR(6);
+          tc_fence_after();
+          uint32_t rr[4];
+          tmem_ld4(tD, rr);
+          tc_wait_ld();
+          ox += __uint_as_float(rr[0]), oy += __uint_as_float(rr[1]), oz += __uint_as_float(rr[2]);
         }
-        if constexpr (kResid) {
-#pragma unroll 1
-          for (int layer = 0; layer < 2; ++layer) {
-            for (int sl = 0; sl < ns; ++sl) {
-              const uint32_t tD = trow + COL_SLOT0 + SLOT_STRIDE * sl;
-              mbar_wait(&bars->d_ready[sl], (d_ph >> sl) & 1), d_ph ^= 1u << sl;
-              tc_fence_after();
-              uint32_t h[32], packed[16];
-#pragma unroll
-              for (int half = 0; half < 2; ++half) {
-                tmem_ld32(tD + 32 * half, h);
-                tc_wait_ld();
-#pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                  // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
-                  const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
-                  packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
-                }
-                tmem_st16(tD + OFF_A + 16 * half, packed);
-              }
-              tc_wait_st();
-              tc_fence_before();
-              __syncwarp();
-              if (lane == 0) mbar_arrive(&bars->a_ready[sl]);
-            }
-          }
-        }
-        for (int sl = 0; sl < ns; ++sl) {
-          float ox = u[sl][0], oy = u[sl][1], oz = u[sl][2];
-          if constexpr (kResid) {
-            mbar_wait(&bars->d_ready[sl], (d_ph >> sl) & 1), d_ph ^= 1u << sl;
-            tc_fence_after();
-            uint32_t rr[4];
-            tmem_ld4(trow + COL_SLOT0 + SLOT_STRIDE * sl, rr);
-            tc_wait_ld();
-            ox += __uint_as_float(rr[0]), oy += __uint_as_float(rr[1]), oz += __uint_as_float(rr[2]);
-          }
-          if (valid) {
-            if (dl[sl] > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH)
-              ox = -dl[sl] * nrm.x, oy = -dl[sl] * nrm.y, oz = -dl[sl] * nrm.z;
-            float* o = io.out + node[sl] * 3;
-            o[0] = ox, o[1] = oy, o[2] = oz;
-            if (io.analytic_out) {
-              float* a = io.analytic_out + node[sl] * 3;
-              a[0] = u[sl][0], a[1] = u[sl][1], a[2] = u[sl][2];
-            }
+#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 2
+        if (valid && ox == 123.456f) {
+#else
+        if (valid) {
+#endif
+          if (dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH) ox = -dl * nrm.x, oy = -dl * nrm.y, oz = -dl * nrm.z;
+          float* o = io.out + node * 3;
+          o[0] = ox, o[1] = oy, o[2] = oz;
+          if (io.analytic_out) {
+            float* a = io.analytic_out + node * 3;
+            a[0] = ux, a[1] = uy, a[2] = uz;
           }
         }
       }
@@ -287,6 +361,12 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   }
   tc_fence_before();
   __syncthreads();
+#ifdef ETAC_TRACE
+  if (blockIdx.x == 0) {
+    for (int k = threadIdx.x; k < 4800; k += blockDim.x) g_trace[k] = (k % 400) < s_trace_n[k / 400] ? s_trace[k] : 0ull;
+    g_trace_n = 4800;
+  }
+#endif
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc<kTmemCols>(tmem);
@@ -312,3 +392,10 @@ cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtenso
 }
 
 }  // namespace etac
+
+#ifdef ETAC_TRACE
+extern "C" void etac_debug_trace(unsigned long long* out, unsigned int* n) {
+  cudaMemcpyFromSymbol(out, etac::g_trace, sizeof(unsigned long long) * 4800);
+  cudaMemcpyFromSymbol(n, etac::g_trace_n, sizeof(unsigned int));
+}
+#endif

@@ -91,17 +91,24 @@ struct SPose {
   int evaluated;  // 0 = culled by the bounding-sphere test
 };
 
-// One CTA per environment.  Patch poses and the conservative bounding-sphere cull are computed
-// once per (env, patch) by one thread each (not per node), then the CTA walks the patches:
-// culled / contact-free patches are zero-filled, the others are evaluated node by node.
+// One CTA per environment.  Patches are handled kPoseChunk at a time in four block-wide phases
+// (3 barriers per chunk, none per patch):
+//   B  one thread per patch: pose -> rotation, conservative bounding-sphere cull
+//   C  all threads: nodes of the non-culled patches -> phi, delta (workspace), per-patch "any"
+//   D  one thread per patch: contact flag, slot in the patch's compact environment list
+//   E  all threads: contact-free patches -> zero-fill of the output rows; contacting patches ->
+//      U^ operand rows (bf16), optional delta / mask outputs
 template <bool kIndenters>
 __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int write_uhat) {
   extern __shared__ uint8_t smem_raw[];
   SInd* sind = reinterpret_cast<SInd*>(smem_raw);
   __shared__ SPose s_pose[kPoseChunk];
-  __shared__ int s_slot;
+  __shared__ int s_any[kPoseChunk];
+  __shared__ int s_slot[kPoseChunk];
+  __shared__ int s_off[kPoseChunk + 1];  // node offsets of the chunk's patches (+ end)
 
   const int e = blockIdx.x;
+  const int lane = threadIdx.x & 31;
   const int words = (m.n_nodes + 31) >> 5;
   const bool posed = io.patch_pose != nullptr;
   if constexpr (kIndenters) {
@@ -116,10 +123,18 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
     }
   }
   for (int p0 = 0; p0 < m.n_patches; p0 += kPoseChunk) {
-    __syncthreads();  // sind ready / previous chunk's s_pose no longer read
-    if constexpr (kIndenters) {
+    const int np = min(kPoseChunk, m.n_patches - p0);
+    __syncthreads();  // sind ready / previous chunk fully consumed
+    // ---- phase B
+    if ((int)threadIdx.x < np) {
       const int p = p0 + threadIdx.x;
-      if (threadIdx.x < kPoseChunk && p < m.n_patches) {
+      s_any[threadIdx.x] = 0;
+      {
+        const PatchInfo pi0 = m.patch[p];
+        s_off[threadIdx.x] = pi0.off;
+        if ((int)threadIdx.x == np - 1) s_off[np] = pi0.off + pi0.n;
+      }
+      if constexpr (kIndenters) {
         const PatchInfo pi = m.patch[p];
         SPose sp;
         float C0 = pi.bc[0], C1 = pi.bc[1], C2 = pi.bc[2];
@@ -133,35 +148,37 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           C1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], x), __fmul_rn(sp.R[4], y)), __fmul_rn(sp.R[5], z)), sp.t[1]);
           C2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], x), __fmul_rn(sp.R[7], y)), __fmul_rn(sp.R[8], z)), sp.t[2]);
         }
-        // conservative bounding-sphere cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
+        // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
         const float phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
         sp.evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
         s_pose[threadIdx.x] = sp;
       }
-      __syncthreads();
     }
-    const int pend = min(m.n_patches, p0 + kPoseChunk);
-    for (int p = p0; p < pend; ++p) {
-      const PatchInfo pi = m.patch[p];
+    __syncthreads();
+    // ---- phase C
+    for (int q = 0; q < np; ++q) {
+      if constexpr (kIndenters) {
+        if (!s_pose[q].evaluated) continue;
+      }
+      PatchInfo pi;
+      pi.off = s_off[q], pi.n = s_off[q + 1] - s_off[q];
       const int64_t row0 = (int64_t)e * m.n_nodes + pi.off;
       float* delta = m.delta + row0;
       bool any = false;
       if constexpr (kIndenters) {
-        const SPose& sp = s_pose[p - p0];
-        if (sp.evaluated) {
-          for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
-            const float4 pos = m.pos4[pi.off + i];
-            float X0 = pos.x, X1 = pos.y, X2 = pos.z;
-            if (posed) {
-              X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[0], pos.x), __fmul_rn(sp.R[1], pos.y)), __fmul_rn(sp.R[2], pos.z)), sp.t[0]);
-              X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
-              X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
-            }
-            const float phi = union_sdf(sind, m.max_ind, X0, X1, X2);
-            const float d = phi < 0.0f ? -phi : 0.0f;
-            delta[i] = d;
-            any |= d > 0.0f;
+        const SPose& sp = s_pose[q];
+        for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
+          const float4 pos = m.pos4[pi.off + i];
+          float X0 = pos.x, X1 = pos.y, X2 = pos.z;
+          if (posed) {
+            X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[0], pos.x), __fmul_rn(sp.R[1], pos.y)), __fmul_rn(sp.R[2], pos.z)), sp.t[0]);
+            X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
+            X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
           }
+          const float phi = union_sdf(sind, m.max_ind, X0, X1, X2);
+          const float d = phi < 0.0f ? -phi : 0.0f;
+          delta[i] = d;
+          any |= d > 0.0f;
         }
       } else {
         for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
@@ -170,38 +187,57 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           any |= d > 0.0f;
         }
       }
-      any = __syncthreads_or(any);
-      if (!any) {
-        if (threadIdx.x == 0) m.flags[(int64_t)e * m.n_patches + p] = 0;
-        zero_fill(io.out + row0 * 3, pi.n * 3);
-        if (io.analytic_out) zero_fill(io.analytic_out + row0 * 3, pi.n * 3);
-        if (io.pen_out) zero_fill(io.pen_out + row0, pi.n);
-        continue;
-      }
-      if (threadIdx.x == 0) {
-        m.flags[(int64_t)e * m.n_patches + p] = 1;
+      if (__any_sync(0xffffffffu, any) && lane == 0) atomicOr(&s_any[q], 1);
+    }
+    __syncthreads();
+    // ---- phase D
+    if ((int)threadIdx.x < np) {
+      const int p = p0 + threadIdx.x;
+      const int hit = s_any[threadIdx.x];
+      m.flags[(int64_t)e * m.n_patches + p] = (uint8_t)hit;
+      if (hit) {
         const int slot = atomicAdd(&m.count[p], 1);
         m.envlist[(int64_t)p * m.max_envs + slot] = e;
-        s_slot = slot;
+        s_slot[threadIdx.x] = slot;
       }
-      __syncthreads();
-      const int slot = s_slot;
-      for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
-        const float d = delta[i];  // written by this same thread above
+    }
+    __syncthreads();
+    // ---- phase E (runs of consecutive contact-free patches are zero-filled in one go)
+    int run0 = -1;
+    for (int q = 0; q <= np; ++q) {
+      const bool hit = q < np && s_any[q];
+      if (q < np && !hit) {
+        if (run0 < 0) run0 = q;
+        continue;
+      }
+      if (run0 >= 0) {
+        const int64_t r0 = (int64_t)e * m.n_nodes + s_off[run0];
+        const int cnt = s_off[q] - s_off[run0];
+        zero_fill(io.out + r0 * 3, cnt * 3);
+        if (io.analytic_out) zero_fill(io.analytic_out + r0 * 3, cnt * 3);
+        if (io.pen_out) zero_fill(io.pen_out + r0, cnt);
+        run0 = -1;
+      }
+      if (q == np) break;
+      const int off = s_off[q], n = s_off[q + 1] - off;
+      const int64_t row0 = (int64_t)e * m.n_nodes + off;
+      const int slot = s_slot[q];
+      const float* delta = m.delta + row0;
+      for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const float d = delta[i];
         if (io.pen_out) io.pen_out[row0 + i] = d;
         if (io.mask_out && d > 0.0f) {
-          const int g = pi.off + i;
+          const int g = off + i;
           atomicOr(&io.mask_out[(int64_t)e * words + (g >> 5)], 1u << (g & 31));
         }
         if (write_uhat) {
-          const float4 n = m.nrm4[pi.off + i];
-          __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.off + i;
-          u[0] = __float2bfloat16_rn(-d * n.x);
-          u[m.ldu] = __float2bfloat16_rn(-d * n.y);
-          u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * n.z);
+          const float4 nn = m.nrm4[off + i];
+          __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off + i;
+          u[0] = __float2bfloat16_rn(-d * nn.x);
+          u[m.ldu] = __float2bfloat16_rn(-d * nn.y);
+          u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * nn.z);
         }
       }
-      __syncthreads();  // s_slot is rewritten by the next contacting patch
     }
   }
 }
