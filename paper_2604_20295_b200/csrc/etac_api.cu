@@ -333,6 +333,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
       chunks.push_back(ChunkInfo{p, pi.off + n0, std::min(kGatherChunk, pi.n - n0)});
   }
   m.n_chunks = (int)chunks.size();
+  m.max_patch_nodes = max_np;
   m.kw = (max_np + 63) / 64 * 64;
   m.ldu = (N + 63) / 64 * 64;
   CK(dev_upload(c, &m.patch, hp.data(), P), "upload patches");

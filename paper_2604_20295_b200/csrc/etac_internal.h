@@ -46,6 +46,7 @@ constexpr int kWImgBytes = kW1ImgBytes + kW2ImgBytes + kW3ImgBytes;
 
 struct DevModel {
   int32_t n_nodes, n_patches, n_chunks;
+  int32_t max_patch_nodes;    // largest patch
   int32_t kw;                 // padded column count of k16 (multiple of 64)
   int32_t ldu;                // row pitch (elements) of uhat_t
   int32_t max_envs, max_ind;

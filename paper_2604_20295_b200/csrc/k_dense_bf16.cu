@@ -6,7 +6,8 @@
 //   S3  residual MLP 9 -> 64 -> 64 -> 3 (SiLU) on the accumulator tile, each layer one small
 //       tcgen05.mma whose A operand is written to TMEM by the epilogue warps and whose B operand
 //       (the weights, biases folded in as an extra K column) stays in shared memory,
-//   S4  mask M_p + combine (Eq. 2) and the store of U[e][i][0..2].
+//   S4  mask M_p + combine (Eq. 2) and the store of U[e][i][0..2]; the rows of
+//       contact-free (env, patch) pairs are zero-filled by the MLP issuer warps (R8).
 //
 // Work item = (patch p, block of 128 nodes, tile of TE contacting environments of that patch).
 // The grid is persistent (2 CTAs per SM); every CTA walks items blockIdx.x, +gridDim.x, ...
@@ -65,6 +66,51 @@ __shared__ unsigned int s_trace_n[12];
 
 struct Item {
   int p, mb, tile, cnt;
+};
+
+// streaming zero-fill of `count` floats at a 4-byte aligned address by one warp
+__device__ __forceinline__ void warp_zero_fill(float* __restrict__ p, int count, int lane) {
+  const int head = min(count, (int)(((16u - (uint32_t)((uintptr_t)p & 15u)) & 15u) >> 2));
+  if (lane < head) __stcs(p + lane, 0.0f);
+  float4* body = reinterpret_cast<float4*>(p + head);
+  const int nvec = (count - head) >> 2;
+  for (int v = lane; v < nvec; v += 32) __stcs(body + v, make_float4(0.f, 0.f, 0.f, 0.f));
+  const int tail0 = head + (nvec << 2);
+  if (tail0 + lane < count) __stcs(p + tail0 + lane, 0.0f);
+}
+
+// Rows of (env, patch) pairs without contact are exactly 0 (R8).  Resumable sweep for one
+// warp: warp `part` of `nparts` takes the pairs 32*part.., 32*(part+nparts)..; lane l looks at pair
+// base+l; one step() zero-fills one run of consecutive contact-free patches of one environment,
+// so that the sweep can be spread over the kernel instead of saturating HBM at its start.
+struct ZeroFill {
+  int64_t base, total, stride;
+  uint32_t mask;
+  __device__ __forceinline__ void init(const DevModel& m, const StepIO& io, int part, int nparts) {
+    total = (int64_t)io.n_envs * m.n_patches, base = (int64_t)part * 32 - (int64_t)nparts * 32;
+    stride = (int64_t)nparts * 32, mask = 0;
+  }
+  __device__ __forceinline__ bool step(const DevModel& m, const StepIO& io, int lane) {  // false: nothing left
+    while (mask == 0) {
+      base += stride;
+      if (base >= total) return false;
+      const int64_t idx = base + lane;
+      mask = __ballot_sync(0xffffffffu, idx < total && m.flags[idx] == 0);
+    }
+    const int P = m.n_patches;
+    const int b = __ffs(mask) - 1;
+    const int64_t pair = base + b;
+    const int e = (int)(pair / P), p = (int)(pair - (int64_t)e * P);
+    int len = 1;
+    while (b + len < 32 && p + len < P && ((mask >> (b + len)) & 1u)) ++len;
+    mask &= ~(((len == 32) ? 0xffffffffu : ((1u << len) - 1u)) << b);
+    const int off = m.patch[p].off;
+    const int cnt = m.patch[p + len - 1].off + m.patch[p + len - 1].n - off;
+    const int64_t r0 = ((int64_t)e * m.n_nodes + off) * 3;
+    warp_zero_fill(io.out + r0, cnt * 3, lane);
+    if (io.analytic_out) warp_zero_fill(io.analytic_out + r0, cnt * 3, lane);
+    return true;
+  }
 };
 
 __device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, const DevModel& m, int w, int& pcur,
@@ -187,6 +233,10 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     // ------------------------------------------------------------------ MLP MMA issuer of slot (warp - 10)
     // One dedicated issuer warp per slot: a tcgen05.mma round trip is ~450 cycles during which the
     // issuing warp makes no progress, so the two slots must not share an issuer.
+    // Between requests the warp zero-fills its share of the output rows of contact-free (env, patch)
+    // pairs, one run per request, so that these stores trickle out next to the MUFU-bound work.
+    ZeroFill zf;
+    zf.init(m, io, blockIdx.x * 2 + (warp - 10), gridDim.x * 2);
     if constexpr (kResid) {
       const int sl = warp - 10;
       constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
@@ -233,9 +283,12 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
             }
             __syncwarp();
             TR(200 + sl * 10 + layer);
+            zf.step(m, io, lane);
           }
         }
       }
+    }
+    while (zf.step(m, io, lane)) {
     }
   } else {
     // ------------------------------------------------------------------ epilogue (thread = node)

@@ -9,8 +9,9 @@
 // Outputs: delta workspace [E x N] (only where the patch was evaluated), per-(env,patch) contact
 // flag, per-patch compact list of contacting environments (slot = position in that list), and,
 // for the tensor-core path, the GEMM B operand U^ = -delta * n as bf16 rows uhat_t[slot*3+c][j].
-// A patch with no active node gets its rows of the output zero-filled here (R8), so
-// the contraction kernels only ever touch contacting (env, patch) pairs.
+// A patch with no active node gets its rows of the output zero-filled (R8) -- here for
+// the gather path, by the idle warps of the fused kernel for the tensor-core path -- so the
+// contraction kernels only ever compute contacting (env, patch) pairs.
 #include "etac_internal.h"
 
 namespace etac {
@@ -42,35 +43,51 @@ __device__ __forceinline__ float len3(float a, float b, float c) {
   return __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(a, a), __fmul_rn(b, b)), __fmul_rn(c, c)));
 }
 
-// Union signed distance at world point X.
+// Signed distance of world point X to one indenter (+inf for an empty slot).
+__device__ __forceinline__ float sdf_one(const SInd& s, float X0, float X1, float X2) {
+  if (s.type == ETAC_IND_NONE) return __int_as_float(0x7f800000);
+  const float d0 = __fsub_rn(X0, s.t[0]), d1 = __fsub_rn(X1, s.t[1]), d2 = __fsub_rn(X2, s.t[2]);
+  // y = R^T d
+  const float y0 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[0], d0), __fmul_rn(s.R[3], d1)), __fmul_rn(s.R[6], d2));
+  const float y1 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[1], d0), __fmul_rn(s.R[4], d1)), __fmul_rn(s.R[7], d2));
+  const float y2 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[2], d0), __fmul_rn(s.R[5], d1)), __fmul_rn(s.R[8], d2));
+  if (s.type == ETAC_IND_SPHERE) return __fsub_rn(len3(y0, y1, y2), s.prm[0]);
+  if (s.type == ETAC_IND_BOX) {
+    const float q0 = __fsub_rn(fabsf(y0), s.prm[0]);
+    const float q1 = __fsub_rn(fabsf(y1), s.prm[1]);
+    const float q2 = __fsub_rn(fabsf(y2), s.prm[2]);
+    const float outside = len3(fmaxf(q0, 0.0f), fmaxf(q1, 0.0f), fmaxf(q2, 0.0f));
+    const float inside = fminf(fmaxf(fmaxf(q0, q1), q2), 0.0f);
+    return __fadd_rn(outside, inside);
+  }
+  // capsule along local z
+  const float L = s.prm[1];
+  const float cz = fminf(fmaxf(y2, -L), L);
+  return __fsub_rn(len3(y0, y1, __fsub_rn(y2, cz)), s.prm[0]);
+}
+
+// Union signed distance at world point X: min over the slots in slot order.
 __device__ __forceinline__ float union_sdf(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2) {
   float phi = __int_as_float(0x7f800000);
-  for (int k = 0; k < n_ind; ++k) {
-    const SInd& s = ind[k];
-    if (s.type == ETAC_IND_NONE) continue;
-    const float d0 = __fsub_rn(X0, s.t[0]), d1 = __fsub_rn(X1, s.t[1]), d2 = __fsub_rn(X2, s.t[2]);
-    // y = R^T d
-    const float y0 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[0], d0), __fmul_rn(s.R[3], d1)), __fmul_rn(s.R[6], d2));
-    const float y1 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[1], d0), __fmul_rn(s.R[4], d1)), __fmul_rn(s.R[7], d2));
-    const float y2 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[2], d0), __fmul_rn(s.R[5], d1)), __fmul_rn(s.R[8], d2));
-    float v;
-    if (s.type == ETAC_IND_SPHERE) {
-      v = __fsub_rn(len3(y0, y1, y2), s.prm[0]);
-    } else if (s.type == ETAC_IND_BOX) {
-      const float q0 = __fsub_rn(fabsf(y0), s.prm[0]);
-      const float q1 = __fsub_rn(fabsf(y1), s.prm[1]);
-      const float q2 = __fsub_rn(fabsf(y2), s.prm[2]);
-      const float outside = len3(fmaxf(q0, 0.0f), fmaxf(q1, 0.0f), fmaxf(q2, 0.0f));
-      const float inside = fminf(fmaxf(fmaxf(q0, q1), q2), 0.0f);
-      v = __fadd_rn(outside, inside);
-    } else {  // capsule along local z
-      const float L = s.prm[1];
-      const float cz = fminf(fmaxf(y2, -L), L);
-      v = __fsub_rn(len3(y0, y1, __fsub_rn(y2, cz)), s.prm[0]);
-    }
-    phi = fminf(phi, v);
-  }
+  for (int k = 0; k < n_ind; ++k) phi = fminf(phi, sdf_one(ind[k], X0, X1, X2));
   return phi;
+}
+
+__device__ __forceinline__ SInd load_indenter(const etac_indenter* __restrict__ p) {
+  SInd s;
+  s.type = p->type;
+  s.prm[0] = p->param[0], s.prm[1] = p->param[1], s.prm[2] = p->param[2];
+  s.t[0] = p->pose[0], s.t[1] = p->pose[1], s.t[2] = p->pose[2];
+  quat_to_rot(p->pose + 3, s.R);
+  return s;
+}
+
+// world position of mesh point x under patch pose (R, t): one fixed order of single-rounded operations
+__device__ __forceinline__ void to_world(const float* R, const float* t, float x, float y, float z, float& X0, float& X1,
+                                         float& X2) {
+  X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(R[0], x), __fmul_rn(R[1], y)), __fmul_rn(R[2], z)), t[0]);
+  X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(R[3], x), __fmul_rn(R[4], y)), __fmul_rn(R[5], z)), t[1]);
+  X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(R[6], x), __fmul_rn(R[7], y)), __fmul_rn(R[8], z)), t[2]);
 }
 
 __device__ __forceinline__ void zero_fill(float* __restrict__ p, int count) {
@@ -213,8 +230,10 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       if (run0 >= 0) {
         const int64_t r0 = (int64_t)e * m.n_nodes + s_off[run0];
         const int cnt = s_off[q] - s_off[run0];
-        zero_fill(io.out + r0 * 3, cnt * 3);
-        if (io.analytic_out) zero_fill(io.analytic_out + r0 * 3, cnt * 3);
+        if (!write_uhat) {  // tensor-core path: the fused kernel's idle warps zero-fill these rows
+          zero_fill(io.out + r0 * 3, cnt * 3);
+          if (io.analytic_out) zero_fill(io.analytic_out + r0 * 3, cnt * 3);
+        }
         if (io.pen_out) zero_fill(io.pen_out + r0, cnt);
         run0 = -1;
       }
@@ -242,8 +261,122 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// S1 for meshes of many small patches (dexterous hand): one WARP per (env, patch) pair.
+// All lanes build the patch rotation and do the conservative bounding-sphere cull against the
+// environment's indenters (warp-uniform, no divergence); a culled warp exits at once.  Otherwise
+// the warp evaluates the nodes -> phi, delta (workspace), warp vote -> contact flag; on contact
+// lane 0 takes a slot in the patch's compact environment list and the warp writes the U^ operand
+// rows.  No block barrier; the indenter lives in registers when there is one slot per environment.
+// Same single-rounded arithmetic in the same order as sdf_penetration_kernel.
+constexpr int kPairWarps = 2;
+
+template <bool kOne>
+__global__ void __launch_bounds__(kPairWarps * 32) sdf_pairs_kernel(DevModel m, StepIO io, int write_uhat) {
+  extern __shared__ uint8_t smem_raw[];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  SInd* sind = reinterpret_cast<SInd*>(smem_raw) + (size_t)wib * (kOne ? 0 : m.max_ind);  // per-warp staging (M > 1)
+  const int P = m.n_patches;
+  const int64_t pair = (int64_t)blockIdx.x * kPairWarps + wib;
+  if (pair >= (int64_t)io.n_envs * P) return;
+  const int e = (int)(pair / P), p = (int)(pair - (int64_t)e * P);
+  const bool posed = io.patch_pose != nullptr;
+  const PatchInfo pi = m.patch[p];
+  const int off = pi.off, n = pi.n;
+  const int64_t row0 = (int64_t)e * m.n_nodes + off;
+
+  float R[9] = {1.f, 0.f, 0.f, 0.f, 1.f, 0.f, 0.f, 0.f, 1.f}, t[3] = {0.f, 0.f, 0.f};
+  float C0 = pi.bc[0], C1 = pi.bc[1], C2 = pi.bc[2];
+  if (posed) {
+    const float* pp = io.patch_pose + pair * 7;
+    const float q[4] = {pp[3], pp[4], pp[5], pp[6]};
+    t[0] = pp[0], t[1] = pp[1], t[2] = pp[2];
+    quat_to_rot(q, R);
+    to_world(R, t, pi.bc[0], pi.bc[1], pi.bc[2], C0, C1, C2);
+  }
+  SInd one;
+  float phi_c;
+  if constexpr (kOne) {
+    one = load_indenter(io.ind + e);
+    phi_c = fminf(__int_as_float(0x7f800000), sdf_one(one, C0, C1, C2));
+  } else {
+    for (int k = lane; k < m.max_ind; k += 32) sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
+    __syncwarp();
+    phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
+  }
+  // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
+  const bool evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
+  bool any = false;
+  float* delta = m.delta + row0;
+  if (evaluated) {
+#pragma unroll 2
+    for (int i = lane; i < n; i += 32) {
+      const float4 pos = m.pos4[off + i];
+      float X0 = pos.x, X1 = pos.y, X2 = pos.z;
+      if (posed) to_world(R, t, pos.x, pos.y, pos.z, X0, X1, X2);
+      float phi;
+      if constexpr (kOne) phi = fminf(__int_as_float(0x7f800000), sdf_one(one, X0, X1, X2));
+      else phi = union_sdf(sind, m.max_ind, X0, X1, X2);
+      const float d = phi < 0.0f ? -phi : 0.0f;
+      delta[i] = d;
+      any |= d > 0.0f;
+    }
+    any = __any_sync(0xffffffffu, any);
+  }
+  int slot = 0;
+  if (lane == 0) {
+    m.flags[pair] = (uint8_t)any;
+    if (any) {
+      slot = atomicAdd(&m.count[p], 1);
+      m.envlist[(int64_t)p * m.max_envs + slot] = e;
+    }
+  }
+  if (any) {
+    slot = __shfl_sync(0xffffffffu, slot, 0);
+    const int words = (m.n_nodes + 31) >> 5;
+#pragma unroll 2
+    for (int i = lane; i < n; i += 32) {
+      const float d = delta[i];  // written by this thread above
+      if (io.pen_out) io.pen_out[row0 + i] = d;
+      if (io.mask_out && d > 0.0f) {
+        const int g = off + i;
+        atomicOr(&io.mask_out[(int64_t)e * words + (g >> 5)], 1u << (g & 31));
+      }
+      if (write_uhat) {
+        const float4 nn = m.nrm4[off + i];
+        __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off + i;
+        u[0] = __float2bfloat16_rn(-d * nn.x);
+        u[m.ldu] = __float2bfloat16_rn(-d * nn.y);
+        u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * nn.z);
+      }
+    }
+  } else {
+    // contact-free pair: optional outputs are zero; for the gather path the output rows too (the
+    // tensor-core path zero-fills them in the fused kernel)
+    if (!write_uhat) {
+      for (int i = lane; i < n * 3; i += 32) io.out[row0 * 3 + i] = 0.0f;
+      if (io.analytic_out)
+        for (int i = lane; i < n * 3; i += 32) io.analytic_out[row0 * 3 + i] = 0.0f;
+    }
+    if (io.pen_out)
+      for (int i = lane; i < n; i += 32) io.pen_out[row0 + i] = 0.0f;
+  }
+}
+
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, bool write_uhat, cudaStream_t s) {
   const unsigned grid = (unsigned)io.n_envs;
+  // many small patches with indenters: one warp per (env, patch) pair; otherwise one CTA per environment
+  if (io.input_mode == ETAC_IN_INDENTERS && m.max_ind >= 1 && m.n_patches >= 4 && m.max_patch_nodes <= 2048) {
+    const int64_t pairs = (int64_t)io.n_envs * m.n_patches;
+    const unsigned pgrid = (unsigned)((pairs + kPairWarps - 1) / kPairWarps);
+    if (m.max_ind == 1) {
+      sdf_pairs_kernel<true><<<pgrid, kPairWarps * 32, 0, s>>>(m, io, write_uhat ? 1 : 0);
+    } else {
+      const size_t smem = sizeof(SInd) * (size_t)m.max_ind * kPairWarps;
+      sdf_pairs_kernel<false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, write_uhat ? 1 : 0);
+    }
+    return cudaGetLastError();
+  }
   if (io.input_mode == ETAC_IN_INDENTERS) {
     const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
     sdf_penetration_kernel<true><<<grid, 256, smem, s>>>(m, io, write_uhat ? 1 : 0);
