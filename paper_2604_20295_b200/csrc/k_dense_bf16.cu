@@ -11,8 +11,9 @@
 //
 // Work item = (patch p, block of 128 nodes, tile of TE contacting environments of that patch).
 // The grid is persistent (2 CTAs per SM); every CTA walks items blockIdx.x, +gridDim.x, ...
-// 12 warps: 0 = TMA producer, 1 = propagation-GEMM MMA issuer (+ TMEM alloc), 2..5 and 6..9 = two
-// epilogue warpgroups (thread = node), 10/11 = MLP MMA issuers of slot 0/1.
+// 12 warps: 0 = TMA producer, 1 = propagation-GEMM MMA issuer (+ TMEM alloc), 2/3 = MLP MMA issuers
+// of slot 0/1, 4..7 and 8..11 = two epilogue warpgroups (thread = node).  setmaxnreg gives the
+// epilogue warps 96 registers and the others 48.
 //
 // TWO environments are in flight per CTA (slots 0/1, each with its own TMEM D/A regions, mbarrier
 // pair and epilogue warpgroup): while the tensor core runs a layer of slot 0, warpgroup 1
@@ -32,6 +33,9 @@ namespace etac {
 constexpr int BM = 128, BK = 64, TE = kDenseTE, BN = kDenseBN, STAGES = 4;
 constexpr int A_STAGE = BM * BK * 2, B_STAGE = BN * BK * 2;
 constexpr int kDenseThreads = 384;
+// setmaxnreg moves registers inside the CTA's launch-time allocation: 12 warps x 80 registers
+constexpr int kRegsCtrl = 48, kRegsEpi = 96;
+static_assert(4 * kRegsCtrl + 8 * kRegsEpi <= 12 * 80, "register pool");
 constexpr uint32_t kTmemCols = 256;
 constexpr uint32_t COL_ACC = 0, COL_SLOT0 = 48, SLOT_STRIDE = 104, OFF_A = 64;
 
@@ -47,22 +51,6 @@ __host__ __device__ constexpr size_t dense_smem_bytes(int n_patches) {
          (size_t)(n_patches + 1) * 4 + 16;
 }
 
-#ifdef ETAC_TRACE
-// timing experiment only: per-warp event log in shared memory (no global traffic while running)
-__device__ unsigned long long g_trace[12 * 400];
-__device__ unsigned int g_trace_n;
-__shared__ unsigned long long s_trace[12 * 400];
-__shared__ unsigned int s_trace_n[12];
-#define TR(tag)                                                                       \
-  do {                                                                                \
-    if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {                                 \
-      unsigned int w_ = threadIdx.x >> 5, i_ = s_trace_n[w_];                         \
-      if (i_ < 400) s_trace[w_ * 400 + i_] = ((unsigned long long)(tag) << 48) | ((unsigned long long)w_ << 40) | (clock64() & 0xFFFFFFFFFFull), s_trace_n[w_] = i_ + 1; \
-    }                                                                                 \
-  } while (0)
-#else
-#define TR(tag)
-#endif
 
 struct Item {
   int p, mb, tile, cnt;
@@ -127,6 +115,18 @@ __device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, co
   return true;
 }
 
+#ifdef ETAC_PROFILE
+// timing experiment only: per-epilogue-warp cycle accumulators [cta][warp 0..7][12]
+__device__ long long g_prof[320 * 8 * 12];
+#define PROF_MARK(i)                         \
+  do {                                       \
+    const long long now_ = clock64();        \
+    prof[i] += now_ - plast, plast = now_;   \
+  } while (0)
+#else
+#define PROF_MARK(i)
+#endif
+
 template <bool kResid>
 __global__ void __launch_bounds__(kDenseThreads, 2)
     dense_bf16_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
@@ -140,9 +140,6 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   int* prefix = reinterpret_cast<int*>(bars + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-#ifdef ETAC_TRACE
-  if (threadIdx.x < 12) s_trace_n[threadIdx.x] = 0;
-#endif
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
@@ -173,6 +170,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   const uint32_t tmem = bars->tmem_base;
 
   if (warp == 0) {
+    reg_dealloc<kRegsCtrl>();
     // ------------------------------------------------------------------ TMA producer
     // (the whole warp runs the loop so that every operand stays warp-uniform; one elected lane issues)
     {
@@ -195,6 +193,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       }
     }
   } else if (warp == 1) {
+    reg_dealloc<kRegsCtrl>();
     // ------------------------------------------------------------------ MMA issuer
     // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are issued by one elected lane.
     {
@@ -229,16 +228,17 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         }
       }
     }
-  } else if (warp >= 10) {
-    // ------------------------------------------------------------------ MLP MMA issuer of slot (warp - 10)
+  } else if (warp < 4) {
+    reg_dealloc<kRegsCtrl>();
+    // ------------------------------------------------------------------ MLP MMA issuer of slot (warp - 2)
     // One dedicated issuer warp per slot: a tcgen05.mma round trip is ~450 cycles during which the
     // issuing warp makes no progress, so the two slots must not share an issuer.
     // Between requests the warp zero-fills its share of the output rows of contact-free (env, patch)
     // pairs, one run per request, so that these stores trickle out next to the MUFU-bound work.
     ZeroFill zf;
-    zf.init(m, io, blockIdx.x * 2 + (warp - 10), gridDim.x * 2);
+    zf.init(m, io, blockIdx.x * 2 + (warp - 2), gridDim.x * 2);
     if constexpr (kResid) {
-      const int sl = warp - 10;
+      const int sl = warp - 2;
       constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
       constexpr uint32_t idesc_o = make_idesc_bf16(BM, 16);
       const uint64_t dW1 = make_desc(smem_u32(sW), 1024, 128, kLayoutNone);
@@ -255,45 +255,36 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
 #pragma unroll 1
           for (int layer = 0; layer < 3; ++layer) {
             mbar_wait(a_ready, a_ph), a_ph ^= 1;
-            TR(100 + sl * 10 + layer);
             tc_fence_after();
             if (elect_one()) {
-#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 4
-              if (layer == 99) {
-#else
               if (layer == 0) {
-#endif
                 mma_ts(tD, tA, dW1, idesc_h, 0);
-#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 4
-              } else if (layer == 98) {
-#else
               } else if (layer == 1) {
-#endif
 #pragma unroll
                 for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
-#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 4
-              } else if (layer == 97) {
-#else
               } else {
-#endif
 #pragma unroll
                 for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
               }
               tc_commit(d_ready);
             }
             __syncwarp();
-            TR(200 + sl * 10 + layer);
+#ifndef ETAC_NOFILL
             zf.step(m, io, lane);
+#endif
           }
         }
       }
     }
+#ifndef ETAC_NOFILL
     while (zf.step(m, io, lane)) {
     }
+#endif
   } else {
+    reg_alloc<kRegsEpi>();
     // ------------------------------------------------------------------ epilogue (thread = node)
     // Two warpgroups; warpgroup s owns TMEM slot s and takes the environments el = s, s+2, ...
-    const int sl = (warp - 2) >> 2;
+    const int sl = (warp - 4) >> 2;
     const uint32_t lane_base = (uint32_t)(warp & 3) * 32;
     const uint32_t trow = tmem + (lane_base << 16);
     const uint32_t tD = trow + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
@@ -309,6 +300,11 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     int pcur = 0;
     uint32_t acc_ph = 0, d_ph = 0;
     Item it;
+#ifdef ETAC_PROFILE
+    long long prof[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+    long long plast = clock64();
+    const long long pstart = plast;
+#endif
     for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
       const PatchInfo pi = m.patch[it.p];
       const int li = it.mb * BM + row;
@@ -326,100 +322,133 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       }
       // lane l prefetches the id of the item's l-th environment (broadcast by shuffle below)
       const int my_env = lane < it.cnt ? m.envlist[(int64_t)it.p * m.max_envs + it.tile * TE + lane] : 0;
+      PROF_MARK(0);  // item setup
       mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
       tc_fence_after();
-#ifdef ETAC_SKEW
-      // De-phase the two warpgroups: both leave the accumulator barrier together and would then
-      // alternate "both on the MUFU pipe" / "both waiting for the tensor core" in lock-step.
-      if (sl == 1) {
-        const long long t0 = clock64();
-        while (clock64() - t0 < ETAC_SKEW) {
-        }
-      }
-#endif
-      for (int el = sl; el < it.cnt; el += 2) {
-#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 3
-        const int env = it.tile * TE + el;
-        const int64_t node = (int64_t)env * m.n_nodes + g;
-        const float dl = 0.0f;
-#else
+      PROF_MARK(1);  // acc_full wait
+      // The units of an item are software-pipelined: while the tensor core runs layer 3 of unit
+      // el, the u_lin of unit el+2 is already fetched from the accumulator, and its layer-1 operand
+      // is written (and requested) before the output of unit el is combined and stored.  Every
+      // TMEM access costs a few hundred cycles of latency; this takes two of them per unit off
+      // the chain's critical path.
+      struct Unit {
+        int64_t node;
+        float ux, uy, uz, dl;
+      };
+      auto fetch_unit = [&](Unit& u, const int el, uint32_t (&ur)[4]) {  // requests only; tc_wait_ld() follows
         const int env = __shfl_sync(0xffffffffu, my_env, el);
-        const int64_t node = (int64_t)env * m.n_nodes + g;
-        const float dl = valid ? m.delta[node] : 0.0f;
-#endif
-        uint32_t ur[4];
+        u.node = (int64_t)env * m.n_nodes + g;
+        u.dl = valid ? m.delta[u.node] : 0.0f;  // consumed when the unit is stored
         tmem_ld4(trow + COL_ACC + 3 * el, ur);
-        tc_wait_ld();
-        const float ux = __uint_as_float(ur[0]), uy = __uint_as_float(ur[1]), uz = __uint_as_float(ur[2]);
-        float ox = ux, oy = uy, oz = uz;
+      };
+      auto request_layer1 = [&](Unit& u, const uint32_t (&ur)[4]) {
+        u.ux = __uint_as_float(ur[0]), u.uy = __uint_as_float(ur[1]), u.uz = __uint_as_float(ur[2]);
         if constexpr (kResid) {
-          a1[0] = pack_bf16(ux, uy);
-          a1[1] = pack_bf16(uz, px);
+          a1[0] = pack_bf16(u.ux, u.uy);
+          a1[1] = pack_bf16(u.uz, px);
           tmem_st8(tA, a1);
           tc_wait_st();
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(a_ready);
-          TR(1);
+        }
+      };
+      // the accumulator is released as soon as this warp has fetched its LAST u_lin of the item, a
+      // whole unit before the item ends: the next item's propagation GEMM runs behind that unit's MLP
+      auto release_acc = [&]() {
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars->acc_empty);
+      };
+      Unit cur, nxt;
+      {
+        uint32_t ur[4];
+        if (sl < it.cnt) {
+          fetch_unit(cur, sl, ur);
+          tc_wait_ld();
+          if (sl + 2 >= it.cnt) release_acc();
+          request_layer1(cur, ur);
+        } else {
+          release_acc();
+        }
+      }
+      PROF_MARK(2);  // first unit of the item: u_lin, layer-1 operand
+      for (int el = sl; el < it.cnt; el += 2) {
+        const bool more = el + 2 < it.cnt;
+        float rx = 0.f, ry = 0.f, rz = 0.f;
+        uint32_t un[4] = {0, 0, 0, 0};
+        if constexpr (kResid) {
 #pragma unroll 1
           for (int layer = 0; layer < 2; ++layer) {
             mbar_wait(d_ready, d_ph), d_ph ^= 1;
-            TR(2 + layer * 2);
             tc_fence_after();
-            uint32_t h[32], packed[16];
+            PROF_MARK(4);  // d_ready wait (layers 1, 2)
+            // both halves are requested at once: one TMEM load latency per layer instead of two
+            uint32_t ha[32], hb[32], packed[16];
+            tmem_ld32(tD, ha);
+            tmem_ld32(tD + 32, hb);
+            tc_wait_ld();
 #pragma unroll
-            for (int half = 0; half < 2; ++half) {
-              tmem_ld32(tD + 32 * half, h);
-              tc_wait_ld();
-#pragma unroll
-              for (int k = 0; k < 16; ++k) {
-                // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
-                const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
-                packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
-              }
-              tmem_st16(tA + 16 * half, packed);
+            for (int k = 0; k < 16; ++k) {
+              // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
+              const float h0 = __uint_as_float(ha[2 * k]), h1 = __uint_as_float(ha[2 * k + 1]);
+              packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
             }
+            tmem_st16(tA, packed);
+#pragma unroll
+            for (int k = 0; k < 16; ++k) {
+              const float h0 = __uint_as_float(hb[2 * k]), h1 = __uint_as_float(hb[2 * k + 1]);
+              packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
+            }
+            tmem_st16(tA + 16, packed);
+            PROF_MARK(6);  // D load + SiLU + operand stores issued
             tc_wait_st();
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(a_ready);
-            TR(3 + layer * 2);
+            PROF_MARK(7);  // store wait + arrive
           }
+          if (more) fetch_unit(nxt, el + 2, un);  // overlaps the layer-3 round trip
           mbar_wait(d_ready, d_ph), d_ph ^= 1;
-          TR(6);
           tc_fence_after();
+          PROF_MARK(8);  // d_ready wait (layer 3)
           uint32_t rr[4];
           tmem_ld4(tD, rr);
           tc_wait_ld();
-          ox += __uint_as_float(rr[0]), oy += __uint_as_float(rr[1]), oz += __uint_as_float(rr[2]);
-        }
-#if defined(ETAC_ABLATE) && ETAC_ABLATE >= 2
-        if (valid && ox == 123.456f) {
-#else
-        if (valid) {
-#endif
-          if (dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH) ox = -dl * nrm.x, oy = -dl * nrm.y, oz = -dl * nrm.z;
-          float* o = io.out + node * 3;
-          o[0] = ox, o[1] = oy, o[2] = oz;
-          if (io.analytic_out) {
-            float* a = io.analytic_out + node * 3;
-            a[0] = ux, a[1] = uy, a[2] = uz;
+          rx = __uint_as_float(rr[0]), ry = __uint_as_float(rr[1]), rz = __uint_as_float(rr[2]);
+          PROF_MARK(9);  // r (and next u_lin) load
+        } else {
+          if (more) {
+            fetch_unit(nxt, el + 2, un);
+            tc_wait_ld();
           }
         }
+        if (more && el + 4 >= it.cnt) release_acc();
+        if (more) request_layer1(nxt, un);  // layer 3 has been read: the operand region is free
+        PROF_MARK(3);  // next unit's layer-1 operand + arrive
+        if (valid) {  // S4: mask M_p + combine (Eq. 2); active rows keep u^ = -delta n in fp32
+          float ox = cur.ux + rx, oy = cur.uy + ry, oz = cur.uz + rz;
+          if (cur.dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH)
+            ox = -cur.dl * nrm.x, oy = -cur.dl * nrm.y, oz = -cur.dl * nrm.z;
+          float* o = io.out + cur.node * 3;
+          __stcs(o, ox), __stcs(o + 1, oy), __stcs(o + 2, oz);
+          if (io.analytic_out) {
+            float* a = io.analytic_out + cur.node * 3;
+            __stcs(a, cur.ux), __stcs(a + 1, cur.uy), __stcs(a + 2, cur.uz);
+          }
+        }
+        cur = nxt;
+        PROF_MARK(10);  // mask, combine, store
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&bars->acc_empty);
     }
+#ifdef ETAC_PROFILE
+    prof[11] = clock64() - pstart;
+    if (lane == 0 && blockIdx.x < 320)
+      for (int i = 0; i < 12; ++i) g_prof[(blockIdx.x * 8 + (warp - 4)) * 12 + i] = prof[i];
+#endif
   }
   tc_fence_before();
   __syncthreads();
-#ifdef ETAC_TRACE
-  if (blockIdx.x == 0) {
-    for (int k = threadIdx.x; k < 4800; k += blockDim.x) g_trace[k] = (k % 400) < s_trace_n[k / 400] ? s_trace[k] : 0ull;
-    g_trace_n = 4800;
-  }
-#endif
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc<kTmemCols>(tmem);
@@ -446,9 +475,7 @@ cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtenso
 
 }  // namespace etac
 
-#ifdef ETAC_TRACE
-extern "C" void etac_debug_trace(unsigned long long* out, unsigned int* n) {
-  cudaMemcpyFromSymbol(out, etac::g_trace, sizeof(unsigned long long) * 4800);
-  cudaMemcpyFromSymbol(n, etac::g_trace_n, sizeof(unsigned int));
-}
+#ifdef ETAC_PROFILE
+extern "C" void etac_debug_prof(long long* out) { cudaMemcpyFromSymbol(out, etac::g_prof, sizeof(long long) * 320 * 8 * 12); }
 #endif
+
