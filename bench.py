@@ -32,8 +32,9 @@ UNIT = "env-steps/s"
 N_INPUT_SETS = 4
 MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728
 # dram__bytes_read.sum + dram__bytes_write.sum of one dense_bf16_kernel launch, from the
-# `ncu --set full` capture summarised in profiles/r01_dense_ncu_full.md (79.3 MB read + 47.9 MB write).
-NCU_TRAFFIC_BYTES = 127.26e6
+# `ncu --set full` capture summarised in profiles/r01b_dense_ncu_full.md (79.3 MB read + 234.1 MB
+# write; the kernel now also zero-fills the rows of contact-free (env, patch) pairs).
+NCU_TRAFFIC_BYTES = 313.43e6
 
 
 def load_peaks():
@@ -70,7 +71,7 @@ class ClockSampler:
         self.p = None
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                       "--format=csv,noheader,nounits", "-lms", "20"], stdout=self.f,
                                       stderr=subprocess.DEVNULL)
         except OSError:
             pass
@@ -232,7 +233,7 @@ def run_ours(a):
     t_tensor = flops / (peak * 1e12)
     t_hbm = wm["b_hbm_min"] / (peaks["hbm_gbs"] * 1e9)
     t_roof = max(t_tensor, t_hbm)
-    cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, 512 if a.envs >= 512 else a.envs)
+    cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, a.envs)   # ~10 s of CPU work at 4096 envs
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -242,13 +243,14 @@ def run_ours(a):
                    "n_nodes": eng.N, "n_patches": eng.P, "precision": "bf16 operands, fp32 accumulate",
                    "contact_pairs_per_step": wm["pairs"], "node_envs_per_step": wm["w_nodeenv"],
                    "l2": f"{N_INPUT_SETS} rotating seeded input sets; 280 MB output + 230 MB workspace per step > 126 MB L2",
+                   "algorithmic_bytes_fused": wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"],
                    "parallelism": f"env-sharded x{world}, no collective"},
         "clocks": clocks,
         "e2e": {"value": world * a.envs * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": n_e2e,
                 "note": "pinned host indenters+patch poses -> device, etac_step, full [E,N,3] fp32 result -> pinned host"},
         "gpu_launches": launches,
-        "kernels_ms": {"sdf_penetration_kernel": ms_s1, "dense_bf16_kernel": ms_fused},
+        "kernels_ms": {"s1_sdf_pairs_kernel_incl_memsets": ms_s1, "dense_bf16_kernel": ms_fused},
         "roofline": {"bound": "tensor", "kernel": "dense_bf16_kernel", "achieved": achieved, "peak": peak,
                      "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES,
                      "peak_src": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['src']})",
@@ -269,7 +271,7 @@ def run_ours(a):
 if __name__ == "__main__":
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--envs", type=int, default=4096)
