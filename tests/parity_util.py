@@ -45,8 +45,10 @@ def run_oracle(wl, *, resid=True, active_mode="passthrough", penetration=None, e
     return O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose, envs=envs)
 
 
-def compare(gpu, ref, tol, envs=None, resid_tol=None, label=""):
-    """gpu: dict from run_gpu (all envs); ref: oracle dict for `envs` (default all)."""
+def compare(gpu, ref, tol, envs=None, resid_tol=None, label="", delta_tol=1e-5):
+    """gpu: dict from run_gpu (all envs); ref: oracle dict for `envs` (default all).
+    delta_tol: fp32-vs-fp64 bound on delta relative to max(1, max delta); the fp32 evaluation of
+    |y| - r loses ~ulp(r), so workloads with very large indenters pass a looser bound."""
     sel = slice(None) if envs is None else np.asarray(list(envs))
     U, A, D, M = gpu["U"][sel], gpu["analytic"][sel], gpu["delta"][sel], gpu["mask"][sel]
     assert np.isfinite(U).all() and np.isfinite(A).all() and np.isfinite(D).all(), f"{label}: unwritten output"
@@ -54,7 +56,7 @@ def compare(gpu, ref, tol, envs=None, resid_tol=None, label=""):
     assert np.array_equal(M, ref["mask"]), f"{label}: mask differs at {np.argwhere(M != ref['mask'])[:5]}"
     assert np.array_equal(D, ref["delta32"]), f"{label}: delta not bit-exact vs the fp32 twin"
     scale_d = max(1.0, float(np.abs(ref["delta"]).max()))
-    assert np.abs(D - ref["delta"]).max() <= 1e-5 * scale_d
+    assert np.abs(D - ref["delta"]).max() <= delta_tol * scale_d
     umax = float(np.abs(ref["U"]).max())
     amax = float(np.abs(ref["analytic"]).max())
     err_u = float(np.abs(U - ref["U"]).max())

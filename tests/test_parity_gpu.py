@@ -162,3 +162,91 @@ def test_full_size_config3_sampled():
     act = gpu["mask"]
     nrm = wl.mesh.normal[None]
     np.testing.assert_array_equal(gpu["U"][act], (-gpu["delta"][..., None] * nrm)[act])   # P7 on every env
+
+
+def _multi_indenter_hand(seed, n_envs, n_ind, posed):
+    """Hand mesh (16 patches) with several indenters per environment pressed on random nodes:
+    exercises the warp-per-(env, patch) S1 kernel with M > 1 (indenters staged per warp)."""
+    base = W.config3(seed, n_envs)
+    mesh = base.mesh
+    rng = np.random.default_rng(100 + seed)
+    ind = W._blank_indenters(n_envs, n_ind)
+    for k in range(n_ind):
+        c = rng.integers(0, mesh.n_nodes, size=n_envs)
+        shape = rng.integers(1, 4, size=n_envs)                       # sphere / box / capsule
+        size = rng.uniform(2.0, 5.0, n_envs)
+        d = rng.uniform(0.1, 1.2, n_envs)
+        centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, d, rng.uniform(0, 6.28, n_envs))
+        use = rng.random(n_envs) < 0.8
+        ind["type"][:, k] = np.where(use, shape, W.IND_NONE)
+        ind["param"][:, k, 0] = size
+        ind["param"][:, k, 1] = np.where(shape == W.IND_CAPSULE, rng.uniform(0.0, 4.0, n_envs), size)
+        ind["param"][:, k, 2] = size
+        ind["pose"][use, k, 0:3] = centre[use]
+        ind["pose"][use, k, 3:7] = q[use]
+    pose = None
+    if posed:                                                         # one rigid motion per env for all patches
+        pose = np.zeros((n_envs, mesh.n_patches, 7), np.float32)
+        Rm = W.random_rotations(rng, n_envs)
+        t = rng.uniform(-20, 20, (n_envs, 3))
+        pose[:, :, 0:3] = t[:, None, :]
+        pose[:, :, 3:7] = W.quat_from_matrix(Rm)[:, None, :]
+        ind["pose"][..., 0:3] = np.einsum("eij,ekj->eki", Rm, ind["pose"][..., 0:3].astype(np.float64)) + t[:, None, :]
+        qi = ind["pose"][..., 3:7].astype(np.float64)
+        from scipy.spatial.transform import Rotation as Rot
+        for e in range(n_envs):
+            ind["pose"][e, :, 3:7] = (Rot.from_matrix(Rm[e]) * Rot.from_quat(qi[e])).as_quat()
+    return W.Workload("hand_multi_ind", mesh, base.alpha, base.weights, n_envs, n_ind, ind, pose, "bf16")
+
+
+@pytest.mark.parametrize("posed", [False, True])
+def test_many_patches_several_indenters(posed):
+    wl = _multi_indenter_hand(5, 29, 3, posed)
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    assert gpu["mask"].any()
+    _report(f"hand M=3 posed={posed}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="hand-multi"))
+    assert gpu["pairs"] == int(ref["contact"].sum())
+    gpu32 = run_gpu(wl, precision="fp32")
+    compare(gpu32, ref, TOL["fp32"], resid_tol=1e-4, label="hand-multi-fp32")
+
+
+@pytest.mark.parametrize("n_nodes,curved,frac", [(256, False, 0.05), (1024, True, 0.20), (1024, False, 0.01)])
+def test_config5_dense_and_sparse_paths(n_nodes, curved, frac):
+    """BASELINE.json configs[4] sweep points at a size the oracle finishes in seconds: the bf16
+    context through the tensor-core path and through the gather path (fp32 arithmetic)."""
+    wl = W.config5(48, n_nodes, curved, frac, "bf16")
+    ref = run_oracle(wl)
+    assert ref["mask"].any()
+    dense = run_gpu(wl, path=T.ETAC_PATH_DENSE)
+    # 20 % contact on the curved sheet needs spheres of r > 100 mm: ulp(r) ~ 1e-5 in fp32
+    _report(f"cfg5 N={n_nodes} dense", compare(dense, ref, TOL["bf16"], resid_tol=5e-2, label="cfg5-dense", delta_tol=1e-4))
+    sparse = run_gpu(wl, path=T.ETAC_PATH_SPARSE)
+    assert sparse["path"] == T.ETAC_PATH_SPARSE
+    _report(f"cfg5 N={n_nodes} sparse", compare(sparse, ref, TOL["fp32"], resid_tol=1e-4, label="cfg5-sparse", delta_tol=1e-4))
+
+
+def test_full_size_config4_sampled():
+    """BASELINE.json configs[3] at full size (4096 envs, one dense K[8192 x 8192], bf16); the
+    oracle checks a sample of environments; invariants hold on every environment."""
+    wl = W.config4(0, 4096)
+    import torch
+    eng = T.Etac(wl, debug_outputs=False)
+    try:
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        eng.out.fill_(float("nan"))
+        U = eng.step(wl.n_envs, dev)
+        torch.cuda.synchronize()
+        envs = [0, 1777, 4095]
+        ref = run_oracle(wl, envs=envs)
+        Us = U[envs].cpu().numpy()
+        umax = float(np.abs(ref["U"]).max())
+        err = float(np.abs(Us - ref["U"]).max())
+        print(f"[parity] cfg4 full: umax={umax:.3e} err={err:.3e} rel={err / umax:.3e}")
+        assert err <= TOL["bf16"] * umax
+        # active rows keep u^ = -delta n exactly (P7) on the sampled envs; everything finite everywhere
+        act = ref["mask"]
+        np.testing.assert_array_equal(Us[act], (-ref["delta32"][..., None] * wl.mesh.normal[None])[act])
+        assert bool(torch.isfinite(U).all())
+        assert T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_CONTACT_PAIRS) == int((np.abs(U.cpu().numpy()).sum((1, 2)) > 0).sum())
+    finally:
+        eng.close()
