@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
 constexpr int kPairWarps = 2;
 
 template <bool kOne>
-__global__ void __launch_bounds__(kPairWarps * 32) sdf_pairs_kernel(DevModel m, StepIO io, int write_uhat) {
+__global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel m, StepIO io, int write_uhat) {
   extern __shared__ uint8_t smem_raw[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   SInd* sind = reinterpret_cast<SInd*>(smem_raw) + (size_t)wib * (kOne ? 0 : m.max_ind);  // per-warp staging (M > 1)
