@@ -123,7 +123,10 @@ etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* ar
 enum { ETAC_OPT_PATH = 1 };
 enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
 /* DENSE : tcgen05 tensor-core contraction K_p . U^ (needs ETAC_PREC_BF16);
- * SPARSE: gather over the active nodes only (Omega U_a literally), fp32 SIMT;
+ * SPARSE: gather over the active nodes only (Omega U_a literally).  FP32 context: fp32 SIMT kernel,
+ *         fp32 MLP.  BF16 context: bf16 K, fp32 u^ and accumulation, tensor-core MLP as in DENSE;
+ *         selecting it allocates the active-node lists (16 bytes x max_envs x N), which is why the
+ *         choice is made with etac_set_option and never inside etac_step;
  * AUTO  : DENSE for BF16 contexts, SPARSE for FP32 contexts. */
 etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value);
 

@@ -152,12 +152,18 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   }
   if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset count", e));
-  if ((e = launch_sdf(ctx->m, io, path == ETAC_PATH_DENSE, s)) != cudaSuccess)
+  // bf16 context: tensor-core MLP either way; DENSE = tcgen05 contraction K.U^, SPARSE = gather over the
+  // active-node lists.  fp32 context: fp32 SIMT gather kernel (which needs S1 to zero-fill).
+  const bool bf16 = ctx->precision == ETAC_PREC_BF16;
+  const bool gather16 = bf16 && path == ETAC_PATH_SPARSE;
+  const int s1_flags = !bf16 ? kS1FillOut : (gather16 ? kS1WriteAlist : kS1WriteUhat);
+  if (gather16 && !ctx->m.alist) return fail(ctx, ETAC_ERR_INVALID_ARG, "select ETAC_PATH_SPARSE with etac_set_option first");
+  if ((e = launch_sdf(ctx->m, io, s1_flags, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
   ++ctx->last_launches;
   if (ev) cudaEventRecord(ev[1], s);
-  if (path == ETAC_PATH_DENSE) {
-    if ((e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, s)) != cudaSuccess)
+  if (bf16) {
+    if ((e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, s)) != cudaSuccess)
       return fail(ctx, ETAC_ERR_CUDA, cuda_msg("dense_bf16_kernel", e));
   } else {
     if ((e = launch_gather_fp32(ctx->m, io, s)) != cudaSuccess)
@@ -428,6 +434,17 @@ etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
     return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_PATH value");
   if (value == ETAC_PATH_DENSE && ctx->precision != ETAC_PREC_BF16)
     return fail(ctx, ETAC_ERR_UNSUPPORTED, "ETAC_PATH_DENSE needs an ETAC_PREC_BF16 context");
+  if (value == ETAC_PATH_SPARSE && ctx->precision == ETAC_PREC_BF16 && !ctx->m.alist) {
+    // workspace of the bf16 gather path: active-node lists (allocated here, never inside etac_step)
+    DeviceGuard guard(ctx->device);
+    ActiveEntry* al = nullptr;
+    int32_t* ac = nullptr;
+    const size_t rows = (size_t)((ctx->m.max_envs + kDenseTE - 1) / kDenseTE) * kDenseTE;
+    cudaError_t e = dev_alloc(ctx, &al, rows * ctx->m.ldu, false);
+    if (e == cudaSuccess) e = dev_alloc(ctx, &ac, (size_t)ctx->m.n_patches * ctx->m.max_envs, true);
+    if (e != cudaSuccess) return fail(ctx, e == cudaErrorMemoryAllocation ? ETAC_ERR_ALLOC : ETAC_ERR_CUDA, cuda_msg("alloc active lists", e));
+    ctx->m.alist = al, ctx->m.acount = ac;
+  }
   ctx->path_opt = (int)value;
   return ETAC_OK;
 }

@@ -44,6 +44,16 @@ constexpr int kW2ImgBytes = 64 * 80 * 2;   // N=64,  K=80   (64 + bias column, p
 constexpr int kW3ImgBytes = 16 * 80 * 2;   // N=16,  K=80   (3 outputs padded to 16)
 constexpr int kWImgBytes = kW1ImgBytes + kW2ImgBytes + kW3ImgBytes;
 
+// Active node of a contacting (env, patch) pair, for the gather form of the propagation:
+// u^ of the node (fp32) and its index within the patch.
+struct __align__(16) ActiveEntry {
+  float ux, uy, uz;
+  int32_t j;
+};
+
+// what S1 writes besides delta / flags / env lists
+enum : int { kS1WriteUhat = 1, kS1WriteAlist = 2, kS1FillOut = 4 };
+
 struct DevModel {
   int32_t n_nodes, n_patches, n_chunks;
   int32_t max_patch_nodes;    // largest patch
@@ -66,6 +76,9 @@ struct DevModel {
   int32_t* count;             // [P] contacting envs per patch (this step)
   int32_t* envlist;           // [P x max_envs]
   uint8_t* flags;             // [max_envs x P]
+  ActiveEntry* alist;         // [max_envs (slots) x ldu]: the active nodes of (slot, patch p) start at
+                              // slot * ldu + off_p, in node order (allocated when the bf16 gather path is first selected)
+  int32_t* acount;            // [P x max_envs]: number of active nodes of (patch, slot)
 };
 
 struct StepIO {
@@ -82,10 +95,10 @@ struct StepIO {
 // kernel launchers (each returns cudaGetLastError())
 cudaError_t launch_build_k(const DevModel& m, float* k32, __nv_bfloat16* k16, cudaStream_t s);
 cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1, float* c1t, cudaStream_t s);
-cudaError_t launch_sdf(const DevModel& m, const StepIO& io, bool write_uhat, cudaStream_t s);
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s);
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                              int n_sm, cudaStream_t s);
+                              int n_sm, bool gather, cudaStream_t s);
 cudaError_t dense_bf16_configure();
 
 }  // namespace etac

@@ -48,13 +48,18 @@ struct __align__(8) DenseBars {
 
 __host__ __device__ constexpr size_t dense_smem_bytes(int n_patches) {
   return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE + B_STAGE) + kWImgBytes + sizeof(DenseBars) +
-         (size_t)(n_patches + 1) * 4 + 16;
+         (size_t)(n_patches + 1) * 4 + 16 + 16 + 8 * 32 * 16;
 }
 
 
 struct Item {
   int p, mb, tile, cnt;
 };
+
+#ifndef ETAC_GATHER_DEPTH
+#define ETAC_GATHER_DEPTH 16
+#endif
+constexpr int kGatherDepth = ETAC_GATHER_DEPTH;  // K loads in flight per thread in the gather form (divides 32)
 
 // streaming zero-fill of `count` floats at a 4-byte aligned address by one warp
 __device__ __forceinline__ void warp_zero_fill(float* __restrict__ p, int count, int lane) {
@@ -127,7 +132,12 @@ __device__ long long g_prof[320 * 8 * 12];
 #define PROF_MARK(i)
 #endif
 
-template <bool kResid>
+// kGather: the propagation is not the dense tensor-core contraction but Omega U_a literally
+// (PAPER.md:L87): every epilogue thread sums K[i][j] u^_j over the ACTIVE nodes j of its unit,
+// read from the compact lists S1 wrote (bf16 K row j, coalesced over i because K is symmetric;
+// fp32 u^ and accumulation).  No TMA, no propagation MMA; the MLP part is unchanged.  It wins
+// when few nodes are in contact (ETAC_PATH_SPARSE on a bf16 context).
+template <bool kResid, bool kGather>
 __global__ void __launch_bounds__(kDenseThreads, 2)
     dense_bf16_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
                       const __grid_constant__ CUtensorMap tmB) {
@@ -138,6 +148,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   uint8_t* sW = sB + STAGES * B_STAGE;
   DenseBars* bars = reinterpret_cast<DenseBars*>(sW + kWImgBytes);
   int* prefix = reinterpret_cast<int*>(bars + 1);
+  uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + (m.n_patches + 1)) + 15) & ~uintptr_t(15));  // 8 warps x 32 entries
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -171,6 +182,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
 
   if (warp == 0) {
     reg_dealloc<kRegsCtrl>();
+    if constexpr (!kGather)
     // ------------------------------------------------------------------ TMA producer
     // (the whole warp runs the loop so that every operand stays warp-uniform; one elected lane issues)
     {
@@ -194,6 +206,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     }
   } else if (warp == 1) {
     reg_dealloc<kRegsCtrl>();
+    if constexpr (!kGather)
     // ------------------------------------------------------------------ MMA issuer
     // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are issued by one elected lane.
     {
@@ -323,8 +336,10 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       // lane l prefetches the id of the item's l-th environment (broadcast by shuffle below)
       const int my_env = lane < it.cnt ? m.envlist[(int64_t)it.p * m.max_envs + it.tile * TE + lane] : 0;
       PROF_MARK(0);  // item setup
-      mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
-      tc_fence_after();
+      if constexpr (!kGather) {
+        mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
+        tc_fence_after();
+      }
       PROF_MARK(1);  // acc_full wait
       // The units of an item are software-pipelined: while the tensor core runs layer 3 of unit
       // el, the u_lin of unit el+2 is already fetched from the accumulator, and its layer-1 operand
@@ -339,7 +354,41 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         const int env = __shfl_sync(0xffffffffu, my_env, el);
         u.node = (int64_t)env * m.n_nodes + g;
         u.dl = valid ? m.delta[u.node] : 0.0f;  // consumed when the unit is stored
-        tmem_ld4(trow + COL_ACC + 3 * el, ur);
+        if constexpr (!kGather) {
+          tmem_ld4(trow + COL_ACC + 3 * el, ur);
+        } else {
+          // Omega U_a: sum over the active nodes of this (env, patch); entry loads are warp-uniform
+          // (broadcast), K row j is read coalesced over the rows i of the warp
+          const int slot = it.tile * TE + el;
+          const int cnt = m.acount[(int64_t)it.p * m.max_envs + slot];
+          const ActiveEntry* __restrict__ al = m.alist + (int64_t)slot * m.ldu + pi.off;
+          const __nv_bfloat16* __restrict__ kcol = m.k16 + (int64_t)pi.off * m.kw + (valid ? li : 0);
+          float ax = 0.f, ay = 0.f, az = 0.f;
+          // 32 entries per sweep: lane l loads entry k0+l (one coalesced 512-byte read) into the
+          // warp's shared-memory staging row; the entries are then read back as broadcasts while
+          // kGatherDepth K loads are in flight per thread
+          float4* stage = reinterpret_cast<float4*>(sGather) + (warp - 4) * 32;
+          for (int k0 = 0; k0 < cnt; k0 += 32) {
+            float4 mine = make_float4(0.f, 0.f, 0.f, 0.f);  // padding entries: u^ = 0, j = 0
+            if (k0 + lane < cnt) mine = __ldg(reinterpret_cast<const float4*>(al + k0 + lane));
+            __syncwarp();
+            stage[lane] = mine;
+            __syncwarp();
+            const int nb = min(32, cnt - k0);
+            for (int q0 = 0; q0 < nb; q0 += kGatherDepth) {  // the loop is bound by loads in flight
+              float kv[kGatherDepth];
+#pragma unroll
+              for (int q = 0; q < kGatherDepth; ++q)
+                kv[q] = __bfloat162float(kcol[(int64_t)__float_as_int(stage[q0 + q].w) * m.kw]);
+#pragma unroll
+              for (int q = 0; q < kGatherDepth; ++q) {
+                const float4 en = stage[q0 + q];
+                ax = fmaf(kv[q], en.x, ax), ay = fmaf(kv[q], en.y, ay), az = fmaf(kv[q], en.z, az);
+              }
+            }
+          }
+          ur[0] = __float_as_uint(ax), ur[1] = __float_as_uint(ay), ur[2] = __float_as_uint(az), ur[3] = 0;
+        }
       };
       auto request_layer1 = [&](Unit& u, const uint32_t (&ur)[4]) {
         u.ux = __uint_as_float(ur[0]), u.uy = __uint_as_float(ur[1]), u.uz = __uint_as_float(ur[2]);
@@ -356,9 +405,11 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       // the accumulator is released as soon as this warp has fetched its LAST u_lin of the item, a
       // whole unit before the item ends: the next item's propagation GEMM runs behind that unit's MLP
       auto release_acc = [&]() {
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&bars->acc_empty);
+        if constexpr (!kGather) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bars->acc_empty);
+        }
       };
       Unit cur, nxt;
       {
@@ -457,19 +508,22 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
 
 cudaError_t dense_bf16_configure() {
   const int bytes = (int)dense_smem_bytes(kMaxPatches);
-  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e != cudaSuccess) return e;
-  return cudaFuncSetAttribute(dense_bf16_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  return e;
 }
 
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                              int n_sm, cudaStream_t s) {
+                              int n_sm, bool gather, cudaStream_t s) {
   const size_t smem = dense_smem_bytes(m.n_patches);
   const int grid = 2 * n_sm;
-  if (m.resid != ETAC_RESID_NONE)
-    dense_bf16_kernel<true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-  else
-    dense_bf16_kernel<false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  const bool resid = m.resid != ETAC_RESID_NONE;
+  if (resid && !gather) dense_bf16_kernel<true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  if (!resid && !gather) dense_bf16_kernel<false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  if (resid && gather) dense_bf16_kernel<true, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  if (!resid && gather) dense_bf16_kernel<false, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
   return cudaGetLastError();
 }
 

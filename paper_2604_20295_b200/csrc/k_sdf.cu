@@ -116,7 +116,9 @@ struct SPose {
 //   E  all threads: contact-free patches -> zero-fill of the output rows; contacting patches ->
 //      U^ operand rows (bf16), optional delta / mask outputs
 template <bool kIndenters>
-__global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int write_uhat) {
+__global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int s1_flags) {
+  const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
+  __shared__ int s_wcnt[8];
   extern __shared__ uint8_t smem_raw[];
   SInd* sind = reinterpret_cast<SInd*>(smem_raw);
   __shared__ SPose s_pose[kPoseChunk];
@@ -230,7 +232,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       if (run0 >= 0) {
         const int64_t r0 = (int64_t)e * m.n_nodes + s_off[run0];
         const int cnt = s_off[q] - s_off[run0];
-        if (!write_uhat) {  // tensor-core path: the fused kernel's idle warps zero-fill these rows
+        if (fill_out) {  // (tensor-core paths: the fused kernel's issuer warps zero-fill these rows)
           zero_fill(io.out + r0 * 3, cnt * 3);
           if (io.analytic_out) zero_fill(io.analytic_out + r0 * 3, cnt * 3);
         }
@@ -242,6 +244,32 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       const int64_t row0 = (int64_t)e * m.n_nodes + off;
       const int slot = s_slot[q];
       const float* delta = m.delta + row0;
+      if (write_alist) {
+        // compact list of the patch's active nodes in node order (block-wide ordered compaction)
+        ActiveEntry* al = m.alist + (int64_t)slot * m.ldu + off;
+        int base = 0;
+        for (int i0 = 0; i0 < n; i0 += blockDim.x) {
+          const int i = i0 + threadIdx.x;
+          const float d = i < n ? delta[i] : 0.0f;
+          const uint32_t bal = __ballot_sync(0xffffffffu, d > 0.0f);
+          if (lane == 0) s_wcnt[threadIdx.x >> 5] = __popc(bal);
+          __syncthreads();
+          int before = base, total = base;
+          for (int w = 0; w < 8; ++w) {
+            if (w < (int)(threadIdx.x >> 5)) before += s_wcnt[w];
+            total += s_wcnt[w];
+          }
+          if (d > 0.0f) {
+            const float4 nn = m.nrm4[off + i];
+            ActiveEntry en;
+            en.ux = -d * nn.x, en.uy = -d * nn.y, en.uz = -d * nn.z, en.j = i;
+            al[before + __popc(bal & ((1u << lane) - 1u))] = en;
+          }
+          base = total;
+          __syncthreads();
+        }
+        if (threadIdx.x == 0) m.acount[(int64_t)(p0 + q) * m.max_envs + slot] = base;
+      }
       for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const float d = delta[i];
         if (io.pen_out) io.pen_out[row0 + i] = d;
@@ -272,7 +300,8 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
 constexpr int kPairWarps = 2;
 
 template <bool kOne>
-__global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel m, StepIO io, int write_uhat) {
+__global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel m, StepIO io, int s1_flags) {
+  const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
   extern __shared__ uint8_t smem_raw[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   SInd* sind = reinterpret_cast<SInd*>(smem_raw) + (size_t)wib * (kOne ? 0 : m.max_ind);  // per-warp staging (M > 1)
@@ -334,6 +363,23 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
   if (any) {
     slot = __shfl_sync(0xffffffffu, slot, 0);
     const int words = (m.n_nodes + 31) >> 5;
+    if (write_alist) {  // compact list of the patch's active nodes, in node order
+      ActiveEntry* al = m.alist + (int64_t)slot * m.ldu + off;
+      int base = 0;
+      for (int i0 = 0; i0 < n; i0 += 32) {
+        const int i = i0 + lane;
+        const float d = i < n ? delta[i] : 0.0f;
+        const uint32_t bal = __ballot_sync(0xffffffffu, d > 0.0f);
+        if (d > 0.0f) {
+          const float4 nn = m.nrm4[off + i];
+          ActiveEntry en;
+          en.ux = -d * nn.x, en.uy = -d * nn.y, en.uz = -d * nn.z, en.j = i;
+          al[base + __popc(bal & ((1u << lane) - 1u))] = en;
+        }
+        base += __popc(bal);
+      }
+      if (lane == 0) m.acount[(int64_t)p * m.max_envs + slot] = base;
+    }
 #pragma unroll 2
     for (int i = lane; i < n; i += 32) {
       const float d = delta[i];  // written by this thread above
@@ -351,9 +397,9 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       }
     }
   } else {
-    // contact-free pair: optional outputs are zero; for the gather path the output rows too (the
-    // tensor-core path zero-fills them in the fused kernel)
-    if (!write_uhat) {
+    // contact-free pair: optional outputs are zero; for the fp32 gather kernel the output rows too
+    // (the tensor-core kernel zero-fills them itself)
+    if (fill_out) {
       for (int i = lane; i < n * 3; i += 32) io.out[row0 * 3 + i] = 0.0f;
       if (io.analytic_out)
         for (int i = lane; i < n * 3; i += 32) io.analytic_out[row0 * 3 + i] = 0.0f;
@@ -363,25 +409,25 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
   }
 }
 
-cudaError_t launch_sdf(const DevModel& m, const StepIO& io, bool write_uhat, cudaStream_t s) {
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s) {
   const unsigned grid = (unsigned)io.n_envs;
   // many small patches with indenters: one warp per (env, patch) pair; otherwise one CTA per environment
   if (io.input_mode == ETAC_IN_INDENTERS && m.max_ind >= 1 && m.n_patches >= 4 && m.max_patch_nodes <= 2048) {
     const int64_t pairs = (int64_t)io.n_envs * m.n_patches;
     const unsigned pgrid = (unsigned)((pairs + kPairWarps - 1) / kPairWarps);
     if (m.max_ind == 1) {
-      sdf_pairs_kernel<true><<<pgrid, kPairWarps * 32, 0, s>>>(m, io, write_uhat ? 1 : 0);
+      sdf_pairs_kernel<true><<<pgrid, kPairWarps * 32, 0, s>>>(m, io, s1_flags);
     } else {
       const size_t smem = sizeof(SInd) * (size_t)m.max_ind * kPairWarps;
-      sdf_pairs_kernel<false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, write_uhat ? 1 : 0);
+      sdf_pairs_kernel<false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
     }
     return cudaGetLastError();
   }
   if (io.input_mode == ETAC_IN_INDENTERS) {
     const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
-    sdf_penetration_kernel<true><<<grid, 256, smem, s>>>(m, io, write_uhat ? 1 : 0);
+    sdf_penetration_kernel<true><<<grid, 256, smem, s>>>(m, io, s1_flags);
   } else {
-    sdf_penetration_kernel<false><<<grid, 256, 0, s>>>(m, io, write_uhat ? 1 : 0);
+    sdf_penetration_kernel<false><<<grid, 256, 0, s>>>(m, io, s1_flags);
   }
   return cudaGetLastError();
 }

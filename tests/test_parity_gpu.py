@@ -43,10 +43,17 @@ def test_config3_bf16_dense_small(n_envs):
     assert gpu["pairs"] == int(ref["contact"].sum())
 
 
-def test_config3_sparse_path_matches_fp32_tolerance():
+def test_config3_sparse_paths():
+    """Omega U_a as a gather over the active nodes: the fp32 SIMT kernel of an fp32 context at the
+    fp32 tolerance, and the bf16-K / tensor-core-MLP form of a bf16 context at the bf16 tolerance."""
     wl = W.config3(2, 24)
+    ref = run_oracle(wl)
+    gpu = run_gpu(wl, path=T.ETAC_PATH_SPARSE, precision="fp32")
+    _report("cfg3 sparse fp32", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="cfg3-sparse"))
+    wl = W.config3(2, 97)          # several env tiles per patch + a ragged one
     gpu = run_gpu(wl, path=T.ETAC_PATH_SPARSE)
-    _report("cfg3 sparse", compare(gpu, run_oracle(wl), TOL["fp32"], resid_tol=1e-4, label="cfg3-sparse"))
+    assert gpu["path"] == T.ETAC_PATH_SPARSE and gpu["launches"] == 2
+    _report("cfg3 sparse bf16", compare(gpu, run_oracle(wl), TOL["bf16"], resid_tol=5e-2, label="cfg3-sparse16"))
 
 
 def test_config4_bf16_dense_small():
@@ -213,7 +220,8 @@ def test_many_patches_several_indenters(posed):
 @pytest.mark.parametrize("n_nodes,curved,frac", [(256, False, 0.05), (1024, True, 0.20), (1024, False, 0.01)])
 def test_config5_dense_and_sparse_paths(n_nodes, curved, frac):
     """BASELINE.json configs[4] sweep points at a size the oracle finishes in seconds: the bf16
-    context through the tensor-core path and through the gather path (fp32 arithmetic)."""
+    context through the tensor-core contraction and through the gather form, the fp32 context
+    through the fp32 gather kernel."""
     wl = W.config5(48, n_nodes, curved, frac, "bf16")
     ref = run_oracle(wl)
     assert ref["mask"].any()
@@ -222,7 +230,9 @@ def test_config5_dense_and_sparse_paths(n_nodes, curved, frac):
     _report(f"cfg5 N={n_nodes} dense", compare(dense, ref, TOL["bf16"], resid_tol=5e-2, label="cfg5-dense", delta_tol=1e-4))
     sparse = run_gpu(wl, path=T.ETAC_PATH_SPARSE)
     assert sparse["path"] == T.ETAC_PATH_SPARSE
-    _report(f"cfg5 N={n_nodes} sparse", compare(sparse, ref, TOL["fp32"], resid_tol=1e-4, label="cfg5-sparse", delta_tol=1e-4))
+    _report(f"cfg5 N={n_nodes} sparse bf16", compare(sparse, ref, TOL["bf16"], resid_tol=5e-2, label="cfg5-sparse16", delta_tol=1e-4))
+    sparse32 = run_gpu(wl, path=T.ETAC_PATH_SPARSE, precision="fp32")
+    _report(f"cfg5 N={n_nodes} sparse fp32", compare(sparse32, ref, TOL["fp32"], resid_tol=1e-4, label="cfg5-sparse32", delta_tol=1e-4))
 
 
 def test_full_size_config4_sampled():
