@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define ETAC_ABI_VERSION 1
+#define ETAC_ABI_VERSION 2
 
 typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
 
@@ -113,6 +113,10 @@ typedef struct {
   uint32_t* d_mask_out;               /* optional device [E x ceil(N/32)]: bit (i%32) of word i/32 = node i active */
   float* d_analytic_out;              /* optional device [E x N x 3]: unmasked K.U^ on ALL rows
                                          (the "linear decay only" term; test hook) */
+  uint8_t* d_contact_out;             /* optional device [E x P]: 1 = some node of the patch is active; with one
+                                         patch per link this is the link-contact vector S_cr of PAPER.md:L224 */
+  int32_t* d_active_count_out;        /* optional device [E]: n_a = number of active nodes of the environment
+                                         (contact ratio R_a = n_a / N) */
 } etac_step_args;
 
 /* Enqueues S1-S4 for n_envs environments on cuda_stream (a cudaStream_t; NULL = default stream).

@@ -143,6 +143,7 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
   io.out = a->d_out, io.pen_out = a->d_penetration_out, io.mask_out = a->d_mask_out;
   io.analytic_out = a->d_analytic_out;
+  io.contact_out = a->d_contact_out, io.nact_out = a->d_active_count_out;
 
   cudaError_t e;
   if (ev) cudaEventRecord(ev[0], s);
@@ -150,6 +151,8 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
     const size_t words = (size_t)((ctx->m.n_nodes + 31) / 32) * a->n_envs;
     if ((e = cudaMemsetAsync(io.mask_out, 0, words * 4, s)) != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset mask", e));
   }
+  if (io.nact_out && (e = cudaMemsetAsync(io.nact_out, 0, sizeof(int32_t) * a->n_envs, s)) != cudaSuccess)
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset active count", e));
   if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset count", e));
   // bf16 context: tensor-core MLP either way; DENSE = tcgen05 contraction K.U^, SPARSE = gather over the

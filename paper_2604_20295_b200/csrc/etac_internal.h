@@ -90,6 +90,8 @@ struct StepIO {
   float* pen_out;
   uint32_t* mask_out;
   float* analytic_out;
+  uint8_t* contact_out;
+  int32_t* nact_out;
 };
 
 // kernel launchers (each returns cudaGetLastError())

@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       const int64_t row0 = (int64_t)e * m.n_nodes + pi.off;
       float* delta = m.delta + row0;
       bool any = false;
+      int nact = 0;
       if constexpr (kIndenters) {
         const SPose& sp = s_pose[q];
         for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
@@ -198,15 +199,21 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           const float d = phi < 0.0f ? -phi : 0.0f;
           delta[i] = d;
           any |= d > 0.0f;
+          nact += d > 0.0f;
         }
       } else {
         for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
           const float d = fmaxf(io.pen_in[row0 + i], 0.0f);
           delta[i] = d;
           any |= d > 0.0f;
+          nact += d > 0.0f;
         }
       }
       if (__any_sync(0xffffffffu, any) && lane == 0) atomicOr(&s_any[q], 1);
+      if (io.nact_out) {
+        nact = __reduce_add_sync(0xffffffffu, nact);
+        if (lane == 0 && nact) atomicAdd(&io.nact_out[e], nact);
+      }
     }
     __syncthreads();
     // ---- phase D
@@ -214,6 +221,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       const int p = p0 + threadIdx.x;
       const int hit = s_any[threadIdx.x];
       m.flags[(int64_t)e * m.n_patches + p] = (uint8_t)hit;
+      if (io.contact_out) io.contact_out[(int64_t)e * m.n_patches + p] = (uint8_t)hit;
       if (hit) {
         const int slot = atomicAdd(&m.count[p], 1);
         m.envlist[(int64_t)p * m.max_envs + slot] = e;
@@ -336,6 +344,7 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
   // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
   const bool evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
   bool any = false;
+  int nact = 0;
   float* delta = m.delta + row0;
   if (evaluated) {
 #pragma unroll 2
@@ -349,12 +358,18 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       const float d = phi < 0.0f ? -phi : 0.0f;
       delta[i] = d;
       any |= d > 0.0f;
+      nact += d > 0.0f;
     }
     any = __any_sync(0xffffffffu, any);
+  }
+  if (io.nact_out && any) {
+    nact = __reduce_add_sync(0xffffffffu, nact);
+    if (lane == 0) atomicAdd(&io.nact_out[e], nact);
   }
   int slot = 0;
   if (lane == 0) {
     m.flags[pair] = (uint8_t)any;
+    if (io.contact_out) io.contact_out[pair] = (uint8_t)any;
     if (any) {
       slot = atomicAdd(&m.count[p], 1);
       m.envlist[(int64_t)p * m.max_envs + slot] = e;

@@ -52,7 +52,7 @@ class etac_step_args(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_envs", C.c_int32), ("input_mode", C.c_int32),
                 ("d_indenters", C.c_void_p), ("d_patch_pose", C.c_void_p), ("d_penetration", C.c_void_p),
                 ("d_out", C.c_void_p), ("d_penetration_out", C.c_void_p), ("d_mask_out", C.c_void_p),
-                ("d_analytic_out", C.c_void_p)]
+                ("d_analytic_out", C.c_void_p), ("d_contact_out", C.c_void_p), ("d_active_count_out", C.c_void_p)]
 
 
 _lib = None
@@ -146,7 +146,7 @@ def etac_destroy(ctx) -> None:
 
 
 def make_step_args(n_envs, out, *, indenters=None, patch_pose=None, penetration=None, penetration_out=None,
-                   mask_out=None, analytic_out=None) -> etac_step_args:
+                   mask_out=None, analytic_out=None, contact_out=None, active_count_out=None) -> etac_step_args:
     a = etac_step_args()
     a.struct_size = C.sizeof(etac_step_args)
     a.n_envs = n_envs
@@ -154,6 +154,7 @@ def make_step_args(n_envs, out, *, indenters=None, patch_pose=None, penetration=
     a.d_indenters, a.d_patch_pose, a.d_penetration = _dptr(indenters), _dptr(patch_pose), _dptr(penetration)
     a.d_out, a.d_penetration_out = _dptr(out), _dptr(penetration_out)
     a.d_mask_out, a.d_analytic_out = _dptr(mask_out), _dptr(analytic_out)
+    a.d_contact_out, a.d_active_count_out = _dptr(contact_out), _dptr(active_count_out)
     return a
 
 
@@ -226,6 +227,8 @@ class Etac:
             self.pen_out = torch.empty((E, self.N), dtype=torch.float32, device=self.device)
             self.mask_out = torch.empty((E, (self.N + 31) // 32), dtype=torch.int32, device=self.device)
             self.analytic = torch.empty((E, self.N, 3), dtype=torch.float32, device=self.device)
+            self.contact = torch.empty((E, self.P), dtype=torch.uint8, device=self.device)
+            self.active_count = torch.empty((E,), dtype=torch.int32, device=self.device)
 
     def upload(self, indenters=None, patch_pose=None, penetration=None):
         t = self.torch
@@ -241,7 +244,8 @@ class Etac:
     def args(self, n_envs, dev):
         kw = dict(dev)
         if self.debug:
-            kw.update(penetration_out=self.pen_out, mask_out=self.mask_out, analytic_out=self.analytic)
+            kw.update(penetration_out=self.pen_out, mask_out=self.mask_out, analytic_out=self.analytic,
+                      contact_out=self.contact, active_count_out=self.active_count)
         return make_step_args(n_envs, self.out, **kw)
 
     def step(self, n_envs, dev):

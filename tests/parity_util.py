@@ -25,11 +25,13 @@ def run_gpu(wl, *, precision=None, path=T.ETAC_PATH_AUTO, resid=True, active_mod
             dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
         # poison the outputs: every element must be overwritten by the step
         eng.out.fill_(float("nan")), eng.analytic.fill_(float("nan")), eng.pen_out.fill_(float("nan"))
+        eng.contact.fill_(77), eng.active_count.fill_(-5)
         for _ in range(steps):
             eng.step(n_envs, dev)
         torch.cuda.synchronize()
         res = {"U": eng.out[:n_envs].cpu().numpy(), "analytic": eng.analytic[:n_envs].cpu().numpy(),
                "delta": eng.pen_out[:n_envs].cpu().numpy(), "mask": eng.mask_bool(n_envs),
+               "contact": eng.contact[:n_envs].cpu().numpy(), "active_count": eng.active_count[:n_envs].cpu().numpy(),
                "pairs": T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_CONTACT_PAIRS),
                "path": T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_PATH),
                "launches": T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_LAUNCHES)}
@@ -55,6 +57,9 @@ def compare(gpu, ref, tol, envs=None, resid_tol=None, label="", delta_tol=1e-5):
     # decisions: bit-exact (taken in fp32 on both sides)
     assert np.array_equal(M, ref["mask"]), f"{label}: mask differs at {np.argwhere(M != ref['mask'])[:5]}"
     assert np.array_equal(D, ref["delta32"]), f"{label}: delta not bit-exact vs the fp32 twin"
+    # link-contact vector and active-node count: integer work, bit-exact
+    assert np.array_equal(gpu["contact"][sel].astype(bool), ref["contact"]), f"{label}: contact vector differs"
+    assert np.array_equal(gpu["active_count"][sel], ref["mask"].sum(1)), f"{label}: active-node count differs"
     scale_d = max(1.0, float(np.abs(ref["delta"]).max()))
     assert np.abs(D - ref["delta"]).max() <= delta_tol * scale_d
     umax = float(np.abs(ref["U"]).max())
