@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define ETAC_ABI_VERSION 2
+#define ETAC_ABI_VERSION 3
 
 typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
 
@@ -59,7 +59,7 @@ typedef struct {
 } etac_indenter; /* 48 bytes */
 
 enum { ETAC_KERNEL_EXP_L2 = 0 };                                  /* Eq. (1): exp(-alpha*|p_j-p_i|_2) */
-enum { ETAC_RESID_NONE = 0, ETAC_RESID_PERNODE_MLP = 1, ETAC_RESID_POINTNET = 2 /* not built: UNSUPPORTED */ };
+enum { ETAC_RESID_NONE = 0, ETAC_RESID_PERNODE_MLP = 1, ETAC_RESID_POINTNET = 2 /* ETAC_PREC_BF16 contexts only */ };
 enum { ETAC_PREC_FP32 = 0, ETAC_PREC_BF16 = 1 };                  /* BF16: 16-bit tensor-core operands, fp32 accumulate */
 enum { ETAC_ACTIVE_PASSTHROUGH = 0, ETAC_ACTIVE_PROPAGATE = 1 };  /* PASSTHROUGH: active rows keep u^ (mask M_p, L99) */
 enum { ETAC_IN_INDENTERS = 0, ETAC_IN_PENETRATION = 1 };
@@ -84,6 +84,13 @@ typedef struct {
   const float *W1, *b1, *W2, *b2, *W3, *b3; /* host, Linear-layer layout [out x in]:
                                   W1[64x9] (input order [u_lin(3), p(3), n(3)]) b1[64] W2[64x64] b2[64] W3[3x64] b3[3];
                                   may be NULL when resid_arch == ETAC_RESID_NONE */
+  const float *E1, *e1, *E2, *e2, *G1, *g1, *D1, *d1, *D2, *d2; /* host, ETAC_RESID_POINTNET (the paper's form of
+                                  Phi; widths are this library's reading, Fig. 3 is an image):
+                                  per node f_i = silu(E2 silu(E1 [p,n,u^] + e1) + e2), E1[64x9] (input order
+                                  [p(3), n(3), u^(3)], L93) e1[64] E2[64x64] e2[64]; per (env, patch)
+                                  g = max_i f_i over all nodes of the patch, g' = silu(G1 g + g1), G1[64x64] g1[64];
+                                  r_i = D2 silu(D1 [f_i; g'] + d1) + d2, D1[64x128] d1[64] D2[3x64] d2[3];
+                                  may be NULL for the other forms */
   int32_t max_envs;            /* workspace sizing, >= 1 */
   int32_t max_indenters;       /* M >= 0: indenter slots per environment */
   int32_t precision;           /* ETAC_PREC_* */

@@ -166,8 +166,10 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   ++ctx->last_launches;
   if (ev) cudaEventRecord(ev[1], s);
   if (bf16) {
-    if ((e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, s)) != cudaSuccess)
+    int n_launch = 1;
+    if ((e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s)) != cudaSuccess)
       return fail(ctx, ETAC_ERR_CUDA, cuda_msg("dense_bf16_kernel", e));
+    ctx->last_launches += n_launch - 1;
   } else {
     if ((e = launch_gather_fp32(ctx->m, io, s)) != cudaSuccess)
       return fail(ctx, ETAC_ERR_CUDA, cuda_msg("gather_fp32_kernel", e));
@@ -232,9 +234,14 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   if (d->precision != ETAC_PREC_FP32 && d->precision != ETAC_PREC_BF16) return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad precision");
   if (d->active_mode != ETAC_ACTIVE_PASSTHROUGH && d->active_mode != ETAC_ACTIVE_PROPAGATE)
     return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad active_mode");
-  if (d->resid_arch == ETAC_RESID_POINTNET) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "ETAC_RESID_POINTNET is not built");
-  if (d->resid_arch != ETAC_RESID_NONE && d->resid_arch != ETAC_RESID_PERNODE_MLP)
+  if (d->resid_arch != ETAC_RESID_NONE && d->resid_arch != ETAC_RESID_PERNODE_MLP && d->resid_arch != ETAC_RESID_POINTNET)
     return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad resid_arch");
+  if (d->resid_arch == ETAC_RESID_POINTNET) {
+    if (d->precision != ETAC_PREC_BF16) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "ETAC_RESID_POINTNET needs an ETAC_PREC_BF16 context");
+    if (d->resid_hidden != kHidden) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "only resid_hidden == 64 is built");
+    if (!d->E1 || !d->e1 || !d->E2 || !d->e2 || !d->G1 || !d->g1 || !d->D1 || !d->d1 || !d->D2 || !d->d2)
+      return fail(nullptr, ETAC_ERR_INVALID_ARG, "PointNet weights missing");
+  }
   if (d->resid_arch == ETAC_RESID_PERNODE_MLP) {
     if (d->resid_hidden != kHidden) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "only resid_hidden == 64 is built");
     if (!d->W1 || !d->b1 || !d->W2 || !d->b2 || !d->W3 || !d->b3) return fail(nullptr, ETAC_ERR_INVALID_ARG, "MLP weights missing");
@@ -391,6 +398,41 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
       put(kW1ImgBytes + kW2ImgBytes, n, 64, 16, d->b3[n]);
     }
     CK(dev_upload(c, &m.wimg, img.data(), img.size()), "upload weight image");
+  }
+
+  if (d->resid_arch == ETAC_RESID_POINTNET) {
+    // bf16 shared-memory image; the 0.5 of silu(x) = h + h*tanh(h), h = x/2, is folded into every layer
+    // that feeds a SiLU.  Layer-1 operand columns are [u^(3), p(3), n(3), 1]; E1's inputs are [p, n, u^].
+    std::vector<uint8_t> img(kPnImgBytes, 0);
+    auto put = [&](size_t base, int n, int k, int rows, float v) {
+      const uint16_t b = f2bf(v);
+      memcpy(&img[base + wimg_off(n, k, rows)], &b, 2);
+    };
+    const size_t o1 = kW1ImgBytes, o2 = o1 + kW2ImgBytes, o3 = o2 + kW2ImgBytes;
+    for (int n = 0; n < 64; ++n) {
+      for (int k = 0; k < 3; ++k) {
+        put(0, n, k, 64, 0.5f * d->E1[n * 9 + 6 + k]);      // u^
+        put(0, n, 3 + k, 64, 0.5f * d->E1[n * 9 + k]);      // p
+        put(0, n, 6 + k, 64, 0.5f * d->E1[n * 9 + 3 + k]);  // n
+      }
+      put(0, n, 9, 64, 0.5f * d->e1[n]);
+      for (int k = 0; k < 64; ++k) put(o1, n, k, 64, 0.5f * d->E2[n * 64 + k]);
+      put(o1, n, 64, 64, 0.5f * d->e2[n]);
+      for (int k = 0; k < 64; ++k) put(o2, n, k, 64, 0.5f * d->D1[n * 128 + k]);  // bias column stays 0: c_(e,p) is added in the epilogue
+    }
+    for (int n = 0; n < 3; ++n) {
+      for (int k = 0; k < 64; ++k) put(o3, n, k, 16, d->D2[n * 64 + k]);
+      put(o3, n, 64, 16, d->d2[n]);
+    }
+    CK(dev_upload(c, &m.wimg_pn, img.data(), img.size()), "upload PointNet weight image");
+    std::vector<float> pf(4096 + 64 + 4096 + 64);
+    memcpy(pf.data(), d->G1, 4096 * 4);
+    memcpy(pf.data() + 4096, d->g1, 64 * 4);
+    for (int n = 0; n < 64; ++n) memcpy(pf.data() + 4160 + n * 64, d->D1 + n * 128 + 64, 64 * 4);
+    memcpy(pf.data() + 4160 + 4096, d->d1, 64 * 4);
+    CK(dev_upload(c, &m.pn_f32, pf.data(), pf.size()), "upload PointNet global MLP");
+    CK(dev_alloc(c, &m.gmax, (size_t)64 * P * d->max_envs, true), "alloc gmax");
+    CK(dev_alloc(c, &m.cvec, (size_t)64 * P * d->max_envs, true), "alloc cvec");
   }
 
   // ---- per-step workspace

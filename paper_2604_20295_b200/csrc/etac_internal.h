@@ -43,6 +43,8 @@ constexpr int kW1ImgBytes = 64 * 16 * 2;   // N=64,  K=16   (9 inputs + bias col
 constexpr int kW2ImgBytes = 64 * 80 * 2;   // N=64,  K=80   (64 + bias column, padded to 5 k-steps)
 constexpr int kW3ImgBytes = 16 * 80 * 2;   // N=16,  K=80   (3 outputs padded to 16)
 constexpr int kWImgBytes = kW1ImgBytes + kW2ImgBytes + kW3ImgBytes;
+// PointNet form: E1 [64 x 16] | E2 [64 x 80] | D1[:, 0:64] [64 x 80, zero bias column] | D2 [16 x 80]
+constexpr int kPnImgBytes = kW1ImgBytes + 2 * kW2ImgBytes + kW3ImgBytes;
 
 // Active node of a contacting (env, patch) pair, for the gather form of the propagation:
 // u^ of the node (fp32) and its index within the patch.
@@ -70,6 +72,10 @@ struct DevModel {
   const float* wf32;          // fp32 weights blob: W1u[64x3] | c1t[64 x N] is separate | W2[64x64] b2[64] W3[3x64] b3[3]
   const float* c1t;           // [64 x N]: W1[:,3:9].[p;n] + b1, transposed for coalescing
   const uint8_t* wimg;        // kWImgBytes
+  const uint8_t* wimg_pn;     // kPnImgBytes (ETAC_RESID_POINTNET)
+  const float* pn_f32;        // G1[64x64] g1[64] D1[:,64:128] as [64x64] d1[64] (fp32, pn_global_kernel)
+  uint32_t* gmax;             // [P x max_envs x 64] max-pooled encoder features as order-preserving keys
+  float* cvec;                // [P x max_envs x 64] c_(e,p) / 2
   // per-step workspace
   float* delta;               // [max_envs x N]
   __nv_bfloat16* uhat_t;      // [3*max_envs (+pad) x ldu]: row slot*3+c, column = node j
@@ -100,7 +106,7 @@ cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1,
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s);
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                              int n_sm, bool gather, cudaStream_t s);
+                              int n_sm, bool gather, int* launches, cudaStream_t s);
 cudaError_t dense_bf16_configure();
 
 }  // namespace etac

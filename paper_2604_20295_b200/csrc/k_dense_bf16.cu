@@ -30,7 +30,7 @@
 
 namespace etac {
 
-constexpr int BM = 128, BK = 64, TE = kDenseTE, BN = kDenseBN, STAGES = 4;
+constexpr int BM = 128, BK = 64, TE = kDenseTE, BN = kDenseBN, STAGES = 4;  // STAGES: upper bound (barrier arrays)
 constexpr int A_STAGE = BM * BK * 2, B_STAGE = BN * BK * 2;
 constexpr int kDenseThreads = 384;
 // setmaxnreg moves registers inside the CTA's launch-time allocation: 12 warps x 80 registers
@@ -46,8 +46,21 @@ struct __align__(8) DenseBars {
   uint32_t pad;
 };
 
-__host__ __device__ constexpr size_t dense_smem_bytes(int n_patches) {
-  return 1024 /*align slack*/ + (size_t)STAGES * (A_STAGE + B_STAGE) + kWImgBytes + sizeof(DenseBars) +
+// Residual variants of the fused kernel (template parameter kMode).  The PointNet form of Phi
+// needs the max-pool over all nodes of a patch before any node can be decoded,
+// so it runs as two passes of this kernel with a tiny per-(env, patch) kernel in between:
+//   kModePnEncode: [u^, p, n] -> E1 -> SiLU -> E2 -> SiLU = f_i, column max over the rows -> gmax
+//   kModePnDecode: propagation as usual; f_i again; D1[:, :64] f_i + c_(e,p) -> SiLU -> D2 -> r
+// where c_(e,p) = D1[:, 64:] silu(G1 g + g1) + d1 comes from pn_global_kernel.
+constexpr int kModeNone = 0, kModePerNode = 1, kModePnEncode = 2, kModePnDecode = 3;
+__host__ __device__ constexpr int mode_layers(int mode) { return mode == 1 ? 3 : mode == 2 ? 2 : mode == 3 ? 4 : 0; }
+__host__ __device__ constexpr int mode_stages(int mode) { return mode == 3 ? 3 : 4; }  // shared memory: 2 CTAs per SM
+__host__ __device__ constexpr int mode_img_bytes(int mode) {
+  return mode == 1 ? kWImgBytes : mode == 2 ? kW1ImgBytes + kW2ImgBytes : mode == 3 ? kPnImgBytes : 0;
+}
+
+__host__ __device__ constexpr size_t dense_smem_bytes(int n_patches, int mode) {
+  return 1024 /*align slack*/ + (size_t)mode_stages(mode) * (A_STAGE + B_STAGE) + mode_img_bytes(mode) + sizeof(DenseBars) +
          (size_t)(n_patches + 1) * 4 + 16 + 16 + 8 * 32 * 16;
 }
 
@@ -137,23 +150,28 @@ __device__ long long g_prof[320 * 8 * 12];
 // read from the compact lists S1 wrote (bf16 K row j, coalesced over i because K is symmetric;
 // fp32 u^ and accumulation).  No TMA, no propagation MMA; the MLP part is unchanged.  It wins
 // when few nodes are in contact (ETAC_PATH_SPARSE on a bf16 context).
-template <bool kResid, bool kGather>
+template <int kMode, bool kGather>
 __global__ void __launch_bounds__(kDenseThreads, 2)
     dense_bf16_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
                       const __grid_constant__ CUtensorMap tmB) {
+  constexpr bool kResid = kMode != kModeNone;
+  constexpr bool kPn = kMode == kModePnEncode || kMode == kModePnDecode;
+  constexpr bool kProp = !kGather && kMode != kModePnEncode;  // TMA + propagation GEMM run
+  constexpr bool kFill = kMode != kModePnEncode;              // the decode pass zero-fills
+  constexpr int kLayers = mode_layers(kMode), kStages = mode_stages(kMode), kImgBytes = mode_img_bytes(kMode);
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sA = smem;
-  uint8_t* sB = smem + STAGES * A_STAGE;
-  uint8_t* sW = sB + STAGES * B_STAGE;
-  DenseBars* bars = reinterpret_cast<DenseBars*>(sW + kWImgBytes);
+  uint8_t* sB = smem + kStages * A_STAGE;
+  uint8_t* sW = sB + kStages * B_STAGE;
+  DenseBars* bars = reinterpret_cast<DenseBars*>(sW + kImgBytes);
   int* prefix = reinterpret_cast<int*>(bars + 1);
   uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + (m.n_patches + 1)) + 15) & ~uintptr_t(15));  // 8 warps x 32 entries
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
+    for (int s = 0; s < kStages; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
     mbar_init(&bars->acc_full, 1);
     mbar_init(&bars->acc_empty, 8);
     for (int s = 0; s < 2; ++s) mbar_init(&bars->a_ready[s], 4), mbar_init(&bars->d_ready[s], 1);
@@ -170,9 +188,9 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   }
   if (warp == 1) tmem_alloc<kTmemCols>(&bars->tmem_base);
   if constexpr (kResid) {
-    const uint4* src = reinterpret_cast<const uint4*>(m.wimg);
+    const uint4* src = reinterpret_cast<const uint4*>(kPn ? m.wimg_pn : m.wimg);
     uint4* dst = reinterpret_cast<uint4*>(sW);
-    for (int k = threadIdx.x; k < kWImgBytes / 16; k += kDenseThreads) dst[k] = src[k];
+    for (int k = threadIdx.x; k < kImgBytes / 16; k += kDenseThreads) dst[k] = src[k];
     fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor-core (async) proxy
   }
   tc_fence_before();
@@ -182,7 +200,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
 
   if (warp == 0) {
     reg_dealloc<kRegsCtrl>();
-    if constexpr (!kGather)
+    if constexpr (kProp)
     // ------------------------------------------------------------------ TMA producer
     // (the whole warp runs the loop so that every operand stays warp-uniform; one elected lane issues)
     {
@@ -200,13 +218,13 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
             tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], pi.off + kb * BK, it.tile * BN);
           }
           __syncwarp();
-          if (++stage == STAGES) stage = 0, ph ^= 1;
+          if (++stage == kStages) stage = 0, ph ^= 1;
         }
       }
     }
   } else if (warp == 1) {
     reg_dealloc<kRegsCtrl>();
-    if constexpr (!kGather)
+    if constexpr (kProp)
     // ------------------------------------------------------------------ MMA issuer
     // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are issued by one elected lane.
     {
@@ -237,7 +255,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
             if (kb == nkb - 1) tc_commit(&bars->acc_full);
           }
           __syncwarp();
-          if (++stage == STAGES) stage = 0, ph ^= 1;
+          if (++stage == kStages) stage = 0, ph ^= 1;
         }
       }
     }
@@ -257,6 +275,8 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       const uint64_t dW1 = make_desc(smem_u32(sW), 1024, 128, kLayoutNone);
       const uint64_t dW2 = make_desc(smem_u32(sW + kW1ImgBytes), 1024, 128, kLayoutNone);
       const uint64_t dW3 = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 256, 128, kLayoutNone);
+      const uint64_t dW3h = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 1024, 128, kLayoutNone);
+      const uint64_t dW4 = make_desc(smem_u32(sW + kW1ImgBytes + 2 * kW2ImgBytes), 256, 128, kLayoutNone);
       const uint32_t tD = tmem + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
       uint64_t* a_ready = &bars->a_ready[sl];
       uint64_t* d_ready = &bars->d_ready[sl];
@@ -266,33 +286,34 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
         for (int el = sl; el < it.cnt; el += 2) {
 #pragma unroll 1
-          for (int layer = 0; layer < 3; ++layer) {
+          for (int layer = 0; layer < kLayers; ++layer) {
             mbar_wait(a_ready, a_ph), a_ph ^= 1;
             tc_fence_after();
             if (elect_one()) {
+              // weight image: [64 x 16] | [64 x 80] | per-node: [16 x 80]; PointNet: [64 x 80] | [16 x 80]
               if (layer == 0) {
                 mma_ts(tD, tA, dW1, idesc_h, 0);
-              } else if (layer == 1) {
+              } else if (layer == kLayers - 1 && kMode != kModePnEncode) {
+                const uint64_t dWo = kMode == kModePnDecode ? dW4 : dW3;
 #pragma unroll
-                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW2 + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
+                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dWo + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
               } else {
+                const uint64_t dWh = layer == 1 ? dW2 : dW3h;
 #pragma unroll
-                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dW3 + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
+                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dWh + (uint64_t)(k * (2048 >> 4)), idesc_h, k != 0);
               }
               tc_commit(d_ready);
             }
             __syncwarp();
-#ifndef ETAC_NOFILL
-            zf.step(m, io, lane);
-#endif
+            if constexpr (kFill) zf.step(m, io, lane);
           }
         }
       }
     }
-#ifndef ETAC_NOFILL
-    while (zf.step(m, io, lane)) {
+    if constexpr (kFill) {
+      while (zf.step(m, io, lane)) {
+      }
     }
-#endif
   } else {
     reg_alloc<kRegsEpi>();
     // ------------------------------------------------------------------ epilogue (thread = node)
@@ -336,7 +357,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       // lane l prefetches the id of the item's l-th environment (broadcast by shuffle below)
       const int my_env = lane < it.cnt ? m.envlist[(int64_t)it.p * m.max_envs + it.tile * TE + lane] : 0;
       PROF_MARK(0);  // item setup
-      if constexpr (!kGather) {
+      if constexpr (kProp) {
         mbar_wait(&bars->acc_full, acc_ph), acc_ph ^= 1;
         tc_fence_after();
       }
@@ -349,13 +370,17 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       struct Unit {
         int64_t node;
         float ux, uy, uz, dl;
+        int slot;  // position of the unit's environment in the patch's contact list
       };
       auto fetch_unit = [&](Unit& u, const int el, uint32_t (&ur)[4]) {  // requests only; tc_wait_ld() follows
         const int env = __shfl_sync(0xffffffffu, my_env, el);
         u.node = (int64_t)env * m.n_nodes + g;
         u.dl = valid ? m.delta[u.node] : 0.0f;  // consumed when the unit is stored
-        if constexpr (!kGather) {
+        u.slot = it.tile * TE + el;
+        if constexpr (kProp) {
           tmem_ld4(trow + COL_ACC + 3 * el, ur);
+        } else if constexpr (kMode == kModePnEncode) {
+          ur[0] = ur[1] = ur[2] = ur[3] = 0;  // the encoder pass has no propagation
         } else {
           // Omega U_a: sum over the active nodes of this (env, patch); entry loads are warp-uniform
           // (broadcast), K row j is read coalesced over the rows i of the warp
@@ -393,8 +418,13 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       auto request_layer1 = [&](Unit& u, const uint32_t (&ur)[4]) {
         u.ux = __uint_as_float(ur[0]), u.uy = __uint_as_float(ur[1]), u.uz = __uint_as_float(ur[2]);
         if constexpr (kResid) {
-          a1[0] = pack_bf16(u.ux, u.uy);
-          a1[1] = pack_bf16(u.uz, px);
+          if constexpr (kPn) {  // PointNet encoder input: u^ = -delta n of the node itself
+            a1[0] = pack_bf16(-u.dl * nrm.x, -u.dl * nrm.y);
+            a1[1] = pack_bf16(-u.dl * nrm.z, px);
+          } else {
+            a1[0] = pack_bf16(u.ux, u.uy);
+            a1[1] = pack_bf16(u.uz, px);
+          }
           tmem_st8(tA, a1);
           tc_wait_st();
           tc_fence_before();
@@ -405,7 +435,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       // the accumulator is released as soon as this warp has fetched its LAST u_lin of the item, a
       // whole unit before the item ends: the next item's propagation GEMM runs behind that unit's MLP
       auto release_acc = [&]() {
-        if constexpr (!kGather) {
+        if constexpr (kProp) {
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(&bars->acc_empty);
@@ -429,44 +459,84 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         float rx = 0.f, ry = 0.f, rz = 0.f;
         uint32_t un[4] = {0, 0, 0, 0};
         if constexpr (kResid) {
+          // SiLU granules after every layer but the last; the decoder's layer 2 adds the
+          // per-(env, patch) vector c (halved like the weights), the encoder's layer 1 is max-pooled
+          const float4* cv = nullptr;
+          if constexpr (kMode == kModePnDecode)
+            cv = reinterpret_cast<const float4*>(m.cvec + ((int64_t)it.p * m.max_envs + cur.slot) * 64);
+          uint32_t pool0 = 0, pool1 = 0;  // lane l: max keys of hidden columns l and 32 + l
+          constexpr int kGranules = kMode == kModePnEncode ? kLayers : kLayers - 1;  // layers followed by a SiLU
 #pragma unroll 1
-          for (int layer = 0; layer < 2; ++layer) {
+          for (int layer = 0; layer < kGranules; ++layer) {
             mbar_wait(d_ready, d_ph), d_ph ^= 1;
             tc_fence_after();
-            PROF_MARK(4);  // d_ready wait (layers 1, 2)
+            PROF_MARK(4);  // d_ready wait
             // both halves are requested at once: one TMEM load latency per layer instead of two
             uint32_t ha[32], hb[32], packed[16];
             tmem_ld32(tD, ha);
             tmem_ld32(tD + 32, hb);
             tc_wait_ld();
+            const bool add_c = kMode == kModePnDecode && layer == 2;
+            const bool pool = kMode == kModePnEncode && layer == 1;
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
-              // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
-              const float h0 = __uint_as_float(ha[2 * k]), h1 = __uint_as_float(ha[2 * k + 1]);
-              packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
-            }
-            tmem_st16(tA, packed);
+            for (int half = 0; half < 2; ++half) {
+              uint32_t(&h)[32] = half ? hb : ha;
+              if (add_c) {
 #pragma unroll
-            for (int k = 0; k < 16; ++k) {
-              const float h0 = __uint_as_float(hb[2 * k]), h1 = __uint_as_float(hb[2 * k + 1]);
-              packed[k] = pack_bf16(fmaf(h0, tanh_approx(h0), h0), fmaf(h1, tanh_approx(h1), h1));
+                for (int k = 0; k < 8; ++k) {
+                  const float4 c4 = __ldg(cv + half * 8 + k);
+                  h[4 * k] = __float_as_uint(__uint_as_float(h[4 * k]) + c4.x);
+                  h[4 * k + 1] = __float_as_uint(__uint_as_float(h[4 * k + 1]) + c4.y);
+                  h[4 * k + 2] = __float_as_uint(__uint_as_float(h[4 * k + 2]) + c4.z);
+                  h[4 * k + 3] = __float_as_uint(__uint_as_float(h[4 * k + 3]) + c4.w);
+                }
+              }
+#pragma unroll
+              for (int k = 0; k < 16; ++k) {
+                // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
+                const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
+                const float y0 = fmaf(h0, tanh_approx(h0), h0), y1 = fmaf(h1, tanh_approx(h1), h1);
+                packed[k] = pack_bf16(y0, y1);
+                if constexpr (kMode == kModePnEncode) {
+                  if (pool) {  // column max over the warp's 32 rows; order-preserving uint keys, 0 = no row
+                    const uint32_t b0 = __float_as_uint(y0), b1 = __float_as_uint(y1);
+                    const uint32_t k0 = valid ? (b0 ^ ((b0 >> 31) ? 0xffffffffu : 0x80000000u)) : 0u;
+                    const uint32_t k1 = valid ? (b1 ^ ((b1 >> 31) ? 0xffffffffu : 0x80000000u)) : 0u;
+                    const uint32_t m0 = __reduce_max_sync(0xffffffffu, k0), m1 = __reduce_max_sync(0xffffffffu, k1);
+                    if (lane == ((2 * k) & 31)) (half ? pool1 : pool0) = m0;
+                    if (lane == ((2 * k + 1) & 31)) (half ? pool1 : pool0) = m1;
+                  }
+                }
+              }
+              if (!pool) tmem_st16(tA + 16 * half, packed);
             }
-            tmem_st16(tA + 16, packed);
             PROF_MARK(6);  // D load + SiLU + operand stores issued
-            tc_wait_st();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(a_ready);
+            if (!pool) {
+              tc_wait_st();
+              tc_fence_before();
+              __syncwarp();
+              if (lane == 0) mbar_arrive(a_ready);
+            }
             PROF_MARK(7);  // store wait + arrive
           }
-          if (more) fetch_unit(nxt, el + 2, un);  // overlaps the layer-3 round trip
-          mbar_wait(d_ready, d_ph), d_ph ^= 1;
-          tc_fence_after();
-          PROF_MARK(8);  // d_ready wait (layer 3)
-          uint32_t rr[4];
-          tmem_ld4(tD, rr);
-          tc_wait_ld();
-          rx = __uint_as_float(rr[0]), ry = __uint_as_float(rr[1]), rz = __uint_as_float(rr[2]);
+          if constexpr (kMode == kModePnEncode) {
+            uint32_t* gm = m.gmax + ((int64_t)it.p * m.max_envs + cur.slot) * 64;
+            atomicMax(gm + lane, pool0);
+            atomicMax(gm + 32 + lane, pool1);
+            if (more) {
+              fetch_unit(nxt, el + 2, un);
+              tc_wait_ld();
+            }
+          } else {
+            if (more) fetch_unit(nxt, el + 2, un);  // overlaps the last layer's round trip
+            mbar_wait(d_ready, d_ph), d_ph ^= 1;
+            tc_fence_after();
+            PROF_MARK(8);  // d_ready wait (last layer)
+            uint32_t rr[4];
+            tmem_ld4(tD, rr);
+            tc_wait_ld();
+            rx = __uint_as_float(rr[0]), ry = __uint_as_float(rr[1]), rz = __uint_as_float(rr[2]);
+          }
           PROF_MARK(9);  // r (and next u_lin) load
         } else {
           if (more) {
@@ -477,7 +547,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         if (more && el + 4 >= it.cnt) release_acc();
         if (more) request_layer1(nxt, un);  // layer 3 has been read: the operand region is free
         PROF_MARK(3);  // next unit's layer-1 operand + arrive
-        if (valid) {  // S4: mask M_p + combine (Eq. 2); active rows keep u^ = -delta n in fp32
+        if (valid && kMode != kModePnEncode) {  // S4: mask M_p + combine (Eq. 2); active rows keep u^ = -delta n in fp32
           float ox = cur.ux + rx, oy = cur.uy + ry, oz = cur.uz + rz;
           if (cur.dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH)
             ox = -cur.dl * nrm.x, oy = -cur.dl * nrm.y, oz = -cur.dl * nrm.z;
@@ -506,24 +576,68 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   }
 }
 
+// c_(e,p) of the PointNet decoder: g = max-pooled features (keys -> floats), g' = silu(G1 g + g1)
+// ("further encoded by another MLP"), c = D1[:, 64:128] g' + d1, stored halved like
+// the decoder weights.  One 64-thread CTA per contacting (patch, slot).
+__global__ void __launch_bounds__(64) pn_global_kernel(DevModel m) {
+  const int p = blockIdx.y, slot = blockIdx.x, k = threadIdx.x;
+  if (slot >= m.count[p]) return;
+  __shared__ float g[64], g2[64];
+  const int64_t base = ((int64_t)p * m.max_envs + slot) * 64;
+  const uint32_t key = m.gmax[base + k];
+  const uint32_t bits = (key >> 31) ? (key ^ 0x80000000u) : ~key;
+  g[k] = __uint_as_float(bits);
+  __syncthreads();
+  const float* G1 = m.pn_f32, *g1 = G1 + 4096, *D1g = g1 + 64, *d1 = D1g + 4096;
+  float a = g1[k];
+  for (int j = 0; j < 64; ++j) a = fmaf(G1[k * 64 + j], g[j], a);
+  g2[k] = a / (1.0f + expf(-a));
+  __syncthreads();
+  float c = d1[k];
+  for (int j = 0; j < 64; ++j) c = fmaf(D1g[k * 64 + j], g2[j], c);
+  m.cvec[base + k] = 0.5f * c;
+}
+
+template <int kMode, bool kGather>
+static cudaError_t configure_one() {
+  return cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)dense_smem_bytes(kMaxPatches, kMode));
+}
+
 cudaError_t dense_bf16_configure() {
-  const int bytes = (int)dense_smem_bytes(kMaxPatches);
-  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaError_t e = configure_one<kModeNone, false>();
+  if (e == cudaSuccess) e = configure_one<kModeNone, true>();
+  if (e == cudaSuccess) e = configure_one<kModePerNode, false>();
+  if (e == cudaSuccess) e = configure_one<kModePerNode, true>();
+  if (e == cudaSuccess) e = configure_one<kModePnEncode, false>();
+  if (e == cudaSuccess) e = configure_one<kModePnDecode, false>();
+  if (e == cudaSuccess) e = configure_one<kModePnDecode, true>();
   return e;
 }
 
+template <int kMode, bool kGather>
+static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int grid,
+                       cudaStream_t s) {
+  dense_bf16_kernel<kMode, kGather><<<grid, kDenseThreads, dense_smem_bytes(m.n_patches, kMode), s>>>(m, io, tmA, tmB);
+}
+
+// Launches S2-S4 for the context's residual form; *launches receives the number of kernels.
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                              int n_sm, bool gather, cudaStream_t s) {
-  const size_t smem = dense_smem_bytes(m.n_patches);
+                              int n_sm, bool gather, int* launches, cudaStream_t s) {
   const int grid = 2 * n_sm;
-  const bool resid = m.resid != ETAC_RESID_NONE;
-  if (resid && !gather) dense_bf16_kernel<true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-  if (!resid && !gather) dense_bf16_kernel<false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-  if (resid && gather) dense_bf16_kernel<true, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-  if (!resid && gather) dense_bf16_kernel<false, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  *launches = 1;
+  if (m.resid == ETAC_RESID_NONE) {
+    gather ? launch_one<kModeNone, true>(m, io, tmA, tmB, grid, s) : launch_one<kModeNone, false>(m, io, tmA, tmB, grid, s);
+  } else if (m.resid == ETAC_RESID_PERNODE_MLP) {
+    gather ? launch_one<kModePerNode, true>(m, io, tmA, tmB, grid, s) : launch_one<kModePerNode, false>(m, io, tmA, tmB, grid, s);
+  } else {  // ETAC_RESID_POINTNET: encode + max-pool, per-(env, patch) vector, decode
+    cudaError_t e = cudaMemsetAsync(m.gmax, 0, sizeof(uint32_t) * 64 * (size_t)m.n_patches * m.max_envs, s);
+    if (e != cudaSuccess) return e;
+    launch_one<kModePnEncode, false>(m, io, tmA, tmB, grid, s);
+    pn_global_kernel<<<dim3((unsigned)io.n_envs, (unsigned)m.n_patches), 64, 0, s>>>(m);
+    gather ? launch_one<kModePnDecode, true>(m, io, tmA, tmB, grid, s) : launch_one<kModePnDecode, false>(m, io, tmA, tmB, grid, s);
+    *launches = 3;
+  }
   return cudaGetLastError();
 }
 

@@ -44,6 +44,8 @@ class etac_model_desc(C.Structure):
                 ("kernel_type", C.c_int32), ("n_alpha", C.c_int32), ("alpha", _fp),
                 ("resid_arch", C.c_int32), ("resid_hidden", C.c_int32),
                 ("W1", _fp), ("b1", _fp), ("W2", _fp), ("b2", _fp), ("W3", _fp), ("b3", _fp),
+                ("E1", _fp), ("e1", _fp), ("E2", _fp), ("e2", _fp), ("G1", _fp), ("g1", _fp),
+                ("D1", _fp), ("d1", _fp), ("D2", _fp), ("d2", _fp),
                 ("max_envs", C.c_int32), ("max_indenters", C.c_int32), ("precision", C.c_int32),
                 ("active_mode", C.c_int32), ("device", C.c_int32)]
 
@@ -118,7 +120,7 @@ def etac_create(node_pos, node_normal, alpha, *, patch_offset=None, adj_rowptr=N
     off, rp, col = _i32(patch_offset), _i32(adj_rowptr), _i32(adj_col)
     w = {k: _f32(v) for k, v in (weights or {}).items()}
     if resid_arch is None:
-        resid_arch = ETAC_RESID_PERNODE_MLP if weights else ETAC_RESID_NONE
+        resid_arch = ETAC_RESID_NONE if not weights else (ETAC_RESID_POINTNET if "E1" in w else ETAC_RESID_PERNODE_MLP)
     d = etac_model_desc()
     d.struct_size = C.sizeof(etac_model_desc)
     d.n_nodes = pos.shape[0]
@@ -128,7 +130,7 @@ def etac_create(node_pos, node_normal, alpha, *, patch_offset=None, adj_rowptr=N
     d.kernel_type = ETAC_KERNEL_EXP_L2
     d.n_alpha, d.alpha = al.shape[0], _p(al, _fp)
     d.resid_arch, d.resid_hidden = resid_arch, resid_hidden
-    for k in ("W1", "b1", "W2", "b2", "W3", "b3"):
+    for k in ("W1", "b1", "W2", "b2", "W3", "b3", "E1", "e1", "E2", "e2", "G1", "g1", "D1", "d1", "D2", "d2"):
         setattr(d, k, _p(w.get(k), _fp))
     d.max_envs, d.max_indenters = max_envs, max_indenters
     d.precision, d.active_mode, d.device = precision, active_mode, device

@@ -217,6 +217,15 @@ def make_weights(cfg: int, seed: int = 0, hidden: int = 64, std: float = 0.02):
     return {k: _f32(rng.normal(0.0, std, size=s)) for k, s in shp.items()}
 
 
+def make_pointnet_weights(cfg: int, seed: int = 0, std: float = 0.1):
+    """Weights of the paper's PointNet form of Phi with this repo's reading of
+    the widths: E1[64,9] e1 E2[64,64] e2 | G1[64,64] g1 | D1[64,128] d1 D2[3,64] d2; N(0,std^2)."""
+    rng = _rng(cfg, 3, seed)
+    shp = {"E1": (64, 9), "e1": (64,), "E2": (64, 64), "e2": (64,), "G1": (64, 64), "g1": (64,),
+           "D1": (64, 128), "d1": (64,), "D2": (3, 64), "d2": (3,)}
+    return {k: _f32(rng.normal(0.0, std, size=s)) for k, s in shp.items()}
+
+
 # --------------------------------------------------------------------------------------
 # workload container
 # --------------------------------------------------------------------------------------

@@ -41,7 +41,8 @@ def run_gpu(wl, *, precision=None, path=T.ETAC_PATH_AUTO, resid=True, active_mod
 
 
 def run_oracle(wl, *, resid=True, active_mode="passthrough", penetration=None, envs=None):
-    m = O.model_from_workload(wl, resid_arch="pernode" if resid else "none", active_mode=active_mode)
+    arch = "none" if not resid else ("pointnet" if "E1" in wl.weights else "pernode")
+    m = O.model_from_workload(wl, resid_arch=arch, active_mode=active_mode)
     if penetration is not None:
         return O.step(m, penetration=penetration, envs=envs)
     return O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose, envs=envs)

@@ -28,7 +28,7 @@ def test_exports_match_header(lib):
     assert declared == set(T.EXPORTS)
     for name in declared:
         assert getattr(lib, name) is not None
-    assert lib.etac_abi_version() == 2
+    assert lib.etac_abi_version() == 3
     assert C.sizeof(T.etac_indenter) == 48 == W.INDENTER_DTYPE.itemsize
 
 
@@ -56,8 +56,12 @@ def test_create_validates_before_cuda(lib):
     assert ei.value.status == T.ETAC_ERR_INVALID_ARG
     with pytest.raises(T.EtacError) as ei:
         T.etac_create(m.pos, m.normal, [0.5], patch_offset=m.patch_offset, weights=wl.weights,
-                      resid_arch=T.ETAC_RESID_POINTNET)
-    assert ei.value.status == T.ETAC_ERR_UNSUPPORTED
+                      resid_arch=T.ETAC_RESID_POINTNET, precision=T.ETAC_PREC_BF16)
+    assert ei.value.status == T.ETAC_ERR_INVALID_ARG and "PointNet" in str(ei.value)     # per-node weights only
+    with pytest.raises(T.EtacError) as ei:
+        T.etac_create(m.pos, m.normal, [0.5], patch_offset=m.patch_offset, weights=W.make_pointnet_weights(1),
+                      precision=T.ETAC_PREC_FP32)
+    assert ei.value.status == T.ETAC_ERR_UNSUPPORTED                                     # bf16 contexts only
     with pytest.raises(T.EtacError) as ei:
         T.etac_create(m.pos, m.normal, [0.5], patch_offset=m.patch_offset, max_envs=0)
     assert ei.value.status == T.ETAC_ERR_INVALID_ARG

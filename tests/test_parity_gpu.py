@@ -260,3 +260,18 @@ def test_full_size_config4_sampled():
         assert T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_CONTACT_PAIRS) == int((np.abs(U.cpu().numpy()).sum((1, 2)) > 0).sum())
     finally:
         eng.close()
+
+
+@pytest.mark.parametrize("n_envs,path", [(29, T.ETAC_PATH_DENSE), (97, T.ETAC_PATH_DENSE), (40, T.ETAC_PATH_SPARSE)])
+def test_pointnet_residual_bf16(n_envs, path):
+    """The paper's form of Phi: per-node encoder, max-pool over the patch,
+    global MLP, decoder on [f_i; g'] -- two passes of the fused kernel against the oracle's
+    residual_pointnet.  N(0, 0.15) weights so that the residual and its global part matter."""
+    import dataclasses
+    wl = dataclasses.replace(W.config3(4, n_envs), weights=W.make_pointnet_weights(3, 1, std=0.15))
+    gpu, ref = run_gpu(wl, path=path), run_oracle(wl)
+    assert gpu["launches"] == 4                      # S1, encode + pool, global MLP, decode
+    st = compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="pointnet")
+    _report(f"pointnet E={n_envs}", st)
+    # the global feature matters: with g' removed (per-node part only) the residual is different
+    assert float(np.abs(ref["U"] - ref["analytic"]).max()) > 1e-2 * float(np.abs(ref["U"]).max())
