@@ -426,9 +426,9 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
     }
     CK(dev_upload(c, &m.wimg_pn, img.data(), img.size()), "upload PointNet weight image");
     std::vector<float> pf(4096 + 64 + 4096 + 64);
-    memcpy(pf.data(), d->G1, 4096 * 4);
+    for (int n = 0; n < 64; ++n)      // both 64 x 64 matrices transposed to [in][out] (coalesced over the outputs)
+      for (int j = 0; j < 64; ++j) pf[j * 64 + n] = d->G1[n * 64 + j], pf[4160 + j * 64 + n] = d->D1[n * 128 + 64 + j];
     memcpy(pf.data() + 4096, d->g1, 64 * 4);
-    for (int n = 0; n < 64; ++n) memcpy(pf.data() + 4160 + n * 64, d->D1 + n * 128 + 64, 64 * 4);
     memcpy(pf.data() + 4160 + 4096, d->d1, 64 * 4);
     CK(dev_upload(c, &m.pn_f32, pf.data(), pf.size()), "upload PointNet global MLP");
     CK(dev_alloc(c, &m.gmax, (size_t)64 * P * d->max_envs, true), "alloc gmax");

@@ -73,7 +73,7 @@ struct DevModel {
   const float* c1t;           // [64 x N]: W1[:,3:9].[p;n] + b1, transposed for coalescing
   const uint8_t* wimg;        // kWImgBytes
   const uint8_t* wimg_pn;     // kPnImgBytes (ETAC_RESID_POINTNET)
-  const float* pn_f32;        // G1[64x64] g1[64] D1[:,64:128] as [64x64] d1[64] (fp32, pn_global_kernel)
+  const float* pn_f32;        // G1^T [in][out] g1[64] D1[:,64:128]^T [in][out] d1[64] (fp32, pn_global_kernel)
   uint32_t* gmax;             // [P x max_envs x 64] max-pooled encoder features as order-preserving keys
   float* cvec;                // [P x max_envs x 64] c_(e,p) / 2
   // per-step workspace

@@ -498,10 +498,9 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
                 const float y0 = fmaf(h0, tanh_approx(h0), h0), y1 = fmaf(h1, tanh_approx(h1), h1);
                 packed[k] = pack_bf16(y0, y1);
                 if constexpr (kMode == kModePnEncode) {
-                  if (pool) {  // column max over the warp's 32 rows; order-preserving uint keys, 0 = no row
-                    const uint32_t b0 = __float_as_uint(y0), b1 = __float_as_uint(y1);
-                    const uint32_t k0 = valid ? (b0 ^ ((b0 >> 31) ? 0xffffffffu : 0x80000000u)) : 0u;
-                    const uint32_t k1 = valid ? (b1 ^ ((b1 >> 31) ? 0xffffffffu : 0x80000000u)) : 0u;
+                  if (pool) {  // column max over the warp's 32 rows.  silu >= -0.279, so 1 + silu is a
+                               // positive float whose bit pattern orders like the value; 0 = no row
+                    const uint32_t k0 = valid ? __float_as_uint(1.0f + y0) : 0u, k1 = valid ? __float_as_uint(1.0f + y1) : 0u;
                     const uint32_t m0 = __reduce_max_sync(0xffffffffu, k0), m1 = __reduce_max_sync(0xffffffffu, k1);
                     if (lane == ((2 * k) & 31)) (half ? pool1 : pool0) = m0;
                     if (lane == ((2 * k + 1) & 31)) (half ? pool1 : pool0) = m1;
@@ -576,26 +575,35 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   }
 }
 
-// c_(e,p) of the PointNet decoder: g = max-pooled features (keys -> floats), g' = silu(G1 g + g1)
+// c_(e,p) of the PointNet decoder: g = max-pooled features (keys = bits of 1 + f), g' = silu(G1 g + g1)
 // ("further encoded by another MLP"), c = D1[:, 64:128] g' + d1, stored halved like
-// the decoder weights.  One 64-thread CTA per contacting (patch, slot).
+// the decoder weights.  A 64-thread CTA stages the two transposed 64 x 64 matrices in shared
+// memory once and walks kPnSlots contact-list slots of one patch.
+constexpr int kPnSlots = 16;
 __global__ void __launch_bounds__(64) pn_global_kernel(DevModel m) {
-  const int p = blockIdx.y, slot = blockIdx.x, k = threadIdx.x;
-  if (slot >= m.count[p]) return;
-  __shared__ float g[64], g2[64];
-  const int64_t base = ((int64_t)p * m.max_envs + slot) * 64;
-  const uint32_t key = m.gmax[base + k];
-  const uint32_t bits = (key >> 31) ? (key ^ 0x80000000u) : ~key;
-  g[k] = __uint_as_float(bits);
-  __syncthreads();
-  const float* G1 = m.pn_f32, *g1 = G1 + 4096, *D1g = g1 + 64, *d1 = D1g + 4096;
-  float a = g1[k];
-  for (int j = 0; j < 64; ++j) a = fmaf(G1[k * 64 + j], g[j], a);
-  g2[k] = a / (1.0f + expf(-a));
-  __syncthreads();
-  float c = d1[k];
-  for (int j = 0; j < 64; ++j) c = fmaf(D1g[k * 64 + j], g2[j], c);
-  m.cvec[base + k] = 0.5f * c;
+  const int p = blockIdx.y, k = threadIdx.x;
+  const int slot0 = blockIdx.x * kPnSlots, cnt = m.count[p];
+  if (slot0 >= cnt) return;
+  __shared__ float sG1[64 * 64], sD1[64 * 64], g[64], g2[64];
+  const float* G1t = m.pn_f32, *g1 = G1t + 4096, *D1gt = g1 + 64, *d1 = D1gt + 4096;  // both matrices [in][out]
+  for (int i = k; i < 4096; i += 64) sG1[i] = G1t[i], sD1[i] = D1gt[i];
+  const float bg = g1[k], bd = d1[k];
+  for (int slot = slot0; slot < min(cnt, slot0 + kPnSlots); ++slot) {
+    const int64_t base = ((int64_t)p * m.max_envs + slot) * 64;
+    const uint32_t key = m.gmax[base + k];
+    __syncthreads();  // previous slot done with g / g2; first pass: weights staged
+    g[k] = __uint_as_float(key) - 1.0f;  // keys are the bit patterns of 1 + f
+    __syncthreads();
+    float a = bg;
+#pragma unroll 8
+    for (int j = 0; j < 64; ++j) a = fmaf(sG1[j * 64 + k], g[j], a);
+    g2[k] = a / (1.0f + expf(-a));
+    __syncthreads();
+    float c = bd;
+#pragma unroll 8
+    for (int j = 0; j < 64; ++j) c = fmaf(sD1[j * 64 + k], g2[j], c);
+    m.cvec[base + k] = 0.5f * c;
+  }
 }
 
 template <int kMode, bool kGather>
@@ -634,7 +642,7 @@ cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtenso
     cudaError_t e = cudaMemsetAsync(m.gmax, 0, sizeof(uint32_t) * 64 * (size_t)m.n_patches * m.max_envs, s);
     if (e != cudaSuccess) return e;
     launch_one<kModePnEncode, false>(m, io, tmA, tmB, grid, s);
-    pn_global_kernel<<<dim3((unsigned)io.n_envs, (unsigned)m.n_patches), 64, 0, s>>>(m);
+    pn_global_kernel<<<dim3((unsigned)((io.n_envs + kPnSlots - 1) / kPnSlots), (unsigned)m.n_patches), 64, 0, s>>>(m);
     gather ? launch_one<kModePnDecode, true>(m, io, tmA, tmB, grid, s) : launch_one<kModePnDecode, false>(m, io, tmA, tmB, grid, s);
     *launches = 3;
   }
