@@ -37,6 +37,18 @@ MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728 (SURVEY.md 
 NCU_TRAFFIC_BYTES = 313.43e6
 
 
+WORKLOADS = {
+    "cfg3": ("cfg3_dexterous_hand_5696 (BASELINE.json configs[2])", lambda seed, envs: W.config3(seed, envs)),
+    # not the headline: the single dense K[8192 x 8192] case, same metric (python bench.py --workload cfg4)
+    "cfg4": ("cfg4_curved_sheet_8192 (BASELINE.json configs[3])", lambda seed, envs: W.config4(seed, envs)),
+}
+
+
+def chosen_of(wl):
+    """[E, P] contact pairs the generator placed (cfg 4: every env presses on its single patch)."""
+    return wl.meta["chosen"] if "chosen" in wl.meta else np.ones((wl.n_envs, wl.mesh.n_patches), dtype=bool)
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -115,8 +127,9 @@ def run_reference(a):
     """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    wl = W.config3(0, a.envs)
-    n_sample = min(a.envs, 96)
+    label, make = WORKLOADS[a.workload]
+    wl = make(0, a.envs)
+    n_sample = min(a.envs, 96 if a.workload == "cfg3" else 8)
     t_w = [time_oracle(wl, n_sample)[0] for _ in range(a.warmup)]
     t0 = time.perf_counter()
     envs_done = 0
@@ -131,7 +144,7 @@ def run_reference(a):
         "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "node_updates_per_s": v * wl.mesh.n_nodes,
-        "config": {"workload": "cfg3_dexterous_hand_5696 (BASELINE.json configs[2])", "n_envs": a.envs,
+        "config": {"workload": label, "n_envs": a.envs,
                    "n_nodes": wl.mesh.n_nodes, "n_patches": wl.mesh.n_patches},
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
                          "sample": f"each step = {n_sample} of {a.envs} envs (stride {max(1, a.envs // n_sample)})"},
@@ -156,7 +169,8 @@ def run_ours(a):
     peaks = load_peaks()
 
     # weak scaling: every rank owns a batch of a.envs environments (its own seeds)
-    sets = [W.config3(rank * N_INPUT_SETS + k, a.envs) for k in range(N_INPUT_SETS)]
+    label, make = WORKLOADS[a.workload]
+    sets = [make(rank * N_INPUT_SETS + k, a.envs) for k in range(N_INPUT_SETS)]
     wl = sets[0]
     eng = T.Etac(wl, device=local)
     stream = torch.cuda.current_stream().cuda_stream
@@ -173,7 +187,7 @@ def run_ours(a):
         T.etac_step(eng.ctx, stream, argv[i % N_INPUT_SETS])
     pairs = T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_CONTACT_PAIRS)
     last_set = sets[(a.warmup - 1) % N_INPUT_SETS]
-    assert pairs == int(last_set.meta["chosen"].sum()), "realised contact pairs differ from the generator's placement"
+    assert pairs == int(chosen_of(last_set).sum()), "realised contact pairs differ from the generator's placement"
 
     # ---- device-resident timing
     sync_all()
@@ -191,16 +205,19 @@ def run_ours(a):
     clocks = clk.stop() if clk else None
 
     # ---- end to end: host buffers in, host buffer out, through the C-ABI call
+    posed = sets[0].patch_pose is not None
     pin = [(torch.from_numpy(np.ascontiguousarray(s.indenters).view(np.uint8).reshape(-1)).pin_memory(),
-            torch.from_numpy(np.ascontiguousarray(s.patch_pose)).pin_memory()) for s in sets]
-    d_ind, d_pose = torch.empty_like(pin[0][0], device="cuda"), torch.empty_like(pin[0][1], device="cuda")
+            torch.from_numpy(np.ascontiguousarray(s.patch_pose)).pin_memory() if posed else None) for s in sets]
+    d_ind = torch.empty_like(pin[0][0], device="cuda")
+    d_pose = torch.empty_like(pin[0][1], device="cuda") if posed else None
     h_out = torch.empty((a.envs, eng.N, 3), dtype=torch.float32).pin_memory()
     e2e_args = T.make_step_args(a.envs, eng.out, indenters=d_ind, patch_pose=d_pose)
     n_e2e = max(3, min(a.steps, 10))
 
     def e2e_step(k):
         d_ind.copy_(pin[k][0], non_blocking=True)
-        d_pose.copy_(pin[k][1], non_blocking=True)
+        if posed:
+            d_pose.copy_(pin[k][1], non_blocking=True)
         T.etac_step(eng.ctx, stream, e2e_args)
         h_out.copy_(eng.out[: a.envs], non_blocking=True)
 
@@ -211,7 +228,7 @@ def run_ours(a):
         e2e_step(i % N_INPUT_SETS)
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t0)
-    h2d = pin[0][0].numel() + pin[0][1].numel() * 4
+    h2d = pin[0][0].numel() + (pin[0][1].numel() * 4 if posed else 0)
     d2h = h_out.numel() * 4
 
     t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device="cuda")
@@ -226,23 +243,24 @@ def run_ours(a):
 
     ms_step = ms / a.steps
     value = world * a.envs / (ms_step * 1e-3)
-    wm = work_model(wl, np.mean([s.meta["chosen"] for s in sets], axis=0) * 1.0)
+    wm = work_model(wl, np.mean([chosen_of(s) for s in sets], axis=0) * 1.0)
     flops = wm["f_prop_dense"] + wm["f_mlp"]
     peak = peaks["bf16_tflops_sustained"]
     achieved = flops / (ms_fused * 1e-3) / 1e12
     t_tensor = flops / (peak * 1e12)
     t_hbm = wm["b_hbm_min"] / (peaks["hbm_gbs"] * 1e9)
     t_roof = max(t_tensor, t_hbm)
-    cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, a.envs)   # ~10 s of CPU work at 4096 envs
+    cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, a.envs if a.workload == "cfg3" else 48)   # ~10 s of CPU work
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "bf16", "data": "synthetic",
         "node_updates_per_s": value * eng.N,
-        "config": {"workload": "cfg3_dexterous_hand_5696 (BASELINE.json configs[2])", "n_envs_per_gpu": a.envs,
+        "config": {"workload": label, "n_envs_per_gpu": a.envs,
                    "n_nodes": eng.N, "n_patches": eng.P, "precision": "bf16 operands, fp32 accumulate",
                    "contact_pairs_per_step": wm["pairs"], "node_envs_per_step": wm["w_nodeenv"],
-                   "l2": f"{N_INPUT_SETS} rotating seeded input sets; 280 MB output + 230 MB workspace per step > 126 MB L2",
+                   "l2": f"{N_INPUT_SETS} rotating seeded input sets; {12 * a.envs * eng.N / 1e6:.0f} MB output + "
+                         f"{10 * a.envs * eng.N / 1e6:.0f} MB workspace per step > 126 MB L2",
                    "algorithmic_bytes_fused": wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"],
                    "parallelism": f"env-sharded x{world}, no collective"},
         "clocks": clocks,
@@ -250,9 +268,9 @@ def run_ours(a):
                 "d2h_bytes_per_step": d2h, "steps": n_e2e,
                 "note": "pinned host indenters+patch poses -> device, etac_step, full [E,N,3] fp32 result -> pinned host"},
         "gpu_launches": launches,
-        "kernels_ms": {"s1_sdf_pairs_kernel_incl_memsets": ms_s1, "dense_bf16_kernel": ms_fused},
+        "kernels_ms": {"s1_sdf_kernel_incl_memsets": ms_s1, "dense_bf16_kernel": ms_fused},
         "roofline": {"bound": "tensor", "kernel": "dense_bf16_kernel", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else None,
                      "peak_src": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['src']})",
                      "flops_per_launch": flops},
         "roofline_step": {"t_roof_us": t_roof * 1e6, "t_tensor_us": t_tensor * 1e6, "t_hbm_us": t_hbm * 1e6,
@@ -275,6 +293,7 @@ if __name__ == "__main__":
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--envs", type=int, default=4096)
+    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     (run_reference if args.impl == "reference" else run_ours)(args)
