@@ -19,7 +19,8 @@ of Phi, ...) are listed in DESIGN.md §3 (R1..R20); each function cites the one 
 Pins (tests/test_oracle_pins.py, ``-m "not gpu"``): closed-form single-point-contact decay,
 lattice row sums, brute-force triple loops, scipy cdist / torch float64 library
 cross-checks, linearity, rigid invariance, SDF spot values, hand-derived worked examples
-under tests/golden/.  Unpinned: numerical agreement with the paper's *trained* Phi and its
+under tests/golden/; the sampled-grid SDF against scipy's RegularGridInterpolator, exactness
+on affine fields and the h^2 interpolation bound on a sphere.  Unpinned: numerical agreement with the paper's *trained* Phi and its
 Table II (no weights / FEM data exist here)  -> "parity unpinned" for that item only; and
 the PointNet form of Phi is pinned only by its structural invariants (hidden widths are not
 given in the paper: Fig. 3 is an image).
@@ -30,7 +31,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-IND_NONE, IND_SPHERE, IND_BOX, IND_CAPSULE = 0, 1, 2, 3
+IND_NONE, IND_SPHERE, IND_BOX, IND_CAPSULE, IND_GRID = 0, 1, 2, 3, 4
 
 
 @dataclass
@@ -42,6 +43,7 @@ class OracleModel:
     weights: dict | None = None   # per-node MLP: W1 b1 W2 b2 W3 b3 (reading R10); None = no residual
     resid_arch: str = "pernode"   # "none" | "pernode" | "pointnet"
     active_mode: str = "passthrough"   # "passthrough" (mask M_p) | "propagate"
+    grids: dict = field(default_factory=dict)   # id -> (values [nz,ny,nx] fp32, origin [3], spacing): sampled SDFs
     _K: dict = field(default_factory=dict)
 
     @property
@@ -112,6 +114,37 @@ def sdf_local(itype, param, y0, y1, y2, dt=np.float64):
     raise ValueError(f"bad indenter type {itype}")
 
 
+def sdf_grid(values, origin, spacing, y0, y1, y2, dt=np.float64):
+    """Signed distance of a SAMPLED object (PAPER.md:L77 detects contact with SDFs against
+    object meshes; a sampled grid is how such an SDF is handed over; R21).
+    values[iz, iy, ix] = SDF sample at origin + spacing*(ix, iy, iz).  Definition: clamp the
+    query point to the grid's box, interpolate the samples TRILINEARLY there (x, then y, then
+    z; lerp written a + f*(b - a)), and add the Euclidean distance from the point to the box.
+    Every operation is rounded to ``dt`` (fp32 twin: no fused multiply-add)."""
+    v = np.asarray(values)
+    nz, ny, nx = v.shape
+    h, inv_h = dt(spacing), dt(1.0) / dt(spacing)
+    y = [np.asarray(y0, dtype=dt), np.asarray(y1, dtype=dt), np.asarray(y2, dtype=dt)]
+    n = [nx, ny, nz]
+    yc, idx, fr = [], [], []
+    for a in range(3):
+        lo = dt(origin[a])
+        hi = lo + h * dt(n[a] - 1)
+        c = np.minimum(np.maximum(y[a], lo), hi)
+        t = (c - lo) * inv_h
+        i = np.minimum(np.floor(t), dt(n[a] - 2)).astype(np.int64)
+        yc.append(c), idx.append(i), fr.append(t - i.astype(dt))
+    ix, iy, iz = idx
+    fx, fy, fz = fr
+    V = lambda dz, dy, dx: v[iz + dz, iy + dy, ix + dx].astype(dt)
+    lerp = lambda a, b, f: a + f * (b - a)
+    c00, c10 = lerp(V(0, 0, 0), V(0, 0, 1), fx), lerp(V(0, 1, 0), V(0, 1, 1), fx)
+    c01, c11 = lerp(V(1, 0, 0), V(1, 0, 1), fx), lerp(V(1, 1, 0), V(1, 1, 1), fx)
+    c = lerp(lerp(c00, c10, fy), lerp(c01, c11, fy), fz)
+    d0, d1, d2 = y[0] - yc[0], y[1] - yc[1], y[2] - yc[2]
+    return c + np.sqrt((d0 * d0 + d1 * d1) + d2 * d2)
+
+
 def signed_distance(model: OracleModel, indenters_e, patch_pose_e=None, dt=np.float64):
     """phi[i] = min over the env's indenters (type != NONE) of sdf_k(R_k^T (x_i - t_k)),
     x_i = R(q_{e,p}) p_i + t_{e,p} (identity if no patch poses); +inf if no indenter.
@@ -143,7 +176,11 @@ def signed_distance(model: OracleModel, indenters_e, patch_pose_e=None, dt=np.fl
         y0 = (R[0, 0] * d0 + R[1, 0] * d1) + R[2, 0] * d2
         y1 = (R[0, 1] * d0 + R[1, 1] * d1) + R[2, 1] * d2
         y2 = (R[0, 2] * d0 + R[1, 2] * d1) + R[2, 2] * d2
-        phi = np.minimum(phi, sdf_local(itype, ind["param"], y0, y1, y2, dt))
+        if itype == IND_GRID:
+            values, origin, spacing = model.grids[int(ind["param"][0])]
+            phi = np.minimum(phi, sdf_grid(values, origin, spacing, y0, y1, y2, dt))
+        else:
+            phi = np.minimum(phi, sdf_local(itype, ind["param"], y0, y1, y2, dt))
     return phi
 
 
@@ -243,4 +280,4 @@ def step(model: OracleModel, indenters=None, patch_pose=None, penetration=None, 
 
 def model_from_workload(wl, resid_arch="pernode", active_mode="passthrough") -> OracleModel:
     return OracleModel(wl.mesh.pos, wl.mesh.normal, wl.mesh.patch_offset, wl.alpha,
-                       wl.weights, resid_arch, active_mode)
+                       wl.weights, resid_arch, active_mode, grids=dict(wl.meta.get("grids", {})))

@@ -320,3 +320,55 @@ def test_fp32_twin_agrees_with_fp64_away_from_the_surface():
             assert np.abs(p32[near] - p64[near]).max() < 1e-4
             far = np.abs(p64) > 1e-4
             assert np.array_equal((p32 < 0)[far], (p64 < 0)[far])
+
+
+# ---------------------------------------------------------------- sampled-grid SDF (R21)
+def _grid_of(fn, n=(9, 11, 13), origin=(-2.0, -2.5, -3.0), h=0.5):
+    nx, ny, nz = n
+    x = origin[0] + h * np.arange(nx)
+    y = origin[1] + h * np.arange(ny)
+    z = origin[2] + h * np.arange(nz)
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    return fn(X, Y, Z).astype(np.float32), (x, y, z)
+
+
+def test_grid_sdf_matches_library_trilinear_interpolation_inside():
+    from scipy.interpolate import RegularGridInterpolator
+    rng = np.random.default_rng(21)
+    vals = rng.normal(size=(13, 11, 9)).astype(np.float32)          # arbitrary samples: pure interpolation
+    origin, h = (-2.0, -2.5, -3.0), 0.5
+    x, y, z = (origin[a] + h * np.arange(n) for a, n in zip(range(3), (9, 11, 13)))
+    rgi = RegularGridInterpolator((z, y, x), vals.astype(np.float64), method="linear")
+    q = np.stack([rng.uniform(x[0], x[-1], 500), rng.uniform(y[0], y[-1], 500), rng.uniform(z[0], z[-1], 500)], 1)
+    got = O.sdf_grid(vals, origin, h, q[:, 0], q[:, 1], q[:, 2])
+    np.testing.assert_allclose(got, rgi(q[:, ::-1]), atol=1e-12)
+    # at a grid point the sample itself comes back
+    assert O.sdf_grid(vals, origin, h, x[3], y[10], z[12]) == pytest.approx(float(vals[12, 10, 3]), abs=1e-12)
+
+
+def test_grid_sdf_is_exact_for_a_plane_and_adds_the_distance_outside():
+    vals, (x, y, z) = _grid_of(lambda X, Y, Z: Z - 0.25)            # half-space z < 0.25: affine => exact
+    origin, h = (-2.0, -2.5, -3.0), 0.5
+    rng = np.random.default_rng(22)
+    q = np.stack([rng.uniform(x[0], x[-1], 200), rng.uniform(y[0], y[-1], 200), rng.uniform(-6.0, 6.0, 200)], 1)
+    got = O.sdf_grid(vals, origin, h, q[:, 0], q[:, 1], q[:, 2])
+    np.testing.assert_allclose(got, q[:, 2] - 0.25 + np.where(q[:, 2] < z[0], 2 * (z[0] - q[:, 2]), 0.0), atol=1e-6)
+    # sideways outside the box: value at the clamped point plus the distance to the box
+    far = O.sdf_grid(vals, origin, h, x[-1] + 3.0, 0.0, 1.0)
+    assert far == pytest.approx((1.0 - 0.25) + 3.0, abs=1e-6)
+
+
+def test_grid_sdf_of_a_sphere_obeys_the_interpolation_bound():
+    R, h = 1.5, 0.25
+    vals, (x, y, z) = _grid_of(lambda X, Y, Z: np.sqrt(X * X + Y * Y + Z * Z) - R, n=(25, 25, 25),
+                               origin=(-3.0, -3.0, -3.0), h=h)
+    rng = np.random.default_rng(23)
+    q = rng.uniform(-2.9, 2.9, (2000, 3))
+    rho = np.linalg.norm(q, axis=1)
+    keep = rho > 1.0
+    got = O.sdf_grid(vals, (-3.0, -3.0, -3.0), h, q[keep, 0], q[keep, 1], q[keep, 2])
+    # trilinear error <= h^2/8 * sum |d2 phi / dx_a^2| <= h^2/8 * 2/rho (Laplacian of |x|), + fp32 samples
+    assert np.all(np.abs(got - (rho[keep] - R)) <= h * h / 8 * 2 / (rho[keep] - h * np.sqrt(3)) + 1e-6)
+    # fp32 twin: same formula, every op in float32, agrees to rounding
+    got32 = O.sdf_grid(vals, (-3.0, -3.0, -3.0), h, q[keep, 0], q[keep, 1], q[keep, 2], np.float32)
+    assert got32.dtype == np.float32 and np.abs(got32 - got).max() < 5e-6
