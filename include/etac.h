@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define ETAC_ABI_VERSION 3
+#define ETAC_ABI_VERSION 4
 
 typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
 
@@ -49,11 +49,12 @@ typedef enum {
 /* Analytic indenters (north_star: "analytic indenter SDFs (sphere/box/capsule poses)").  The
  * signed distance is exact (1-Lipschitz), negative inside.  PAPER.md:L77 detects contact with
  * SDFs against object meshes; several indenters per environment are united by min. */
-typedef enum { ETAC_IND_NONE = 0, ETAC_IND_SPHERE = 1, ETAC_IND_BOX = 2, ETAC_IND_CAPSULE = 3 } etac_ind_type;
+typedef enum { ETAC_IND_NONE = 0, ETAC_IND_SPHERE = 1, ETAC_IND_BOX = 2, ETAC_IND_CAPSULE = 3, ETAC_IND_GRID = 4 } etac_ind_type;
 
 typedef struct {
   int32_t type;   /* etac_ind_type; NONE slots are skipped */
-  float param[3]; /* sphere {r,-,-}; box {hx,hy,hz} half extents; capsule {r, half length along local z, -} */
+  float param[3]; /* sphere {r,-,-}; box {hx,hy,hz} half extents; capsule {r, half length along local z, -};
+                     grid {grid id as a float,-,-}: a sampled SDF registered with etac_set_sdf_grid */
   float pose[7];  /* {px,py,pz, qx,qy,qz,qw}: unit quaternion, Isaac-Gym order; world frame */
   float _pad;
 } etac_indenter; /* 48 bytes */
@@ -152,6 +153,16 @@ enum {
   ETAC_INFO_SM_COUNT = 8
 };
 etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value);
+
+/* Sampled signed-distance field of an arbitrary object (PAPER.md:L77 queries SDFs against object
+ * meshes; this is how such a field is handed over).  values[(iz*ny + iy)*nx + ix] (host, fp32) is the
+ * SDF at origin + spacing*(ix, iy, iz) in the object's frame; an indenter of type ETAC_IND_GRID with
+ * param[0] = grid_id places it with its pose.  The field at a point is the trilinear interpolation of
+ * the samples at the point clamped to the grid's box plus the distance from the point to the box.
+ * grid_id in [0, 8); nx, ny, nz >= 2; spacing > 0.  Copies the samples; replacing a grid synchronises
+ * the device first.  Not to be called concurrently with etac_step on the same ctx. */
+etac_status etac_set_sdf_grid(etac_ctx* ctx, int32_t grid_id, int32_t nx, int32_t ny, int32_t nz,
+                              const float* origin, float spacing, const float* values);
 
 /* Message of the last failure on this ctx ("" if none); ctx-owned, valid until the next call.
  * With ctx == NULL returns the message of the last failed etac_create on this thread. */

@@ -494,6 +494,34 @@ etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
   return ETAC_OK;
 }
 
+etac_status etac_set_sdf_grid(etac_ctx* ctx, int32_t grid_id, int32_t nx, int32_t ny, int32_t nz, const float* origin,
+                              float spacing, const float* values) {
+  if (!ctx) return ETAC_ERR_INVALID_ARG;
+  if (grid_id < 0 || grid_id >= kMaxGrids) return fail(ctx, ETAC_ERR_INVALID_ARG, "grid_id out of range");
+  if (nx < 2 || ny < 2 || nz < 2 || !origin || !values || !(spacing > 0.0f) || !isfinite(spacing))
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "bad SDF grid");
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, ETAC_ERR_CUDA, "cudaSetDevice failed");
+  GridDesc& g = ctx->m.grid[grid_id];
+  cudaError_t e = cudaSuccess;
+  if (g.v) {  // replacing: nothing in flight may still read the old samples
+    if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("synchronize", e));
+    cudaFree(const_cast<float*>(g.v));
+    ctx->allocs.erase(std::remove(ctx->allocs.begin(), ctx->allocs.end(), (void*)g.v), ctx->allocs.end());
+    g.v = nullptr;
+  }
+  float* dv = nullptr;
+  const size_t count = (size_t)nx * ny * nz;
+  if ((e = dev_alloc(ctx, &dv, count, false)) != cudaSuccess)
+    return fail(ctx, e == cudaErrorMemoryAllocation ? ETAC_ERR_ALLOC : ETAC_ERR_CUDA, cuda_msg("alloc SDF grid", e));
+  if ((e = cudaMemcpy(dv, values, count * sizeof(float), cudaMemcpyHostToDevice)) != cudaSuccess)
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("upload SDF grid", e));
+  g.v = dv, g.nx = nx, g.ny = ny, g.nz = nz;
+  g.o[0] = origin[0], g.o[1] = origin[1], g.o[2] = origin[2];
+  g.h = spacing, g.inv_h = 1.0f / spacing;
+  return ETAC_OK;
+}
+
 etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value) {
   if (!ctx || !value) return ETAC_ERR_INVALID_ARG;
   switch (key) {

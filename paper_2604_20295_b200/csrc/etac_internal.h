@@ -56,6 +56,15 @@ struct __align__(16) ActiveEntry {
 // what S1 writes besides delta / flags / env lists
 enum : int { kS1WriteUhat = 1, kS1WriteAlist = 2, kS1FillOut = 4 };
 
+// Sampled SDF of an object (ETAC_IND_GRID): values[(iz*ny + iy)*nx + ix] at origin + h*(ix, iy, iz).
+constexpr int kMaxGrids = 8;
+struct GridDesc {
+  const float* v;  // device, NULL = slot unused
+  int32_t nx, ny, nz;
+  float o[3];
+  float h, inv_h;  // inv_h = 1.0f / h (IEEE fp32 division)
+};
+
 struct DevModel {
   int32_t n_nodes, n_patches, n_chunks;
   int32_t max_patch_nodes;    // largest patch
@@ -82,6 +91,7 @@ struct DevModel {
   int32_t* count;             // [P] contacting envs per patch (this step)
   int32_t* envlist;           // [P x max_envs]
   uint8_t* flags;             // [max_envs x P]
+  GridDesc grid[kMaxGrids];   // sampled-SDF objects (etac_set_sdf_grid)
   ActiveEntry* alist;         // [max_envs (slots) x ldu]: the active nodes of (slot, patch p) start at
                               // slot * ldu + off_p, in node order (allocated when the bf16 gather path is first selected)
   int32_t* acount;            // [P x max_envs]: number of active nodes of (patch, slot)

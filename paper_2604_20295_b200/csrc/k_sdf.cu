@@ -43,8 +43,35 @@ __device__ __forceinline__ float len3(float a, float b, float c) {
   return __fsqrt_rn(__fadd_rn(__fadd_rn(__fmul_rn(a, a), __fmul_rn(b, b)), __fmul_rn(c, c)));
 }
 
+// Sampled SDF (R21): clamp to the grid's box, trilinear interpolation of the samples
+// (x, then y, then z; lerp = a + f*(b - a)), plus the distance from the point to the box.  Same
+// single-rounded operations in the same order as the oracle's fp32 twin.
+__device__ __forceinline__ float sdf_grid(const GridDesc& g, float y0, float y1, float y2) {
+  const float y[3] = {y0, y1, y2};
+  const int n[3] = {g.nx, g.ny, g.nz};
+  float yc[3], f[3];
+  int i[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const float lo = g.o[a], hi = __fadd_rn(lo, __fmul_rn(g.h, (float)(n[a] - 1)));
+    yc[a] = fminf(fmaxf(y[a], lo), hi);
+    const float t = __fmul_rn(__fsub_rn(yc[a], lo), g.inv_h);
+    const float fl = fminf(floorf(t), (float)(n[a] - 2));
+    i[a] = (int)fl;
+    f[a] = __fsub_rn(t, fl);
+  }
+  const float* v = g.v + ((int64_t)i[2] * g.ny + i[1]) * g.nx + i[0];
+  const int64_t sy = g.nx, sz = (int64_t)g.nx * g.ny;
+  auto lerp = [](float a, float b, float t) { return __fadd_rn(a, __fmul_rn(t, __fsub_rn(b, a))); };
+  const float c00 = lerp(v[0], v[1], f[0]), c10 = lerp(v[sy], v[sy + 1], f[0]);
+  const float c01 = lerp(v[sz], v[sz + 1], f[0]), c11 = lerp(v[sz + sy], v[sz + sy + 1], f[0]);
+  const float c = lerp(lerp(c00, c10, f[1]), lerp(c01, c11, f[1]), f[2]);
+  return __fadd_rn(c, len3(__fsub_rn(y0, yc[0]), __fsub_rn(y1, yc[1]), __fsub_rn(y2, yc[2])));
+}
+
 // Signed distance of world point X to one indenter (+inf for an empty slot).
-__device__ __forceinline__ float sdf_one(const SInd& s, float X0, float X1, float X2) {
+template <bool kGrid>
+__device__ __forceinline__ float sdf_one(const SInd& s, float X0, float X1, float X2, const GridDesc* grids) {
   if (s.type == ETAC_IND_NONE) return __int_as_float(0x7f800000);
   const float d0 = __fsub_rn(X0, s.t[0]), d1 = __fsub_rn(X1, s.t[1]), d2 = __fsub_rn(X2, s.t[2]);
   // y = R^T d
@@ -52,6 +79,14 @@ __device__ __forceinline__ float sdf_one(const SInd& s, float X0, float X1, floa
   const float y1 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[1], d0), __fmul_rn(s.R[4], d1)), __fmul_rn(s.R[7], d2));
   const float y2 = __fadd_rn(__fadd_rn(__fmul_rn(s.R[2], d0), __fmul_rn(s.R[5], d1)), __fmul_rn(s.R[8], d2));
   if (s.type == ETAC_IND_SPHERE) return __fsub_rn(len3(y0, y1, y2), s.prm[0]);
+  if constexpr (kGrid) {  // compiled only into the variants launched once a grid is registered
+    if (s.type == ETAC_IND_GRID) {
+      const GridDesc& g = grids[min(max((int)s.prm[0], 0), kMaxGrids - 1)];
+      return g.v ? sdf_grid(g, y0, y1, y2) : __int_as_float(0x7f800000);
+    }
+  } else {
+    if (s.type == ETAC_IND_GRID) return __int_as_float(0x7f800000);  // no grid registered: empty slot
+  }
   if (s.type == ETAC_IND_BOX) {
     const float q0 = __fsub_rn(fabsf(y0), s.prm[0]);
     const float q1 = __fsub_rn(fabsf(y1), s.prm[1]);
@@ -67,10 +102,27 @@ __device__ __forceinline__ float sdf_one(const SInd& s, float X0, float X1, floa
 }
 
 // Union signed distance at world point X: min over the slots in slot order.
-__device__ __forceinline__ float union_sdf(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2) {
+template <bool kGrid>
+__device__ __forceinline__ float union_sdf(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2,
+                                           const GridDesc* grids) {
   float phi = __int_as_float(0x7f800000);
-  for (int k = 0; k < n_ind; ++k) phi = fminf(phi, sdf_one(ind[k], X0, X1, X2));
+  for (int k = 0; k < n_ind; ++k) phi = fminf(phi, sdf_one<kGrid>(ind[k], X0, X1, X2, grids));
   return phi;
+}
+
+// Lower bound of the union SDF over a ball of radius rad around X, for the conservative culls:
+// the analytic SDFs are 1-Lipschitz; a sampled one is bounded by sqrt(3) inside its box (each
+// partial derivative of the trilinear interpolant <= the samples' Lipschitz constant) plus 1
+// for the distance term outside.
+template <bool kGrid>
+__device__ __forceinline__ float union_sdf_lower(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2,
+                                                 float rad, const GridDesc* grids) {
+  float lo = __int_as_float(0x7f800000);
+  for (int k = 0; k < n_ind; ++k) {
+    const float L = (kGrid && ind[k].type == ETAC_IND_GRID) ? 2.7320508f : 1.0f;
+    lo = fminf(lo, sdf_one<kGrid>(ind[k], X0, X1, X2, grids) - L * rad);
+  }
+  return lo;
 }
 
 __device__ __forceinline__ SInd load_indenter(const etac_indenter* __restrict__ p) {
@@ -115,7 +167,7 @@ struct SPose {
 //   D  one thread per patch: contact flag, slot in the patch's compact environment list
 //   E  all threads: contact-free patches -> zero-fill of the output rows; contacting patches ->
 //      U^ operand rows (bf16), optional delta / mask outputs
-template <bool kIndenters>
+template <bool kIndenters, bool kGrid>
 __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int s1_flags) {
   const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
   __shared__ int s_wcnt[8];
@@ -168,8 +220,8 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           C2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], x), __fmul_rn(sp.R[7], y)), __fmul_rn(sp.R[8], z)), sp.t[2]);
         }
         // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
-        const float phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
-        sp.evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
+        const float phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid);
+        sp.evaluated = !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
         s_pose[threadIdx.x] = sp;
       }
     }
@@ -195,7 +247,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
             X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
             X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
           }
-          const float phi = union_sdf(sind, m.max_ind, X0, X1, X2);
+          const float phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid);
           const float d = phi < 0.0f ? -phi : 0.0f;
           delta[i] = d;
           any |= d > 0.0f;
@@ -307,7 +359,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
 // Same single-rounded arithmetic in the same order as sdf_penetration_kernel.
 constexpr int kPairWarps = 2;
 
-template <bool kOne>
+template <bool kOne, bool kGrid>
 __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel m, StepIO io, int s1_flags) {
   const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
   extern __shared__ uint8_t smem_raw[];
@@ -332,17 +384,17 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
     to_world(R, t, pi.bc[0], pi.bc[1], pi.bc[2], C0, C1, C2);
   }
   SInd one;
-  float phi_c;
+  float phi_lo;
   if constexpr (kOne) {
     one = load_indenter(io.ind + e);
-    phi_c = fminf(__int_as_float(0x7f800000), sdf_one(one, C0, C1, C2));
+    phi_lo = union_sdf_lower<kGrid>(&one, 1, C0, C1, C2, pi.brad, m.grid);
   } else {
     for (int k = lane; k < m.max_ind; k += 32) sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
     __syncwarp();
-    phi_c = union_sdf(sind, m.max_ind, C0, C1, C2);
+    phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid);
   }
-  // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
-  const bool evaluated = !(phi_c - pi.brad > 0.01f + 1e-5f * fabsf(phi_c));
+  // conservative cull: phi(x_i) >= phi(c) - L * brad on the patch's bounding sphere
+  const bool evaluated = !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
   bool any = false;
   int nact = 0;
   float* delta = m.delta + row0;
@@ -353,8 +405,8 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       float X0 = pos.x, X1 = pos.y, X2 = pos.z;
       if (posed) to_world(R, t, pos.x, pos.y, pos.z, X0, X1, X2);
       float phi;
-      if constexpr (kOne) phi = fminf(__int_as_float(0x7f800000), sdf_one(one, X0, X1, X2));
-      else phi = union_sdf(sind, m.max_ind, X0, X1, X2);
+      if constexpr (kOne) phi = fminf(__int_as_float(0x7f800000), sdf_one<kGrid>(one, X0, X1, X2, m.grid));
+      else phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid);
       const float d = phi < 0.0f ? -phi : 0.0f;
       delta[i] = d;
       any |= d > 0.0f;
@@ -426,23 +478,25 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
 
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s) {
   const unsigned grid = (unsigned)io.n_envs;
+  bool grids = false;  // the sampled-SDF code is only in the variants launched once a grid is registered
+  for (int k = 0; k < kMaxGrids; ++k) grids |= m.grid[k].v != nullptr;
   // many small patches with indenters: one warp per (env, patch) pair; otherwise one CTA per environment
   if (io.input_mode == ETAC_IN_INDENTERS && m.max_ind >= 1 && m.n_patches >= 4 && m.max_patch_nodes <= 2048) {
     const int64_t pairs = (int64_t)io.n_envs * m.n_patches;
     const unsigned pgrid = (unsigned)((pairs + kPairWarps - 1) / kPairWarps);
-    if (m.max_ind == 1) {
-      sdf_pairs_kernel<true><<<pgrid, kPairWarps * 32, 0, s>>>(m, io, s1_flags);
-    } else {
-      const size_t smem = sizeof(SInd) * (size_t)m.max_ind * kPairWarps;
-      sdf_pairs_kernel<false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
-    }
+    const size_t smem = m.max_ind == 1 ? 0 : sizeof(SInd) * (size_t)m.max_ind * kPairWarps;
+    if (m.max_ind == 1 && !grids) sdf_pairs_kernel<true, false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
+    if (m.max_ind == 1 && grids) sdf_pairs_kernel<true, true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
+    if (m.max_ind != 1 && !grids) sdf_pairs_kernel<false, false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
+    if (m.max_ind != 1 && grids) sdf_pairs_kernel<false, true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
     return cudaGetLastError();
   }
   if (io.input_mode == ETAC_IN_INDENTERS) {
     const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
-    sdf_penetration_kernel<true><<<grid, 256, smem, s>>>(m, io, s1_flags);
+    if (grids) sdf_penetration_kernel<true, true><<<grid, 256, smem, s>>>(m, io, s1_flags);
+    else sdf_penetration_kernel<true, false><<<grid, 256, smem, s>>>(m, io, s1_flags);
   } else {
-    sdf_penetration_kernel<false><<<grid, 256, 0, s>>>(m, io, s1_flags);
+    sdf_penetration_kernel<false, false><<<grid, 256, 0, s>>>(m, io, s1_flags);
   }
   return cudaGetLastError();
 }

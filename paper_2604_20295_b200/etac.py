@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libetac.so")
 
 ETAC_OK, ETAC_ERR_INVALID_ARG, ETAC_ERR_UNSUPPORTED, ETAC_ERR_ALLOC, ETAC_ERR_CUDA, ETAC_ERR_CAPACITY = range(6)
-ETAC_IND_NONE, ETAC_IND_SPHERE, ETAC_IND_BOX, ETAC_IND_CAPSULE = range(4)
+ETAC_IND_NONE, ETAC_IND_SPHERE, ETAC_IND_BOX, ETAC_IND_CAPSULE, ETAC_IND_GRID = range(5)
 ETAC_KERNEL_EXP_L2 = 0
 ETAC_RESID_NONE, ETAC_RESID_PERNODE_MLP, ETAC_RESID_POINTNET = range(3)
 ETAC_PREC_FP32, ETAC_PREC_BF16 = 0, 1
@@ -28,7 +28,7 @@ ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
  ETAC_INFO_LAST_LAUNCHES, ETAC_INFO_LAST_CONTACT_PAIRS, ETAC_INFO_SM_COUNT) = range(1, 9)
 
 EXPORTS = ["etac_create", "etac_destroy", "etac_step", "etac_set_option", "etac_get_info", "etac_last_error",
-           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps"]
+           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid"]
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -78,6 +78,7 @@ def load() -> C.CDLL:
         lib.etac_patches_from_adjacency.argtypes = [C.c_int32, _ip, _ip, _ip, C.c_int32, _ip]
         lib.etac_abi_version.restype = C.c_int32
         lib.etac_time_steps.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_step_args), C.c_int32, _fp, _fp]
+        lib.etac_set_sdf_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
         for name in EXPORTS:
             getattr(lib, name)
         _lib = lib
@@ -179,6 +180,14 @@ def etac_get_info(ctx, key) -> int:
     return v.value
 
 
+def etac_set_sdf_grid(ctx, grid_id, values, origin, spacing) -> None:
+    """values: [nz, ny, nx] fp32 samples (x fastest), origin [3], spacing."""
+    v = _f32(values)
+    nz, ny, nx = v.shape
+    o = _f32(np.asarray(origin, dtype=np.float32).reshape(3))
+    _check(ctx, load().etac_set_sdf_grid(ctx, int(grid_id), nx, ny, nz, _p(o, _fp), C.c_float(float(spacing)), _p(v, _fp)))
+
+
 def etac_last_error(ctx=None) -> str:
     return (load().etac_last_error(ctx) or b"").decode()
 
@@ -221,6 +230,8 @@ class Etac:
         self.ctx = etac_create(m.pos, m.normal, wl.alpha, patch_offset=m.patch_offset, adj_rowptr=m.adj_rowptr,
                                adj_col=m.adj_col, weights=wl.weights if resid else None, max_envs=self.max_envs,
                                max_indenters=wl.max_indenters, precision=prec, active_mode=active_mode, device=device)
+        for gid, (values, origin, spacing) in getattr(wl, "meta", {}).get("grids", {}).items():
+            etac_set_sdf_grid(self.ctx, gid, values, origin, spacing)
         self.N, self.P = m.n_nodes, m.n_patches
         E = self.max_envs
         self.out = torch.empty((E, self.N, 3), dtype=torch.float32, device=self.device)

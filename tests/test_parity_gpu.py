@@ -303,3 +303,44 @@ def test_two_contexts_on_two_streams_are_independent():
     for _ in range(8):
         T.Etac(wa).close()
     assert torch.cuda.mem_get_info()[0] >= free0 - (8 << 20)     # no leak across create/destroy
+
+
+def _grid_workload(mesh_kind, n_envs, seed):
+    """Objects given as SAMPLED signed-distance fields (ETAC_IND_GRID): a rounded box sampled at
+    0.5 mm on a 41^3 grid, pressed on random nodes; half of the envs also get an analytic sphere."""
+    rng = np.random.default_rng(300 + seed)
+    base = W.config3(seed, n_envs) if mesh_kind == "hand" else W.config2(seed, n_envs)
+    mesh = base.mesh
+    h, n = 0.5, 41
+    ax = -10.0 + h * np.arange(n)
+    Z, Y, X = np.meshgrid(ax, ax, ax, indexing="ij")
+    q = np.stack([np.abs(X) - 4.0, np.abs(Y) - 3.0, np.abs(Z) - 5.0], 0)             # box 4 x 3 x 5 ...
+    vals = (np.linalg.norm(np.maximum(q, 0), axis=0) + np.minimum(q.max(0), 0) - 1.0).astype(np.float32)   # ... rounded by 1
+    ind = W._blank_indenters(n_envs, 2)
+    c = rng.integers(0, mesh.n_nodes, n_envs)
+    d = rng.uniform(0.2, 1.4, n_envs)
+    centre, quat = W._press_on_node(mesh.pos, mesh.normal, c, None, np.full(n_envs, 6.0), d, rng.uniform(0, 6.28, n_envs))
+    ind["type"][:, 0] = T.ETAC_IND_GRID
+    ind["param"][:, 0, 0] = 2.0                                                        # grid id
+    ind["pose"][:, 0, 0:3], ind["pose"][:, 0, 3:7] = centre, quat
+    c2 = rng.integers(0, mesh.n_nodes, n_envs)
+    use = rng.random(n_envs) < 0.5
+    cs, qs = W._press_on_node(mesh.pos, mesh.normal, c2, None, np.full(n_envs, 3.0), rng.uniform(0.1, 1.0, n_envs), np.zeros(n_envs))
+    ind["type"][:, 1] = np.where(use, W.IND_SPHERE, W.IND_NONE)
+    ind["param"][:, 1, 0] = 3.0
+    ind["pose"][use, 1, 0:3], ind["pose"][use, 1, 3:7] = cs[use], qs[use]
+    meta = {"grids": {2: (vals, (-10.0, -10.0, -10.0), h)}}
+    return W.Workload("grid_sdf_" + mesh_kind, mesh, base.alpha, base.weights, n_envs, 2, ind, None, base.precision, meta)
+
+
+@pytest.mark.parametrize("mesh_kind,n_envs", [("hand", 21), ("cap", 12)])
+def test_sampled_sdf_grid_indenters(mesh_kind, n_envs):
+    wl = _grid_workload(mesh_kind, n_envs, 1)
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    assert ref["mask"].any() and ref["mask"].sum() > 50
+    tol = TOL[wl.precision]
+    _report(f"grid sdf {mesh_kind}", compare(gpu, ref, tol, resid_tol=5e-2 if wl.precision == "bf16" else 1e-4,
+                                             label="grid-sdf", delta_tol=1e-4))
+    # the sampled field is close to the analytic rounded box it was sampled from (h^2 bound): the
+    # penetrations differ by well under the grid spacing
+    assert float(np.abs(ref["delta"]).max()) > 0.2
