@@ -132,7 +132,7 @@ typedef struct {
 etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args);
 
 /* Options / introspection. */
-enum { ETAC_OPT_PATH = 1 };
+enum { ETAC_OPT_PATH = 1, ETAC_OPT_ABLATION = 2 };
 enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
 /* DENSE : tcgen05 tensor-core contraction K_p . U^ (needs ETAC_PREC_BF16);
  * SPARSE: gather over the active nodes only (Omega U_a literally).  FP32 context: fp32 SIMT kernel,
@@ -140,6 +140,10 @@ enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
  *         selecting it allocates the active-node lists (16 bytes x max_envs x N), which is why the
  *         choice is made with etac_set_option and never inside etac_step;
  * AUTO  : DENSE for BF16 contexts, SPARSE for FP32 contexts. */
+/* ETAC_OPT_ABLATION: the rows of Table II as run-time modes.  FULL (default):
+ * U_p = Omega U_a + Phi_p.  RESIDUAL_ONLY: U_p = Phi_p ("Residual Network Only").  "Linear Decay
+ * Only" is a context created with ETAC_RESID_NONE. */
+enum { ETAC_ABLATE_FULL = 0, ETAC_ABLATE_RESIDUAL_ONLY = 1 };
 etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value);
 
 enum {

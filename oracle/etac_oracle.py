@@ -43,6 +43,7 @@ class OracleModel:
     weights: dict | None = None   # per-node MLP: W1 b1 W2 b2 W3 b3 (reading R10); None = no residual
     resid_arch: str = "pernode"   # "none" | "pernode" | "pointnet"
     active_mode: str = "passthrough"   # "passthrough" (mask M_p) | "propagate"
+    ablation: str = "full"        # "full" | "residual_only" (Table II rows)
     grids: dict = field(default_factory=dict)   # id -> (values [nz,ny,nx] fp32, origin [3], spacing): sampled SDFs
     _K: dict = field(default_factory=dict)
 
@@ -271,7 +272,7 @@ def step(model: OracleModel, indenters=None, patch_pose=None, penetration=None, 
                 r = residual_pointnet(model.weights, uhat[lo:hi], pos[lo:hi], nrm[lo:hi])
             else:
                 raise ValueError(model.resid_arch)
-            U = ulin + r
+            U = ulin + r if model.ablation == "full" else r + 0.0 * ulin   # "Residual Network Only": U_p = Phi_p
             if model.active_mode == "passthrough":                # mask M_p, reading R4
                 U = np.where(act[:, None], uhat[lo:hi], U)
             out["U"][oi, lo:hi] = U

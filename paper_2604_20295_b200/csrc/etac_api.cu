@@ -474,6 +474,11 @@ etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* ar
 
 etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return ETAC_ERR_INVALID_ARG;
+  if (key == ETAC_OPT_ABLATION) {
+    if (value != ETAC_ABLATE_FULL && value != ETAC_ABLATE_RESIDUAL_ONLY) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_ABLATION value");
+    ctx->m.residual_only = value == ETAC_ABLATE_RESIDUAL_ONLY;
+    return ETAC_OK;
+  }
   if (key != ETAC_OPT_PATH) return fail(ctx, ETAC_ERR_INVALID_ARG, "unknown option");
   if (value != ETAC_PATH_AUTO && value != ETAC_PATH_DENSE && value != ETAC_PATH_SPARSE)
     return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_PATH value");

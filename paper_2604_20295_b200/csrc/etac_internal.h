@@ -72,6 +72,7 @@ struct DevModel {
   int32_t ldu;                // row pitch (elements) of uhat_t
   int32_t max_envs, max_ind;
   int32_t resid, active_mode;
+  int32_t residual_only;      // ETAC_OPT_ABLATION: passive rows get Phi_p without the linear term
   const float4* pos4;         // [N] (x,y,z,0)
   const float4* nrm4;         // [N]
   const PatchInfo* patch;     // [P]

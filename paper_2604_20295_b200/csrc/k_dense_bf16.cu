@@ -547,7 +547,8 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         if (more) request_layer1(nxt, un);  // layer 3 has been read: the operand region is free
         PROF_MARK(3);  // next unit's layer-1 operand + arrive
         if (valid && kMode != kModePnEncode) {  // S4: mask M_p + combine (Eq. 2); active rows keep u^ = -delta n in fp32
-          float ox = cur.ux + rx, oy = cur.uy + ry, oz = cur.uz + rz;
+          const float lin = m.residual_only ? 0.0f : 1.0f;  // Table II ablation "Residual Network Only"
+          float ox = fmaf(lin, cur.ux, rx), oy = fmaf(lin, cur.uy, ry), oz = fmaf(lin, cur.uz, rz);
           if (cur.dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH)
             ox = -cur.dl * nrm.x, oy = -cur.dl * nrm.y, oz = -cur.dl * nrm.z;
           float* o = io.out + cur.node * 3;

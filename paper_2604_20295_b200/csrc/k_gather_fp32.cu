@@ -100,7 +100,8 @@ __global__ void __launch_bounds__(kGatherChunk) gather_fp32_kernel(DevModel m, S
       r1 = fmaf(W3[kHidden + k2], h2, r1);
       r2 = fmaf(W3[2 * kHidden + k2], h2, r2);
     }
-    ox += r0, oy += r1, oz += r2;
+    if (m.residual_only) ox = r0, oy = r1, oz = r2;  // Table II ablation "Residual Network Only"
+    else ox += r0, oy += r1, oz += r2;
   }
   const float d = delta[li];
   if (d > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH) {

@@ -22,7 +22,8 @@ ETAC_RESID_NONE, ETAC_RESID_PERNODE_MLP, ETAC_RESID_POINTNET = range(3)
 ETAC_PREC_FP32, ETAC_PREC_BF16 = 0, 1
 ETAC_ACTIVE_PASSTHROUGH, ETAC_ACTIVE_PROPAGATE = 0, 1
 ETAC_IN_INDENTERS, ETAC_IN_PENETRATION = 0, 1
-ETAC_OPT_PATH = 1
+ETAC_OPT_PATH, ETAC_OPT_ABLATION = 1, 2
+ETAC_ABLATE_FULL, ETAC_ABLATE_RESIDUAL_ONLY = 0, 1
 ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
 (ETAC_INFO_N_NODES, ETAC_INFO_N_PATCHES, ETAC_INFO_MAX_ENVS, ETAC_INFO_DEVICE_BYTES, ETAC_INFO_LAST_PATH,
  ETAC_INFO_LAST_LAUNCHES, ETAC_INFO_LAST_CONTACT_PAIRS, ETAC_INFO_SM_COUNT) = range(1, 9)

@@ -344,3 +344,26 @@ def test_sampled_sdf_grid_indenters(mesh_kind, n_envs):
     # the sampled field is close to the analytic rounded box it was sampled from (h^2 bound): the
     # penetrations differ by well under the grid spacing
     assert float(np.abs(ref["delta"]).max()) > 0.2
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_ablation_residual_only(precision):
+    """Table II's "Residual Network Only" row as a run-time mode: passive rows get Phi_p alone."""
+    import dataclasses
+    from oracle import etac_oracle as O
+    wl = dataclasses.replace(W.config3(11, 19), weights=W.make_weights(3, 2, std=0.2))
+    m = O.model_from_workload(wl)
+    m.ablation = "residual_only"
+    ref = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)
+    import torch
+    eng = T.Etac(wl, precision=precision, debug_outputs=True)
+    try:
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_ABLATION, T.ETAC_ABLATE_RESIDUAL_ONLY)
+        U = eng.step(wl.n_envs, eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)).cpu().numpy()
+    finally:
+        eng.close()
+    full = run_oracle(wl)
+    assert np.abs(ref["U"] - full["U"]).max() > 0.1                      # the mode changes the answer
+    tol = (1e-4 if precision == "fp32" else 5e-2) * np.abs(ref["U"][~ref["mask"]]).max()
+    assert np.abs(U - ref["U"])[~ref["mask"]].max() <= tol
+    np.testing.assert_allclose(U[ref["mask"]], full["U"][ref["mask"]], atol=2e-5)            # active rows keep u^
