@@ -15,7 +15,8 @@
  *     "device" pointers must be CUDA device memory on the ctx's device, owned by the caller and
  *     kept alive until the stream reaches the end of the step.
  *   - etac_step only enqueues work on the given CUDA stream: no host synchronisation, no
- *     allocation, no host<->device copy of per-step data.  One in-flight stream per ctx;
+ *     allocation, no host<->device copy of per-step data (so a step can be captured in a CUDA graph and
+ *     replayed).  One in-flight stream per ctx;
  *     different ctxs are independent.  Each step depends only on its arguments (the model is
  *     quasi-static).
  *   - Units are the caller's: alpha is in 1/(unit of node_pos).  The synthetic workloads use mm.

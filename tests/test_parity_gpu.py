@@ -367,3 +367,29 @@ def test_ablation_residual_only(precision):
     tol = (1e-4 if precision == "fp32" else 5e-2) * np.abs(ref["U"][~ref["mask"]]).max()
     assert np.abs(U - ref["U"])[~ref["mask"]].max() <= tol
     np.testing.assert_allclose(U[ref["mask"]], full["U"][ref["mask"]], atol=2e-5)            # active rows keep u^
+
+
+def test_step_is_capturable_in_a_cuda_graph():
+    """etac_step only enqueues (no sync, no allocation, no host copy): it can be captured in a
+    CUDA graph and replayed; the replays give the eager result bit for bit."""
+    import torch
+    for wl in (W.config2(13, 16), W.config3(13, 40)):
+        eng = T.Etac(wl)
+        try:
+            dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+            eager = eng.step(wl.n_envs, dev).clone()
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            side = torch.cuda.Stream()
+            with torch.cuda.stream(side):
+                eng.step(wl.n_envs, dev)                      # warm-up on the capture stream
+                torch.cuda.synchronize()
+                with torch.cuda.graph(g, stream=side):
+                    eng.step(wl.n_envs, dev)
+            for _ in range(3):
+                eng.out.fill_(float("nan"))
+                g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(eng.out[: wl.n_envs], eager)
+        finally:
+            eng.close()
