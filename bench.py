@@ -129,7 +129,10 @@ def run_reference(a):
         return
     label, make = WORKLOADS[a.workload]
     wl = make(0, a.envs)
-    n_sample = min(a.envs, 96 if a.workload == "cfg3" else 8)
+    # each step = the oracle on a strided sample of the batch, sized from a probe so that the whole
+    # --steps K --warmup W run stays within about two minutes
+    probe_rate = time_oracle(wl, min(a.envs, 8))[0]
+    n_sample = int(max(4, min(a.envs, 96, 120.0 * probe_rate / max(1, a.steps + a.warmup))))
     t_w = [time_oracle(wl, n_sample)[0] for _ in range(a.warmup)]
     t0 = time.perf_counter()
     envs_done = 0
