@@ -176,15 +176,26 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     mbar_init(&bars->acc_empty, 8);
     for (int s = 0; s < 2; ++s) mbar_init(&bars->a_ready[s], 4), mbar_init(&bars->d_ready[s], 1);
     fence_barrier_init();
-    int acc = 0;
-    prefix[0] = 0;
-    for (int p = 0; p < m.n_patches; ++p) {
-      const int cnt = m.count[p];
-      acc += ((cnt + TE - 1) / TE) * ((m.patch[p].n + BM - 1) / BM);
-      prefix[p + 1] = acc;
-    }
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB);
+  }
+  if (warp == 2) {
+    // prefix[p] = first work index of patch p: warp scan, 32 patches per sweep (the per-patch counts
+    // and sizes are global loads: issued in parallel instead of one dependent chain by one thread)
+    int carry = 0;
+    for (int p0 = 0; p0 < m.n_patches; p0 += 32) {
+      const int p = p0 + lane;
+      int v = 0;
+      if (p < m.n_patches) v = ((m.count[p] + TE - 1) / TE) * ((m.patch[p].n + BM - 1) / BM);
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int o = __shfl_up_sync(0xffffffffu, v, d);
+        if (lane >= d) v += o;
+      }
+      if (p < m.n_patches) prefix[p + 1] = carry + v;
+      carry += __shfl_sync(0xffffffffu, v, 31);
+    }
+    if (lane == 0) prefix[0] = 0;
   }
   if (warp == 1) tmem_alloc<kTmemCols>(&bars->tmem_base);
   if constexpr (kResid) {
