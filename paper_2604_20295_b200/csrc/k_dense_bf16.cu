@@ -20,6 +20,14 @@
 // evaluates the SiLUs of slot 1 and vice versa; with 2 CTAs per SM every SM sub-partition has 4
 // epilogue warps to hide the MMA round trips and TMEM load latency behind the MUFU pipe.
 //
+// Within a slot the units of an item are software-pipelined (the next unit's u_lin is fetched behind
+// the last layer's round trip, its layer-1 operand is requested before the current unit is stored)
+// and the accumulator is released one unit before the item ends.
+//
+// Template variants (one source, see kMode / kGather below): per-node MLP or none; the PointNet form
+// of Phi as an encoder pass with max-pool and a decoder pass; and the gather form of the propagation
+// (Omega U_a over the active-node lists) instead of the dense contraction.
+//
 // TMEM columns (fp32 lanes = nodes):   [0,48)   u_lin accumulator, column 3*env+c
 //   slot s at 48 + 104*s:              [+0,+64)   D: pre-activations of the current MLP layer
 //                                      [+64,+104) A: bf16 layer input; layer 1 uses words 0..7
