@@ -393,10 +393,9 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
       for (int k = 0; k < 64; ++k) put(kW1ImgBytes, n, k, 64, 0.5f * d->W2[n * 64 + k]);
       put(kW1ImgBytes, n, 64, 64, 0.5f * d->b2[n]);
     }
-    for (int n = 0; n < 3; ++n) {
-      for (int k = 0; k < 64; ++k) put(kW1ImgBytes + kW2ImgBytes, n, k, 16, d->W3[n * 64 + k]);
-      put(kW1ImgBytes + kW2ImgBytes, n, 64, 16, d->b3[n]);
-    }
+    memcpy(m.wout, d->W3, 192 * 4);  // the output layer runs on the FMA pipe in fp32
+    memcpy(m.wout + 192, d->b3, 3 * 4);
+    m.wout[195] = 0.0f;
     CK(dev_upload(c, &m.wimg, img.data(), img.size()), "upload weight image");
   }
 
@@ -408,7 +407,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
       const uint16_t b = f2bf(v);
       memcpy(&img[base + wimg_off(n, k, rows)], &b, 2);
     };
-    const size_t o1 = kW1ImgBytes, o2 = o1 + kW2ImgBytes, o3 = o2 + kW2ImgBytes;
+    const size_t o1 = kW1ImgBytes, o2 = o1 + kW2ImgBytes;
     for (int n = 0; n < 64; ++n) {
       for (int k = 0; k < 3; ++k) {
         put(0, n, k, 64, 0.5f * d->E1[n * 9 + 6 + k]);      // u^
@@ -420,10 +419,9 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
       put(o1, n, 64, 64, 0.5f * d->e2[n]);
       for (int k = 0; k < 64; ++k) put(o2, n, k, 64, 0.5f * d->D1[n * 128 + k]);  // bias column stays 0: c_(e,p) is added in the epilogue
     }
-    for (int n = 0; n < 3; ++n) {
-      for (int k = 0; k < 64; ++k) put(o3, n, k, 16, d->D2[n * 64 + k]);
-      put(o3, n, 64, 16, d->d2[n]);
-    }
+    memcpy(m.wout, d->D2, 192 * 4);
+    memcpy(m.wout + 192, d->d2, 3 * 4);
+    m.wout[195] = 0.0f;
     CK(dev_upload(c, &m.wimg_pn, img.data(), img.size()), "upload PointNet weight image");
     std::vector<float> pf(4096 + 64 + 4096 + 64);
     for (int n = 0; n < 64; ++n)      // both 64 x 64 matrices transposed to [in][out] (coalesced over the outputs)

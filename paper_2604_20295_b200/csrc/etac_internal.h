@@ -41,10 +41,11 @@ constexpr int kDenseBN = kDenseTE * 3;
 // SWIZZLE_NONE core-matrix layout; see k_dense_bf16.cu).
 constexpr int kW1ImgBytes = 64 * 16 * 2;   // N=64,  K=16   (9 inputs + bias column)
 constexpr int kW2ImgBytes = 64 * 80 * 2;   // N=64,  K=80   (64 + bias column, padded to 5 k-steps)
-constexpr int kW3ImgBytes = 16 * 80 * 2;   // N=16,  K=80   (3 outputs padded to 16)
-constexpr int kWImgBytes = kW1ImgBytes + kW2ImgBytes + kW3ImgBytes;
+// The output layer (3 x 64) is not an MMA: the epilogue applies it with FFMAs to the fp32 SiLU
+// outputs it holds in registers (DevModel::wout), which saves one tensor-core round trip per unit.
+constexpr int kWImgBytes = kW1ImgBytes + kW2ImgBytes;
 // PointNet form: E1 [64 x 16] | E2 [64 x 80] | D1[:, 0:64] [64 x 80, zero bias column] | D2 [16 x 80]
-constexpr int kPnImgBytes = kW1ImgBytes + 2 * kW2ImgBytes + kW3ImgBytes;
+constexpr int kPnImgBytes = kW1ImgBytes + 2 * kW2ImgBytes;
 
 // Active node of a contacting (env, patch) pair, for the gather form of the propagation:
 // u^ of the node (fp32) and its index within the patch.
@@ -86,6 +87,7 @@ struct DevModel {
   const float* pn_f32;        // G1^T [in][out] g1[64] D1[:,64:128]^T [in][out] d1[64] (fp32, pn_global_kernel)
   uint32_t* gmax;             // [P x max_envs x 64] max-pooled encoder features as order-preserving keys
   float* cvec;                // [P x max_envs x 64] c_(e,p) / 2
+  float wout[196];            // output layer of Phi in fp32: W3 (or D2) [3 x 64] row-major, then b3 (d2) at 192..194
   // per-step workspace
   float* delta;               // [max_envs x N]
   __nv_bfloat16* uhat_t;      // [3*max_envs (+pad) x ldu]: row slot*3+c, column = node j

@@ -3,9 +3,11 @@
 //   S2  u_lin = K_p . U^  as a dense bf16 contraction with fp32 accumulation in TMEM
 //       ("propagation matrix Omega ... computed as Omega U_a"; the zero rows of the
 //       zero-padded U^ contribute nothing, R3),
-//   S3  residual MLP 9 -> 64 -> 64 -> 3 (SiLU) on the accumulator tile, each layer one small
-//       tcgen05.mma whose A operand is written to TMEM by the epilogue warps and whose B operand
-//       (the weights, biases folded in as an extra K column) stays in shared memory,
+//   S3  residual MLP 9 -> 64 -> 64 -> 3 (SiLU) on the accumulator tile: the two hidden layers are
+//       small tcgen05.mma's whose A operand is written to TMEM by the epilogue warps and whose B
+//       operand (the weights, biases folded in as an extra K column) stays in shared memory; the
+//       3 x 64 output layer is applied in fp32 by the epilogue to the SiLU outputs it holds in
+//       registers (packed fma.rn.f32x2), which saves a tensor-core round trip per unit,
 //   S4  mask M_p + combine (Eq. 2) and the store of U[e][i][0..2]; the rows of
 //       contact-free (env, patch) pairs are zero-filled by the MLP issuer warps (R8).
 //
@@ -31,8 +33,8 @@
 // TMEM columns (fp32 lanes = nodes):   [0,48)   u_lin accumulator, column 3*env+c
 //   slot s at 48 + 104*s:              [+0,+64)   D: pre-activations of the current MLP layer
 //                                      [+64,+104) A: bf16 layer input; layer 1 uses words 0..7
-//                                                 [u_lin(3), p(3), n(3), 1, 0..], layers 2/3 use
-//                                                 64 activations + a ones column (word 32)
+//                                                 [u_lin(3), p(3), n(3), 1, 0..], the K = 80 layers
+//                                                 use 64 activations + a ones column (word 32)
 #include "etac_internal.h"
 #include "sm100_prims.cuh"
 
@@ -61,7 +63,8 @@ struct __align__(8) DenseBars {
 //   kModePnDecode: propagation as usual; f_i again; D1[:, :64] f_i + c_(e,p) -> SiLU -> D2 -> r
 // where c_(e,p) = D1[:, 64:] silu(G1 g + g1) + d1 comes from pn_global_kernel.
 constexpr int kModeNone = 0, kModePerNode = 1, kModePnEncode = 2, kModePnDecode = 3;
-__host__ __device__ constexpr int mode_layers(int mode) { return mode == 1 ? 3 : mode == 2 ? 2 : mode == 3 ? 4 : 0; }
+// layers that run as MMAs, each followed by a SiLU granule (the 3 x 64 output layer runs in the epilogue)
+__host__ __device__ constexpr int mode_layers(int mode) { return mode == 1 ? 2 : mode == 2 ? 2 : mode == 3 ? 3 : 0; }
 __host__ __device__ constexpr int mode_stages(int mode) { return mode == 3 ? 3 : 4; }  // shared memory: 2 CTAs per SM
 __host__ __device__ constexpr int mode_img_bytes(int mode) {
   return mode == 1 ? kWImgBytes : mode == 2 ? kW1ImgBytes + kW2ImgBytes : mode == 3 ? kPnImgBytes : 0;
@@ -248,13 +251,8 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are issued by one elected lane.
     {
       constexpr uint32_t idesc_prop = make_idesc_bf16(BM, BN);
-      constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
-      constexpr uint32_t idesc_o = make_idesc_bf16(BM, 16);
-      const uint64_t dW1 = make_desc(smem_u32(sW), 1024, 128, kLayoutNone);
-      const uint64_t dW2 = make_desc(smem_u32(sW + kW1ImgBytes), 1024, 128, kLayoutNone);
-      const uint64_t dW3 = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 256, 128, kLayoutNone);
       int pcur = 0, stage = 0;
-      uint32_t ph = 0, acc_ph = 0, a_ph = 0;
+      uint32_t ph = 0, acc_ph = 0;
       Item it;
       for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
         const int nkb = (m.patch[it.p].n + BK - 1) / BK;
@@ -290,12 +288,9 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     if constexpr (kResid) {
       const int sl = warp - 2;
       constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
-      constexpr uint32_t idesc_o = make_idesc_bf16(BM, 16);
       const uint64_t dW1 = make_desc(smem_u32(sW), 1024, 128, kLayoutNone);
       const uint64_t dW2 = make_desc(smem_u32(sW + kW1ImgBytes), 1024, 128, kLayoutNone);
-      const uint64_t dW3 = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 256, 128, kLayoutNone);
       const uint64_t dW3h = make_desc(smem_u32(sW + kW1ImgBytes + kW2ImgBytes), 1024, 128, kLayoutNone);
-      const uint64_t dW4 = make_desc(smem_u32(sW + kW1ImgBytes + 2 * kW2ImgBytes), 256, 128, kLayoutNone);
       const uint32_t tD = tmem + COL_SLOT0 + SLOT_STRIDE * sl, tA = tD + OFF_A;
       uint64_t* a_ready = &bars->a_ready[sl];
       uint64_t* d_ready = &bars->d_ready[sl];
@@ -309,13 +304,9 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
             mbar_wait(a_ready, a_ph), a_ph ^= 1;
             tc_fence_after();
             if (elect_one()) {
-              // weight image: [64 x 16] | [64 x 80] | per-node: [16 x 80]; PointNet: [64 x 80] | [16 x 80]
+              // weight image: [64 x 16] | [64 x 80] | PointNet decoder: [64 x 80]
               if (layer == 0) {
                 mma_ts(tD, tA, dW1, idesc_h, 0);
-              } else if (layer == kLayers - 1 && kMode != kModePnEncode) {
-                const uint64_t dWo = kMode == kModePnDecode ? dW4 : dW3;
-#pragma unroll
-                for (int k = 0; k < 5; ++k) mma_ts(tD, tA + 8 * k, dWo + (uint64_t)(k * (512 >> 4)), idesc_o, k != 0);
               } else {
                 const uint64_t dWh = layer == 1 ? dW2 : dW3h;
 #pragma unroll
@@ -381,7 +372,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         tc_fence_after();
       }
       PROF_MARK(1);  // acc_full wait
-      // The units of an item are software-pipelined: while the tensor core runs layer 3 of unit
+      // The units of an item are software-pipelined: while the tensor core runs the last MMA layer of unit
       // el, the u_lin of unit el+2 is already fetched from the accumulator, and its layer-1 operand
       // is written (and requested) before the output of unit el is combined and stored.  Every
       // TMEM access costs a few hundred cycles of latency; this takes two of them per unit off
@@ -477,94 +468,119 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         const bool more = el + 2 < it.cnt;
         float rx = 0.f, ry = 0.f, rz = 0.f;
         uint32_t un[4] = {0, 0, 0, 0};
+        // The next unit's layer-1 operand and request; the operand region is free once the last MMA layer
+        // has been read.  Placement matters more than it should: issuing this (or the accumulator
+        // release, or anything else with a warp-level sync) between the TMEM loads of the last
+        // granule and its SiLUs costs 5-8 % (measured), so it sits after the granule.
+        auto request_next = [&]() {
+          if (more && el + 4 >= it.cnt) release_acc();
+          if (more) request_layer1(nxt, un);
+          PROF_MARK(3);  // next unit's layer-1 operand + arrive
+        };
         if constexpr (kResid) {
-          // SiLU granules after every layer but the last; the decoder's layer 2 adds the
-          // per-(env, patch) vector c (halved like the weights), the encoder's layer 1 is max-pooled
-          const float4* cv = nullptr;
-          if constexpr (kMode == kModePnDecode)
-            cv = reinterpret_cast<const float4*>(m.cvec + ((int64_t)it.p * m.max_envs + cur.slot) * 64);
-          uint32_t pool0 = 0, pool1 = 0;  // lane l: max keys of hidden columns l and 32 + l
-          constexpr int kGranules = kMode == kModePnEncode ? kLayers : kLayers - 1;  // layers followed by a SiLU
+          // One SiLU granule per MMA layer.  The inner granules write the next layer's bf16 operand
+          // back to TMEM and request the layer; the last one keeps its fp32 outputs in registers and
+          // applies the 3 x 64 output layer on the FMA pipe (per-node MLP / decoder) or max-pools
+          // them over the rows (encoder).  The decoder's last layer adds the per-(env, patch)
+          // vector c (halved like the weights).
+          uint32_t ha[32], hb[32];
 #pragma unroll 1
-          for (int layer = 0; layer < kGranules; ++layer) {
+          for (int layer = 0; layer < kLayers - 1; ++layer) {
             mbar_wait(d_ready, d_ph), d_ph ^= 1;
             tc_fence_after();
             PROF_MARK(4);  // d_ready wait
             // both halves are requested at once: one TMEM load latency per layer instead of two
-            uint32_t ha[32], hb[32], packed[16];
+            uint32_t packed[16];
             tmem_ld32(tD, ha);
             tmem_ld32(tD + 32, hb);
             tc_wait_ld();
-            const bool add_c = kMode == kModePnDecode && layer == 2;
-            const bool pool = kMode == kModePnEncode && layer == 1;
 #pragma unroll
             for (int half = 0; half < 2; ++half) {
               uint32_t(&h)[32] = half ? hb : ha;
-              if (add_c) {
-#pragma unroll
-                for (int k = 0; k < 8; ++k) {
-                  const float4 c4 = __ldg(cv + half * 8 + k);
-                  h[4 * k] = __float_as_uint(__uint_as_float(h[4 * k]) + c4.x);
-                  h[4 * k + 1] = __float_as_uint(__uint_as_float(h[4 * k + 1]) + c4.y);
-                  h[4 * k + 2] = __float_as_uint(__uint_as_float(h[4 * k + 2]) + c4.z);
-                  h[4 * k + 3] = __float_as_uint(__uint_as_float(h[4 * k + 3]) + c4.w);
-                }
-              }
 #pragma unroll
               for (int k = 0; k < 16; ++k) {
                 // D holds x/2 (0.5 folded into the weights): silu(x) = x*sigmoid(x) = h + h*tanh(h)
-                const float h0 = __uint_as_float(h[2 * k]), h1 = __uint_as_float(h[2 * k + 1]);
-                const float y0 = fmaf(h0, tanh_approx(h0), h0), y1 = fmaf(h1, tanh_approx(h1), h1);
+                float y0, y1;
+                unpack_f32x2(silu_half_x2(__uint_as_float(h[2 * k]), __uint_as_float(h[2 * k + 1])), y0, y1);
                 packed[k] = pack_bf16(y0, y1);
-                if constexpr (kMode == kModePnEncode) {
-                  if (pool) {  // column max over the warp's 32 rows.  silu >= -0.279, so 1 + silu is a
-                               // positive float whose bit pattern orders like the value; 0 = no row
-                    const uint32_t k0 = valid ? __float_as_uint(1.0f + y0) : 0u, k1 = valid ? __float_as_uint(1.0f + y1) : 0u;
-                    const uint32_t m0 = __reduce_max_sync(0xffffffffu, k0), m1 = __reduce_max_sync(0xffffffffu, k1);
-                    if (lane == ((2 * k) & 31)) (half ? pool1 : pool0) = m0;
-                    if (lane == ((2 * k + 1) & 31)) (half ? pool1 : pool0) = m1;
-                  }
-                }
               }
-              if (!pool) tmem_st16(tA + 16 * half, packed);
+              tmem_st16(tA + 16 * half, packed);
             }
             PROF_MARK(6);  // D load + SiLU + operand stores issued
-            if (!pool) {
-              tc_wait_st();
-              tc_fence_before();
-              __syncwarp();
-              if (lane == 0) mbar_arrive(a_ready);
-            }
+            tc_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(a_ready);
             PROF_MARK(7);  // store wait + arrive
           }
+          // ---- last granule
+          if (more) fetch_unit(nxt, el + 2, un);  // overlaps the last layer's round trip
+          mbar_wait(d_ready, d_ph), d_ph ^= 1;
+          tc_fence_after();
+          PROF_MARK(8);  // d_ready wait (last layer)
+          tmem_ld32(tD, ha);
+          tmem_ld32(tD + 32, hb);
+          tc_wait_ld();
+          PROF_MARK(9);  // D (and next u_lin) load
           if constexpr (kMode == kModePnEncode) {
+            uint32_t pool0 = 0, pool1 = 0;  // lane l: max keys of hidden columns l and 32 + l
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+              uint32_t(&h)[32] = half ? hb : ha;
+#pragma unroll
+              for (int k = 0; k < 32; ++k) {
+                // column max over the warp's 32 rows.  silu >= -0.279, so 1 + silu is a positive
+                // float whose bit pattern orders like the value; 0 = no row
+                const float h0 = __uint_as_float(h[k]);
+                const float y0 = fmaf(h0, tanh_approx(h0), h0);
+                const uint32_t k0 = valid ? __float_as_uint(1.0f + y0) : 0u;
+                const uint32_t m0 = __reduce_max_sync(0xffffffffu, k0);
+                if (lane == k) (half ? pool1 : pool0) = m0;
+              }
+            }
             uint32_t* gm = m.gmax + ((int64_t)it.p * m.max_envs + cur.slot) * 64;
             atomicMax(gm + lane, pool0);
             atomicMax(gm + 32 + lane, pool1);
-            if (more) {
-              fetch_unit(nxt, el + 2, un);
-              tc_wait_ld();
-            }
           } else {
-            if (more) fetch_unit(nxt, el + 2, un);  // overlaps the last layer's round trip
-            mbar_wait(d_ready, d_ph), d_ph ^= 1;
-            tc_fence_after();
-            PROF_MARK(8);  // d_ready wait (last layer)
-            uint32_t rr[4];
-            tmem_ld4(tD, rr);
-            tc_wait_ld();
-            rx = __uint_as_float(rr[0]), ry = __uint_as_float(rr[1]), rz = __uint_as_float(rr[2]);
+            const float4* cv = nullptr;
+            if constexpr (kMode == kModePnDecode)
+              cv = reinterpret_cast<const float4*>(m.cvec + ((int64_t)it.p * m.max_envs + cur.slot) * 64);
+            // even / odd hidden columns accumulate in the two halves of packed fp32x2 registers
+            uint64_t ax = pack_f32x2(m.wout[192], 0.f), ay = pack_f32x2(m.wout[193], 0.f), az = pack_f32x2(m.wout[194], 0.f);
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+              uint32_t(&h)[32] = half ? hb : ha;
+#pragma unroll
+              for (int k4 = 0; k4 < 8; ++k4) {
+                float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                if constexpr (kMode == kModePnDecode) c4 = __ldg(cv + half * 8 + k4);
+                const float cc[4] = {c4.x, c4.y, c4.z, c4.w};
+#pragma unroll
+                for (int q = 0; q < 4; q += 2) {
+                  const int k = 4 * k4 + q, col = 32 * half + k;
+                  float h0 = __uint_as_float(h[k]), h1 = __uint_as_float(h[k + 1]);
+                  if constexpr (kMode == kModePnDecode) h0 += cc[q], h1 += cc[q + 1];
+                  const uint64_t y = silu_half_x2(h0, h1);
+                  ax = fma_f32x2(y, pack_f32x2(m.wout[col], m.wout[col + 1]), ax);
+                  ay = fma_f32x2(y, pack_f32x2(m.wout[64 + col], m.wout[65 + col]), ay);
+                  az = fma_f32x2(y, pack_f32x2(m.wout[128 + col], m.wout[129 + col]), az);
+                }
+              }
+            }
+            float lo, hi;
+            unpack_f32x2(ax, lo, hi), rx = lo + hi;
+            unpack_f32x2(ay, lo, hi), ry = lo + hi;
+            unpack_f32x2(az, lo, hi), rz = lo + hi;
           }
-          PROF_MARK(9);  // r (and next u_lin) load
+          request_next();
+          PROF_MARK(5);  // last granule: SiLU + output layer / pool
         } else {
           if (more) {
             fetch_unit(nxt, el + 2, un);
             tc_wait_ld();
           }
+          request_next();
         }
-        if (more && el + 4 >= it.cnt) release_acc();
-        if (more) request_layer1(nxt, un);  // layer 3 has been read: the operand region is free
-        PROF_MARK(3);  // next unit's layer-1 operand + arrive
         if (valid && kMode != kModePnEncode) {  // S4: mask M_p + combine (Eq. 2); active rows keep u^ = -delta n in fp32
           const float lin = m.residual_only ? 0.0f : 1.0f;  // Table II ablation "Residual Network Only"
           float ox = fmaf(lin, cur.ux, rx), oy = fmaf(lin, cur.uy, ry), oz = fmaf(lin, cur.uz, rz);
