@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define ETAC_ABI_VERSION 4
+#define ETAC_ABI_VERSION 5
 
 typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
 
@@ -116,8 +116,11 @@ typedef struct {
   const float* d_patch_pose;          /* device [E x P x 7] {t, q} of every patch in the indenters' world frame,
                                          or NULL = identity */
   const float* d_penetration;         /* device [E x N] (PENETRATION mode): delta; negatives clamp to 0 */
-  float* d_out;                       /* device [E x N x 3] fp32 displacement, REQUIRED, fully overwritten;
-                                         patch-local frame (u^ = -delta * n with the create-time normal) */
+  void* d_out;                        /* device displacement U, REQUIRED: element (e, i, c) at index
+                                         e*out_env_stride + 3*i + c of an array of out_dtype; the 3N elements of
+                                         every environment are fully overwritten, the gaps of a strided layout are
+                                         not touched; patch-local frame (u^ = -delta * n with the create-time normal).
+                                         Alignment: that of one element */
   float* d_penetration_out;           /* optional device [E x N]: delta */
   uint32_t* d_mask_out;               /* optional device [E x ceil(N/32)]: bit (i%32) of word i/32 = node i active */
   float* d_analytic_out;              /* optional device [E x N x 3]: unmasked K.U^ on ALL rows
@@ -126,6 +129,11 @@ typedef struct {
                                          patch per link this is the link-contact vector S_cr of PAPER.md:L224 */
   int32_t* d_active_count_out;        /* optional device [E]: n_a = number of active nodes of the environment
                                          (contact ratio R_a = n_a / N) */
+  int64_t out_env_stride;             /* elements between consecutive environments in d_out; 0 = 3N (packed),
+                                         else >= 3N: U lands inside a wider per-env observation row (the n x 3
+                                         tensor is the policy observation) */
+  int32_t out_dtype;                  /* ETAC_OUT_*: fp32 (default) or bf16 (round to nearest even of the fp32 result) */
+  int32_t reserved;                   /* 0 */
 } etac_step_args;
 
 /* Enqueues S1-S4 for n_envs environments on cuda_stream (a cudaStream_t; NULL = default stream).
@@ -142,9 +150,12 @@ enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
  *         choice is made with etac_set_option and never inside etac_step;
  * AUTO  : DENSE for BF16 contexts, SPARSE for FP32 contexts. */
 /* ETAC_OPT_ABLATION: the rows of Table II as run-time modes.  FULL (default):
- * U_p = Omega U_a + Phi_p.  RESIDUAL_ONLY: U_p = Phi_p ("Residual Network Only").  "Linear Decay
- * Only" is a context created with ETAC_RESID_NONE. */
-enum { ETAC_ABLATE_FULL = 0, ETAC_ABLATE_RESIDUAL_ONLY = 1 };
+ * U_p = M_p (Omega U_a + Phi_p) + active part.  RESIDUAL_ONLY: Phi_p without the linear term ("Residual
+ * Network Only").  LINEAR_ONLY: Omega U_a without Phi_p ("Linear Decay Only"; same result as a context
+ * created with ETAC_RESID_NONE).  NO_PROPAGATION: U = U^, i.e. the penalty displacement -delta*n of the
+ * nodes in contact and 0 elsewhere (what a penalty-based simulator without propagation reports). */
+enum { ETAC_ABLATE_FULL = 0, ETAC_ABLATE_RESIDUAL_ONLY = 1, ETAC_ABLATE_LINEAR_ONLY = 2, ETAC_ABLATE_NO_PROPAGATION = 3 };
+enum { ETAC_OUT_F32 = 0, ETAC_OUT_BF16 = 1 };
 etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value);
 
 enum {

@@ -43,7 +43,8 @@ class OracleModel:
     weights: dict | None = None   # per-node MLP: W1 b1 W2 b2 W3 b3 (reading R10); None = no residual
     resid_arch: str = "pernode"   # "none" | "pernode" | "pointnet"
     active_mode: str = "passthrough"   # "passthrough" (mask M_p) | "propagate"
-    ablation: str = "full"        # "full" | "residual_only" (Table II rows)
+    ablation: str = "full"        # Table II rows: "full" | "residual_only" | "linear_only";
+                                  # "no_propagation": U = U_hat, penalty displacement of the contact nodes only
     grids: dict = field(default_factory=dict)   # id -> (values [nz,ny,nx] fp32, origin [3], spacing): sampled SDFs
     _K: dict = field(default_factory=dict)
 
@@ -264,7 +265,10 @@ def step(model: OracleModel, indenters=None, patch_pose=None, penetration=None, 
             ulin = K[:, act] @ uhat[lo:hi][act]
             out["analytic"][oi, lo:hi] = ulin
             # ---- O4 (Eq. 2)
-            if model.resid_arch == "none":
+            if model.ablation == "no_propagation":                # nothing but the contact nodes moves
+                out["U"][oi, lo:hi] = uhat[lo:hi]
+                continue
+            if model.resid_arch == "none" or model.ablation == "linear_only":   # "Linear Decay Only"
                 r = 0.0
             elif model.resid_arch == "pernode":
                 r = residual_pernode(model.weights, ulin, pos[lo:hi], nrm[lo:hi])
@@ -272,7 +276,9 @@ def step(model: OracleModel, indenters=None, patch_pose=None, penetration=None, 
                 r = residual_pointnet(model.weights, uhat[lo:hi], pos[lo:hi], nrm[lo:hi])
             else:
                 raise ValueError(model.resid_arch)
-            U = ulin + r if model.ablation == "full" else r + 0.0 * ulin   # "Residual Network Only": U_p = Phi_p
+            if model.ablation not in ("full", "residual_only", "linear_only"):
+                raise ValueError(model.ablation)
+            U = r + 0.0 * ulin if model.ablation == "residual_only" else ulin + r   # "Residual Network Only": U_p = Phi_p
             if model.active_mode == "passthrough":                # mask M_p, reading R4
                 U = np.where(act[:, None], uhat[lo:hi], U)
             out["U"][oi, lo:hi] = U

@@ -124,6 +124,12 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   if (a->input_mode != ETAC_IN_INDENTERS && a->input_mode != ETAC_IN_PENETRATION)
     return fail(ctx, ETAC_ERR_INVALID_ARG, "bad input_mode");
   if (!a->d_out) return fail(ctx, ETAC_ERR_INVALID_ARG, "d_out is required");
+  if (a->out_dtype != ETAC_OUT_F32 && a->out_dtype != ETAC_OUT_BF16) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad out_dtype");
+  if (a->out_env_stride != 0 && a->out_env_stride < 3 * (int64_t)ctx->m.n_nodes)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "out_env_stride < 3 * n_nodes");
+  if (a->reserved != 0) return fail(ctx, ETAC_ERR_INVALID_ARG, "reserved must be 0");
+  if (reinterpret_cast<uintptr_t>(a->d_out) % (a->out_dtype == ETAC_OUT_BF16 ? 2 : 4))
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "d_out is not aligned to its element type");
   if (a->input_mode == ETAC_IN_INDENTERS && ctx->m.max_ind > 0 && !a->d_indenters)
     return fail(ctx, ETAC_ERR_INVALID_ARG, "d_indenters is NULL");
   if (a->input_mode == ETAC_IN_PENETRATION && !a->d_penetration)
@@ -142,6 +148,8 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   io.n_envs = a->n_envs, io.input_mode = a->input_mode;
   io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
   io.out = a->d_out, io.pen_out = a->d_penetration_out, io.mask_out = a->d_mask_out;
+  io.out_stride = a->out_env_stride ? a->out_env_stride : 3 * (int64_t)ctx->m.n_nodes;
+  io.out_bf16 = a->out_dtype == ETAC_OUT_BF16;
   io.analytic_out = a->d_analytic_out;
   io.contact_out = a->d_contact_out, io.nact_out = a->d_active_count_out;
 
@@ -159,20 +167,36 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   // active-node lists.  fp32 context: fp32 SIMT gather kernel (which needs S1 to zero-fill).
   const bool bf16 = ctx->precision == ETAC_PREC_BF16;
   const bool gather16 = bf16 && path == ETAC_PATH_SPARSE;
-  const int s1_flags = !bf16 ? kS1FillOut : (gather16 ? kS1WriteAlist : kS1WriteUhat);
+  const int abl = ctx->m.ablation;
+  const int s1_flags = abl == ETAC_ABLATE_NO_PROPAGATION ? 0 : !bf16 ? kS1FillOut : (gather16 ? kS1WriteAlist : kS1WriteUhat);
   if (gather16 && !ctx->m.alist) return fail(ctx, ETAC_ERR_INVALID_ARG, "select ETAC_PATH_SPARSE with etac_set_option first");
   if ((e = launch_sdf(ctx->m, io, s1_flags, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
   ++ctx->last_launches;
   if (ev) cudaEventRecord(ev[1], s);
-  if (bf16) {
+  if (abl == ETAC_ABLATE_NO_PROPAGATION) {
+    if ((e = launch_penalty_only(ctx->m, io, s)) != cudaSuccess)
+      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("penalty_only_kernel", e));
+  } else if (bf16) {
     int n_launch = 1;
-    if ((e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s)) != cudaSuccess)
-      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("dense_bf16_kernel", e));
+    if (abl == ETAC_ABLATE_LINEAR_ONLY) {  // "Linear Decay Only": the kernels compiled without Phi
+      DevModel lin = ctx->m;
+      lin.resid = ETAC_RESID_NONE;
+      e = launch_dense_bf16(lin, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s);
+    } else {
+      e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s);
+    }
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("dense_bf16_kernel", e));
     ctx->last_launches += n_launch - 1;
   } else {
-    if ((e = launch_gather_fp32(ctx->m, io, s)) != cudaSuccess)
-      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("gather_fp32_kernel", e));
+    if (abl == ETAC_ABLATE_LINEAR_ONLY) {
+      DevModel lin = ctx->m;
+      lin.resid = ETAC_RESID_NONE;
+      e = launch_gather_fp32(lin, io, s);
+    } else {
+      e = launch_gather_fp32(ctx->m, io, s);
+    }
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("gather_fp32_kernel", e));
   }
   ++ctx->last_launches;
   if (ev) cudaEventRecord(ev[2], s);
@@ -473,8 +497,9 @@ etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* ar
 etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
   if (!ctx) return ETAC_ERR_INVALID_ARG;
   if (key == ETAC_OPT_ABLATION) {
-    if (value != ETAC_ABLATE_FULL && value != ETAC_ABLATE_RESIDUAL_ONLY) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_ABLATION value");
+    if (value < ETAC_ABLATE_FULL || value > ETAC_ABLATE_NO_PROPAGATION) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_ABLATION value");
     ctx->m.residual_only = value == ETAC_ABLATE_RESIDUAL_ONLY;
+    ctx->m.ablation = (int32_t)value;
     return ETAC_OK;
   }
   if (key != ETAC_OPT_PATH) return fail(ctx, ETAC_ERR_INVALID_ARG, "unknown option");

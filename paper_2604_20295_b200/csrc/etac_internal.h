@@ -74,6 +74,7 @@ struct DevModel {
   int32_t max_envs, max_ind;
   int32_t resid, active_mode;
   int32_t residual_only;      // ETAC_OPT_ABLATION: passive rows get Phi_p without the linear term
+  int32_t ablation;           // ETAC_ABLATE_* (LINEAR_ONLY / NO_PROPAGATION select other kernels on the host)
   const float4* pos4;         // [N] (x,y,z,0)
   const float4* nrm4;         // [N]
   const PatchInfo* patch;     // [P]
@@ -105,7 +106,9 @@ struct StepIO {
   const etac_indenter* ind;
   const float* patch_pose;
   const float* pen_in;
-  float* out;
+  void* out;                  // fp32 or bf16 elements (out_bf16), environment e at element e * out_stride
+  int64_t out_stride;
+  int32_t out_bf16;
   float* pen_out;
   uint32_t* mask_out;
   float* analytic_out;
@@ -113,11 +116,50 @@ struct StepIO {
   int32_t* nact_out;
 };
 
+#ifdef __CUDACC__
+// ---- output element access (etac_step_args: d_out, out_env_stride, out_dtype)
+// Streaming zero fill of nbytes (even, < 2^31) at a 2-byte aligned address by nthreads (>= 8) cooperating threads.
+__device__ __forceinline__ void zero_fill_bytes(void* ptr, int nbytes, int tid, int nthreads) {
+  char* p = static_cast<char*>(ptr);
+  const int head = min((int)((16u - (uint32_t)((uintptr_t)p & 15u)) & 15u), nbytes);
+  if (2 * tid < head) __stcs(reinterpret_cast<unsigned short*>(p + 2 * tid), (unsigned short)0);
+  uint4* body = reinterpret_cast<uint4*>(p + head);
+  const int nvec = (nbytes - head) >> 4;
+  for (int v = tid; v < nvec; v += nthreads) __stcs(body + v, make_uint4(0u, 0u, 0u, 0u));
+  const int tail0 = head + (nvec << 4);
+  if (tail0 + 2 * tid < nbytes) __stcs(reinterpret_cast<unsigned short*>(p + tail0 + 2 * tid), (unsigned short)0);
+}
+// rows [g0, g0 + n_rows) of environment env of the displacement output := 0
+__device__ __forceinline__ void zero_out_rows(const StepIO& io, int env, int g0, int n_rows, int tid, int nthreads) {
+  const int sh = io.out_bf16 ? 1 : 2;
+  char* p = static_cast<char*>(io.out) + (((int64_t)env * io.out_stride + 3 * g0) << sh);
+  zero_fill_bytes(p, (n_rows * 3) << sh, tid, nthreads);
+}
+// U[env][g][0..2] := (x, y, z), streaming; kDtype: ETAC_OUT_F32 / ETAC_OUT_BF16, or -1 = io.out_bf16 decides
+template <int kDtype = -1>
+__device__ __forceinline__ void store_out3_at(const StepIO& io, int64_t o, float x, float y, float z) {
+  if (kDtype == ETAC_OUT_BF16 || (kDtype < 0 && io.out_bf16)) {
+    unsigned short* q = static_cast<unsigned short*>(io.out) + o;
+    __stcs(q, __bfloat16_as_ushort(__float2bfloat16_rn(x)));
+    __stcs(q + 1, __bfloat16_as_ushort(__float2bfloat16_rn(y)));
+    __stcs(q + 2, __bfloat16_as_ushort(__float2bfloat16_rn(z)));
+  } else {
+    float* q = static_cast<float*>(io.out) + o;
+    __stcs(q, x), __stcs(q + 1, y), __stcs(q + 2, z);
+  }
+}
+template <int kDtype = -1>
+__device__ __forceinline__ void store_out3(const StepIO& io, int env, int g, float x, float y, float z) {
+  store_out3_at<kDtype>(io, (int64_t)env * io.out_stride + 3 * (int64_t)g, x, y, z);
+}
+#endif
+
 // kernel launchers (each returns cudaGetLastError())
 cudaError_t launch_build_k(const DevModel& m, float* k32, __nv_bfloat16* k16, cudaStream_t s);
 cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1, float* c1t, cudaStream_t s);
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s);
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
+cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
                               int n_sm, bool gather, int* launches, cudaStream_t s);
 cudaError_t dense_bf16_configure();

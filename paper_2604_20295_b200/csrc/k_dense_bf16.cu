@@ -123,9 +123,8 @@ struct ZeroFill {
     mask &= ~(((len == 32) ? 0xffffffffu : ((1u << len) - 1u)) << b);
     const int off = m.patch[p].off;
     const int cnt = m.patch[p + len - 1].off + m.patch[p + len - 1].n - off;
-    const int64_t r0 = ((int64_t)e * m.n_nodes + off) * 3;
-    warp_zero_fill(io.out + r0, cnt * 3, lane);
-    if (io.analytic_out) warp_zero_fill(io.analytic_out + r0, cnt * 3, lane);
+    zero_out_rows(io, e, off, cnt, lane, 32);
+    if (io.analytic_out) warp_zero_fill(io.analytic_out + ((int64_t)e * m.n_nodes + off) * 3, cnt * 3, lane);
     return true;
   }
 };
@@ -161,7 +160,7 @@ __device__ long long g_prof[320 * 8 * 12];
 // read from the compact lists S1 wrote (bf16 K row j, coalesced over i because K is symmetric;
 // fp32 u^ and accumulation).  No TMA, no propagation MMA; the MLP part is unchanged.  It wins
 // when few nodes are in contact (ETAC_PATH_SPARSE on a bf16 context).
-template <int kMode, bool kGather>
+template <int kMode, bool kGather, bool kOutBf16>
 __global__ void __launch_bounds__(kDenseThreads, 2)
     dense_bf16_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
                       const __grid_constant__ CUtensorMap tmB) {
@@ -581,13 +580,19 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
           }
           request_next();
         }
+        // (the environment id is re-read from the prefetched list here rather than kept in a register
+        // through the MLP: the register allocation of this loop is fragile)
+        const int cur_env = __shfl_sync(0xffffffffu, my_env, el);
         if (valid && kMode != kModePnEncode) {  // S4: mask M_p + combine (Eq. 2); active rows keep u^ = -delta n in fp32
           const float lin = m.residual_only ? 0.0f : 1.0f;  // Table II ablation "Residual Network Only"
           float ox = fmaf(lin, cur.ux, rx), oy = fmaf(lin, cur.uy, ry), oz = fmaf(lin, cur.uz, rz);
           if (cur.dl > 0.0f && m.active_mode == ETAC_ACTIVE_PASSTHROUGH)
-            ox = -cur.dl * nrm.x, oy = -cur.dl * nrm.y, oz = -cur.dl * nrm.z;
-          float* o = io.out + cur.node * 3;
-          __stcs(o, ox), __stcs(o + 1, oy), __stcs(o + 2, oz);
+          {
+            // (reloaded for the few active rows instead of held in three registers through the MLP)
+            const float4 nn = kPn ? nrm : m.nrm4[g];
+            ox = -cur.dl * nn.x, oy = -cur.dl * nn.y, oz = -cur.dl * nn.z;
+          }
+          store_out3<kOutBf16 ? ETAC_OUT_BF16 : ETAC_OUT_F32>(io, cur_env, g, ox, oy, oz);
           if (io.analytic_out) {
             float* a = io.analytic_out + cur.node * 3;
             __stcs(a, cur.ux), __stcs(a + 1, cur.uy), __stcs(a + 2, cur.uz);
@@ -644,8 +649,11 @@ __global__ void __launch_bounds__(64) pn_global_kernel(DevModel m) {
 
 template <int kMode, bool kGather>
 static cudaError_t configure_one() {
-  return cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)dense_smem_bytes(kMaxPatches, kMode));
+  const int bytes = (int)dense_smem_bytes(kMaxPatches, kMode);
+  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess && kMode != kModePnEncode)  // the encoder pass writes no displacement
+    e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  return e;
 }
 
 cudaError_t dense_bf16_configure() {
@@ -659,10 +667,19 @@ cudaError_t dense_bf16_configure() {
   return e;
 }
 
-template <int kMode, bool kGather>
+template <int kMode>
 static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int grid,
-                       cudaStream_t s) {
-  dense_bf16_kernel<kMode, kGather><<<grid, kDenseThreads, dense_smem_bytes(m.n_patches, kMode), s>>>(m, io, tmA, tmB);
+                       bool gather, cudaStream_t s) {
+  const size_t smem = dense_smem_bytes(m.n_patches, kMode);
+  if constexpr (kMode == kModePnEncode) {
+    dense_bf16_kernel<kMode, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  } else if (gather) {
+    if (io.out_bf16) dense_bf16_kernel<kMode, true, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    else dense_bf16_kernel<kMode, true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  } else {
+    if (io.out_bf16) dense_bf16_kernel<kMode, false, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    else dense_bf16_kernel<kMode, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  }
 }
 
 // Launches S2-S4 for the context's residual form; *launches receives the number of kernels.
@@ -671,15 +688,15 @@ cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtenso
   const int grid = 2 * n_sm;
   *launches = 1;
   if (m.resid == ETAC_RESID_NONE) {
-    gather ? launch_one<kModeNone, true>(m, io, tmA, tmB, grid, s) : launch_one<kModeNone, false>(m, io, tmA, tmB, grid, s);
+    launch_one<kModeNone>(m, io, tmA, tmB, grid, gather, s);
   } else if (m.resid == ETAC_RESID_PERNODE_MLP) {
-    gather ? launch_one<kModePerNode, true>(m, io, tmA, tmB, grid, s) : launch_one<kModePerNode, false>(m, io, tmA, tmB, grid, s);
+    launch_one<kModePerNode>(m, io, tmA, tmB, grid, gather, s);
   } else {  // ETAC_RESID_POINTNET: encode + max-pool, per-(env, patch) vector, decode
     cudaError_t e = cudaMemsetAsync(m.gmax, 0, sizeof(uint32_t) * 64 * (size_t)m.n_patches * m.max_envs, s);
     if (e != cudaSuccess) return e;
-    launch_one<kModePnEncode, false>(m, io, tmA, tmB, grid, s);
+    launch_one<kModePnEncode>(m, io, tmA, tmB, grid, false, s);
     pn_global_kernel<<<dim3((unsigned)((io.n_envs + kPnSlots - 1) / kPnSlots), (unsigned)m.n_patches), 64, 0, s>>>(m);
-    gather ? launch_one<kModePnDecode, true>(m, io, tmA, tmB, grid, s) : launch_one<kModePnDecode, false>(m, io, tmA, tmB, grid, s);
+    launch_one<kModePnDecode>(m, io, tmA, tmB, grid, gather, s);
     *launches = 3;
   }
   return cudaGetLastError();

@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(kGatherChunk) gather_fp32_kernel(DevModel m, S
     ox = -d * n.x, oy = -d * n.y, oz = -d * n.z;
   }
   const int64_t o = ((int64_t)e * m.n_nodes + g) * 3;
-  io.out[o] = ox, io.out[o + 1] = oy, io.out[o + 2] = oz;
+  store_out3(io, e, g, ox, oy, oz);
   if (io.analytic_out) io.analytic_out[o] = ax, io.analytic_out[o + 1] = ay, io.analytic_out[o + 2] = az;
 }
 

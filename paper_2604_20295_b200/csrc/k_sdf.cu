@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
         const int64_t r0 = (int64_t)e * m.n_nodes + s_off[run0];
         const int cnt = s_off[q] - s_off[run0];
         if (fill_out) {  // (tensor-core paths: the fused kernel's issuer warps zero-fill these rows)
-          zero_fill(io.out + r0 * 3, cnt * 3);
+          zero_out_rows(io, e, s_off[run0], cnt, threadIdx.x, blockDim.x);
           if (io.analytic_out) zero_fill(io.analytic_out + r0 * 3, cnt * 3);
         }
         if (io.pen_out) zero_fill(io.pen_out + r0, cnt);
@@ -467,13 +467,38 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
     // contact-free pair: optional outputs are zero; for the fp32 gather kernel the output rows too
     // (the tensor-core kernel zero-fills them itself)
     if (fill_out) {
-      for (int i = lane; i < n * 3; i += 32) io.out[row0 * 3 + i] = 0.0f;
+      zero_out_rows(io, e, off, n, lane, 32);
       if (io.analytic_out)
         for (int i = lane; i < n * 3; i += 32) io.analytic_out[row0 * 3 + i] = 0.0f;
     }
     if (io.pen_out)
       for (int i = lane; i < n; i += 32) io.pen_out[row0 + i] = 0.0f;
   }
+}
+
+// ETAC_ABLATE_NO_PROPAGATION: U = U^, the penalty displacement -delta * n of the nodes in contact and 0
+// elsewhere (no K, no Phi).  Reads S1's delta (valid for the contacting pairs) and pair flags.
+__global__ void __launch_bounds__(256) penalty_only_kernel(DevModel m, StepIO io) {
+  const int e = blockIdx.x, p = blockIdx.y;
+  const PatchInfo pi = m.patch[p];
+  const bool hit = m.flags[(int64_t)e * m.n_patches + p] != 0;
+  for (int i = blockIdx.z * 256 + threadIdx.x; i < pi.n; i += gridDim.z * 256) {
+    const int g = pi.off + i;
+    const float d = hit ? m.delta[(int64_t)e * m.n_nodes + g] : 0.0f;
+    const float4 nn = m.nrm4[g];
+    const bool act = d > 0.0f;
+    store_out3(io, e, g, act ? -d * nn.x : 0.0f, act ? -d * nn.y : 0.0f, act ? -d * nn.z : 0.0f);
+    if (io.analytic_out) {
+      float* a = io.analytic_out + ((int64_t)e * m.n_nodes + g) * 3;
+      a[0] = 0.0f, a[1] = 0.0f, a[2] = 0.0f;
+    }
+  }
+}
+
+cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s) {
+  const dim3 grid(io.n_envs, m.n_patches, min(64, (m.max_patch_nodes + 255) / 256));
+  penalty_only_kernel<<<grid, 256, 0, s>>>(m, io);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s) {

@@ -23,7 +23,8 @@ ETAC_PREC_FP32, ETAC_PREC_BF16 = 0, 1
 ETAC_ACTIVE_PASSTHROUGH, ETAC_ACTIVE_PROPAGATE = 0, 1
 ETAC_IN_INDENTERS, ETAC_IN_PENETRATION = 0, 1
 ETAC_OPT_PATH, ETAC_OPT_ABLATION = 1, 2
-ETAC_ABLATE_FULL, ETAC_ABLATE_RESIDUAL_ONLY = 0, 1
+ETAC_ABLATE_FULL, ETAC_ABLATE_RESIDUAL_ONLY, ETAC_ABLATE_LINEAR_ONLY, ETAC_ABLATE_NO_PROPAGATION = range(4)
+ETAC_OUT_F32, ETAC_OUT_BF16 = 0, 1
 ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
 (ETAC_INFO_N_NODES, ETAC_INFO_N_PATCHES, ETAC_INFO_MAX_ENVS, ETAC_INFO_DEVICE_BYTES, ETAC_INFO_LAST_PATH,
  ETAC_INFO_LAST_LAUNCHES, ETAC_INFO_LAST_CONTACT_PAIRS, ETAC_INFO_SM_COUNT) = range(1, 9)
@@ -55,7 +56,8 @@ class etac_step_args(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_envs", C.c_int32), ("input_mode", C.c_int32),
                 ("d_indenters", C.c_void_p), ("d_patch_pose", C.c_void_p), ("d_penetration", C.c_void_p),
                 ("d_out", C.c_void_p), ("d_penetration_out", C.c_void_p), ("d_mask_out", C.c_void_p),
-                ("d_analytic_out", C.c_void_p), ("d_contact_out", C.c_void_p), ("d_active_count_out", C.c_void_p)]
+                ("d_analytic_out", C.c_void_p), ("d_contact_out", C.c_void_p), ("d_active_count_out", C.c_void_p),
+                ("out_env_stride", C.c_int64), ("out_dtype", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None
@@ -150,7 +152,8 @@ def etac_destroy(ctx) -> None:
 
 
 def make_step_args(n_envs, out, *, indenters=None, patch_pose=None, penetration=None, penetration_out=None,
-                   mask_out=None, analytic_out=None, contact_out=None, active_count_out=None) -> etac_step_args:
+                   mask_out=None, analytic_out=None, contact_out=None, active_count_out=None,
+                   out_env_stride=0, out_dtype=ETAC_OUT_F32) -> etac_step_args:
     a = etac_step_args()
     a.struct_size = C.sizeof(etac_step_args)
     a.n_envs = n_envs
@@ -159,6 +162,7 @@ def make_step_args(n_envs, out, *, indenters=None, patch_pose=None, penetration=
     a.d_out, a.d_penetration_out = _dptr(out), _dptr(penetration_out)
     a.d_mask_out, a.d_analytic_out = _dptr(mask_out), _dptr(analytic_out)
     a.d_contact_out, a.d_active_count_out = _dptr(contact_out), _dptr(active_count_out)
+    a.out_env_stride, a.out_dtype, a.reserved = out_env_stride, out_dtype, 0
     return a
 
 
@@ -255,12 +259,15 @@ class Etac:
             dev["penetration"] = t.from_numpy(np.ascontiguousarray(penetration, dtype=np.float32)).to(self.device)
         return dev
 
-    def args(self, n_envs, dev):
+    def args(self, n_envs, dev, out=None, **opts):
+        """Step arguments; `out` (a CUDA tensor: fp32 or bf16, possibly a wider observation buffer)
+        together with out_env_stride / out_dtype in `opts` replaces the engine's packed fp32 output."""
         kw = dict(dev)
+        kw.update(opts)
         if self.debug:
             kw.update(penetration_out=self.pen_out, mask_out=self.mask_out, analytic_out=self.analytic,
                       contact_out=self.contact, active_count_out=self.active_count)
-        return make_step_args(n_envs, self.out, **kw)
+        return make_step_args(n_envs, self.out if out is None else out, **kw)
 
     def step(self, n_envs, dev):
         stream = self.torch.cuda.current_stream(self.device).cuda_stream

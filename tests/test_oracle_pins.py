@@ -288,6 +288,24 @@ def test_mode_reductions():
     assert np.abs(prop["U"][act] - full["U"][act]).max() > 1e-3
 
 
+def test_ablation_modes_reduce_to_their_definitions():
+    """Table II rows as oracle modes: "linear_only" is the model without Phi,
+    "residual_only" + "linear_only" add up to "full" on the passive rows, "no_propagation" is U^."""
+    wl = W.config2(seed=5, n_envs=3)
+    def run(abl, **kw):
+        m = O.model_from_workload(wl, **kw)
+        m.ablation = abl
+        return O.step(m, indenters=wl.indenters)
+    full, lin, res, nop = run("full"), run("linear_only"), run("residual_only"), run("no_propagation")
+    none = run("full", resid_arch="none")
+    np.testing.assert_array_equal(lin["U"], none["U"])
+    passive = ~full["mask"]
+    np.testing.assert_allclose((lin["U"] + res["U"])[passive], full["U"][passive], rtol=0, atol=1e-12)
+    nrm = wl.mesh.normal.astype(np.float64)
+    np.testing.assert_array_equal(nop["U"], -full["delta"][:, :, None] * nrm[None])
+    assert np.all(nop["U"][passive] == 0) and np.abs(nop["U"][full["mask"]]).max() > 0.05
+
+
 # ---------------------------------------------------------------- P12
 def test_pointnet_branch_is_permutation_equivariant():
     rng = np.random.default_rng(8)

@@ -150,6 +150,15 @@ def test_patches_derived_from_adjacency_on_device():
     with pytest.raises(T.EtacError) as ei:
         T.etac_step(ctx, None, T.make_step_args(4, None, indenters=out))
     assert ei.value.status == T.ETAC_ERR_INVALID_ARG
+    for bad in (dict(out_dtype=2), dict(out_env_stride=3 * 5696 - 1), dict(out_env_stride=-1)):
+        with pytest.raises(T.EtacError) as ei:
+            T.etac_step(ctx, None, T.make_step_args(4, out, indenters=out, **bad))
+        assert ei.value.status == T.ETAC_ERR_INVALID_ARG
+    with pytest.raises(T.EtacError) as ei:                               # fp32 output at an odd 2-byte address
+        T.etac_step(ctx, None, T.make_step_args(4, out.data_ptr() + 2, indenters=out))
+    assert ei.value.status == T.ETAC_ERR_INVALID_ARG
+    with pytest.raises(T.EtacError):
+        T.etac_set_option(ctx, T.ETAC_OPT_ABLATION, 4)
     T.etac_step(ctx, None, T.make_step_args(0, out, indenters=out))       # no-op
     T.etac_destroy(ctx)
 
@@ -367,6 +376,77 @@ def test_ablation_residual_only(precision):
     tol = (1e-4 if precision == "fp32" else 5e-2) * np.abs(ref["U"][~ref["mask"]]).max()
     assert np.abs(U - ref["U"])[~ref["mask"]].max() <= tol
     np.testing.assert_allclose(U[ref["mask"]], full["U"][ref["mask"]], atol=2e-5)            # active rows keep u^
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+@pytest.mark.parametrize("mode", ["linear_only", "no_propagation"])
+def test_ablation_linear_only_and_no_propagation(precision, mode):
+    """The other Table II rows as run-time modes of a context that has Phi: "Linear Decay Only"
+     and the penalty displacement without propagation."""
+    import dataclasses
+    from oracle import etac_oracle as O
+    wl = dataclasses.replace(W.config3(12, 21), weights=W.make_weights(3, 2, std=0.2))
+    m = O.model_from_workload(wl)
+    m.ablation = mode
+    ref = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)
+    eng = T.Etac(wl, precision=precision, debug_outputs=True)
+    try:
+        code = {"linear_only": T.ETAC_ABLATE_LINEAR_ONLY, "no_propagation": T.ETAC_ABLATE_NO_PROPAGATION}[mode]
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_ABLATION, code)
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        U = eng.step(wl.n_envs, dev).cpu().numpy()
+        assert np.array_equal(eng.mask_bool(wl.n_envs), ref["mask"])
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_ABLATION, T.ETAC_ABLATE_FULL)      # and back
+        U_full = eng.step(wl.n_envs, dev).cpu().numpy()
+    finally:
+        eng.close()
+    full = run_oracle(wl)
+    assert np.abs(ref["U"] - full["U"]).max() > 0.05                     # the mode changes the answer
+    scale = np.abs(full["U"]).max()
+    if mode == "no_propagation":
+        assert np.all(U[~ref["mask"]] == 0)                              # nothing but the contact nodes moves
+        np.testing.assert_allclose(U, ref["U"], rtol=0, atol=2e-5)
+    else:
+        assert np.abs(U - ref["U"]).max() <= TOL[precision] * scale
+    assert np.abs(U_full - full["U"]).max() <= (5e-2 if precision == "bf16" else 1e-4) * scale
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+@pytest.mark.parametrize("path", ["dense", "sparse"])
+def test_bf16_output_in_a_strided_observation_buffer(precision, path):
+    """out_dtype = BF16 and out_env_stride: U lands, rounded to bf16, inside a wider per-env observation
+    row (the n x 3 tensor is the policy observation); the rest of the row is untouched."""
+    import torch
+    if precision == "fp32" and path == "dense":
+        pytest.skip("the dense contraction needs a bf16 context")
+    wl = W.config3(14, 37)
+    ref = run_oracle(wl)
+    eng = T.Etac(wl, precision=precision)
+    try:
+        if path == "sparse":
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, T.ETAC_PATH_SPARSE)
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        N, E = eng.N, wl.n_envs
+        stream = torch.cuda.current_stream().cuda_stream
+        for dtype, code, pad_front, pad_back in ((torch.bfloat16, T.ETAC_OUT_BF16, 7, 5), (torch.float32, T.ETAC_OUT_F32, 3, 11)):
+            stride = pad_front + 3 * N + pad_back
+            obs = torch.full((E, stride), -7.0, dtype=dtype, device=eng.device)
+            out = obs.data_ptr() + pad_front * obs.element_size()          # odd offsets: element alignment only
+            T.etac_step(eng.ctx, stream, eng.args(E, dev, out=out, out_env_stride=stride, out_dtype=code))
+            torch.cuda.synchronize()
+            got = obs.float().cpu().numpy()
+            assert np.all(got[:, :pad_front] == -7.0) and np.all(got[:, pad_front + 3 * N:] == -7.0)
+            U = got[:, pad_front:pad_front + 3 * N].reshape(E, N, 3)
+            packed = eng.step(E, dev).float().cpu().numpy()
+            if dtype == torch.float32:
+                assert np.array_equal(U, packed)                          # same kernels, other addresses
+            else:                                                          # = the fp32 result rounded to bf16
+                want = torch.from_numpy(packed).to(torch.bfloat16).float().numpy()
+                assert np.array_equal(U, want)
+            scale = np.abs(ref["U"]).max()
+            assert np.abs(U - ref["U"]).max() <= (TOL[precision] + (2.0 ** -8 if dtype == torch.bfloat16 else 0)) * scale
+    finally:
+        eng.close()
 
 
 def test_step_is_capturable_in_a_cuda_graph():
