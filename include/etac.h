@@ -57,7 +57,10 @@ typedef struct {
   float param[3]; /* sphere {r,-,-}; box {hx,hy,hz} half extents; capsule {r, half length along local z, -};
                      grid {grid id as a float,-,-}: a sampled SDF registered with etac_set_sdf_grid */
   float pose[7];  /* {px,py,pz, qx,qy,qz,qw}: unit quaternion, Isaac-Gym order; world frame */
-  float _pad;
+  int32_t skip_patch1; /* self-contact (PAPER.md:L77 detects contact between the hand's own links too): the
+                     other links' collision shapes are passed as indenters at their link poses, and the
+                     shape of the link a patch is mounted on must not press on that patch: the patch with
+                     index skip_patch1 - 1 ignores this indenter; 0 = no patch does */
 } etac_indenter; /* 48 bytes */
 
 enum { ETAC_KERNEL_EXP_L2 = 0 };                                  /* Eq. (1): exp(-alpha*|p_j-p_i|_2) */

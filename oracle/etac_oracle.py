@@ -150,6 +150,8 @@ def sdf_grid(values, origin, spacing, y0, y1, y2, dt=np.float64):
 def signed_distance(model: OracleModel, indenters_e, patch_pose_e=None, dt=np.float64):
     """phi[i] = min over the env's indenters (type != NONE) of sdf_k(R_k^T (x_i - t_k)),
     x_i = R(q_{e,p}) p_i + t_{e,p} (identity if no patch poses); +inf if no indenter.
+    Self-contact: an indenter with skip_patch1 = p + 1 is the collision shape of the link
+    patch p is mounted on and is left out of that patch's union (the other patches see it).
     PAPER.md:L77 'contact events are first detected using SDFs between nodes and objects';
     union of several indenters = min (reading R6).  ``dt=np.float32`` gives the fp32
     decision twin: same formulas, same order, every op rounded to fp32."""
@@ -180,9 +182,15 @@ def signed_distance(model: OracleModel, indenters_e, patch_pose_e=None, dt=np.fl
         y2 = (R[0, 2] * d0 + R[1, 2] * d1) + R[2, 2] * d2
         if itype == IND_GRID:
             values, origin, spacing = model.grids[int(ind["param"][0])]
-            phi = np.minimum(phi, sdf_grid(values, origin, spacing, y0, y1, y2, dt))
+            phi_k = sdf_grid(values, origin, spacing, y0, y1, y2, dt)
         else:
-            phi = np.minimum(phi, sdf_local(itype, ind["param"], y0, y1, y2, dt))
+            phi_k = sdf_local(itype, ind["param"], y0, y1, y2, dt)
+        skip = int(ind["skip_patch1"]) - 1 if "skip_patch1" in ind.dtype.names else -1
+        if 0 <= skip < model.n_patches:
+            lo, hi = int(model.patch_offset[skip]), int(model.patch_offset[skip + 1])
+            phi_k = phi_k.copy()
+            phi_k[lo:hi] = np.inf
+        phi = np.minimum(phi, phi_k)
     return phi
 
 

@@ -18,6 +18,7 @@ namespace etac {
 
 struct SInd {
   int type;
+  int skip1;  // etac_indenter::skip_patch1 (self-contact: patch skip1 - 1 ignores this indenter)
   float prm[3];
   float t[3];
   float R[9];
@@ -104,9 +105,10 @@ __device__ __forceinline__ float sdf_one(const SInd& s, float X0, float X1, floa
 // Union signed distance at world point X: min over the slots in slot order.
 template <bool kGrid>
 __device__ __forceinline__ float union_sdf(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2,
-                                           const GridDesc* grids) {
+                                           const GridDesc* grids, int p1) {  // p1 = patch + 1 (self-contact skip)
   float phi = __int_as_float(0x7f800000);
-  for (int k = 0; k < n_ind; ++k) phi = fminf(phi, sdf_one<kGrid>(ind[k], X0, X1, X2, grids));
+  for (int k = 0; k < n_ind; ++k)
+    if (ind[k].skip1 != p1) phi = fminf(phi, sdf_one<kGrid>(ind[k], X0, X1, X2, grids));
   return phi;
 }
 
@@ -116,9 +118,10 @@ __device__ __forceinline__ float union_sdf(const SInd* __restrict__ ind, int n_i
 // for the distance term outside.
 template <bool kGrid>
 __device__ __forceinline__ float union_sdf_lower(const SInd* __restrict__ ind, int n_ind, float X0, float X1, float X2,
-                                                 float rad, const GridDesc* grids) {
+                                                 float rad, const GridDesc* grids, int p1) {
   float lo = __int_as_float(0x7f800000);
   for (int k = 0; k < n_ind; ++k) {
+    if (ind[k].skip1 == p1) continue;
     const float L = (kGrid && ind[k].type == ETAC_IND_GRID) ? 2.7320508f : 1.0f;
     lo = fminf(lo, sdf_one<kGrid>(ind[k], X0, X1, X2, grids) - L * rad);
   }
@@ -128,6 +131,7 @@ __device__ __forceinline__ float union_sdf_lower(const SInd* __restrict__ ind, i
 __device__ __forceinline__ SInd load_indenter(const etac_indenter* __restrict__ p) {
   SInd s;
   s.type = p->type;
+  s.skip1 = p->skip_patch1;
   s.prm[0] = p->param[0], s.prm[1] = p->param[1], s.prm[2] = p->param[2];
   s.t[0] = p->pose[0], s.t[1] = p->pose[1], s.t[2] = p->pose[2];
   quat_to_rot(p->pose + 3, s.R);
@@ -184,13 +188,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
   const bool posed = io.patch_pose != nullptr;
   if constexpr (kIndenters) {
     for (int k = threadIdx.x; k < m.max_ind; k += blockDim.x) {
-      const etac_indenter in = io.ind[(int64_t)e * m.max_ind + k];
-      SInd s;
-      s.type = in.type;
-      s.prm[0] = in.param[0], s.prm[1] = in.param[1], s.prm[2] = in.param[2];
-      s.t[0] = in.pose[0], s.t[1] = in.pose[1], s.t[2] = in.pose[2];
-      quat_to_rot(in.pose + 3, s.R);
-      sind[k] = s;
+      sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
     }
   }
   for (int p0 = 0; p0 < m.n_patches; p0 += kPoseChunk) {
@@ -220,7 +218,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           C2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], x), __fmul_rn(sp.R[7], y)), __fmul_rn(sp.R[8], z)), sp.t[2]);
         }
         // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
-        const float phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid);
+        const float phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
         sp.evaluated = !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
         s_pose[threadIdx.x] = sp;
       }
@@ -247,7 +245,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
             X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
             X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
           }
-          const float phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid);
+          const float phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid, p0 + q + 1);
           const float d = phi < 0.0f ? -phi : 0.0f;
           delta[i] = d;
           any |= d > 0.0f;
@@ -387,11 +385,12 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
   float phi_lo;
   if constexpr (kOne) {
     one = load_indenter(io.ind + e);
-    phi_lo = union_sdf_lower<kGrid>(&one, 1, C0, C1, C2, pi.brad, m.grid);
+    if (one.skip1 == p + 1) one.type = ETAC_IND_NONE;  // the shape of this patch's own link
+    phi_lo = union_sdf_lower<kGrid>(&one, 1, C0, C1, C2, pi.brad, m.grid, p + 1);
   } else {
     for (int k = lane; k < m.max_ind; k += 32) sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
     __syncwarp();
-    phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid);
+    phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
   }
   // conservative cull: phi(x_i) >= phi(c) - L * brad on the patch's bounding sphere
   const bool evaluated = !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
@@ -406,7 +405,7 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       if (posed) to_world(R, t, pos.x, pos.y, pos.z, X0, X1, X2);
       float phi;
       if constexpr (kOne) phi = fminf(__int_as_float(0x7f800000), sdf_one<kGrid>(one, X0, X1, X2, m.grid));
-      else phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid);
+      else phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid, p + 1);
       const float d = phi < 0.0f ? -phi : 0.0f;
       delta[i] = d;
       any |= d > 0.0f;

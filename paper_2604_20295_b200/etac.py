@@ -37,7 +37,7 @@ _ip = C.POINTER(C.c_int32)
 
 
 class etac_indenter(C.Structure):
-    _fields_ = [("type", C.c_int32), ("param", C.c_float * 3), ("pose", C.c_float * 7), ("_pad", C.c_float)]
+    _fields_ = [("type", C.c_int32), ("param", C.c_float * 3), ("pose", C.c_float * 7), ("skip_patch1", C.c_int32)]
 
 
 class etac_model_desc(C.Structure):

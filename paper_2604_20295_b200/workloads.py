@@ -25,7 +25,7 @@ IND_NONE, IND_SPHERE, IND_BOX, IND_CAPSULE = 0, 1, 2, 3
 
 #: mirrors ``etac_indenter`` in include/etac.h (48 bytes)
 INDENTER_DTYPE = np.dtype(
-    [("type", "<i4"), ("param", "<f4", (3,)), ("pose", "<f4", (7,)), ("_pad", "<f4")]
+    [("type", "<i4"), ("param", "<f4", (3,)), ("pose", "<f4", (7,)), ("skip_patch1", "<i4")]
 )
 assert INDENTER_DTYPE.itemsize == 48
 

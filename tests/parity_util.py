@@ -7,6 +7,7 @@ import numpy as np
 
 from oracle import etac_oracle as O
 from paper_2604_20295_b200 import etac as T
+from paper_2604_20295_b200 import workloads as W
 
 TOL = {"fp32": 1e-4, "bf16": 2e-2}
 
@@ -85,3 +86,49 @@ def compare(gpu, ref, tol, envs=None, resid_tol=None, label="", delta_tol=1e-5):
         stats["rel_r"] = err_r / max(rmax, 1e-30)
         assert err_r <= resid_tol * rmax, f"{label}: residual err {err_r:.3e} > {resid_tol}*{rmax:.3e}"
     return stats
+
+
+def self_contact_workload(mesh, caps, seed, n_envs, n_ind, precision="bf16", weights=None, alpha=0.5):
+    """Self-contact: the patches listed in ``caps`` = {patch: cap radius} sit on links whose
+    collision shape is a sphere a little larger than the cap (it would press on every node of its own
+    patch).  Per env one such link A is pressed onto a node of another patch B; slot 0 of the indenters is
+    A's shape at A's pose with skip_patch1 = A + 1, the other slots are free objects pressed on other
+    patches.  Every patch has its own rigid pose; patches not involved are parked apart."""
+    rng = np.random.default_rng(4000 + seed)
+    P, N = mesh.n_patches, mesh.n_nodes
+    off = np.asarray(mesh.patch_offset)
+    pos, nrm = mesh.pos.astype(np.float64), mesh.normal.astype(np.float64)
+    ind = W._blank_indenters(n_envs, n_ind)
+    pose = np.zeros((n_envs, P, 7), np.float32)
+    meta = {"A": [], "B": []}
+    for e in range(n_envs):
+        Rm = W.random_rotations(rng, P)
+        t = np.stack([60.0 * (np.arange(P) - P // 2), np.zeros(P), np.zeros(P)], 1) + rng.uniform(-5, 5, (P, 3))
+        A = int(rng.choice(list(caps)))
+        B = int(rng.choice([p for p in range(P) if p != A]))
+        r_link = caps[A] + 0.25
+        c = int(rng.integers(off[B], off[B + 1]))
+        depth = rng.uniform(0.2, 1.0)
+        centre_local = pos[c] + nrm[c] * (r_link - depth)            # A's sphere centre in B's frame
+        t[B] = t[A] - Rm[B] @ centre_local                            # ... lands on A's world centre t[A]
+        pose[e, :, 0:3] = t
+        pose[e, :, 3:7] = W.quat_from_matrix(Rm)
+        ind["type"][e, 0], ind["param"][e, 0, 0] = W.IND_SPHERE, r_link
+        ind["pose"][e, 0, 0:3], ind["pose"][e, 0, 3:7] = t[A], [0, 0, 0, 1]
+        ind["skip_patch1"][e, 0] = A + 1
+        others = [p for p in range(P) if p not in (A, B)]
+        for k in range(1, n_ind):                                     # free objects on other patches
+            if not others or rng.random() < 0.3:
+                continue
+            C = int(rng.choice(others))
+            cc = np.array([rng.integers(off[C], off[C + 1])])
+            size = rng.uniform(2.0, 4.0, 1)
+            cl, q = W._press_on_node(mesh.pos, mesh.normal, cc, None, size, rng.uniform(0.2, 0.9, 1), rng.uniform(0, 6.28, 1))
+            from scipy.spatial.transform import Rotation as Rot
+            ind["type"][e, k], ind["param"][e, k] = W.IND_CAPSULE, [size[0], rng.uniform(0, 3), 0]
+            ind["pose"][e, k, 0:3] = Rm[C] @ cl[0] + t[C]
+            ind["pose"][e, k, 3:7] = (Rot.from_matrix(Rm[C]) * Rot.from_quat(q[0])).as_quat()
+        meta["A"].append(A), meta["B"].append(B)
+    wl = W.Workload("self_contact", mesh, np.asarray([alpha], np.float32), weights or W.make_weights(3, seed), n_envs,
+                    n_ind, ind, pose, precision, meta)
+    return wl

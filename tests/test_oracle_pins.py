@@ -306,6 +306,34 @@ def test_ablation_modes_reduce_to_their_definitions():
     assert np.all(nop["U"][passive] == 0) and np.abs(nop["U"][full["mask"]]).max() > 0.05
 
 
+def test_self_contact_skip_is_per_patch():
+    """Self-contact: a link's collision shape is an indenter for every patch but its own.
+    Brute force per patch: with the skip, patch A sees only the other indenters; every other patch sees the
+    plain union."""
+    from parity_util import self_contact_workload
+    mesh = W.assemble([W.fib_cap(6.0, 72), W.flat_pad(10, 12, 1.0), W.fib_cap(5.0, 60)])
+    wl = self_contact_workload(mesh, {0: 6.0, 2: 5.0}, seed=3, n_envs=6, n_ind=2, precision="fp32")
+    m = O.model_from_workload(wl)
+    off = np.asarray(mesh.patch_offset)
+    for e in range(wl.n_envs):
+        A, B = wl.meta["A"][e], wl.meta["B"][e]
+        phi = O.signed_distance(m, wl.indenters[e], wl.patch_pose[e])
+        plain = wl.indenters[e].copy()
+        plain["skip_patch1"] = 0
+        phi_plain = O.signed_distance(m, plain, wl.patch_pose[e])
+        without = plain.copy()
+        without["type"][0] = W.IND_NONE
+        phi_without = O.signed_distance(m, without, wl.patch_pose[e])
+        sl = slice(off[A], off[A + 1])
+        np.testing.assert_array_equal(phi[sl], phi_without[sl])
+        rest = np.ones(mesh.n_nodes, bool)
+        rest[sl] = False
+        np.testing.assert_array_equal(phi[rest], phi_plain[rest])
+        # the own shape alone would press on every node of A by 0.25; B is pressed by A's shape
+        np.testing.assert_allclose(phi_plain[sl], -0.25, atol=5e-6)   # fp32 poses and positions
+        assert (phi_plain[sl] < 0).all() and (phi[off[B]:off[B + 1]] < 0).any()
+
+
 # ---------------------------------------------------------------- P12
 def test_pointnet_branch_is_permutation_equivariant():
     rng = np.random.default_rng(8)

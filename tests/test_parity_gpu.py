@@ -378,6 +378,31 @@ def test_ablation_residual_only(precision):
     np.testing.assert_allclose(U[ref["mask"]], full["U"][ref["mask"]], atol=2e-5)            # active rows keep u^
 
 
+@pytest.mark.parametrize("kind,n_ind", [("hand", 1), ("hand", 3), ("few_patches", 2)])
+def test_self_contact_between_links(kind, n_ind):
+    """Self-contact: link collision shapes as indenters with skip_patch1, through the
+    warp-per-pair S1 kernel with one and with several indenters and through the CTA-per-env kernel."""
+    from parity_util import self_contact_workload
+    if kind == "hand":
+        wl = self_contact_workload(W.hand_mesh(), {p: 9.0 for p in range(5)}, 7, 23, n_ind)
+    else:
+        mesh = W.assemble([W.fib_cap(6.0, 72), W.flat_pad(10, 12, 1.0), W.fib_cap(5.0, 60)])
+        wl = self_contact_workload(mesh, {0: 6.0, 2: 5.0}, 8, 17, n_ind)
+    ref = run_oracle(wl)
+    off = np.asarray(wl.mesh.patch_offset)
+    for e in range(wl.n_envs):                                  # the skip is what keeps patch A free of its own link
+        A, B = wl.meta["A"][e], wl.meta["B"][e]
+        assert ref["mask"][e, off[B]:off[B + 1]].any()
+        if n_ind == 1:
+            assert not ref["mask"][e, off[A]:off[A + 1]].any()
+    for precision in ("bf16", "fp32"):
+        gpu = run_gpu(wl, precision=precision)
+        _report(f"self-contact {kind} M={n_ind} {precision}",
+                compare(gpu, ref, TOL[precision], resid_tol=5e-2 if precision == "bf16" else 1e-4, label="self-contact",
+                        delta_tol=1e-4))       # world coordinates of a few hundred mm: ulp of the fp32 twin
+        assert gpu["pairs"] == int(ref["contact"].sum())
+
+
 @pytest.mark.parametrize("precision", ["fp32", "bf16"])
 @pytest.mark.parametrize("mode", ["linear_only", "no_propagation"])
 def test_ablation_linear_only_and_no_propagation(precision, mode):
