@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define ETAC_ABI_VERSION 5
+#define ETAC_ABI_VERSION 6
 
 typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
 
@@ -192,6 +192,31 @@ const char* etac_last_error(const etac_ctx* ctx);
  * a contiguous index range, ETAC_ERR_CAPACITY if cap is too small. */
 etac_status etac_patches_from_adjacency(int32_t n_nodes, const int32_t* adj_rowptr, const int32_t* adj_col,
                                         int32_t* off, int32_t cap, int32_t* n_patches);
+
+/* Backward pass for the calibration of Eq. (3) ("alpha and the residual network are
+ * obtained by minimising || U_p - U_p* ||_2 by gradient descent"; Table I lists differentiability).
+ * Given the upstream gradient G = dL/dU of one step (same inputs as etac_step), returns dL/dalpha and
+ * dL/d(weights of the per-node residual MLP).  Rows that Eq. (2) overwrites with u^ (the active nodes,
+ * ETAC_ACTIVE_PASSTHROUGH) and rows of contact-free (env, patch) pairs carry no gradient.  Gradients
+ * with respect to the poses / penetrations are not computed.  Arithmetic: fp32 on the fp32 copies of
+ * K and the weights, whatever the context's precision; sums over environments use fp32 atomics, so
+ * repeated calls agree to rounding, not bit for bit.  Contexts with ETAC_RESID_POINTNET and ablation
+ * modes other than FULL: ETAC_ERR_UNSUPPORTED.  Enqueues on cuda_stream, no host synchronisation. */
+typedef struct {
+  uint32_t struct_size;               /* = sizeof(etac_backward_args) */
+  int32_t n_envs;                     /* 1..max_envs (0 is a no-op) */
+  int32_t input_mode;                 /* ETAC_IN_*, as in etac_step_args */
+  const etac_indenter* d_indenters;   /* device [E x max_indenters] */
+  const float* d_patch_pose;          /* device [E x P x 7] or NULL */
+  const float* d_penetration;         /* device [E x N] (PENETRATION mode) */
+  const float* d_grad_out;            /* device [E x N x 3] fp32: dL/dU, REQUIRED */
+  float* d_grad_alpha;                /* device [n_alpha] fp32, REQUIRED, overwritten: dL/dalpha (per patch if the
+                                         context was created with n_alpha = P) */
+  float* d_grad_weights;              /* device [4995] fp32, overwritten, or NULL: dL/d W1[64x9] b1[64] W2[64x64]
+                                         b2[64] W3[3x64] b3[3], in this order; must be NULL for ETAC_RESID_NONE */
+} etac_backward_args;
+#define ETAC_GRAD_WEIGHTS_LEN 4995
+etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* args);
 
 /* Library ABI version (ETAC_ABI_VERSION the .so was built with). */
 int32_t etac_abi_version(void);

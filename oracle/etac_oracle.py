@@ -23,7 +23,8 @@ under tests/golden/; the sampled-grid SDF against scipy's RegularGridInterpolato
 on affine fields and the h^2 interpolation bound on a sphere.  Unpinned: numerical agreement with the paper's *trained* Phi and its
 Table II (no weights / FEM data exist here)  -> "parity unpinned" for that item only; and
 the PointNet form of Phi is pinned only by its structural invariants (hidden widths are not
-given in the paper: Fig. 3 is an image).
+given in the paper: Fig. 3 is an image).  The backward pass (calibration gradients of Eq. 3)
+is in etac_oracle_grad.py, pinned by finite differences of this module.
 """
 from __future__ import annotations
 

@@ -1,0 +1,83 @@
+"""CPU oracle for the backward pass of the ETac tactile update  --  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Same rules as ``etac_oracle.py`` (only tests / smoke / bench baselines may import it; no code shared
+with the CUDA path).  It differentiates exactly what ``etac_oracle.step`` computes:
+
+  L(alpha, Phi) is any scalar function of U with G = dL/dU given (calibration, PAPER.md:L104-L108,
+  Eq. (3): L = || U_p - U_p* ||_2 fitted by gradient descent; Table I lists differentiability).
+
+  For a row i of a contacting (env, patch) that the mask of Eq. (2) does not overwrite with u^
+      U_i = u_i + Phi(u_i, p_i, n_i),  u_i = sum_{j active} K_ij u^_j,  K_ij = exp(-alpha d_ij)   (Eq. 1-2)
+      dK_ij / dalpha = -d_ij K_ij                       (d_ij = ||p_j - p_i||_2 from the positions)
+      dL/dalpha = sum_i (G_i + J^T G_i) . sum_j dK_ij/dalpha u^_j ,   J = dPhi/du at row i
+      dL/dW     = the chain rule through the per-node MLP 9 -> 64 -> 64 -> 3 (SiLU), written out
+  Rows overwritten with u^ = -delta n (active rows, "passthrough") and rows of contact-free pairs do not
+  depend on alpha or Phi.  The contact set is held fixed (it does not depend on alpha or Phi).
+
+float64 numpy, one (env, patch) at a time, no fusion.  Pins (tests/test_oracle_pins.py): central
+finite differences of ``etac_oracle.step`` (itself pinned) with respect to alpha and to sampled
+weights of every layer, and torch float64 autograd of the same MLP.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import etac_oracle as O
+
+
+def silu_prime(z):
+    s = 1.0 / (1.0 + np.exp(-z))
+    return s * (1.0 + z * (1.0 - s))
+
+
+def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetration=None, envs=None):
+    """G: dL/dU [E', N, 3] for the listed envs (default all).  Returns float64 gradients
+    {"alpha": [n_alpha], "W1": [64, 9], "b1", "W2", "b2", "W3", "b3"} (weights only for the per-node form)."""
+    if model.resid_arch not in ("none", "pernode") or model.ablation != "full":
+        raise ValueError("backward oracle: per-node / no residual, full pipeline only")
+    fwd = O.step(model, indenters=indenters, patch_pose=patch_pose, penetration=penetration, envs=envs)
+    alpha = np.atleast_1d(np.asarray(model.alpha, dtype=np.float64))
+    grads = {"alpha": np.zeros(alpha.shape[0])}
+    mlp = model.resid_arch == "pernode"
+    if mlp:
+        w = {k: np.asarray(v, dtype=np.float64) for k, v in model.weights.items()}
+        for k in ("W1", "b1", "W2", "b2", "W3", "b3"):
+            grads[k] = np.zeros_like(w[k])
+    pos = model.pos.astype(np.float64)
+    nrm = model.normal.astype(np.float64)
+    G = np.asarray(G, dtype=np.float64)
+    for oi in range(G.shape[0]):
+        delta, active = fwd["delta"][oi], fwd["mask"][oi]
+        uhat = -delta[:, None] * nrm
+        for p in range(model.n_patches):
+            lo, hi = int(model.patch_offset[p]), int(model.patch_offset[p + 1])
+            act = active[lo:hi]
+            if not act.any():
+                continue
+            K = O.kernel_block(model, p)
+            P = pos[lo:hi]
+            dist = np.sqrt(((P[:, None, :] - P[None, :, :]) ** 2).sum(-1))
+            dK = -dist * K                                        # dK/dalpha, Eq. (1)
+            ua = uhat[lo:hi][act]
+            ulin = K[:, act] @ ua
+            v = dK[:, act] @ ua
+            rows = ~act if model.active_mode == "passthrough" else np.ones_like(act)
+            g = np.where(rows[:, None], G[oi, lo:hi], 0.0)
+            glin = g.copy()
+            if mlp:
+                x9 = np.concatenate([ulin, P, nrm[lo:hi]], axis=1)
+                z1 = x9 @ w["W1"].T + w["b1"]
+                h1 = O.silu(z1)
+                z2 = h1 @ w["W2"].T + w["b2"]
+                h2 = O.silu(z2)
+                grads["W3"] += g.T @ h2
+                grads["b3"] += g.sum(0)
+                gz2 = (g @ w["W3"]) * silu_prime(z2)
+                grads["W2"] += gz2.T @ h1
+                grads["b2"] += gz2.sum(0)
+                gz1 = (gz2 @ w["W2"]) * silu_prime(z1)
+                grads["W1"] += gz1.T @ x9
+                grads["b1"] += gz1.sum(0)
+                glin += (gz1 @ w["W1"])[:, 0:3]
+            grads["alpha"][p if alpha.shape[0] > 1 else 0] += float((glin * v).sum())
+    return grads

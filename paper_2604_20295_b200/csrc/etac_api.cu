@@ -15,7 +15,7 @@ struct etac_ctx {
   DevModel m{};
   std::vector<void*> allocs;
   size_t bytes = 0;
-  int device = 0, n_sm = 0, precision = 0, path_opt = ETAC_PATH_AUTO;
+  int device = 0, n_sm = 0, precision = 0, path_opt = ETAC_PATH_AUTO, n_alpha = 1;
   int last_path = ETAC_PATH_AUTO, last_launches = 0;
   CUtensorMap tmA{}, tmB{};
   bool have_tm = false;
@@ -472,6 +472,8 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
     c->have_tm = true;
     CK(dense_bf16_configure(), "cudaFuncSetAttribute(dense_bf16_kernel)");
   }
+  c->n_alpha = d->n_alpha;
+  CK(backward_configure(), "cudaFuncSetAttribute(backward_kernel)");
   CK(cudaDeviceSynchronize(), "create-time kernels");
 #undef CK
   *out = c;
@@ -570,6 +572,43 @@ etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value) {
     }
     default: return ETAC_ERR_INVALID_ARG;
   }
+}
+
+etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* a) {
+  if (!ctx) return ETAC_ERR_INVALID_ARG;
+  cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+  if (!a || a->struct_size != sizeof(etac_backward_args)) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_backward_args");
+  if (a->n_envs < 0) return fail(ctx, ETAC_ERR_INVALID_ARG, "n_envs < 0");
+  if (a->n_envs > ctx->m.max_envs) return fail(ctx, ETAC_ERR_CAPACITY, "n_envs > max_envs");
+  if (a->input_mode != ETAC_IN_INDENTERS && a->input_mode != ETAC_IN_PENETRATION)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "bad input_mode");
+  if (!a->d_grad_out || !a->d_grad_alpha) return fail(ctx, ETAC_ERR_INVALID_ARG, "d_grad_out and d_grad_alpha are required");
+  if (a->input_mode == ETAC_IN_INDENTERS && ctx->m.max_ind > 0 && !a->d_indenters)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "d_indenters is NULL");
+  if (a->input_mode == ETAC_IN_PENETRATION && !a->d_penetration)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "d_penetration is NULL");
+  if (ctx->m.resid == ETAC_RESID_POINTNET) return fail(ctx, ETAC_ERR_UNSUPPORTED, "etac_backward: per-node residual only");
+  if (ctx->m.ablation != ETAC_ABLATE_FULL) return fail(ctx, ETAC_ERR_UNSUPPORTED, "etac_backward: ETAC_ABLATE_FULL only");
+  if (ctx->m.resid == ETAC_RESID_NONE && a->d_grad_weights)
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "d_grad_weights given for a context without a residual network");
+  ctx->last_stream = s;
+  if (a->n_envs == 0) return ETAC_OK;
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, ETAC_ERR_CUDA, "cudaSetDevice failed");
+  StepIO io{};
+  io.n_envs = a->n_envs, io.input_mode = a->input_mode;
+  io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
+  cudaError_t e;
+  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess ||
+      (e = cudaMemsetAsync(a->d_grad_alpha, 0, sizeof(float) * ctx->n_alpha, s)) != cudaSuccess ||
+      (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * ETAC_GRAD_WEIGHTS_LEN, s)) != cudaSuccess))
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset", e));
+  if ((e = launch_sdf(ctx->m, io, 0, s)) != cudaSuccess)  // S1: delta and the pair flags only
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
+  if ((e = launch_backward(ctx->m, io, a->d_grad_out, a->d_grad_alpha, ctx->n_alpha, a->d_grad_weights, ctx->n_sm, s)) != cudaSuccess)
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("backward_kernel", e));
+  ctx->last_launches = 2;
+  return ETAC_OK;
 }
 
 etac_status etac_time_steps(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args, int32_t iters,

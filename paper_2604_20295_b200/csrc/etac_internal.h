@@ -160,6 +160,9 @@ cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1,
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s);
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
+cudaError_t backward_configure();
+cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,
+                            float* grad_w, int n_sm, cudaStream_t s);
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
                               int n_sm, bool gather, int* launches, cudaStream_t s);
 cudaError_t dense_bf16_configure();

@@ -30,7 +30,7 @@ ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
  ETAC_INFO_LAST_LAUNCHES, ETAC_INFO_LAST_CONTACT_PAIRS, ETAC_INFO_SM_COUNT) = range(1, 9)
 
 EXPORTS = ["etac_create", "etac_destroy", "etac_step", "etac_set_option", "etac_get_info", "etac_last_error",
-           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid"]
+           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward"]
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -60,6 +60,15 @@ class etac_step_args(C.Structure):
                 ("out_env_stride", C.c_int64), ("out_dtype", C.c_int32), ("reserved", C.c_int32)]
 
 
+class etac_backward_args(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_envs", C.c_int32), ("input_mode", C.c_int32),
+                ("d_indenters", C.c_void_p), ("d_patch_pose", C.c_void_p), ("d_penetration", C.c_void_p),
+                ("d_grad_out", C.c_void_p), ("d_grad_alpha", C.c_void_p), ("d_grad_weights", C.c_void_p)]
+
+
+ETAC_GRAD_WEIGHTS_LEN = 4995
+GRAD_WEIGHTS_LAYOUT = (("W1", (64, 9)), ("b1", (64,)), ("W2", (64, 64)), ("b2", (64,)), ("W3", (3, 64)), ("b3", (3,)))
+
 _lib = None
 
 
@@ -81,6 +90,7 @@ def load() -> C.CDLL:
         lib.etac_patches_from_adjacency.argtypes = [C.c_int32, _ip, _ip, _ip, C.c_int32, _ip]
         lib.etac_abi_version.restype = C.c_int32
         lib.etac_time_steps.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_step_args), C.c_int32, _fp, _fp]
+        lib.etac_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_backward_args)]
         lib.etac_set_sdf_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
         for name in EXPORTS:
             getattr(lib, name)
@@ -209,6 +219,28 @@ def etac_patches_from_adjacency(n_nodes, adj_rowptr, adj_col):
     if st != ETAC_OK:
         raise EtacError(st, "etac_patches_from_adjacency")
     return off[: n.value + 1].copy()
+
+
+def etac_backward(ctx, stream, n_envs, grad_out, grad_alpha, grad_weights=None, *, indenters=None, patch_pose=None,
+                  penetration=None) -> None:
+    """dL/dalpha and dL/d(MLP weights) of one step from dL/dU (device tensors / addresses; marshalling only)."""
+    a = etac_backward_args()
+    a.struct_size = C.sizeof(etac_backward_args)
+    a.n_envs = n_envs
+    a.input_mode = ETAC_IN_PENETRATION if penetration is not None else ETAC_IN_INDENTERS
+    a.d_indenters, a.d_patch_pose, a.d_penetration = _dptr(indenters), _dptr(patch_pose), _dptr(penetration)
+    a.d_grad_out, a.d_grad_alpha, a.d_grad_weights = _dptr(grad_out), _dptr(grad_alpha), _dptr(grad_weights)
+    _check(ctx, load().etac_backward(ctx, stream, C.byref(a)))
+
+
+def split_grad_weights(flat):
+    """[4995] -> {"W1": [64, 9], "b1": [64], ...} views in the order of etac_backward_args.d_grad_weights."""
+    out, o = {}, 0
+    for name, shape in GRAD_WEIGHTS_LAYOUT:
+        n = int(np.prod(shape))
+        out[name] = flat[o:o + n].reshape(shape)
+        o += n
+    return out
 
 
 def etac_time_steps(ctx, stream, args: etac_step_args, iters: int, per_kernel: bool = False):

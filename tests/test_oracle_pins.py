@@ -334,6 +334,63 @@ def test_self_contact_skip_is_per_patch():
         assert (phi_plain[sl] < 0).all() and (phi[off[B]:off[B + 1]] < 0).any()
 
 
+def _grad_case(n_alpha_per_patch, active_mode="passthrough", resid_arch="pernode"):
+    import dataclasses
+    mesh = W.assemble([W.fib_cap(6.0, 72), W.flat_pad(10, 12, 1.0)])
+    rng = np.random.default_rng(77)
+    E = 3
+    ind = W._blank_indenters(E, 2)
+    for k in range(2):
+        c = rng.integers(0, mesh.n_nodes, size=E)
+        size = rng.uniform(2.0, 4.0, E)
+        centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, rng.uniform(0.2, 1.0, E), rng.uniform(0, 6.28, E))
+        ind["type"][:, k], ind["param"][:, k, 0] = W.IND_SPHERE, size
+        ind["pose"][:, k, 0:3], ind["pose"][:, k, 3:7] = centre, q
+    alpha = np.asarray([0.45, 0.7] if n_alpha_per_patch else [0.5], np.float32)
+    wl = W.Workload("grad_case", mesh, alpha, W.make_weights(9, 1, std=0.3), E, 2, ind, None, "fp32")
+    target = rng.normal(0, 0.2, (E, mesh.n_nodes, 3))
+
+    def loss(wl_):
+        U = O.step(O.model_from_workload(wl_, resid_arch=resid_arch, active_mode=active_mode), indenters=wl_.indenters)["U"]
+        return 0.5 * float(((U - target) ** 2).sum()), U
+    return wl, target, loss, dataclasses
+
+
+@pytest.mark.parametrize("per_patch,active_mode,resid_arch", [(True, "passthrough", "pernode"), (False, "propagate", "pernode"),
+                                                               (True, "passthrough", "none")])
+def test_backward_oracle_matches_finite_differences(per_patch, active_mode, resid_arch):
+    """The gradient oracle against its definition: central differences of the (pinned) forward oracle's
+    loss 0.5*||U - U*||^2 (Eq. 3) in alpha and in sampled weights of every layer."""
+    from oracle import etac_oracle_grad as OG
+    wl, target, loss, dataclasses = _grad_case(per_patch, active_mode, resid_arch)
+    _, U = loss(wl)
+    m = O.model_from_workload(wl, resid_arch=resid_arch, active_mode=active_mode)
+    g = OG.backward(m, U - target, indenters=wl.indenters)
+    eps = 1e-6
+    for k in range(len(wl.alpha)):
+        a = wl.alpha.astype(np.float64)
+        ap, am = a.copy(), a.copy()
+        ap[k] += eps
+        am[k] -= eps
+        fd = (loss(dataclasses.replace(wl, alpha=ap))[0] - loss(dataclasses.replace(wl, alpha=am))[0]) / (2 * eps)
+        assert abs(fd - g["alpha"][k]) <= 1e-6 * max(1.0, abs(fd)), (k, fd, g["alpha"][k])
+    assert np.abs(g["alpha"]).min() > 1e-3                        # the case exercises every alpha
+    if resid_arch == "none":
+        return
+    rng = np.random.default_rng(5)
+    for name in ("W1", "b1", "W2", "b2", "W3", "b3"):
+        base = wl.weights[name].astype(np.float64)
+        for _ in range(3):
+            idx = tuple(rng.integers(0, s) for s in base.shape)
+            wp, wm = base.copy(), base.copy()
+            wp[idx] += eps
+            wm[idx] -= eps
+            fd = (loss(dataclasses.replace(wl, weights={**wl.weights, name: wp}))[0]
+                  - loss(dataclasses.replace(wl, weights={**wl.weights, name: wm}))[0]) / (2 * eps)
+            assert abs(fd - g[name][idx]) <= 2e-6 * max(1.0, abs(fd)), (name, idx, fd, g[name][idx])
+        assert np.abs(g[name]).max() > 1e-4
+
+
 # ---------------------------------------------------------------- P12
 def test_pointnet_branch_is_permutation_equivariant():
     rng = np.random.default_rng(8)

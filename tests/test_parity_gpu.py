@@ -474,6 +474,66 @@ def test_bf16_output_in_a_strided_observation_buffer(precision, path):
         eng.close()
 
 
+def _backward_case(kind):
+    import dataclasses
+    if kind == "hand_bf16":
+        wl = dataclasses.replace(W.config3(15, 19), weights=W.make_weights(3, 4, std=0.2))
+        return wl, "bf16", T.ETAC_ACTIVE_PASSTHROUGH, True
+    mesh = W.assemble([W.fib_cap(6.0, 72), W.flat_pad(10, 20, 1.0), W.half_cylinder(5.0, 12.0, 9, 15)])   # ragged: 72, 200, 135
+    rng = np.random.default_rng(31)
+    E = 9
+    ind = W._blank_indenters(E, 2)
+    for k in range(2):
+        c = rng.integers(0, mesh.n_nodes, size=E)
+        size = rng.uniform(2.0, 4.0, E)
+        centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, rng.uniform(0.2, 1.0, E), rng.uniform(0, 6.28, E))
+        ind["type"][:, k], ind["param"][:, k, 0] = W.IND_SPHERE, size
+        ind["pose"][:, k, 0:3], ind["pose"][:, k, 3:7] = centre, q
+    alpha = np.asarray([0.45, 0.7, 0.55], np.float32)
+    wl = W.Workload("grad_case", mesh, alpha, W.make_weights(9, 1, std=0.3), E, 2, ind, None, "fp32")
+    mode = T.ETAC_ACTIVE_PROPAGATE if kind == "propagate" else T.ETAC_ACTIVE_PASSTHROUGH
+    return wl, "fp32", mode, kind != "no_resid"
+
+
+@pytest.mark.parametrize("kind", ["per_patch_alpha", "propagate", "no_resid", "hand_bf16"])
+def test_backward_against_the_gradient_oracle(kind):
+    """etac_backward (calibration gradients of Eq. 3) against oracle/etac_oracle_grad.py
+    (itself pinned by finite differences): dL/dalpha and dL/d(MLP weights) for L = 0.5*||U - U*||^2.
+    fp32 arithmetic, fp32 atomics across CTAs: 2e-5 of the largest entry of each tensor (measured: 1e-8 .. 6e-7)."""
+    import torch
+    from oracle import etac_oracle as O, etac_oracle_grad as OG
+    wl, precision, mode, resid = _backward_case(kind)
+    m = O.model_from_workload(wl, resid_arch="pernode" if resid else "none",
+                              active_mode="propagate" if mode == T.ETAC_ACTIVE_PROPAGATE else "passthrough")
+    U = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)["U"]
+    G = U - np.random.default_rng(3).normal(0, 0.2, U.shape)
+    ref = OG.backward(m, G, indenters=wl.indenters, patch_pose=wl.patch_pose)
+    eng = T.Etac(wl, precision=precision, active_mode=mode, resid=resid)
+    try:
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        d_G = torch.from_numpy(G.astype(np.float32)).to(eng.device)
+        g_alpha = torch.full((len(wl.alpha),), 7.0, device=eng.device)
+        g_w = torch.full((T.ETAC_GRAD_WEIGHTS_LEN,), 7.0, device=eng.device) if resid else None
+        stream = torch.cuda.current_stream().cuda_stream
+        for _ in range(2):                                                # the outputs are overwritten, not accumulated
+            T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, g_w, **dev)
+        torch.cuda.synchronize()
+        got = {"alpha": g_alpha.cpu().numpy().astype(np.float64)}
+        if resid:
+            got.update({k: v.astype(np.float64) for k, v in T.split_grad_weights(g_w.cpu().numpy()).items()})
+        U_fwd = eng.step(wl.n_envs, dev).cpu().numpy()                    # the forward still works afterwards
+    finally:
+        eng.close()
+    assert set(got) == set(ref)
+    for k in ref:
+        scale = np.abs(ref[k]).max()
+        assert scale > 1e-4, k
+        err = np.abs(got[k] - ref[k]).max()
+        print(f"[backward {kind}] {k}: max|ref| {scale:.4g} max err {err:.3g} ({err / scale:.2e} rel)")
+        assert err <= 2e-5 * scale, (k, err, scale)
+    assert np.abs(U_fwd - U).max() <= (2e-2 if precision == "bf16" else 1e-4) * np.abs(U).max()
+
+
 def test_step_is_capturable_in_a_cuda_graph():
     """etac_step only enqueues (no sync, no allocation, no host copy): it can be captured in a
     CUDA graph and replayed; the replays give the eager result bit for bit."""
