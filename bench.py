@@ -32,9 +32,9 @@ UNIT = "env-steps/s"
 N_INPUT_SETS = 4
 MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728
 # dram__bytes_read.sum + dram__bytes_write.sum of one dense_bf16_kernel launch, from the
-# `ncu --set full` capture summarised in profiles/r01b_dense_ncu_full.md (79.3 MB read + 234.1 MB
-# write; the kernel now also zero-fills the rows of contact-free (env, patch) pairs).
-NCU_TRAFFIC_BYTES = 313.43e6
+# `ncu --set full` capture summarised in profiles/r01c_dense_ncu_full.md (79.2 MB read + 232.2 MB
+# write; the kernel also zero-fills the rows of contact-free (env, patch) pairs).
+NCU_TRAFFIC_BYTES = 311.37e6
 
 
 WORKLOADS = {
