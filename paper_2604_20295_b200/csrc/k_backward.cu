@@ -11,18 +11,23 @@
 //   dL/dW       += the usual MLP backward of G_i
 // Active rows of Eq. (2) are u^ itself and carry no gradient to alpha or Phi.
 //
-// The grid is persistent (one CTA per SM, 128 threads).  Per item every thread runs forward and
-// backward of its node with its activations in registers and leaves h1, dz1, dz2, h2 as columns of
-// four [64 x 128] shared-memory arrays; the weight gradients are then CTA-level products of those
-// arrays (dW2 = dZ2^T H1 as a 4 x 8 register tile per thread), accumulated in registers over all
-// items of the CTA and added to the global result once at the end (fp32 atomics: the sum order
-// across CTAs is not fixed, results agree to fp32 rounding).
+// The grid is persistent (one CTA per SM, 512 threads: four threads per node, each owning 16 of the
+// 64 hidden units, so that 16 warps hide each other's FMA and shared-memory latencies; the
+// activations take 1 KB of shared memory per node, which limits an SM to 128 nodes in flight).
+// Per item the threads run forward and backward of their node's MLP and leave h1, dz1, dz2, h2 as
+// columns of four [64 x 128] shared-memory arrays; the weight gradients are then CTA-level products
+// of those arrays (dW2 = dZ2^T H1 as 4 x 4 register tiles over half the nodes each), accumulated
+// in registers over all items of the CTA and added to the global result once at the end (fp32
+// atomics: the sum order across CTAs is not fixed, results agree to fp32 rounding).
 #include "etac_internal.h"
 
 namespace etac {
 
 namespace {
-constexpr int kT = kGatherChunk;        // threads per CTA = nodes per item
+constexpr int kT = kGatherChunk;        // nodes per item
+constexpr int kParts = 4;               // threads per node: part s owns the hidden units 16 s .. 16 s + 15
+constexpr int kThreads = kT * kParts;   // 512: thread t = s * 128 + i (s is warp-uniform)
+constexpr int kHp = kHidden / kParts;   // 16
 constexpr int kLd = kT + 1;             // row pitch of the [64][128] arrays (conflict-free column and row access)
 constexpr int kWf32 = 64 * 3 + 64 * 64 + 64 + 3 * 64 + 3;  // W1u | W2 | b2 | W3 | b3 (DevModel::wf32)
 
@@ -34,10 +39,10 @@ struct BwdSmem {
   float D[kHidden * kLd];  // h2
   float X[9 * kLd];        // layer-1 input [u(3), p(3), n(3)] per node
   float G[3 * kLd];        // upstream gradient of the rows that carry one (0 elsewhere)
+  float L[kParts][3][kT];  // per-part shares of W1u^T dz1
   float u[kT][3];
   int j[kT];
   int wcnt[kT / 32];
-  float red[kT / 32];
 };
 
 __device__ __forceinline__ void silu_and_grad(float z, float& y, float& dy) {
@@ -47,31 +52,35 @@ __device__ __forceinline__ void silu_and_grad(float z, float& y, float& dy) {
 }
 }  // namespace
 
-__global__ void __launch_bounds__(kT, 1) backward_kernel(DevModel m, StepIO io, const float* __restrict__ grad_out,
-                                                         float* __restrict__ grad_alpha, int n_alpha,
-                                                         float* __restrict__ grad_w) {
+__global__ void __launch_bounds__(kThreads, 1) backward_kernel(DevModel m, StepIO io, const float* __restrict__ grad_out,
+                                                               float* __restrict__ grad_alpha, int n_alpha,
+                                                               float* __restrict__ grad_w) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
   BwdSmem& S = *reinterpret_cast<BwdSmem*>(smem_raw);
-  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int t = threadIdx.x, lane = t & 31;
+  const int part = t / kT, i = t - part * kT, warp_i = i >> 5;  // node slot i, its warp within the part
+  const int k0 = part * kHp;
   const bool mlp = m.resid == ETAC_RESID_PERNODE_MLP;
   if (mlp)
-    for (int k = t; k < kWf32; k += kT) S.w[k] = m.wf32[k];
+    for (int k = t; k < kWf32; k += kThreads) S.w[k] = m.wf32[k];
   const float* W1u = S.w;
   const float* W2 = S.w + 192;
   const float* b2 = W2 + 4096;
   const float* W3 = b2 + 64;
 
-  // per-thread shares of the weight gradients, accumulated over all items of this CTA
-  const int kt = 4 * (t & 15), jt = 8 * (t >> 4);  // dW2 tile: rows kt..kt+3 (layer-2 output), columns jt..jt+7
-  float gw2[4][8];
+  // per-thread shares of the weight gradients, accumulated over all items of this CTA.
+  // dW2 = dZ2^T H1: 4 x 4 tile (rows kt.., columns jt..) over the nodes [ih, ih + 64) of the item
+  const int tile = t & 255, ih = (t >> 8) * (kT / 2);
+  const int kt = 4 * (tile & 15), jt = 4 * (tile >> 4);
+  float gw2[4][4];
 #pragma unroll
   for (int a = 0; a < 4; ++a)
 #pragma unroll
-    for (int b = 0; b < 8; ++b) gw2[a][b] = 0.f;
-  float gw1[5] = {0.f, 0.f, 0.f, 0.f, 0.f};  // dW1 entries t, t+128, ... (< 576) in [64 x 9] order
-  float gw3[2] = {0.f, 0.f};                 // dW3 entries t, t+128 (< 192) in [3 x 64] order
-  float gb = 0.f;                            // t < 64: db1[t]; else db2[t - 64]
-  float gb3 = 0.f;                           // t < 3: db3[t]
+    for (int b = 0; b < 4; ++b) gw2[a][b] = 0.f;
+  float gw1[2] = {0.f, 0.f};  // dW1 entries t, t + 512 (< 576) in [64 x 9] order
+  float gw3 = 0.f;            // t < 192: dW3 entry t in [3 x 64] order
+  float gb = 0.f;             // t < 64: db1[t]; t < 128: db2[t - 64]
+  float gb3 = 0.f;            // t < 3: db3[t]
   __syncthreads();
 
   const int64_t n_items = (int64_t)m.n_chunks * io.n_envs;
@@ -80,26 +89,27 @@ __global__ void __launch_bounds__(kT, 1) backward_kernel(DevModel m, StepIO io, 
     const ChunkInfo ch = m.chunk[item - (int64_t)e * m.n_chunks];
     if (!m.flags[(int64_t)e * m.n_patches + ch.patch]) continue;  // contact-free pair: U = 0, no gradient
     const PatchInfo pi = m.patch[ch.patch];
-    const bool valid = t < ch.count;
-    const int g = ch.node0 + (valid ? t : 0);
+    const bool valid = i < ch.count;
+    const int g = ch.node0 + (valid ? i : 0);
     const int li = g - pi.off;
     const float* __restrict__ delta = m.delta + (int64_t)e * m.n_nodes + pi.off;
     const float* __restrict__ K = m.k32 + pi.k32_off;
 
-    // ---- u_i = sum_j K_ij u^_j and v_i = sum_j K_ij ln K_ij u^_j over the active nodes j (node order)
+    // ---- u_i = sum_j K_ij u^_j and v_i = sum_j K_ij ln K_ij u^_j over the active nodes j (node order);
+    // part 0 compacts the active nodes, every part runs the (short) sum for its copy of node i
     float ax = 0.f, ay = 0.f, az = 0.f, vx = 0.f, vy = 0.f, vz = 0.f;
     for (int base = 0; base < pi.n; base += kT) {
-      const int j = base + t;
-      const float d = j < pi.n ? delta[j] : 0.0f;
+      const int j = base + i;
+      const float d = (part == 0 && j < pi.n) ? delta[j] : 0.0f;
       const bool act = d > 0.0f;
       const unsigned bal = __ballot_sync(0xffffffffu, act);
-      if (lane == 0) S.wcnt[warp] = __popc(bal);
+      if (part == 0 && lane == 0) S.wcnt[warp_i] = __popc(bal);
       __syncthreads();
       int pre = 0, total = 0;
 #pragma unroll
       for (int w = 0; w < kT / 32; ++w) {
         const int c = S.wcnt[w];
-        pre += w < warp ? c : 0;
+        pre += w < warp_i ? c : 0;
         total += c;
       }
       if (act) {
@@ -124,29 +134,39 @@ __global__ void __launch_bounds__(kT, 1) backward_kernel(DevModel m, StepIO io, 
       const float* go = grad_out + ((int64_t)e * m.n_nodes + g) * 3;
       g0 = go[0], g1 = go[1], g2 = go[2];
     }
-    float l0 = g0, l1 = g1, l2 = g2;  // dL/du_i = G_i + J_Phi,u^T G_i
+    float l0 = g0, l1 = g1, l2 = g2;  // dL/du_i = G_i + J_Phi,u^T G_i (completed by part 0 below)
     if (mlp) {
-      const float4 pos = m.pos4[g], nrm = m.nrm4[g];
-      S.X[0 * kLd + t] = ax, S.X[1 * kLd + t] = ay, S.X[2 * kLd + t] = az;
-      S.X[3 * kLd + t] = pos.x, S.X[4 * kLd + t] = pos.y, S.X[5 * kLd + t] = pos.z;
-      S.X[6 * kLd + t] = nrm.x, S.X[7 * kLd + t] = nrm.y, S.X[8 * kLd + t] = nrm.z;
-      S.G[0 * kLd + t] = g0, S.G[1 * kLd + t] = g1, S.G[2 * kLd + t] = g2;
-      // forward layer 1 (position / normal part precomputed at create: c1t), activations in registers
+      if (part == 0) {
+        const float4 pos = m.pos4[g], nrm = m.nrm4[g];
+        S.X[0 * kLd + i] = ax, S.X[1 * kLd + i] = ay, S.X[2 * kLd + i] = az;
+        S.X[3 * kLd + i] = pos.x, S.X[4 * kLd + i] = pos.y, S.X[5 * kLd + i] = pos.z;
+        S.X[6 * kLd + i] = nrm.x, S.X[7 * kLd + i] = nrm.y, S.X[8 * kLd + i] = nrm.z;
+        S.G[0 * kLd + i] = g0, S.G[1 * kLd + i] = g1, S.G[2 * kLd + i] = g2;
+      }
+      // forward layer 1 for this part's hidden units (position / normal part precomputed at create: c1t)
+      {
+        float z[kHp];
+#pragma unroll
+        for (int q = 0; q < kHp; ++q) z[q] = m.c1t[(int64_t)(k0 + q) * m.n_nodes + g];
+#pragma unroll
+        for (int q = 0; q < kHp; ++q) {
+          const int k = k0 + q;
+          float zz = z[q], y, dy;
+          zz = fmaf(W1u[k * 3 + 0], ax, zz), zz = fmaf(W1u[k * 3 + 1], ay, zz), zz = fmaf(W1u[k * 3 + 2], az, zz);
+          silu_and_grad(zz, y, dy);
+          S.A[k * kLd + i] = dy;
+          S.B[k * kLd + i] = y;
+        }
+      }
+      __syncthreads();  // h1 of every node complete
       float h[kHidden];
 #pragma unroll
-      for (int k = 0; k < kHidden; ++k) h[k] = m.c1t[(int64_t)k * m.n_nodes + g];  // 64 independent loads in flight
-#pragma unroll
-      for (int k = 0; k < kHidden; ++k) {
-        float z = h[k];
-        z = fmaf(W1u[k * 3 + 0], ax, z), z = fmaf(W1u[k * 3 + 1], ay, z), z = fmaf(W1u[k * 3 + 2], az, z);
-        float dy;
-        silu_and_grad(z, h[k], dy);
-        S.A[k * kLd + t] = dy;
-        S.B[k * kLd + t] = h[k];
-      }
-      // forward layer 2 and, in the same sweep, dz2 = (W3^T G) * silu'(z2); two rows and two partial sums
-      // per row at a time: with one warp per SM sub-partition the FMA latency is not hidden otherwise
-      for (int k2 = 0; k2 < kHidden; k2 += 2) {
+      for (int k = 0; k < kHidden; ++k) h[k] = S.B[k * kLd + i];
+      // forward layer 2 for this part's rows and, in the same sweep, dz2 = (W3^T G) * silu'(z2);
+      // two rows and two partial sums per row at a time (FMA latency)
+#pragma unroll 1
+      for (int q = 0; q < kHp; q += 2) {
+        const int k2 = k0 + q;
         float za = b2[k2], zb = b2[k2 + 1], zc = 0.f, zd = 0.f;
         const float4* wa = reinterpret_cast<const float4*>(W2 + k2 * kHidden);
         const float4* wb = reinterpret_cast<const float4*>(W2 + (k2 + 1) * kHidden);
@@ -159,97 +179,94 @@ __global__ void __launch_bounds__(kT, 1) backward_kernel(DevModel m, StepIO io, 
           zb = fmaf(v.z, h[4 * k + 2], zb), zd = fmaf(v.w, h[4 * k + 3], zd);
         }
 #pragma unroll
-        for (int q = 0; q < 2; ++q) {
-          const int kk = k2 + q;
+        for (int r = 0; r < 2; ++r) {
+          const int kk = k2 + r;
           float y, dy;
-          silu_and_grad(q ? zb + zd : za + zc, y, dy);
+          silu_and_grad(r ? zb + zd : za + zc, y, dy);
           const float gh2 = fmaf(W3[kk], g0, fmaf(W3[kHidden + kk], g1, W3[2 * kHidden + kk] * g2));
-          S.C[kk * kLd + t] = gh2 * dy;
-          S.D[kk * kLd + t] = y;
+          S.C[kk * kLd + i] = gh2 * dy;
+          S.D[kk * kLd + i] = y;
         }
       }
-      // dh1 = W2^T dz2 (h[] is reused), dz1 = dh1 * silu'(z1), dL/du += W1u^T dz1
+      __syncthreads();  // dz2 of every node complete
+      // dh1 = W2^T dz2 for this part's 16 hidden units, dz1 = dh1 * silu'(z1), share of W1u^T dz1
 #pragma unroll
-      for (int k = 0; k < kHidden; ++k) h[k] = 0.f;
+      for (int k = 0; k < kHidden; ++k) h[k] = S.C[k * kLd + i];  // dz2 of node i
+      float gh[kHp];
+#pragma unroll
+      for (int q = 0; q < kHp; ++q) gh[q] = 0.f;
+#pragma unroll
       for (int k2 = 0; k2 < kHidden; ++k2) {
-        const float gz = S.C[k2 * kLd + t];
-        const float4* w = reinterpret_cast<const float4*>(W2 + k2 * kHidden);
+        const float4* w = reinterpret_cast<const float4*>(W2 + k2 * kHidden + k0);
 #pragma unroll
-        for (int k = 0; k < kHidden / 4; ++k) {
-          const float4 wv = w[k];
-          h[4 * k + 0] = fmaf(wv.x, gz, h[4 * k + 0]), h[4 * k + 1] = fmaf(wv.y, gz, h[4 * k + 1]);
-          h[4 * k + 2] = fmaf(wv.z, gz, h[4 * k + 2]), h[4 * k + 3] = fmaf(wv.w, gz, h[4 * k + 3]);
+        for (int q = 0; q < kHp / 4; ++q) {
+          const float4 wv = w[q];
+          gh[4 * q + 0] = fmaf(wv.x, h[k2], gh[4 * q + 0]), gh[4 * q + 1] = fmaf(wv.y, h[k2], gh[4 * q + 1]);
+          gh[4 * q + 2] = fmaf(wv.z, h[k2], gh[4 * q + 2]), gh[4 * q + 3] = fmaf(wv.w, h[k2], gh[4 * q + 3]);
         }
       }
+      float p0 = 0.f, p1 = 0.f, p2 = 0.f;
 #pragma unroll
-      for (int k = 0; k < kHidden; ++k) {
-        const float gz1 = h[k] * S.A[k * kLd + t];
-        S.A[k * kLd + t] = gz1;
-        l0 = fmaf(W1u[k * 3 + 0], gz1, l0), l1 = fmaf(W1u[k * 3 + 1], gz1, l1), l2 = fmaf(W1u[k * 3 + 2], gz1, l2);
+      for (int q = 0; q < kHp; ++q) {
+        const int k = k0 + q;
+        const float gz1 = gh[q] * S.A[k * kLd + i];
+        S.A[k * kLd + i] = gz1;
+        p0 = fmaf(W1u[k * 3 + 0], gz1, p0), p1 = fmaf(W1u[k * 3 + 1], gz1, p1), p2 = fmaf(W1u[k * 3 + 2], gz1, p2);
       }
+      S.L[part][0][i] = p0, S.L[part][1][i] = p1, S.L[part][2][i] = p2;
+      __syncthreads();  // dz1 and the shares of W1u^T dz1 complete
+#pragma unroll
+      for (int s = 0; s < kParts; ++s) l0 += S.L[s][0][i], l1 += S.L[s][1][i], l2 += S.L[s][2][i];
     }
-    // ---- dL/dalpha of this item: sum_i dL/du_i . v_i / alpha
-    {
+    // ---- dL/dalpha of this item: sum_i dL/du_i . v_i / alpha (part 0's warps, one atomic each)
+    if (part == 0) {
       float ga = carries ? (l0 * vx + l1 * vy + l2 * vz) / pi.alpha : 0.0f;
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) ga += __shfl_xor_sync(0xffffffffu, ga, o);
-      if (lane == 0) S.red[warp] = ga;
-    }
-    __syncthreads();  // columns of A, B, C, D, X, G and red[] complete
-    if (t == 0) {
-      float ga = 0.f;
-#pragma unroll
-      for (int w = 0; w < kT / 32; ++w) ga += S.red[w];
-      atomicAdd(&grad_alpha[n_alpha == 1 ? 0 : ch.patch], ga);
+      if (lane == 0) atomicAdd(&grad_alpha[n_alpha == 1 ? 0 : ch.patch], ga);
     }
     if (mlp) {
       // ---- weight gradients as CTA-level products over the item's 128 nodes
-      for (int i = 0; i < kT; ++i) {
-        float a[4], b[8];
+#pragma unroll 4
+      for (int n = ih; n < ih + kT / 2; ++n) {
+        float a[4], b[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) a[q] = S.C[(kt + q) * kLd + i];
-#pragma unroll
-        for (int q = 0; q < 8; ++q) b[q] = S.B[(jt + q) * kLd + i];
+        for (int q = 0; q < 4; ++q) a[q] = S.C[(kt + q) * kLd + n], b[q] = S.B[(jt + q) * kLd + n];
 #pragma unroll
         for (int q = 0; q < 4; ++q)
 #pragma unroll
-          for (int r = 0; r < 8; ++r) gw2[q][r] = fmaf(a[q], b[r], gw2[q][r]);
+          for (int r = 0; r < 4; ++r) gw2[q][r] = fmaf(a[q], b[r], gw2[q][r]);
       }
 #pragma unroll
-      for (int q = 0; q < 5; ++q) {
-        const int idx = t + q * kT;  // (k, c) = (idx / 9, idx % 9)
+      for (int q = 0; q < 2; ++q) {
+        const int idx = t + q * kThreads;  // (k, c) = (idx / 9, idx % 9)
         if (idx < kHidden * 9) {
           const float* zr = S.A + (idx / 9) * kLd;
           const float* xr = S.X + (idx % 9) * kLd;
           float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-          for (int i = 0; i < kT; i += 4)
-            s0 = fmaf(zr[i], xr[i], s0), s1 = fmaf(zr[i + 1], xr[i + 1], s1), s2 = fmaf(zr[i + 2], xr[i + 2], s2),
-            s3 = fmaf(zr[i + 3], xr[i + 3], s3);
+          for (int n = 0; n < kT; n += 4)
+            s0 = fmaf(zr[n], xr[n], s0), s1 = fmaf(zr[n + 1], xr[n + 1], s1), s2 = fmaf(zr[n + 2], xr[n + 2], s2),
+            s3 = fmaf(zr[n + 3], xr[n + 3], s3);
           gw1[q] += (s0 + s1) + (s2 + s3);
         }
       }
-#pragma unroll
-      for (int q = 0; q < 2; ++q) {
-        const int idx = t + q * kT;  // (c, k) = (idx / 64, idx % 64)
-        if (idx < 3 * kHidden) {
-          const float* gr = S.G + (idx / kHidden) * kLd;
-          const float* hr = S.D + (idx % kHidden) * kLd;
-          float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-          for (int i = 0; i < kT; i += 4)
-            s0 = fmaf(gr[i], hr[i], s0), s1 = fmaf(gr[i + 1], hr[i + 1], s1), s2 = fmaf(gr[i + 2], hr[i + 2], s2),
-            s3 = fmaf(gr[i + 3], hr[i + 3], s3);
-          gw3[q] += (s0 + s1) + (s2 + s3);
-        }
-      }
-      {
-        const float* zr = (t < kHidden ? S.A : S.C) + (t & (kHidden - 1)) * kLd;
+      if (t < 3 * kHidden) {  // (c, k) = (t / 64, t % 64)
+        const float* gr = S.G + (t / kHidden) * kLd;
+        const float* hr = S.D + (t % kHidden) * kLd;
         float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
-        for (int i = 0; i < kT; i += 4) s0 += zr[i], s1 += zr[i + 1], s2 += zr[i + 2], s3 += zr[i + 3];
+        for (int n = 0; n < kT; n += 4)
+          s0 = fmaf(gr[n], hr[n], s0), s1 = fmaf(gr[n + 1], hr[n + 1], s1), s2 = fmaf(gr[n + 2], hr[n + 2], s2),
+          s3 = fmaf(gr[n + 3], hr[n + 3], s3);
+        gw3 += (s0 + s1) + (s2 + s3);
+      } else if (t >= 256 && t < 256 + 2 * kHidden) {  // (other warps than the dW3 ones)
+        const int k = t - 256;
+        const float* zr = (k < kHidden ? S.A : S.C) + (k & (kHidden - 1)) * kLd;
+        float s0 = 0.f, s1 = 0.f, s2 = 0.f, s3 = 0.f;
+        for (int n = 0; n < kT; n += 4) s0 += zr[n], s1 += zr[n + 1], s2 += zr[n + 2], s3 += zr[n + 3];
         gb += (s0 + s1) + (s2 + s3);
-      }
-      if (t < 3) {
+      } else if (t >= 384 && t < 387) {
         float s = 0.f;
-        for (int i = 0; i < kT; ++i) s += S.G[t * kLd + i];
+        for (int n = 0; n < kT; ++n) s += S.G[(t - 384) * kLd + n];
         gb3 += s;
       }
     }
@@ -264,17 +281,15 @@ __global__ void __launch_bounds__(kT, 1) backward_kernel(DevModel m, StepIO io, 
     float* gW3 = gb2 + 64;
     float* gB3 = gW3 + 192;
 #pragma unroll
-    for (int q = 0; q < 5; ++q)
-      if (t + q * kT < 576) atomicAdd(&gW1[t + q * kT], gw1[q]);
-    atomicAdd(t < kHidden ? &gb1[t] : &gb2[t - kHidden], gb);
+    for (int q = 0; q < 2; ++q)
+      if (t + q * kThreads < 576) atomicAdd(&gW1[t + q * kThreads], gw1[q]);
 #pragma unroll
     for (int q = 0; q < 4; ++q)
 #pragma unroll
-      for (int r = 0; r < 8; ++r) atomicAdd(&gW2[(kt + q) * kHidden + jt + r], gw2[q][r]);
-#pragma unroll
-    for (int q = 0; q < 2; ++q)
-      if (t + q * kT < 192) atomicAdd(&gW3[t + q * kT], gw3[q]);
-    if (t < 3) atomicAdd(&gB3[t], gb3);
+      for (int r = 0; r < 4; ++r) atomicAdd(&gW2[(kt + q) * kHidden + jt + r], gw2[q][r]);
+    if (t < 3 * kHidden) atomicAdd(&gW3[t], gw3);
+    if (t >= 256 && t < 256 + 2 * kHidden) atomicAdd(t - 256 < kHidden ? &gb1[t - 256] : &gb2[t - 256 - kHidden], gb);
+    if (t >= 384 && t < 387) atomicAdd(&gB3[t - 384], gb3);
   }
 }
 
@@ -284,7 +299,7 @@ cudaError_t backward_configure() {
 
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,
                             float* grad_w, int n_sm, cudaStream_t s) {
-  backward_kernel<<<n_sm, kT, sizeof(BwdSmem), s>>>(m, io, grad_out, grad_alpha, n_alpha, grad_w);
+  backward_kernel<<<n_sm, kThreads, sizeof(BwdSmem), s>>>(m, io, grad_out, grad_alpha, n_alpha, grad_w);
   return cudaGetLastError();
 }
 
