@@ -218,6 +218,19 @@ typedef struct {
 #define ETAC_GRAD_WEIGHTS_LEN 4995
 etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* args);
 
+/* Replaces the calibrated parameters of a context in place (one gradient-descent step of Eq. (3)):
+ * alpha ([n_alpha], same n_alpha as at create; NULL = keep; K is rebuilt on the device) and / or the six
+ * arrays of the per-node MLP (all six or none; layouts as in etac_model_desc).  Host pointers, copied.
+ * Synchronises the device before and after; not to be called concurrently with etac_step /
+ * etac_backward on the same ctx.  The result is the same as a context created with these parameters. */
+typedef struct {
+  uint32_t struct_size;   /* = sizeof(etac_params) */
+  int32_t n_alpha;
+  const float* alpha;
+  const float *W1, *b1, *W2, *b2, *W3, *b3;
+} etac_params;
+etac_status etac_update_params(etac_ctx* ctx, const etac_params* params);
+
 /* Library ABI version (ETAC_ABI_VERSION the .so was built with). */
 int32_t etac_abi_version(void);
 

@@ -21,6 +21,11 @@ struct etac_ctx {
   bool have_tm = false;
   cudaStream_t last_stream = nullptr;
   std::string err;
+  // writable aliases of the parameter-dependent device buffers (etac_update_params)
+  std::vector<PatchInfo> hp;
+  float* k32_w = nullptr;
+  __nv_bfloat16* k16_w = nullptr;
+  float *dW1_w = nullptr, *db1_w = nullptr;
 };
 
 static thread_local std::string g_create_err;
@@ -201,6 +206,41 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   ++ctx->last_launches;
   if (ev) cudaEventRecord(ev[2], s);
   return ETAC_OK;
+}
+
+// Host staging of the per-node MLP: the fp32 blob of the SIMT kernels (W1u | W2 | b2 | W3 | b3) and the
+// bf16 shared-memory image of the tensor-core path.  The epilogue evaluates silu(x) = h + h*tanh(h) with
+// h = x/2, so the 0.5 is folded into layers 1 and 2 (exact); the output layer runs on the FMA pipe in
+// fp32 (DevModel::wout).
+struct PerNodeStage {
+  std::vector<float> wf;
+  std::vector<uint8_t> img;
+  float wout[196];
+};
+void stage_pernode(const float* W1, const float* b1, const float* W2, const float* b2, const float* W3, const float* b3,
+                   PerNodeStage* st) {
+  st->wf.assign(64 * 3 + 64 * 64 + 64 + 3 * 64 + 3, 0.f);
+  float* q = st->wf.data();
+  for (int k = 0; k < 64; ++k)
+    for (int cc = 0; cc < 3; ++cc) *q++ = W1[k * 9 + cc];
+  memcpy(q, W2, 4096 * 4), q += 4096;
+  memcpy(q, b2, 64 * 4), q += 64;
+  memcpy(q, W3, 192 * 4), q += 192;
+  memcpy(q, b3, 3 * 4);
+  st->img.assign(kWImgBytes, 0);
+  auto put = [&](size_t base, int n, int k, int rows, float v) {
+    const uint16_t b = f2bf(v);
+    memcpy(&st->img[base + wimg_off(n, k, rows)], &b, 2);
+  };
+  for (int n = 0; n < 64; ++n) {
+    for (int k = 0; k < 9; ++k) put(0, n, k, 64, 0.5f * W1[n * 9 + k]);
+    put(0, n, 9, 64, 0.5f * b1[n]);
+    for (int k = 0; k < 64; ++k) put(kW1ImgBytes, n, k, 64, 0.5f * W2[n * 64 + k]);
+    put(kW1ImgBytes, n, 64, 64, 0.5f * b2[n]);
+  }
+  memcpy(st->wout, W3, 192 * 4);
+  memcpy(st->wout + 192, b3, 3 * 4);
+  st->wout[195] = 0.0f;
 }
 
 }  // namespace
@@ -384,43 +424,23 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   CK(dev_alloc(c, &k32, (size_t)k32_total, false), "alloc K fp32");
   CK(dev_alloc(c, &k16, (size_t)N * m.kw, true), "alloc K bf16");
   m.k32 = k32, m.k16 = k16;
+  c->k32_w = k32, c->k16_w = k16, c->hp = hp;
   CK(launch_build_k(m, k32, k16, 0), "build_k_kernel");
 
   if (d->resid_arch == ETAC_RESID_PERNODE_MLP) {
-    // fp32 blob for the SIMT path
-    std::vector<float> wf(64 * 3 + 64 * 64 + 64 + 3 * 64 + 3);
-    float* q = wf.data();
-    for (int k = 0; k < 64; ++k)
-      for (int cc = 0; cc < 3; ++cc) *q++ = d->W1[k * 9 + cc];
-    memcpy(q, d->W2, 4096 * 4), q += 4096;
-    memcpy(q, d->b2, 64 * 4), q += 64;
-    memcpy(q, d->W3, 192 * 4), q += 192;
-    memcpy(q, d->b3, 3 * 4);
-    CK(dev_upload(c, &m.wf32, wf.data(), wf.size()), "upload weights");
+    PerNodeStage st;
+    stage_pernode(d->W1, d->b1, d->W2, d->b2, d->W3, d->b3, &st);
+    CK(dev_upload(c, &m.wf32, st.wf.data(), st.wf.size()), "upload weights");
     const float *dW1 = nullptr, *db1 = nullptr;
     CK(dev_upload(c, &dW1, d->W1, 64 * 9), "upload W1");
     CK(dev_upload(c, &db1, d->b1, 64), "upload b1");
+    c->dW1_w = const_cast<float*>(dW1), c->db1_w = const_cast<float*>(db1);
     float* c1t = nullptr;
     CK(dev_alloc(c, &c1t, (size_t)64 * N, false), "alloc c1");
     m.c1t = c1t;
     CK(launch_build_c1(m, dW1, db1, c1t, 0), "build_c1_kernel");
-    // bf16 shared-memory image for the tensor-core path.  The epilogue evaluates
-    // silu(x) = h + h*tanh(h) with h = x/2, so the 0.5 is folded into layers 1 and 2 (exact).
-    std::vector<uint8_t> img(kWImgBytes, 0);
-    auto put = [&](size_t base, int n, int k, int rows, float v) {
-      const uint16_t b = f2bf(v);
-      memcpy(&img[base + wimg_off(n, k, rows)], &b, 2);
-    };
-    for (int n = 0; n < 64; ++n) {
-      for (int k = 0; k < 9; ++k) put(0, n, k, 64, 0.5f * d->W1[n * 9 + k]);
-      put(0, n, 9, 64, 0.5f * d->b1[n]);
-      for (int k = 0; k < 64; ++k) put(kW1ImgBytes, n, k, 64, 0.5f * d->W2[n * 64 + k]);
-      put(kW1ImgBytes, n, 64, 64, 0.5f * d->b2[n]);
-    }
-    memcpy(m.wout, d->W3, 192 * 4);  // the output layer runs on the FMA pipe in fp32
-    memcpy(m.wout + 192, d->b3, 3 * 4);
-    m.wout[195] = 0.0f;
-    CK(dev_upload(c, &m.wimg, img.data(), img.size()), "upload weight image");
+    memcpy(m.wout, st.wout, sizeof(m.wout));
+    CK(dev_upload(c, &m.wimg, st.img.data(), st.img.size()), "upload weight image");
   }
 
   if (d->resid_arch == ETAC_RESID_POINTNET) {
@@ -572,6 +592,46 @@ etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value) {
     }
     default: return ETAC_ERR_INVALID_ARG;
   }
+}
+
+etac_status etac_update_params(etac_ctx* ctx, const etac_params* p) {
+  if (!ctx) return ETAC_ERR_INVALID_ARG;
+  if (!p || p->struct_size != sizeof(etac_params)) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_params");
+  const float* w[6] = {p->W1, p->b1, p->W2, p->b2, p->W3, p->b3};
+  int n_w = 0;
+  for (const float* q : w) n_w += q != nullptr;
+  if (n_w != 0 && n_w != 6) return fail(ctx, ETAC_ERR_INVALID_ARG, "give all six weight arrays or none");
+  if (n_w && ctx->m.resid != ETAC_RESID_PERNODE_MLP)
+    return fail(ctx, ETAC_ERR_UNSUPPORTED, "weights can be replaced on ETAC_RESID_PERNODE_MLP contexts only");
+  if (p->alpha) {
+    if (p->n_alpha != ctx->n_alpha) return fail(ctx, ETAC_ERR_INVALID_ARG, "n_alpha differs from the context's");
+    for (int k = 0; k < p->n_alpha; ++k)
+      if (!(p->alpha[k] > 0.0f) || !isfinite(p->alpha[k])) return fail(ctx, ETAC_ERR_INVALID_ARG, "alpha must be > 0");
+  }
+  DeviceGuard guard(ctx->device);
+  if (!guard.ok) return fail(ctx, ETAC_ERR_CUDA, "cudaSetDevice failed");
+  cudaError_t e = cudaDeviceSynchronize();  // steps in flight read the old parameters
+  if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("cudaDeviceSynchronize", e));
+  DevModel& m = ctx->m;
+  if (p->alpha) {  // Eq. (1): K_p is rebuilt on the device
+    for (int q = 0; q < m.n_patches; ++q) ctx->hp[q].alpha = p->alpha[ctx->n_alpha == 1 ? 0 : q];
+    e = cudaMemcpy(const_cast<PatchInfo*>(m.patch), ctx->hp.data(), sizeof(PatchInfo) * m.n_patches, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_build_k(m, ctx->k32_w, ctx->k16_w, 0);
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("rebuild K", e));
+  }
+  if (n_w) {
+    PerNodeStage st;
+    stage_pernode(p->W1, p->b1, p->W2, p->b2, p->W3, p->b3, &st);
+    e = cudaMemcpy(const_cast<float*>(m.wf32), st.wf.data(), st.wf.size() * 4, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->dW1_w, p->W1, 64 * 9 * 4, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->db1_w, p->b1, 64 * 4, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = launch_build_c1(m, ctx->dW1_w, ctx->db1_w, const_cast<float*>(m.c1t), 0);
+    if (e == cudaSuccess) e = cudaMemcpy(const_cast<uint8_t*>(m.wimg), st.img.data(), st.img.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("restage weights", e));
+    memcpy(m.wout, st.wout, sizeof(m.wout));
+  }
+  if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("update kernels", e));
+  return ETAC_OK;
 }
 
 etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* a) {

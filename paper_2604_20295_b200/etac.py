@@ -30,7 +30,7 @@ ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
  ETAC_INFO_LAST_LAUNCHES, ETAC_INFO_LAST_CONTACT_PAIRS, ETAC_INFO_SM_COUNT) = range(1, 9)
 
 EXPORTS = ["etac_create", "etac_destroy", "etac_step", "etac_set_option", "etac_get_info", "etac_last_error",
-           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward"]
+           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward", "etac_update_params"]
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -66,6 +66,11 @@ class etac_backward_args(C.Structure):
                 ("d_grad_out", C.c_void_p), ("d_grad_alpha", C.c_void_p), ("d_grad_weights", C.c_void_p)]
 
 
+class etac_params(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("n_alpha", C.c_int32), ("alpha", _fp),
+                ("W1", _fp), ("b1", _fp), ("W2", _fp), ("b2", _fp), ("W3", _fp), ("b3", _fp)]
+
+
 ETAC_GRAD_WEIGHTS_LEN = 4995
 GRAD_WEIGHTS_LAYOUT = (("W1", (64, 9)), ("b1", (64,)), ("W2", (64, 64)), ("b2", (64,)), ("W3", (3, 64)), ("b3", (3,)))
 
@@ -90,6 +95,7 @@ def load() -> C.CDLL:
         lib.etac_patches_from_adjacency.argtypes = [C.c_int32, _ip, _ip, _ip, C.c_int32, _ip]
         lib.etac_abi_version.restype = C.c_int32
         lib.etac_time_steps.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_step_args), C.c_int32, _fp, _fp]
+        lib.etac_update_params.argtypes = [C.c_void_p, C.POINTER(etac_params)]
         lib.etac_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_backward_args)]
         lib.etac_set_sdf_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
         for name in EXPORTS:
@@ -231,6 +237,23 @@ def etac_backward(ctx, stream, n_envs, grad_out, grad_alpha, grad_weights=None, 
     a.d_indenters, a.d_patch_pose, a.d_penetration = _dptr(indenters), _dptr(patch_pose), _dptr(penetration)
     a.d_grad_out, a.d_grad_alpha, a.d_grad_weights = _dptr(grad_out), _dptr(grad_alpha), _dptr(grad_weights)
     _check(ctx, load().etac_backward(ctx, stream, C.byref(a)))
+
+
+def etac_update_params(ctx, alpha=None, weights=None) -> None:
+    """Replace alpha and / or the per-node MLP weights ({"W1": ..., ..., "b3": ...}) of a context in place."""
+    p = etac_params()
+    p.struct_size = C.sizeof(etac_params)
+    keep = []
+    if alpha is not None:
+        a = np.ascontiguousarray(alpha, dtype=np.float32).reshape(-1)
+        keep.append(a)
+        p.n_alpha, p.alpha = a.size, a.ctypes.data_as(_fp)
+    if weights is not None:
+        for k in ("W1", "b1", "W2", "b2", "W3", "b3"):
+            w = np.ascontiguousarray(weights[k], dtype=np.float32)
+            keep.append(w)
+            setattr(p, k, w.ctypes.data_as(_fp))
+    _check(ctx, load().etac_update_params(ctx, C.byref(p)))
 
 
 def split_grad_weights(flat):

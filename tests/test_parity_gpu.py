@@ -534,6 +534,69 @@ def test_backward_against_the_gradient_oracle(kind):
     assert np.abs(U_fwd - U).max() <= (2e-2 if precision == "bf16" else 1e-4) * np.abs(U).max()
 
 
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_update_params_equals_a_fresh_context(precision):
+    """etac_update_params (a gradient-descent step of Eq. 3 writes alpha and Phi back): the context then
+    gives bit for bit what a context created with the new parameters gives."""
+    import dataclasses
+    wl_a = W.config3(16, 11)
+    wl_b = dataclasses.replace(wl_a, alpha=np.asarray([0.8], np.float32), weights=W.make_weights(3, 9, std=0.15))
+    dev_kw = dict(indenters=wl_a.indenters, patch_pose=wl_a.patch_pose)
+    eng_b = T.Etac(wl_b, precision=precision)
+    U_b = eng_b.step(wl_b.n_envs, eng_b.upload(**dev_kw)).cpu().numpy()
+    eng_b.close()
+    eng = T.Etac(wl_a, precision=precision)
+    try:
+        dev = eng.upload(**dev_kw)
+        U_a = eng.step(wl_a.n_envs, dev).cpu().numpy()
+        T.etac_update_params(eng.ctx, alpha=wl_b.alpha, weights=wl_b.weights)
+        U_ab = eng.step(wl_a.n_envs, dev).cpu().numpy()
+        T.etac_update_params(eng.ctx, alpha=wl_a.alpha)                      # alpha alone, back
+        T.etac_update_params(eng.ctx, weights=wl_a.weights)                  # weights alone, back
+        U_aa = eng.step(wl_a.n_envs, dev).cpu().numpy()
+        with pytest.raises(T.EtacError):
+            T.etac_update_params(eng.ctx, alpha=np.asarray([0.5, 0.6], np.float32))   # n_alpha differs
+        with pytest.raises(T.EtacError):
+            T.etac_update_params(eng.ctx, alpha=np.asarray([-1.0], np.float32))
+    finally:
+        eng.close()
+    assert np.abs(U_a - U_b).max() > 1e-2
+    assert np.array_equal(U_ab, U_b) and np.array_equal(U_aa, U_a)
+
+
+def test_calibration_recovers_alpha_of_a_synthetic_teacher():
+    """Eq. (3) end to end on synthetic data (the paper's FEM data is not available): displacements of a
+    teacher with hidden alpha* (one per patch) are the targets; Adam on dL/dalpha from etac_backward, written
+    back with etac_update_params, recovers alpha* from a start 30-40 % off."""
+    import dataclasses
+    import torch
+    wl, precision, mode, _ = _backward_case("per_patch_alpha")
+    a_star = wl.alpha.astype(np.float64)
+    dev_kw = dict(indenters=wl.indenters, patch_pose=wl.patch_pose)
+    teacher = T.Etac(wl, precision=precision)
+    target = teacher.step(wl.n_envs, teacher.upload(**dev_kw)).clone()
+    teacher.close()
+    a = a_star * np.asarray([0.65, 1.35, 0.7])
+    eng = T.Etac(dataclasses.replace(wl, alpha=a.astype(np.float32)), precision=precision)
+    try:
+        dev = eng.upload(**dev_kw)
+        stream = torch.cuda.current_stream().cuda_stream
+        g_alpha = torch.empty(3, device=eng.device)
+        m1, m2, losses = np.zeros(3), np.zeros(3), []
+        for it in range(1, 121):
+            G = eng.step(wl.n_envs, dev) - target
+            losses.append(0.5 * float((G * G).sum()))
+            T.etac_backward(eng.ctx, stream, wl.n_envs, G.contiguous(), g_alpha, None, **dev)
+            g = g_alpha.cpu().numpy().astype(np.float64)
+            m1, m2 = 0.9 * m1 + 0.1 * g, 0.999 * m2 + 0.001 * g * g
+            a = a - 0.02 * (m1 / (1 - 0.9 ** it)) / (np.sqrt(m2 / (1 - 0.999 ** it)) + 1e-12)
+            T.etac_update_params(eng.ctx, alpha=a.astype(np.float32))
+    finally:
+        eng.close()
+    print(f"[calibration] alpha {a} vs {a_star}; loss {losses[0]:.4g} -> {losses[-1]:.4g}")
+    assert np.abs(a - a_star).max() < 0.02 and losses[-1] < 1e-3 * losses[0]
+
+
 def test_step_is_capturable_in_a_cuda_graph():
     """etac_step only enqueues (no sync, no allocation, no host copy): it can be captured in a
     CUDA graph and replayed; the replays give the eager result bit for bit."""
