@@ -234,10 +234,32 @@ def run_ours(a):
     h2d = pin[0][0].numel() + (pin[0][1].numel() * 4 if posed else 0)
     d2h = h_out.numel() * 4
 
-    t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device="cuda")
+    # the same loop with the result packed as bf16 by the kernel (etac_step_args.out_dtype): the PCIe
+    # copy of the result dominates the end-to-end number, this halves it.  Extra information only:
+    # "e2e" above is the fp32 result.
+    d_out16 = torch.empty((a.envs, eng.N, 3), dtype=torch.bfloat16, device="cuda")
+    h_out16 = torch.empty((a.envs, eng.N, 3), dtype=torch.bfloat16).pin_memory()
+    e2e16_args = T.make_step_args(a.envs, d_out16, indenters=d_ind, patch_pose=d_pose, out_dtype=T.ETAC_OUT_BF16)
+
+    def e2e16_step(k):
+        d_ind.copy_(pin[k][0], non_blocking=True)
+        if posed:
+            d_pose.copy_(pin[k][1], non_blocking=True)
+        T.etac_step(eng.ctx, stream, e2e16_args)
+        h_out16.copy_(d_out16, non_blocking=True)
+
+    e2e16_step(0)
+    sync_all()
+    t0 = time.perf_counter()
+    for i in range(n_e2e):
+        e2e16_step(i % N_INPUT_SETS)
+    torch.cuda.synchronize()
+    e2e16_ms = 1e3 * (time.perf_counter() - t0)
+
+    t = torch.tensor([ms, e2e_ms, e2e16_ms], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(t[0]), float(t[1])
+    ms, e2e_ms, e2e16_ms = float(t[0]), float(t[1]), float(t[2])
     if rank != 0:
         eng.close()
         if dist is not None:
@@ -270,6 +292,8 @@ def run_ours(a):
         "e2e": {"value": world * a.envs * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": n_e2e,
                 "note": "pinned host indenters+patch poses -> device, etac_step, full [E,N,3] fp32 result -> pinned host"},
+        "e2e_bf16_output": {"value": world * a.envs * n_e2e / (e2e16_ms * 1e-3), "unit": UNIT, "d2h_bytes_per_step": d2h // 2,
+                            "note": "same loop, result written as bf16 by the kernel (out_dtype); not the headline"},
         "gpu_launches": launches,
         "kernels_ms": {"s1_sdf_kernel_incl_memsets": ms_s1, "dense_bf16_kernel": ms_fused},
         "roofline": {"bound": "tensor", "kernel": "dense_bf16_kernel", "achieved": achieved, "peak": peak,
