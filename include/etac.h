@@ -197,8 +197,8 @@ etac_status etac_patches_from_adjacency(int32_t n_nodes, const int32_t* adj_rowp
  * obtained by minimising || U_p - U_p* ||_2 by gradient descent"; Table I lists differentiability).
  * Given the upstream gradient G = dL/dU of one step (same inputs as etac_step), returns dL/dalpha and
  * dL/d(weights of the per-node residual MLP).  Rows that Eq. (2) overwrites with u^ (the active nodes,
- * ETAC_ACTIVE_PASSTHROUGH) and rows of contact-free (env, patch) pairs carry no gradient.  Gradients
- * with respect to the poses / penetrations are not computed.  Arithmetic: fp32 on the fp32 copies of
+ * ETAC_ACTIVE_PASSTHROUGH) and rows of contact-free (env, patch) pairs carry no gradient to them.  Optionally
+ * also dL/d(penetration); gradients with respect to poses are not computed.  Arithmetic: fp32 on the fp32 copies of
  * K and the weights, whatever the context's precision; sums over environments use fp32 atomics, so
  * repeated calls agree to rounding, not bit for bit.  Contexts with ETAC_RESID_POINTNET and ablation
  * modes other than FULL: ETAC_ERR_UNSUPPORTED.  Enqueues on cuda_stream, no host synchronisation. */
@@ -214,6 +214,9 @@ typedef struct {
                                          context was created with n_alpha = P) */
   float* d_grad_weights;              /* device [4995] fp32, overwritten, or NULL: dL/d W1[64x9] b1[64] W2[64x64]
                                          b2[64] W3[3x64] b3[3], in this order; must be NULL for ETAC_RESID_NONE */
+  float* d_grad_penetration;          /* device [E x N] fp32, overwritten, or NULL: dL/ddelta for the nodes in contact
+                                         (u^ = -delta n, L77; the contact set is held fixed, 0 for the other nodes).
+                                         The caller chains it to object / link poses through its SDF gradients */
 } etac_backward_args;
 #define ETAC_GRAD_WEIGHTS_LEN 4995
 etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* args);

@@ -12,11 +12,13 @@ with the CUDA path).  It differentiates exactly what ``etac_oracle.step`` comput
       dL/dalpha = sum_i (G_i + J^T G_i) . sum_j dK_ij/dalpha u^_j ,   J = dPhi/du at row i
       dL/dW     = the chain rule through the per-node MLP 9 -> 64 -> 64 -> 3 (SiLU), written out
   Rows overwritten with u^ = -delta n (active rows, "passthrough") and rows of contact-free pairs do not
-  depend on alpha or Phi.  The contact set is held fixed (it does not depend on alpha or Phi).
+  depend on alpha or Phi.  dL/ddelta_j of the nodes in contact follows from u^_j = -delta_j n_j (PAPER.md:L77 +
+  DESIGN.md R5): dL/ddelta_j = -n_j . (sum_i K_ij dL/du_i + G_j if row j is u^_j itself); 0 for the other nodes.
+  The contact set is held fixed (it does not depend on alpha or Phi).
 
 float64 numpy, one (env, patch) at a time, no fusion.  Pins (tests/test_oracle_pins.py): central
-finite differences of ``etac_oracle.step`` (itself pinned) with respect to alpha and to sampled
-weights of every layer, and torch float64 autograd of the same MLP.
+finite differences of ``etac_oracle.step`` (itself pinned) with respect to alpha, to sampled weights
+of every layer and (penetration input mode) to the penetration of sampled contact nodes.
 """
 from __future__ import annotations
 
@@ -32,12 +34,14 @@ def silu_prime(z):
 
 def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetration=None, envs=None):
     """G: dL/dU [E', N, 3] for the listed envs (default all).  Returns float64 gradients
-    {"alpha": [n_alpha], "W1": [64, 9], "b1", "W2", "b2", "W3", "b3"} (weights only for the per-node form)."""
+    {"alpha": [n_alpha], "delta": [E', N], "W1": [64, 9], "b1", "W2", "b2", "W3", "b3"} (weights only for the
+    per-node form)."""
     if model.resid_arch not in ("none", "pernode") or model.ablation != "full":
         raise ValueError("backward oracle: per-node / no residual, full pipeline only")
+    G = np.asarray(G, dtype=np.float64)
     fwd = O.step(model, indenters=indenters, patch_pose=patch_pose, penetration=penetration, envs=envs)
     alpha = np.atleast_1d(np.asarray(model.alpha, dtype=np.float64))
-    grads = {"alpha": np.zeros(alpha.shape[0])}
+    grads = {"alpha": np.zeros(alpha.shape[0]), "delta": np.zeros((G.shape[0], model.n_nodes))}
     mlp = model.resid_arch == "pernode"
     if mlp:
         w = {k: np.asarray(v, dtype=np.float64) for k, v in model.weights.items()}
@@ -45,7 +49,6 @@ def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetrati
             grads[k] = np.zeros_like(w[k])
     pos = model.pos.astype(np.float64)
     nrm = model.normal.astype(np.float64)
-    G = np.asarray(G, dtype=np.float64)
     for oi in range(G.shape[0]):
         delta, active = fwd["delta"][oi], fwd["mask"][oi]
         uhat = -delta[:, None] * nrm
@@ -80,4 +83,9 @@ def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetrati
                 grads["b1"] += gz1.sum(0)
                 glin += (gz1 @ w["W1"])[:, 0:3]
             grads["alpha"][p if alpha.shape[0] > 1 else 0] += float((glin * v).sum())
+            # u^_j = -delta_j n_j: dL/ddelta_j = -n_j . (sum_i K_ij dL/du_i + G_j if row j is u^_j itself)
+            back = K[:, act].T @ glin
+            if model.active_mode == "passthrough":
+                back = back + G[oi, lo:hi][act]
+            grads["delta"][oi, lo:hi][act] = -(nrm[lo:hi][act] * back).sum(1)
     return grads

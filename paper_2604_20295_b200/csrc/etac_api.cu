@@ -661,11 +661,13 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
   cudaError_t e;
   if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess ||
       (e = cudaMemsetAsync(a->d_grad_alpha, 0, sizeof(float) * ctx->n_alpha, s)) != cudaSuccess ||
-      (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * ETAC_GRAD_WEIGHTS_LEN, s)) != cudaSuccess))
+      (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * ETAC_GRAD_WEIGHTS_LEN, s)) != cudaSuccess) ||
+      (a->d_grad_penetration &&
+       (e = cudaMemsetAsync(a->d_grad_penetration, 0, sizeof(float) * (size_t)a->n_envs * ctx->m.n_nodes, s)) != cudaSuccess))
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset", e));
   if ((e = launch_sdf(ctx->m, io, 0, s)) != cudaSuccess)  // S1: delta and the pair flags only
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
-  if ((e = launch_backward(ctx->m, io, a->d_grad_out, a->d_grad_alpha, ctx->n_alpha, a->d_grad_weights, ctx->n_sm, s)) != cudaSuccess)
+  if ((e = launch_backward(ctx->m, io, a->d_grad_out, a->d_grad_alpha, ctx->n_alpha, a->d_grad_weights, a->d_grad_penetration, ctx->n_sm, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("backward_kernel", e));
   ctx->last_launches = 2;
   return ETAC_OK;

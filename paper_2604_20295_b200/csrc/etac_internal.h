@@ -162,7 +162,7 @@ cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t backward_configure();
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,
-                            float* grad_w, int n_sm, cudaStream_t s);
+                            float* grad_w, float* grad_delta, int n_sm, cudaStream_t s);
 cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
                               int n_sm, bool gather, int* launches, cudaStream_t s);
 cudaError_t dense_bf16_configure();

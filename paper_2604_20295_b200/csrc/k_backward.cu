@@ -10,6 +10,8 @@
 //   dL/dalpha   += (G_i + J_Phi,u^T G_i) . sum_j dK_ij/dalpha u^_j
 //   dL/dW       += the usual MLP backward of G_i
 // Active rows of Eq. (2) are u^ itself and carry no gradient to alpha or Phi.
+// Optionally also dL/ddelta (the penetrations of the nodes in contact; the contact set is held fixed),
+// from which a caller chains to object / link poses through its SDF gradients.
 //
 // The grid is persistent (one CTA per SM, 512 threads: four threads per node, each owning 16 of the
 // 64 hidden units, so that 16 warps hide each other's FMA and shared-memory latencies; the
@@ -54,7 +56,8 @@ __device__ __forceinline__ void silu_and_grad(float z, float& y, float& dy) {
 
 __global__ void __launch_bounds__(kThreads, 1) backward_kernel(DevModel m, StepIO io, const float* __restrict__ grad_out,
                                                                float* __restrict__ grad_alpha, int n_alpha,
-                                                               float* __restrict__ grad_w) {
+                                                               float* __restrict__ grad_w,
+                                                               float* __restrict__ grad_delta) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
   BwdSmem& S = *reinterpret_cast<BwdSmem*>(smem_raw);
   const int t = threadIdx.x, lane = t & 31;
@@ -218,6 +221,47 @@ __global__ void __launch_bounds__(kThreads, 1) backward_kernel(DevModel m, StepI
 #pragma unroll
       for (int s = 0; s < kParts; ++s) l0 += S.L[s][0][i], l1 += S.L[s][1][i], l2 += S.L[s][2][i];
     }
+    // ---- dL/ddelta_j of the patch's active nodes j (optional): u^_j = -delta_j n_j, so
+    //   dL/ddelta_j = -n_j . ( sum_{i carrying a gradient} K_ij dL/du_i  +  G_j if row j is u^_j itself )
+    // The active nodes are compacted again (their normals this time); part s takes every fourth of them,
+    // reduces K_ij (dL/du_i . n_j) over its copy of the item's nodes and adds it with one atomic per warp.
+    if (grad_delta) {
+      float* gd = grad_delta + (int64_t)e * m.n_nodes + pi.off;
+      if (part == 0 && valid && !carries) {  // active row of Eq. (2): U_j = u^_j
+        const float* go = grad_out + ((int64_t)e * m.n_nodes + g) * 3;
+        const float4 nn = m.nrm4[g];
+        atomicAdd(&gd[li], -(nn.x * go[0] + nn.y * go[1] + nn.z * go[2]));
+      }
+      for (int base = 0; base < pi.n; base += kT) {
+        const int j = base + i;
+        const bool act = part == 0 && j < pi.n && delta[j] > 0.0f;
+        const unsigned bal = __ballot_sync(0xffffffffu, act);
+        if (part == 0 && lane == 0) S.wcnt[warp_i] = __popc(bal);
+        __syncthreads();
+        int pre = 0, total = 0;
+#pragma unroll
+        for (int w = 0; w < kT / 32; ++w) {
+          const int c = S.wcnt[w];
+          pre += w < warp_i ? c : 0;
+          total += c;
+        }
+        if (act) {
+          const int slot = pre + __popc(bal & ((1u << lane) - 1u));
+          const float4 n = m.nrm4[pi.off + j];
+          S.j[slot] = j;
+          S.u[slot][0] = n.x, S.u[slot][1] = n.y, S.u[slot][2] = n.z;
+        }
+        __syncthreads();
+        for (int a = part; a < total; a += kParts) {
+          float c = 0.0f;
+          if (carries) c = K[(int64_t)S.j[a] * pi.n + li] * (l0 * S.u[a][0] + l1 * S.u[a][1] + l2 * S.u[a][2]);
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+          if (lane == 0 && c != 0.0f) atomicAdd(&gd[S.j[a]], -c);
+        }
+        __syncthreads();
+      }
+    }
     // ---- dL/dalpha of this item: sum_i dL/du_i . v_i / alpha (part 0's warps, one atomic each)
     if (part == 0) {
       float ga = carries ? (l0 * vx + l1 * vy + l2 * vz) / pi.alpha : 0.0f;
@@ -298,8 +342,8 @@ cudaError_t backward_configure() {
 }
 
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,
-                            float* grad_w, int n_sm, cudaStream_t s) {
-  backward_kernel<<<n_sm, kThreads, sizeof(BwdSmem), s>>>(m, io, grad_out, grad_alpha, n_alpha, grad_w);
+                            float* grad_w, float* grad_delta, int n_sm, cudaStream_t s) {
+  backward_kernel<<<n_sm, kThreads, sizeof(BwdSmem), s>>>(m, io, grad_out, grad_alpha, n_alpha, grad_w, grad_delta);
   return cudaGetLastError();
 }
 

@@ -375,6 +375,23 @@ def test_backward_oracle_matches_finite_differences(per_patch, active_mode, resi
         fd = (loss(dataclasses.replace(wl, alpha=ap))[0] - loss(dataclasses.replace(wl, alpha=am))[0]) / (2 * eps)
         assert abs(fd - g["alpha"][k]) <= 1e-6 * max(1.0, abs(fd)), (k, fd, g["alpha"][k])
     assert np.abs(g["alpha"]).min() > 1e-3                        # the case exercises every alpha
+    # dL/ddelta in penetration input mode (the contact set stays fixed under a small change of a positive delta)
+    pen = O.step(m, indenters=wl.indenters)["delta"].astype(np.float32).astype(np.float64)   # the input is fp32
+    eps_p = 2.0 ** -12                                            # d +- eps_p is exact in fp32
+
+    def loss_pen(d):
+        U_ = O.step(m, penetration=d)["U"]
+        return 0.5 * float(((U_ - target) ** 2).sum()), U_
+    _, U_pen = loss_pen(pen)
+    gp = OG.backward(m, U_pen - target, penetration=pen)["delta"]
+    act = np.argwhere(pen > 0.05)
+    assert np.all(gp[pen == 0] == 0) and len(act) > 10
+    for e_, j_ in act[:: max(1, len(act) // 6)]:
+        dp, dm = pen.copy(), pen.copy()
+        dp[e_, j_] += eps_p
+        dm[e_, j_] -= eps_p
+        fd = (loss_pen(dp)[0] - loss_pen(dm)[0]) / (2 * eps_p)
+        assert abs(fd - gp[e_, j_]) <= 1e-5 * max(1.0, abs(fd)), (e_, j_, fd, gp[e_, j_])
     if resid_arch == "none":
         return
     rng = np.random.default_rng(5)

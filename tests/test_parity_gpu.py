@@ -514,11 +514,12 @@ def test_backward_against_the_gradient_oracle(kind):
         d_G = torch.from_numpy(G.astype(np.float32)).to(eng.device)
         g_alpha = torch.full((len(wl.alpha),), 7.0, device=eng.device)
         g_w = torch.full((T.ETAC_GRAD_WEIGHTS_LEN,), 7.0, device=eng.device) if resid else None
+        g_pen = torch.full((wl.n_envs, eng.N), 7.0, device=eng.device)
         stream = torch.cuda.current_stream().cuda_stream
         for _ in range(2):                                                # the outputs are overwritten, not accumulated
-            T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, g_w, **dev)
+            T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, g_w, grad_penetration=g_pen, **dev)
         torch.cuda.synchronize()
-        got = {"alpha": g_alpha.cpu().numpy().astype(np.float64)}
+        got = {"alpha": g_alpha.cpu().numpy().astype(np.float64), "delta": g_pen.cpu().numpy().astype(np.float64)}
         if resid:
             got.update({k: v.astype(np.float64) for k, v in T.split_grad_weights(g_w.cpu().numpy()).items()})
         U_fwd = eng.step(wl.n_envs, dev).cpu().numpy()                    # the forward still works afterwards
