@@ -1,5 +1,5 @@
 """Times one ETAC_RESID_POINTNET step on the cfg-3 hand workload (4096 envs): the command behind
-profiles/r01b_pointnet_launch_list.md.
+profiles/r01c_pointnet_backward_launch_list.md.
 
     python -m paper_2604_20295_b200.examples.pointnet_step
 """
