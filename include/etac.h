@@ -245,6 +245,15 @@ int32_t etac_abi_version(void);
 etac_status etac_time_steps(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args, int32_t iters,
                             float* ms_per_step, float* ms_kernels);
 
+/* Measurement helper for bench.py's roofline (not on the hot path): runs a microbenchmark of independent
+ * tanh.approx.f32 chains on every SM of the current device, on cuda_stream, and returns the measured rate of
+ * the special-function pipe in results per second (*ops_per_s, host pointer) and, if not NULL, per clock and
+ * SM at the device's nominal maximum clock (*ops_per_clk_per_sm).  The fused kernel evaluates 128 SiLUs
+ * (one MUFU.TANH each) per node-environment of a contacting pair, BASELINE.json configs[0] "2x64 SiLU"; this
+ * rate is the denominator of its "alu" roofline.  Synchronises the stream.
+ * Errors: ETAC_ERR_INVALID_ARG (NULL ops_per_s), ETAC_ERR_CUDA. */
+etac_status etac_measure_sfu_rate(void* cuda_stream, double* ops_per_s, double* ops_per_clk_per_sm);
+
 #ifdef __cplusplus
 }
 #endif

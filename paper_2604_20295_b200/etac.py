@@ -30,7 +30,8 @@ ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
  ETAC_INFO_LAST_LAUNCHES, ETAC_INFO_LAST_CONTACT_PAIRS, ETAC_INFO_SM_COUNT) = range(1, 9)
 
 EXPORTS = ["etac_create", "etac_destroy", "etac_step", "etac_set_option", "etac_get_info", "etac_last_error",
-           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward", "etac_update_params"]
+           "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward", "etac_update_params",
+           "etac_measure_sfu_rate"]
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -98,6 +99,7 @@ def load() -> C.CDLL:
         lib.etac_time_steps.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_step_args), C.c_int32, _fp, _fp]
         lib.etac_update_params.argtypes = [C.c_void_p, C.POINTER(etac_params)]
         lib.etac_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_backward_args)]
+        lib.etac_measure_sfu_rate.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         lib.etac_set_sdf_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
         for name in EXPORTS:
             getattr(lib, name)
@@ -273,6 +275,15 @@ def etac_time_steps(ctx, stream, args: etac_step_args, iters: int, per_kernel: b
     mk = (C.c_float * 2)()
     _check(ctx, load().etac_time_steps(ctx, stream, C.byref(args), iters, C.byref(ms), mk if per_kernel else None))
     return (ms.value, [mk[0], mk[1]]) if per_kernel else ms.value
+
+
+def etac_measure_sfu_rate(stream):
+    """(results/s, results per clock and SM at the nominal maximum clock) of the special-function pipe."""
+    a, b = C.c_double(), C.c_double()
+    st = load().etac_measure_sfu_rate(stream, C.byref(a), C.byref(b))
+    if st != 0:
+        raise EtacError(st, "etac_measure_sfu_rate")
+    return a.value, b.value
 
 
 # ------------------------------------------------------------------ convenience wrapper (marshalling only)

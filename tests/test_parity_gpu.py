@@ -622,3 +622,13 @@ def test_step_is_capturable_in_a_cuda_graph():
             assert torch.equal(eng.out[: wl.n_envs], eager)
         finally:
             eng.close()
+
+
+def test_sfu_rate_microbenchmark_is_plausible():
+    """bench.py's "alu" roofline divides by this live measurement: it must be a whole-device rate of the order
+    of 16 results per clock and SM (four sub-partitions x four lanes), not a launch-bound or optimised-away one."""
+    import torch
+    ops_s, per_clk_sm = T.etac_measure_sfu_rate(torch.cuda.current_stream().cuda_stream)
+    n_sm = torch.cuda.get_device_properties(0).multi_processor_count
+    assert 8.0 <= per_clk_sm <= 17.0, per_clk_sm
+    assert ops_s > 1e9 * n_sm
