@@ -278,8 +278,9 @@ def run_ours(a):
     t_hbm = wm["b_hbm_min"] / (peaks["hbm_gbs"] * 1e9)
     t_roof = max(t_tensor, t_hbm)
     # Floors of the fused kernel on the three units it loads: tensor pipe, HBM, and the special-function pipe
-    # (128 SiLUs = 128 MUFU.TANH per node-environment of a contacting pair).  The roofline is the slowest of
-    # them; "roofline" reports that one and "roofline_tensor" keeps the contract's tensor figure beside it.
+    # (128 SiLUs = 128 MUFU.TANH per node-environment of a contacting pair).  "roofline" is the contract's
+    # (tensor peak / HBM); the activation-pipe bound is reported beside it as "roofline_sfu"
+    # against a rate measured live, and does not replace the contract fraction.
     acts = 128.0 * wm["w_nodeenv"]
     t_sfu = acts / sfu_ops_s
     t_hbm_fused = (wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"]) / (peaks["hbm_gbs"] * 1e9)
@@ -291,7 +292,6 @@ def run_ours(a):
                 "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else None,
                 "peak_src": f"etac_measure_sfu_rate, live on this device: {sfu_per_clk_sm:.2f} MUFU results per clock and SM",
                 "activations_per_launch": acts, "pipe": "MUFU (special-function unit)"}
-    binding = roof_sfu if t_sfu >= max(t_tensor, t_hbm_fused) else roof_tensor
     cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, a.envs if a.workload == "cfg3" else 48)   # ~10 s of CPU work
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
@@ -313,7 +313,7 @@ def run_ours(a):
                             "note": "same loop, result written as bf16 by the kernel (out_dtype); not the headline"},
         "gpu_launches": launches,
         "kernels_ms": {"s1_sdf_kernel_incl_memsets": ms_s1, "dense_bf16_kernel": ms_fused},
-        "roofline": binding, "roofline_tensor": roof_tensor,
+        "roofline": roof_tensor, "roofline_sfu": roof_sfu,
         "roofline_floors_us": {"tensor": t_tensor * 1e6, "hbm": t_hbm_fused * 1e6, "sfu": t_sfu * 1e6},
         "roofline_step": {"t_roof_us": t_roof * 1e6, "t_tensor_us": t_tensor * 1e6, "t_hbm_us": t_hbm * 1e6,
                           "roof_dense_frac": t_roof / (ms_step * 1e-3),
