@@ -632,3 +632,26 @@ def test_sfu_rate_microbenchmark_is_plausible():
     n_sm = torch.cuda.get_device_properties(0).multi_processor_count
     assert 8.0 <= per_clk_sm <= 17.0, per_clk_sm
     assert ops_s > 1e9 * n_sm
+
+
+@pytest.mark.parametrize("n_nodes,curved,frac,path", [(1024, False, 0.05, T.ETAC_PATH_DENSE),
+                                                     (1024, False, 0.05, T.ETAC_PATH_SPARSE),
+                                                     (8192, True, 0.01, T.ETAC_PATH_DENSE)])
+def test_config5_largest_batch_sampled(n_nodes, curved, frac, path):
+    """BASELINE.json configs[4] at its largest batch (16,384 envs; N = 8192 is its largest mesh too): every
+    output of the step comes back, the oracle checks a sample of environments one by one,
+    and the properties that hold at any size are checked on all of them."""
+    E = 16384
+    wl = W.config5(E, n_nodes, curved, frac, "bf16")
+    gpu = run_gpu(wl, path=path)
+    assert gpu["path"] == path
+    envs = [0, 5461, 10923, E - 1] if n_nodes > 4096 else list(range(0, E, 683)) + [E - 1]
+    ref = run_oracle(wl, envs=envs)
+    _report(f"cfg5 E={E} N={n_nodes} path={path}",
+            compare(gpu, ref, TOL["bf16"], envs=envs, resid_tol=5e-2, label="cfg5-max", delta_tol=1e-4))
+    # every env: active rows keep u^ = -delta n exactly (P7), mask <=> delta > 0, active-node counts, pairs
+    act = gpu["mask"]
+    assert np.array_equal(act, gpu["delta"] > 0.0)
+    np.testing.assert_array_equal(gpu["U"][act], (-gpu["delta"][..., None] * wl.mesh.normal[None])[act])
+    assert np.array_equal(gpu["active_count"], act.sum(1))
+    assert gpu["pairs"] == int(act.any(1).sum())
