@@ -79,6 +79,10 @@ __host__ __device__ constexpr size_t dense_smem_bytes(int n_patches, int mode) {
 struct Item {
   int p, mb, tile, cnt;
 };
+#ifndef ETAC_GROUP_MB
+#define ETAC_GROUP_MB 40
+#endif
+constexpr int kGroupBytes = ETAC_GROUP_MB << 20;  // U^ operand bytes of one group of env tiles (L2-resident share)
 
 #ifndef ETAC_GATHER_DEPTH
 #define ETAC_GATHER_DEPTH 16
@@ -136,9 +140,20 @@ __device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, co
   const int cnt = m.count[pcur];
   const int tiles = (cnt + TE - 1) / TE;
   const int r = w - prefix[pcur];
+  // Item order inside a patch: env tiles in groups of G whose U^ operand tiles (BN x n bf16 each) stay
+  // resident in L2 together; a group sweeps all node blocks before the next group starts, the tile is the
+  // fast index.  One group (G >= tiles, every small patch) is the plain order mb = r / tiles.  Without the
+  // groups a large single patch (cfg 4: 256 tiles x 786 KB = 201 MB > L2) re-reads every U^ tile from HBM
+  // once per node block.
+  const int n = m.patch[pcur].n;
+  const int nmb = (n + BM - 1) / BM;
+  const int G = max(1, min(tiles, kGroupBytes / (BN * 2 * max(n, 1))));
+  const int g = r / (G * nmb);
+  const int rem = r - g * G * nmb;
+  const int gsz = min(G, tiles - g * G);
   it.p = pcur;
-  it.mb = r / tiles;
-  it.tile = r - it.mb * tiles;
+  it.mb = rem / gsz;
+  it.tile = g * G + (rem - it.mb * gsz);
   it.cnt = min(TE, cnt - it.tile * TE);
   return true;
 }
