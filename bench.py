@@ -32,9 +32,11 @@ UNIT = "env-steps/s"
 N_INPUT_SETS = 4
 MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728
 # dram__bytes_read.sum + dram__bytes_write.sum of one dense_bf16_kernel launch, from the
-# `ncu --set full` capture summarised in profiles/r01c_dense_ncu_full.md (79.2 MB read + 232.2 MB
-# write; the kernel also zero-fills the rows of contact-free (env, patch) pairs).
-NCU_TRAFFIC_BYTES = 311.37e6
+# `ncu --set full` capture summarised in profiles/r01d_dense_ncu_full.md (79.2 MB read + 232.4 MB
+# write; the kernel also zero-fills the rows of contact-free (env, patch) pairs); cfg 4: the counters
+# in profiles/r01d_cfg4_item_order.md (1.26 GB read + 0.395 GB write).
+NCU_TRAFFIC_BYTES = 311.54e6
+NCU_TRAFFIC_BYTES_CFG4 = 1655.0e6
 
 
 WORKLOADS = {
@@ -300,11 +302,11 @@ def run_ours(a):
     t_sfu = acts / sfu_ops_s
     t_hbm_fused = (wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"]) / (peaks["hbm_gbs"] * 1e9)
     roof_tensor = {"bound": "tensor", "kernel": "dense_bf16_kernel", "achieved": achieved, "peak": peak,
-                   "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else None,
+                   "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else NCU_TRAFFIC_BYTES_CFG4,
                    "peak_src": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['src']})", "flops_per_launch": flops}
     roof_sfu = {"bound": "alu", "kernel": "dense_bf16_kernel", "achieved": acts / (ms_fused * 1e-3) / 1e12,
                 "peak": sfu_ops_s / 1e12, "unit": "Tactivation/s", "frac": t_sfu / (ms_fused * 1e-3),
-                "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else None,
+                "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else NCU_TRAFFIC_BYTES_CFG4,
                 "peak_src": f"etac_measure_sfu_rate, live on this device: {sfu_per_clk_sm:.2f} MUFU results per clock and SM",
                 "activations_per_launch": acts, "pipe": "MUFU (special-function unit)"}
     cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, a.envs if a.workload == "cfg3" else 48)   # ~10 s of CPU work
