@@ -365,6 +365,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   DevModel& m = c->m;
   m.n_nodes = N, m.n_patches = P, m.max_envs = d->max_envs, m.max_ind = d->max_indenters;
   m.resid = d->resid_arch, m.active_mode = d->active_mode;
+  m.group_bytes = 40 << 20;
 
   auto bail = [&](etac_status st, const std::string& msg) {
     g_create_err = msg;
@@ -522,6 +523,11 @@ etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
     if (value < ETAC_ABLATE_FULL || value > ETAC_ABLATE_NO_PROPAGATION) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_ABLATION value");
     ctx->m.residual_only = value == ETAC_ABLATE_RESIDUAL_ONLY;
     ctx->m.ablation = (int32_t)value;
+    return ETAC_OK;
+  }
+  if (key == ETAC_OPT_L2_GROUP_BYTES) {
+    if (value < 1 || value > (int64_t)1 << 30) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad ETAC_OPT_L2_GROUP_BYTES value");
+    ctx->m.group_bytes = (int32_t)value;
     return ETAC_OK;
   }
   if (key != ETAC_OPT_PATH) return fail(ctx, ETAC_ERR_INVALID_ARG, "unknown option");

@@ -74,6 +74,7 @@ struct DevModel {
   int32_t max_envs, max_ind;
   int32_t resid, active_mode;
   int32_t residual_only;      // ETAC_OPT_ABLATION: passive rows get Phi_p without the linear term
+  int32_t group_bytes;        // ETAC_OPT_L2_GROUP_BYTES: U^ operand bytes of one group of env tiles (fused kernel)
   int32_t ablation;           // ETAC_ABLATE_* (LINEAR_ONLY / NO_PROPAGATION select other kernels on the host)
   const float4* pos4;         // [N] (x,y,z,0)
   const float4* nrm4;         // [N]

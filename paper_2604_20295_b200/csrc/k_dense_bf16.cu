@@ -72,17 +72,13 @@ __host__ __device__ constexpr int mode_img_bytes(int mode) {
 
 __host__ __device__ constexpr size_t dense_smem_bytes(int n_patches, int mode) {
   return 1024 /*align slack*/ + (size_t)mode_stages(mode) * (A_STAGE + B_STAGE) + mode_img_bytes(mode) + sizeof(DenseBars) +
-         (size_t)(n_patches + 1) * 4 + 16 + 16 + 8 * 32 * 16;
+         (size_t)(5 * n_patches + 4) * 4 + 16 + 16 + 8 * 32 * 16;
 }
 
 
 struct Item {
   int p, mb, tile, cnt;
 };
-#ifndef ETAC_GROUP_MB
-#define ETAC_GROUP_MB 40
-#endif
-constexpr int kGroupBytes = ETAC_GROUP_MB << 20;  // U^ operand bytes of one group of env tiles (L2-resident share)
 
 #ifndef ETAC_GATHER_DEPTH
 #define ETAC_GATHER_DEPTH 16
@@ -133,28 +129,39 @@ struct ZeroFill {
   }
 };
 
+// prefix[0..P]: first work index of every patch.  kGrouped: four more ints per patch behind it (contacting
+// envs, env tiles, env tiles per group G, G x node blocks), written once by the prologue.
+// Item order inside a patch.  Plain (kGrouped = false): node block mb = r / tiles, the env tile is the fast
+// index.  Grouped: env tiles in groups of G whose U^ operand tiles (BN x n bf16 each) stay resident in L2
+// together; a group sweeps all node blocks before the next group starts.  Without the groups a large single
+// patch (cfg 4: 256 tiles x 786 KB = 201 MB > L2) re-reads every U^ tile from HBM once per node block.  The
+// grouped decode is its own instantiation, launched only when a patch's operand can exceed ETAC_OPT_L2_GROUP_BYTES: the
+// epilogue's schedule is sensitive to every instruction of the item set-up (cfg 3: 334 us plain, 336-345 us
+// with the grouped decode in its three variants).
+__host__ __device__ constexpr int kPrefixInts(int n_patches) { return n_patches + 1; }
+template <bool kGrouped>
 __device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, const DevModel& m, int w, int& pcur,
                                             Item& it) {
   if (w >= prefix[n_patches]) return false;
   while (prefix[pcur + 1] <= w) ++pcur;
-  const int cnt = m.count[pcur];
-  const int tiles = (cnt + TE - 1) / TE;
   const int r = w - prefix[pcur];
-  // Item order inside a patch: env tiles in groups of G whose U^ operand tiles (BN x n bf16 each) stay
-  // resident in L2 together; a group sweeps all node blocks before the next group starts, the tile is the
-  // fast index.  One group (G >= tiles, every small patch) is the plain order mb = r / tiles.  Without the
-  // groups a large single patch (cfg 4: 256 tiles x 786 KB = 201 MB > L2) re-reads every U^ tile from HBM
-  // once per node block.
-  const int n = m.patch[pcur].n;
-  const int nmb = (n + BM - 1) / BM;
-  const int G = max(1, min(tiles, kGroupBytes / (BN * 2 * max(n, 1))));
-  const int g = r / (G * nmb);
-  const int rem = r - g * G * nmb;
-  const int gsz = min(G, tiles - g * G);
   it.p = pcur;
-  it.mb = rem / gsz;
-  it.tile = g * G + (rem - it.mb * gsz);
-  it.cnt = min(TE, cnt - it.tile * TE);
+  if constexpr (!kGrouped) {
+    const int cnt = m.count[pcur];
+    const int tiles = (cnt + TE - 1) / TE;
+    it.mb = r / tiles;
+    it.tile = r - it.mb * tiles;
+    it.cnt = min(TE, cnt - it.tile * TE);
+  } else {
+    const int* pinfo = prefix + kPrefixInts(n_patches) + 4 * pcur;
+    const int cnt = pinfo[0], tiles = pinfo[1], G = pinfo[2], GN = pinfo[3];
+    const int g = r / GN;
+    const int rem = r - g * GN;
+    const int gsz = min(G, tiles - g * G);
+    it.mb = rem / gsz;
+    it.tile = g * G + (rem - it.mb * gsz);
+    it.cnt = min(TE, cnt - it.tile * TE);
+  }
   return true;
 }
 
@@ -175,7 +182,7 @@ __device__ long long g_prof[320 * 8 * 12];
 // read from the compact lists S1 wrote (bf16 K row j, coalesced over i because K is symmetric;
 // fp32 u^ and accumulation).  No TMA, no propagation MMA; the MLP part is unchanged.  It wins
 // when few nodes are in contact (ETAC_PATH_SPARSE on a bf16 context).
-template <int kMode, bool kGather, bool kOutBf16>
+template <int kMode, bool kGather, bool kOutBf16, bool kGrouped>
 __global__ void __launch_bounds__(kDenseThreads, 2)
     dense_bf16_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
                       const __grid_constant__ CUtensorMap tmB) {
@@ -191,7 +198,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   uint8_t* sW = sB + kStages * B_STAGE;
   DenseBars* bars = reinterpret_cast<DenseBars*>(sW + kImgBytes);
   int* prefix = reinterpret_cast<int*>(bars + 1);
-  uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + (m.n_patches + 1)) + 15) & ~uintptr_t(15));  // 8 warps x 32 entries
+  uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + kPrefixInts(m.n_patches) + 4 * m.n_patches) + 15) & ~uintptr_t(15));  // 8 warps x 32 entries
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -211,7 +218,16 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     for (int p0 = 0; p0 < m.n_patches; p0 += 32) {
       const int p = p0 + lane;
       int v = 0;
-      if (p < m.n_patches) v = ((m.count[p] + TE - 1) / TE) * ((m.patch[p].n + BM - 1) / BM);
+      if (p < m.n_patches) {
+        const int cnt = m.count[p], n = m.patch[p].n;
+        const int tiles = (cnt + TE - 1) / TE, nmb = (n + BM - 1) / BM;
+        if constexpr (kGrouped) {
+          const int G = max(1, min(tiles, m.group_bytes / (BN * 2 * max(n, 1))));
+          int* pinfo = prefix + kPrefixInts(m.n_patches) + 4 * p;
+          pinfo[0] = cnt, pinfo[1] = tiles, pinfo[2] = G, pinfo[3] = max(G * nmb, 1);
+        }
+        v = tiles * nmb;
+      }
 #pragma unroll
       for (int d = 1; d < 32; d <<= 1) {
         const int o = __shfl_up_sync(0xffffffffu, v, d);
@@ -243,7 +259,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       int pcur = 0, stage = 0;
       uint32_t ph = 0;
       Item it;
-      for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+      for (int w = blockIdx.x; decode_item<kGrouped>(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
         const PatchInfo pi = m.patch[it.p];
         const int nkb = (pi.n + BK - 1) / BK;
         for (int kb = 0; kb < nkb; ++kb) {
@@ -268,7 +284,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       int pcur = 0, stage = 0;
       uint32_t ph = 0, acc_ph = 0;
       Item it;
-      for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+      for (int w = blockIdx.x; decode_item<kGrouped>(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
         const int nkb = (m.patch[it.p].n + BK - 1) / BK;
         mbar_wait(&bars->acc_empty, acc_ph ^ 1);
         acc_ph ^= 1;
@@ -311,7 +327,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       int pcur = 0;
       uint32_t a_ph = 0;
       Item it;
-      for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+      for (int w = blockIdx.x; decode_item<kGrouped>(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
         for (int el = sl; el < it.cnt; el += 2) {
 #pragma unroll 1
           for (int layer = 0; layer < kLayers; ++layer) {
@@ -363,7 +379,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
     long long plast = clock64();
     const long long pstart = plast;
 #endif
-    for (int w = blockIdx.x; decode_item(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
+    for (int w = blockIdx.x; decode_item<kGrouped>(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
       const PatchInfo pi = m.patch[it.p];
       const int li = it.mb * BM + row;
       const bool valid = li < pi.n;
@@ -665,9 +681,13 @@ __global__ void __launch_bounds__(64) pn_global_kernel(DevModel m) {
 template <int kMode, bool kGather>
 static cudaError_t configure_one() {
   const int bytes = (int)dense_smem_bytes(kMaxPatches, kMode);
-  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
   if (e == cudaSuccess && kMode != kModePnEncode)  // the encoder pass writes no displacement
-    e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if constexpr (!kGather && kMode != kModePnEncode) {  // grouped item order: dense propagation only
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  }
   return e;
 }
 
@@ -686,14 +706,19 @@ template <int kMode>
 static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int grid,
                        bool gather, cudaStream_t s) {
   const size_t smem = dense_smem_bytes(m.n_patches, kMode);
+  // grouped item order only where a patch's U^ operand (3 bf16 rows of n nodes per env) can exceed the L2 share
+  const bool grouped = !gather && (size_t)io.n_envs * (size_t)m.max_patch_nodes * 6 > (size_t)m.group_bytes;
   if constexpr (kMode == kModePnEncode) {
-    dense_bf16_kernel<kMode, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    dense_bf16_kernel<kMode, false, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
   } else if (gather) {
-    if (io.out_bf16) dense_bf16_kernel<kMode, true, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-    else dense_bf16_kernel<kMode, true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    if (io.out_bf16) dense_bf16_kernel<kMode, true, true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    else dense_bf16_kernel<kMode, true, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+  } else if (grouped) {
+    if (io.out_bf16) dense_bf16_kernel<kMode, false, true, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    else dense_bf16_kernel<kMode, false, false, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
   } else {
-    if (io.out_bf16) dense_bf16_kernel<kMode, false, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-    else dense_bf16_kernel<kMode, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    if (io.out_bf16) dense_bf16_kernel<kMode, false, true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    else dense_bf16_kernel<kMode, false, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
   }
 }
 

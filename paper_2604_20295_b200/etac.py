@@ -22,7 +22,7 @@ ETAC_RESID_NONE, ETAC_RESID_PERNODE_MLP, ETAC_RESID_POINTNET = range(3)
 ETAC_PREC_FP32, ETAC_PREC_BF16 = 0, 1
 ETAC_ACTIVE_PASSTHROUGH, ETAC_ACTIVE_PROPAGATE = 0, 1
 ETAC_IN_INDENTERS, ETAC_IN_PENETRATION = 0, 1
-ETAC_OPT_PATH, ETAC_OPT_ABLATION = 1, 2
+ETAC_OPT_PATH, ETAC_OPT_ABLATION, ETAC_OPT_L2_GROUP_BYTES = 1, 2, 3
 ETAC_ABLATE_FULL, ETAC_ABLATE_RESIDUAL_ONLY, ETAC_ABLATE_LINEAR_ONLY, ETAC_ABLATE_NO_PROPAGATION = range(4)
 ETAC_OUT_F32, ETAC_OUT_BF16 = 0, 1
 ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2

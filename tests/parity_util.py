@@ -13,13 +13,15 @@ TOL = {"fp32": 1e-4, "bf16": 2e-2}
 
 
 def run_gpu(wl, *, precision=None, path=T.ETAC_PATH_AUTO, resid=True, active_mode=T.ETAC_ACTIVE_PASSTHROUGH,
-            penetration=None, max_envs=None, n_envs=None, steps=1):
+            penetration=None, max_envs=None, n_envs=None, steps=1, group_bytes=None):
     import torch
     n_envs = wl.n_envs if n_envs is None else n_envs
     eng = T.Etac(wl, precision=precision, resid=resid, active_mode=active_mode, debug_outputs=True,
                  max_envs=max_envs or max(n_envs, 1))
     try:
         T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+        if group_bytes is not None:
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_L2_GROUP_BYTES, group_bytes)
         if penetration is not None:
             dev = eng.upload(penetration=penetration)
         else:

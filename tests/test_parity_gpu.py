@@ -655,3 +655,22 @@ def test_config5_largest_batch_sampled(n_nodes, curved, frac, path):
     np.testing.assert_array_equal(gpu["U"][act], (-gpu["delta"][..., None] * wl.mesh.normal[None])[act])
     assert np.array_equal(gpu["active_count"], act.sum(1))
     assert gpu["pairs"] == int(act.any(1).sum())
+
+
+@pytest.mark.parametrize("cfg,n_envs,group_bytes", [("cfg4", 40, 1 << 10), ("cfg4", 40, 1700 << 10), ("cfg3", 200, 120 << 10)])
+def test_grouped_item_order_is_only_scheduling(cfg, n_envs, group_bytes):
+    """ETAC_OPT_L2_GROUP_BYTES forced small: the fused kernel's grouped item order (groups of 1 env tile; of 2 with
+    a ragged last group; several patches with different tile counts) against the oracle on every env, and bit for
+    bit against the plain order."""
+    wl = W.config4(3, n_envs) if cfg == "cfg4" else W.config3(3, n_envs)
+    ref = run_oracle(wl)
+    plain = run_gpu(wl)
+    grouped = run_gpu(wl, group_bytes=group_bytes)
+    _report(f"{cfg} grouped {group_bytes}", compare(grouped, ref, TOL["bf16"], resid_tol=5e-2, label="grouped", delta_tol=1e-4))
+    assert np.array_equal(grouped["U"], plain["U"]) and np.array_equal(grouped["analytic"], plain["analytic"])
+    with pytest.raises(T.EtacError):
+        eng = T.Etac(wl)
+        try:
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_L2_GROUP_BYTES, 0)
+        finally:
+            eng.close()
