@@ -179,6 +179,8 @@ def run_ours(a):
     wl = sets[0]
     eng = T.Etac(wl, device=local)
     stream = torch.cuda.current_stream().cuda_stream
+    if a.l2_group_mb:
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_L2_GROUP_BYTES, a.l2_group_mb << 20)
     devs = [eng.upload(indenters=s.indenters, patch_pose=s.patch_pose) for s in sets]
     argv = [eng.args(a.envs, d) for d in devs]
 
@@ -353,6 +355,8 @@ if __name__ == "__main__":
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--envs", type=int, default=4096)
     ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
+    ap.add_argument("--l2-group-mb", type=int, default=0,
+                    help="experiments: ETAC_OPT_L2_GROUP_BYTES in MiB (0 = library default, 1024 = one group)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     (run_reference if args.impl == "reference" else run_ours)(args)
