@@ -158,6 +158,7 @@ __device__ __forceinline__ void zero_fill(float* __restrict__ p, int count) {
 }
 
 constexpr int kPoseChunk = 32;
+constexpr int kNodeChunk = 4;  // nodes per thread evaluated against one indenter held in registers
 struct SPose {
   float R[9];
   float t[3];
@@ -237,19 +238,39 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       int nact = 0;
       if constexpr (kIndenters) {
         const SPose& sp = s_pose[q];
-        for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
-          const float4 pos = m.pos4[pi.off + i];
-          float X0 = pos.x, X1 = pos.y, X2 = pos.z;
-          if (posed) {
-            X0 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[0], pos.x), __fmul_rn(sp.R[1], pos.y)), __fmul_rn(sp.R[2], pos.z)), sp.t[0]);
-            X1 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
-            X2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
+        // kNodeChunk nodes per thread at a time with the indenter loop outside: an indenter's 17 words are
+        // read from shared memory once per chunk instead of once per node; the union is still the min over
+        // the slots in slot order, node by node
+        for (int i0 = threadIdx.x; i0 < pi.n; i0 += blockDim.x * kNodeChunk) {
+          float X[kNodeChunk][3], phi[kNodeChunk];
+#pragma unroll
+          for (int c = 0; c < kNodeChunk; ++c) {
+            const int i = min(i0 + c * (int)blockDim.x, pi.n - 1);
+            const float4 pos = m.pos4[pi.off + i];
+            X[c][0] = pos.x, X[c][1] = pos.y, X[c][2] = pos.z;
+            if (posed) {
+              X[c][0] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[0], pos.x), __fmul_rn(sp.R[1], pos.y)), __fmul_rn(sp.R[2], pos.z)), sp.t[0]);
+              X[c][1] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[3], pos.x), __fmul_rn(sp.R[4], pos.y)), __fmul_rn(sp.R[5], pos.z)), sp.t[1]);
+              X[c][2] = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], pos.x), __fmul_rn(sp.R[7], pos.y)), __fmul_rn(sp.R[8], pos.z)), sp.t[2]);
+            }
+            phi[c] = __int_as_float(0x7f800000);
           }
-          const float phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid, p0 + q + 1);
-          const float d = phi < 0.0f ? -phi : 0.0f;
-          delta[i] = d;
-          any |= d > 0.0f;
-          nact += d > 0.0f;
+          for (int k = 0; k < m.max_ind; ++k) {
+            if (sind[k].skip1 == p0 + q + 1) continue;
+            const SInd s = sind[k];
+#pragma unroll
+            for (int c = 0; c < kNodeChunk; ++c) phi[c] = fminf(phi[c], sdf_one<kGrid>(s, X[c][0], X[c][1], X[c][2], m.grid));
+          }
+#pragma unroll
+          for (int c = 0; c < kNodeChunk; ++c) {
+            const int i = i0 + c * (int)blockDim.x;
+            if (i < pi.n) {
+              const float d = phi[c] < 0.0f ? -phi[c] : 0.0f;
+              delta[i] = d;
+              any |= d > 0.0f;
+              nact += d > 0.0f;
+            }
+          }
         }
       } else {
         for (int i = threadIdx.x; i < pi.n; i += blockDim.x) {
