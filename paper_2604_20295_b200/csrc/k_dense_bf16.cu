@@ -70,8 +70,12 @@ __host__ __device__ constexpr int mode_img_bytes(int mode) {
   return mode == 1 ? kWImgBytes : mode == 2 ? kW1ImgBytes + kW2ImgBytes : mode == 3 ? kPnImgBytes : 0;
 }
 
-__host__ __device__ constexpr size_t dense_smem_bytes(int n_patches, int mode) {
-  return 1024 /*align slack*/ + (size_t)mode_stages(mode) * (A_STAGE + B_STAGE) + mode_img_bytes(mode) + sizeof(DenseBars) +
+// The big-patch instantiation (kGrouped) keeps an item's u_lin in a per-thread shared-memory stash (24 fp32 per
+// epilogue thread) and pays for it with one pipeline stage.
+constexpr int kStashBytes = 8 * 3 * 256 * 4;
+__host__ __device__ constexpr size_t dense_smem_bytes(int n_patches, int mode, bool big = false) {
+  return 1024 /*align slack*/ + (size_t)(mode_stages(mode) - (big ? 1 : 0)) * (A_STAGE + B_STAGE) + (big ? kStashBytes : 0) +
+         mode_img_bytes(mode) + sizeof(DenseBars) +
          (size_t)(5 * n_patches + 4) * 4 + 16 + 16 + 8 * 32 * 16;
 }
 
@@ -190,7 +194,8 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   constexpr bool kPn = kMode == kModePnEncode || kMode == kModePnDecode;
   constexpr bool kProp = !kGather && kMode != kModePnEncode;  // TMA + propagation GEMM run
   constexpr bool kFill = kMode != kModePnEncode;              // the decode pass zero-fills
-  constexpr int kLayers = mode_layers(kMode), kStages = mode_stages(kMode), kImgBytes = mode_img_bytes(kMode);
+  constexpr int kLayers = mode_layers(kMode), kStages = mode_stages(kMode) - (kGrouped ? 1 : 0), kImgBytes = mode_img_bytes(kMode);
+  constexpr bool kStash = kGrouped && kProp;  // u_lin of an item parked in shared memory, accumulator released at once
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sA = smem;
@@ -199,6 +204,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
   DenseBars* bars = reinterpret_cast<DenseBars*>(sW + kImgBytes);
   int* prefix = reinterpret_cast<int*>(bars + 1);
   uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + kPrefixInts(m.n_patches) + 4 * m.n_patches) + 15) & ~uintptr_t(15));  // 8 warps x 32 entries
+  float* sStash = reinterpret_cast<float*>(sGather + 8 * 32 * 16);  // kStash: [unit of the slot 0..7][component][epilogue thread]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -402,6 +408,31 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         tc_fence_after();
       }
       PROF_MARK(1);  // acc_full wait
+      if constexpr (kStash) {
+        // Big patches: the propagation GEMM of an item is as long as its MLP work, and with one accumulator
+        // the two would alternate.  Every epilogue thread parks the u_lin of its (up to 8) units of the item
+        // in its own shared-memory words (nobody else reads them: no barrier) and the accumulator goes back
+        // to the MMA warp at once, so the next item's GEMM runs under this item's MLP.
+        float* st = sStash + (threadIdx.x - 128);
+#pragma unroll
+        for (int k0 = 0; k0 < 8; k0 += 4) {  // four units at a time: 16 registers in flight
+          if (sl + 2 * k0 < it.cnt) {
+            uint32_t q[4][4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) tmem_ld4(trow + COL_ACC + 3 * min(sl + 2 * (k0 + k), TE - 1), q[k]);
+            tc_wait_ld();
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+              st[(k0 + k) * 768] = __uint_as_float(q[k][0]);
+              st[(k0 + k) * 768 + 256] = __uint_as_float(q[k][1]);
+              st[(k0 + k) * 768 + 512] = __uint_as_float(q[k][2]);
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars->acc_empty);
+      }
       // The units of an item are software-pipelined: while the tensor core runs the last MMA layer of unit
       // el, the u_lin of unit el+2 is already fetched from the accumulator, and its layer-1 operand
       // is written (and requested) before the output of unit el is combined and stored.  Every
@@ -417,7 +448,10 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
         u.node = (int64_t)env * m.n_nodes + g;
         u.dl = valid ? m.delta[u.node] : 0.0f;  // consumed when the unit is stored
         u.slot = it.tile * TE + el;
-        if constexpr (kProp) {
+        if constexpr (kStash) {
+          const float* st = sStash + ((el - sl) >> 1) * (3 * 256) + (threadIdx.x - 128);
+          ur[0] = __float_as_uint(st[0]), ur[1] = __float_as_uint(st[256]), ur[2] = __float_as_uint(st[512]), ur[3] = 0;
+        } else if constexpr (kProp) {
           tmem_ld4(trow + COL_ACC + 3 * el, ur);
         } else if constexpr (kMode == kModePnEncode) {
           ur[0] = ur[1] = ur[2] = ur[3] = 0;  // the encoder pass has no propagation
@@ -475,7 +509,7 @@ __global__ void __launch_bounds__(kDenseThreads, 2)
       // the accumulator is released as soon as this warp has fetched its LAST u_lin of the item, a
       // whole unit before the item ends: the next item's propagation GEMM runs behind that unit's MLP
       auto release_acc = [&]() {
-        if constexpr (kProp) {
+        if constexpr (kProp && !kStash) {
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(&bars->acc_empty);
@@ -680,13 +714,13 @@ __global__ void __launch_bounds__(64) pn_global_kernel(DevModel m) {
 
 template <int kMode, bool kGather>
 static cudaError_t configure_one() {
-  const int bytes = (int)dense_smem_bytes(kMaxPatches, kMode);
+  const int bytes = (int)dense_smem_bytes(kMaxPatches, kMode), bytes_big = (int)dense_smem_bytes(kMaxPatches, kMode, true);
   cudaError_t e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
   if (e == cudaSuccess && kMode != kModePnEncode)  // the encoder pass writes no displacement
     e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, kGather, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
   if constexpr (!kGather && kMode != kModePnEncode) {  // grouped item order: dense propagation only
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes_big);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(dense_bf16_kernel<kMode, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes_big);
   }
   return e;
 }
@@ -714,8 +748,9 @@ static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& t
     if (io.out_bf16) dense_bf16_kernel<kMode, true, true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
     else dense_bf16_kernel<kMode, true, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
   } else if (grouped) {
-    if (io.out_bf16) dense_bf16_kernel<kMode, false, true, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
-    else dense_bf16_kernel<kMode, false, false, true><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
+    const size_t smem_big = dense_smem_bytes(m.n_patches, kMode, true);
+    if (io.out_bf16) dense_bf16_kernel<kMode, false, true, true><<<grid, kDenseThreads, smem_big, s>>>(m, io, tmA, tmB);
+    else dense_bf16_kernel<kMode, false, false, true><<<grid, kDenseThreads, smem_big, s>>>(m, io, tmA, tmB);
   } else {
     if (io.out_bf16) dense_bf16_kernel<kMode, false, true, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
     else dense_bf16_kernel<kMode, false, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
