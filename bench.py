@@ -34,9 +34,9 @@ MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728 (SURVEY.md 
 # dram__bytes_read.sum + dram__bytes_write.sum of one dense_bf16_kernel launch, from the
 # `ncu --set full` capture summarised in profiles/r01d_dense_ncu_full.md (79.2 MB read + 232.4 MB
 # write; the kernel also zero-fills the rows of contact-free (env, patch) pairs); cfg 4: the counters
-# in profiles/r01d_cfg4_item_order.md (1.26 GB read + 0.395 GB write).
+# in profiles/r01d_cfg4_item_order.md, first column (1.47 GB read + 0.41 GB write).
 NCU_TRAFFIC_BYTES = 311.54e6
-NCU_TRAFFIC_BYTES_CFG4 = 1655.0e6
+NCU_TRAFFIC_BYTES_CFG4 = 1877.3e6
 
 
 WORKLOADS = {
