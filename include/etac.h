@@ -159,8 +159,8 @@ enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
  * nodes in contact and 0 elsewhere (what a penalty-based simulator without propagation reports). */
 /* ETAC_OPT_L2_GROUP_BYTES (default 40 MiB, >= 1): scheduling only, results do not depend on it.  The dense
  * contraction K_p . U^ walks a patch's work in groups of environment tiles whose U^ operand (6 bytes x nodes
- * of the patch per environment) fits this share of L2; when n_envs x 6 x (largest patch) is below it the
- * plain order is used (cfg 4). */
+ * of the patch per environment) fits this share of L2; when n_envs x 6 x (largest patch) is below it (and no patch
+ * has 2048 nodes or more) the plain order is used (cfg 4). */
 enum { ETAC_ABLATE_FULL = 0, ETAC_ABLATE_RESIDUAL_ONLY = 1, ETAC_ABLATE_LINEAR_ONLY = 2, ETAC_ABLATE_NO_PROPAGATION = 3 };
 enum { ETAC_OUT_F32 = 0, ETAC_OUT_BF16 = 1 };
 etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value);

@@ -740,8 +740,10 @@ template <int kMode>
 static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int grid,
                        bool gather, cudaStream_t s) {
   const size_t smem = dense_smem_bytes(m.n_patches, kMode);
-  // grouped item order only where a patch's U^ operand (3 bf16 rows of n nodes per env) can exceed the L2 share
-  const bool grouped = !gather && (size_t)io.n_envs * (size_t)m.max_patch_nodes * 6 > (size_t)m.group_bytes;
+  // big-patch instantiation (grouped item order + u_lin stash): where a patch's U^ operand (3 bf16 rows of n nodes
+  // per env) can exceed the L2 share, or a patch is large enough for its propagation GEMM (2.75 n cycles per item)
+  // to matter next to the MLP of the item's 16 units
+  const bool grouped = !gather && ((size_t)io.n_envs * (size_t)m.max_patch_nodes * 6 > (size_t)m.group_bytes || m.max_patch_nodes >= 2048);
   if constexpr (kMode == kModePnEncode) {
     dense_bf16_kernel<kMode, false, false, false><<<grid, kDenseThreads, smem, s>>>(m, io, tmA, tmB);
   } else if (gather) {
