@@ -34,7 +34,7 @@
 extern "C" {
 #endif
 
-#define ETAC_ABI_VERSION 6
+#define ETAC_ABI_VERSION 7
 
 typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it makes */
 

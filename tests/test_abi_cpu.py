@@ -28,7 +28,7 @@ def test_exports_match_header(lib):
     assert declared == set(T.EXPORTS)
     for name in declared:
         assert getattr(lib, name) is not None
-    assert lib.etac_abi_version() == 6
+    assert lib.etac_abi_version() == 7
     assert C.sizeof(T.etac_indenter) == 48 == W.INDENTER_DTYPE.itemsize
 
 
