@@ -674,3 +674,35 @@ def test_grouped_item_order_is_only_scheduling(cfg, n_envs, group_bytes):
             T.etac_set_option(eng.ctx, T.ETAC_OPT_L2_GROUP_BYTES, 0)
         finally:
             eng.close()
+
+
+@pytest.mark.parametrize("out_bf16", [False, True])
+def test_big_patch_instantiation_pointnet_and_linear_only(out_bf16):
+    """One patch of 8192 nodes takes the big-patch instantiation of the fused kernel (grouped item order, u_lin
+    parked in shared memory, one pipeline stage fewer) at any batch size: its PointNet decode pass, its
+    no-residual form and its bf16-output store against the oracle (the per-node form is in the cfg-4 tests)."""
+    import dataclasses
+    import torch
+    base = W.config4(5, 19)                           # two env tiles, the second ragged
+    wl = dataclasses.replace(base, weights=W.make_pointnet_weights(3, 2, std=0.15))
+    ref = run_oracle(wl)
+    if not out_bf16:
+        gpu = run_gpu(wl)
+        assert gpu["launches"] == 4
+        _report("big-patch pointnet", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="big-pointnet", delta_tol=1e-4))
+        lin, ref_lin = run_gpu(base, resid=False), run_oracle(base, resid=False)
+        _report("big-patch linear", compare(lin, ref_lin, TOL["bf16"], label="big-linear", delta_tol=1e-4))
+    else:
+        eng = T.Etac(wl)
+        try:
+            dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+            out16 = torch.full((wl.n_envs, eng.N, 3), float("nan"), dtype=torch.bfloat16, device="cuda")
+            T.etac_step(eng.ctx, torch.cuda.current_stream().cuda_stream,
+                        T.make_step_args(wl.n_envs, out16, indenters=dev["indenters"], patch_pose=dev.get("patch_pose"),
+                                         out_dtype=T.ETAC_OUT_BF16))
+            torch.cuda.synchronize()
+            U = out16.float().cpu().numpy()
+        finally:
+            eng.close()
+        umax = float(np.abs(ref["U"]).max())
+        assert np.isfinite(U).all() and np.abs(U - ref["U"]).max() <= (TOL["bf16"] + 2.0 ** -8) * umax
