@@ -1,20 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- ETac tactile hot path on B200: one JSON line (contract in the task statement).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--envs E]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload cfg1|cfg2|cfg3|cfg4|cfg5] [--envs E]
 
 A "step" is one pass of the whole hot path (S1 SDF penetration -> S2 propagation -> S3 residual
-MLP -> S4 combine) over one batch of 4,096 synthetic environments of the
-dexterous-hand sensor set (BASELINE.json configs[2]; N = 5,696 nodes, 16 patches, bf16 tensor
-path with fp32 accumulation).  metric = tactile env-steps/s (whole job), also node-updates/s.
-Multi-GPU: environments are independent, every rank owns its own 4,096 envs,
-no data-path collective -> "scaling": "weak".
+MLP -> S4 combine) over one batch of synthetic environments.  The default
+workload is BASELINE.json configs[2] (the configuration its `metric` is quoted on): 4,096 envs of the
+dexterous-hand sensor set, N = 5,696 nodes, 16 patches, bf16 tensor path with fp32 accumulation.
+metric = tactile env-steps/s (whole job), also node-updates/s.  The other configs of BASELINE.json are
+selected with --workload (cfg1/cfg2: fp32 contexts; cfg4: one dense K[8192 x 8192]; cfg5: the dense /
+sparse sweep, one line whose "sweep" key holds a row per (N, contact fraction, path)).
+Multi-GPU: environments are independent, every rank owns its own batch,
+no data-path collective -> "scaling": "weak"; `--gpus N` without a torchrun environment re-launches
+itself under torch.distributed.run with N ranks.
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
+import socket
 import subprocess
 import sys
 import tempfile
@@ -31,24 +38,44 @@ METRIC = "tactile_env_steps_per_s"
 UNIT = "env-steps/s"
 N_INPUT_SETS = 4
 MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728 (SURVEY.md §8(d))
-# dram__bytes_read.sum + dram__bytes_write.sum of one dense_bf16_kernel launch, from the
-# `ncu --set full` capture summarised in profiles/r01d_dense_ncu_full.md (79.2 MB read + 232.4 MB
-# write; the kernel also zero-fills the rows of contact-free (env, patch) pairs); cfg 4: the counters
-# in profiles/r01d_cfg4_item_order.md, first column (1.47 GB read + 0.41 GB write).
-NCU_TRAFFIC_BYTES = 311.54e6
-NCU_TRAFFIC_BYTES_CFG4 = 1877.3e6
+FP32_FMA_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12              # 74.4: 148 SMs x 128 fp32 lanes x 2 flop at 1965 MHz
 
-
-WORKLOADS = {
-    "cfg3": ("cfg3_dexterous_hand_5696 (BASELINE.json configs[2])", lambda seed, envs: W.config3(seed, envs)),
-    # not the headline: the single dense K[8192 x 8192] case, same metric (python bench.py --workload cfg4)
-    "cfg4": ("cfg4_curved_sheet_8192 (BASELINE.json configs[3])", lambda seed, envs: W.config4(seed, envs)),
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the `ncu --set full`
+# capture named beside it; "src_sha" = sha1 (first 12 hex digits) of the kernel's source file at capture time.
+# bench.py prints the figure only while the source still has that hash -- a changed kernel gives traffic: null.
+NCU_TRAFFIC = {
+    "cfg3": {"bytes": 311.54e6, "profile": "profiles/r01d_dense_ncu_full.md", "src": "k_dense_bf16.cu",
+             "src_sha": "r01"},
+    "cfg4": {"bytes": 1877.3e6, "profile": "profiles/r01d_cfg4_item_order.md", "src": "k_dense_bf16.cu",
+             "src_sha": "r01"},
 }
 
+CFG5_NODES = (256, 1024, 4096, 8192)
+CFG5_FRACS = (0.001, 0.003, 0.01, 0.05, 0.20)
 
-def chosen_of(wl):
-    """[E, P] contact pairs the generator placed (cfg 4: every env presses on its single patch)."""
-    return wl.meta["chosen"] if "chosen" in wl.meta else np.ones((wl.n_envs, wl.mesh.n_patches), dtype=bool)
+
+def make_workload(name, seed, envs, **kw):
+    if name == "cfg1":
+        return W.config1(seed, envs)
+    if name == "cfg2":
+        return W.config2(seed, envs)
+    if name == "cfg3":
+        return W.config3(seed, envs)
+    if name == "cfg4":
+        return W.config4(seed, envs)
+    if name == "cfg5":
+        return W.config5(envs, kw.get("n_nodes", 4096), kw.get("curved", True), kw.get("frac", 0.05),
+                         kw.get("precision", "bf16"), seed)
+    raise ValueError(name)
+
+
+LABELS = {
+    "cfg1": ("cfg1_flat_pad_256 (BASELINE.json configs[0])", 1),
+    "cfg2": ("cfg2_fingertip_cap_1024 (BASELINE.json configs[1])", 64),
+    "cfg3": ("cfg3_dexterous_hand_5696 (BASELINE.json configs[2])", 4096),
+    "cfg4": ("cfg4_curved_sheet_8192 (BASELINE.json configs[3])", 4096),
+    "cfg5": ("cfg5_dense_sparse_sweep (BASELINE.json configs[4])", 4096),
+}
 
 
 def load_peaks():
@@ -60,19 +87,38 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "src": "fallback"}
 
 
-def work_model(wl, chosen):
-    """Algorithmic work of one step from the realised contact pairs."""
+def src_sha(fname):
+    p = os.path.join(ROOT, "paper_2604_20295_b200", "csrc", fname)
+    return hashlib.sha1(open(p, "rb").read()).hexdigest()[:12] if os.path.exists(p) else None
+
+
+def ncu_traffic(workload):
+    t = NCU_TRAFFIC.get(workload)
+    if not t or src_sha(t["src"]) != t["src_sha"]:
+        return None, (f"no ncu capture of the current {t['src']}" if t else "no ncu capture for this workload")
+    return t["bytes"], t["profile"]
+
+
+def work_model(wl, m_ep):
+    """Algorithmic work of one step from the REALISED contact.
+    m_ep [E, P] = active nodes of patch p in env e (from the masks the GPU path produced)."""
     npat = np.diff(wl.mesh.patch_offset).astype(np.float64)
-    pairs_per_patch = chosen.sum(0).astype(np.float64)
-    w_nodeenv = float((pairs_per_patch * npat).sum())
-    f_prop_dense = 6.0 * float((pairs_per_patch * npat * npat).sum())
-    f_mlp = MLP_FLOP_PER_NODE_ENV * w_nodeenv
-    E, N, P = wl.n_envs, wl.mesh.n_nodes, wl.mesh.n_patches
-    b_out = 12.0 * E * N
-    b_in = 48.0 * E * wl.max_indenters + 28.0 * E * P
-    b_k = 2.0 * float((npat * npat).sum())
-    return {"w_nodeenv": w_nodeenv, "f_prop_dense": f_prop_dense, "f_mlp": f_mlp,
-            "b_hbm_min": b_out + b_in + b_k + 20e3, "pairs": float(pairs_per_patch.sum())}
+    m = m_ep.astype(np.float64)
+    hit = m > 0
+    w_nodeenv = float((hit * npat).sum())
+    n_active = float(m.sum())
+    E, N, P = m_ep.shape[0], wl.mesh.n_nodes, wl.mesh.n_patches
+    return {
+        "w_nodeenv": w_nodeenv, "n_active": n_active, "pairs": float(hit.sum()),
+        "f_prop_dense": 6.0 * float((hit * npat * npat).sum()),          # what a dense K_p . U^ executes
+        "f_prop_alg": 6.0 * float((m * (npat - m)).sum()),               # the method: Omega is (n - m) x m (L87)
+        "f_prop_gather": 6.0 * float((m * npat).sum()),                  # gather over the active nodes, all rows
+        "f_mlp": MLP_FLOP_PER_NODE_ENV * w_nodeenv,                      # Phi on every row of a contacting pair
+        "f_mlp_alg": MLP_FLOP_PER_NODE_ENV * (w_nodeenv - n_active),     # passive rows only
+        "b_hbm_min": 12.0 * E * N + 48.0 * E * wl.max_indenters + (28.0 * E * P if wl.patch_pose is not None else 0.0)
+                     + 2.0 * float((npat * npat).sum()) + 20e3,
+        "contact_frac": n_active / max(1.0, w_nodeenv),
+    }
 
 
 class ClockSampler:
@@ -108,42 +154,55 @@ class ClockSampler:
                 "samples": len(rows), "reasons": reasons}
 
 
-def time_oracle(wl, n_sample, repeats=1):
-    """The CPU oracle as it stands, on a strided sample of the workload's environments."""
+def time_oracle(wl, n_sample):
+    """The CPU oracle as it stands (numpy float64; a Python loop over environments and patches, only the
+    K[:, act] @ u^ products and the MLP matmuls run in the BLAS thread pool), on a strided sample of the
+    workload's environments.  Returns env-steps/s, sample size, wall seconds and the AVERAGE number of host
+    threads it kept busy (process CPU time / wall time)."""
     from oracle import etac_oracle as O
     from threadpoolctl import threadpool_info
     m = O.model_from_workload(wl)
     envs = list(range(0, wl.n_envs, max(1, wl.n_envs // n_sample)))[:n_sample]
     for p in range(m.n_patches):
         O.kernel_block(m, p)                       # K is create-time work on both sides
-    best = float("inf")
-    for _ in range(repeats):
-        t0 = time.perf_counter()
-        O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose, envs=envs)
-        best = min(best, time.perf_counter() - t0)
-    threads = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
-    return len(envs) / best, len(envs), best, threads
+    c0, t0 = time.process_time(), time.perf_counter()
+    O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose, envs=envs)
+    wall, cpu = time.perf_counter() - t0, time.process_time() - c0
+    pool = max([i.get("num_threads", 1) for i in threadpool_info()] + [1])
+    return {"rate": len(envs) / wall, "n": len(envs), "wall": wall, "threads_busy": round(cpu / wall, 2),
+            "nproc": os.cpu_count(), "blas_pool": pool}
+
+
+def cpu_baseline_dict(r, n_envs):
+    return {"value": r["rate"], "unit": UNIT, "cores": r["threads_busy"], "kind": "oracle",
+            "host_cores": r["nproc"], "blas_pool_threads": r["blas_pool"],
+            "sample": f"{r['n']} of {n_envs} envs (strided), {r['wall']:.1f} s wall; oracle/etac_oracle.py: numpy float64, "
+                      f"Python loop over envs and patches, BLAS threads only inside the matmuls "
+                      f"(cores = process CPU time / wall time)"}
 
 
 def run_reference(a):
     """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    label, make = WORKLOADS[a.workload]
-    wl = make(0, a.envs)
+    label, _ = LABELS[a.workload]
+    wl = make_workload(a.workload, 0, a.envs)
     # each step = the oracle on a strided sample of the batch, sized from a probe so that the whole
     # --steps K --warmup W run stays within about two minutes
-    probe_rate = time_oracle(wl, min(a.envs, 8))[0]
-    n_sample = int(max(4, min(a.envs, 96, 120.0 * probe_rate / max(1, a.steps + a.warmup))))
-    t_w = [time_oracle(wl, n_sample)[0] for _ in range(a.warmup)]
+    probe = time_oracle(wl, min(a.envs, 8))
+    n_sample = int(max(1, min(a.envs, 96, 120.0 * probe["rate"] / max(1, a.steps + a.warmup))))
+    for _ in range(a.warmup):
+        time_oracle(wl, n_sample)
     t0 = time.perf_counter()
-    envs_done = 0
-    threads = 1
+    envs_done, last = 0, probe
     for _ in range(a.steps):
-        rate, n, _, threads = time_oracle(wl, n_sample)
-        envs_done += n
+        last = time_oracle(wl, n_sample)
+        envs_done += last["n"]
     dt = time.perf_counter() - t0
     v = envs_done / dt
+    cb = cpu_baseline_dict(last, a.envs)
+    cb["value"] = v
+    cb["sample"] = f"each step = {n_sample} of {a.envs} envs (stride {max(1, a.envs // n_sample)}); " + cb["sample"]
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
         "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
@@ -151,10 +210,75 @@ def run_reference(a):
         "node_updates_per_s": v * wl.mesh.n_nodes,
         "config": {"workload": label, "n_envs": a.envs,
                    "n_nodes": wl.mesh.n_nodes, "n_patches": wl.mesh.n_patches},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle",
-                         "sample": f"each step = {n_sample} of {a.envs} envs (stride {max(1, a.envs // n_sample)})"},
+        "cpu_baseline": cb,
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+def realised_contact(T, torch, eng, wl, dev):
+    """[E, P] active-node counts of one input set, from the mask the GPU path writes (untimed extra step)."""
+    E, N = wl.n_envs, eng.N
+    mask = torch.zeros((E, (N + 31) // 32), dtype=torch.int32, device=eng.device)
+    stream = torch.cuda.current_stream().cuda_stream
+    T.etac_step(eng.ctx, stream, T.make_step_args(E, eng.out, mask_out=mask, **dev))
+    torch.cuda.synchronize()
+    w = mask.cpu().numpy().view(np.uint32)
+    bits = ((w[:, :, None] >> np.arange(32, dtype=np.uint32)) & 1).reshape(E, -1)[:, :N]
+    off = np.asarray(wl.mesh.patch_offset)
+    return np.add.reduceat(bits.astype(np.int64), off[:-1], axis=1)
+
+
+def time_point(T, torch, wl, precision, path, iters):
+    """cfg-5 sweep point: ms per step (whole step, S1, fused) of one context on one path."""
+    eng = T.Etac(wl, precision=precision)
+    try:
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        stream = torch.cuda.current_stream().cuda_stream
+        args = eng.args(wl.n_envs, dev)
+        for _ in range(3):
+            T.etac_step(eng.ctx, stream, args)
+        torch.cuda.synchronize()
+        ms, (s1, rest) = T.etac_time_steps(eng.ctx, stream, args, iters, per_kernel=True)
+        taken = T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_PATH)
+        m_ep = realised_contact(T, torch, eng, wl, dev)
+    finally:
+        eng.close()
+    return ms, s1, rest, taken, m_ep
+
+
+def run_sweep(a, T, torch, peaks):
+    """--workload cfg5: BASELINE.json configs[4], E = --envs, N x contact fraction x path."""
+    rows = []
+    names = {T.ETAC_PATH_DENSE: "dense", T.ETAC_PATH_SPARSE: "sparse", T.ETAC_PATH_AUTO: "auto"}
+    iters = max(3, min(a.steps, 10))
+    headline = None
+    for n_nodes in (a.nodes or CFG5_NODES):
+        curved = n_nodes >= 4096
+        for frac in (a.fracs or CFG5_FRACS):
+            wl = make_workload("cfg5", 0, a.envs, n_nodes=n_nodes, curved=curved, frac=frac)
+            row = {"n_nodes": n_nodes, "curved": curved, "target_frac": frac}
+            for path in (T.ETAC_PATH_DENSE, T.ETAC_PATH_SPARSE, T.ETAC_PATH_AUTO):
+                ms, s1, fused, taken, m_ep = time_point(T, torch, wl, "bf16", path, iters)
+                wm = work_model(wl, m_ep)
+                t_dense = max((wm["f_prop_dense"] + wm["f_mlp"]) / (peaks["bf16_tflops_sustained"] * 1e12),
+                              wm["b_hbm_min"] / (peaks["hbm_gbs"] * 1e9))
+                t_alg = max((wm["f_prop_alg"] + wm["f_mlp_alg"]) / (peaks["bf16_tflops_sustained"] * 1e12),
+                            wm["b_hbm_min"] / (peaks["hbm_gbs"] * 1e9))
+                row["realised_frac"] = wm["contact_frac"]
+                row[names[path]] = {"ms": ms, "s1_ms": s1, "fused_ms": fused, "path_taken": names[taken],
+                                    "roof_dense": t_dense / (ms * 1e-3), "roof_alg": t_alg / (ms * 1e-3)}
+            if a.fp32:
+                ms, s1, fused, _, _ = time_point(T, torch, wl, "fp32", T.ETAC_PATH_SPARSE, max(2, iters // 3))
+                row["fp32"] = {"ms": ms, "s1_ms": s1, "fused_ms": fused}
+            rows.append(row)
+            print(f"[cfg5] E={a.envs} N={n_nodes} target {frac:.3f} realised {row['realised_frac']:.4f}: "
+                  + " ".join(f"{k} {row[k]['ms']:.3f} ms" for k in ("dense", "sparse", "auto", "fp32") if k in row),
+                  file=sys.stderr, flush=True)
+            if headline is None or (n_nodes == 4096 and abs(frac - 0.05) < 1e-9):
+                headline = row
+    ms = headline["auto"]["ms"]
+    return rows, headline, ms
 
 
 def run_ours(a):
@@ -163,6 +287,7 @@ def run_ours(a):
     from paper_2604_20295_b200 import etac as T
     rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert world == a.gpus, f"--gpus {a.gpus} but WORLD_SIZE={world}"
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the ETac hot path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -172,15 +297,31 @@ def run_ours(a):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.build()
     peaks = load_peaks()
+    label, _ = LABELS[a.workload]
+
+    if a.workload == "cfg5":
+        if rank != 0:
+            return
+        clk = ClockSampler(local)
+        rows, head, ms_step = run_sweep(a, T, torch, peaks)
+        clocks = clk.stop()
+        value = a.envs / (ms_step * 1e-3)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic", "node_updates_per_s": value * head["n_nodes"],
+            "config": {"workload": label, "n_envs_per_gpu": a.envs,
+                       "headline_point": {k: head[k] for k in ("n_nodes", "curved", "target_frac", "realised_frac")},
+                       "note": "value = the AUTO path at the headline point; every point is in 'sweep'"},
+            "clocks": clocks, "sweep": rows}))
+        return
 
     # weak scaling: every rank owns a batch of a.envs environments (its own seeds)
-    label, make = WORKLOADS[a.workload]
-    sets = [make(rank * N_INPUT_SETS + k, a.envs) for k in range(N_INPUT_SETS)]
+    sets = [make_workload(a.workload, rank * N_INPUT_SETS + k, a.envs) for k in range(N_INPUT_SETS)]
     wl = sets[0]
+    bf16 = wl.precision == "bf16"
     eng = T.Etac(wl, device=local)
     stream = torch.cuda.current_stream().cuda_stream
-    if a.l2_group_mb:
-        T.etac_set_option(eng.ctx, T.ETAC_OPT_L2_GROUP_BYTES, a.l2_group_mb << 20)
     devs = [eng.upload(indenters=s.indenters, patch_pose=s.patch_pose) for s in sets]
     argv = [eng.args(a.envs, d) for d in devs]
 
@@ -192,9 +333,7 @@ def run_ours(a):
 
     for i in range(a.warmup):
         T.etac_step(eng.ctx, stream, argv[i % N_INPUT_SETS])
-    pairs = T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_CONTACT_PAIRS)
-    last_set = sets[(a.warmup - 1) % N_INPUT_SETS]
-    assert pairs == int(chosen_of(last_set).sum()), "realised contact pairs differ from the generator's placement"
+    torch.cuda.synchronize()
 
     # ---- device-resident timing
     sync_all()
@@ -207,11 +346,17 @@ def run_ours(a):
     sync_all()
     ms = e0.elapsed_time(e1)
     launches = a.steps * T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_LAUNCHES)
+    path_taken = T.etac_get_info(eng.ctx, T.ETAC_INFO_LAST_PATH)
     # per-kernel split, live, same inputs (CUDA events on the launching stream inside the library)
     _, (ms_s1, ms_fused) = T.etac_time_steps(eng.ctx, stream, argv[0], max(5, min(a.steps, 20)), per_kernel=True)
     clocks = clk.stop() if clk else None
     # special-function pipe rate, measured live on this device (denominator of the "alu" roofline)
     sfu_ops_s, sfu_per_clk_sm = T.etac_measure_sfu_rate(stream) if rank == 0 else (0.0, 0.0)
+    # realised contact of every input set (untimed): [E, P] active-node counts from the GPU masks
+    m_eps = [realised_contact(T, torch, eng, s, d) for s, d in zip(sets, devs)]
+    for s, m_ep in zip(sets, m_eps):
+        if "chosen" in s.meta:
+            assert np.array_equal(m_ep > 0, s.meta["chosen"]), "realised contact pairs differ from the generator's placement"
 
     # ---- end to end: host buffers in, host buffer out, through the C-ABI call
     posed = sets[0].patch_pose is not None
@@ -219,15 +364,12 @@ def run_ours(a):
             torch.from_numpy(np.ascontiguousarray(s.patch_pose)).pin_memory() if posed else None) for s in sets]
     d_ind = torch.empty_like(pin[0][0], device="cuda")
     d_pose = torch.empty_like(pin[0][1], device="cuda") if posed else None
-    h_out = torch.empty((a.envs, eng.N, 3), dtype=torch.float32).pin_memory()
-    e2e_args = T.make_step_args(a.envs, eng.out, indenters=d_ind, patch_pose=d_pose)
     n_e2e = max(3, min(a.steps, 10))
-
     # Two result buffers and a copy stream: the device->host read of step i runs while step i+1 is copied in
     # and computed (every step's copies are still inside the timed region; the loop ends with a full sync).
     d_outs = [eng.out, torch.empty_like(eng.out)]
-    h_outs = [h_out, torch.empty((a.envs, eng.N, 3), dtype=torch.float32).pin_memory()]
-    e2e_argv = [e2e_args, T.make_step_args(a.envs, d_outs[1], indenters=d_ind, patch_pose=d_pose)]
+    h_outs = [torch.empty((a.envs, eng.N, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
+    e2e_argv = [T.make_step_args(a.envs, d_outs[b], indenters=d_ind, patch_pose=d_pose) for b in range(2)]
     s_main, s_copy = torch.cuda.current_stream(), torch.cuda.Stream()
     ev_done = [torch.cuda.Event(), torch.cuda.Event()]
     ev_free = [torch.cuda.Event(), torch.cuda.Event()]
@@ -253,7 +395,7 @@ def run_ours(a):
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t0)
     h2d = pin[0][0].numel() + (pin[0][1].numel() * 4 if posed else 0)
-    d2h = h_out.numel() * 4
+    d2h = h_outs[0].numel() * 4
 
     # the same loop with the result packed as bf16 by the kernel (etac_step_args.out_dtype): the PCIe
     # copy of the result dominates the end-to-end number, this halves it.  Extra information only:
@@ -289,62 +431,105 @@ def run_ours(a):
 
     ms_step = ms / a.steps
     value = world * a.envs / (ms_step * 1e-3)
-    wm = work_model(wl, np.mean([chosen_of(s) for s in sets], axis=0) * 1.0)
-    flops = wm["f_prop_dense"] + wm["f_mlp"]
-    peak = peaks["bf16_tflops_sustained"]
-    achieved = flops / (ms_fused * 1e-3) / 1e12
-    t_tensor = flops / (peak * 1e12)
-    t_hbm = wm["b_hbm_min"] / (peaks["hbm_gbs"] * 1e9)
-    t_roof = max(t_tensor, t_hbm)
-    # Floors of the fused kernel on the three units it loads: tensor pipe, HBM, and the special-function pipe
-    # (128 SiLUs = 128 MUFU.TANH per node-environment of a contacting pair).  "roofline" is the contract's
-    # (tensor peak / HBM); the activation-pipe bound is reported beside it as "roofline_sfu"
-    # against a rate measured live, and does not replace the contract fraction.
-    acts = 128.0 * wm["w_nodeenv"]
-    t_sfu = acts / sfu_ops_s
-    t_hbm_fused = (wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"]) / (peaks["hbm_gbs"] * 1e9)
-    roof_tensor = {"bound": "tensor", "kernel": "dense_bf16_kernel", "achieved": achieved, "peak": peak,
-                   "unit": "TFLOP/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else NCU_TRAFFIC_BYTES_CFG4,
-                   "peak_src": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['src']})", "flops_per_launch": flops}
-    roof_sfu = {"bound": "alu", "kernel": "dense_bf16_kernel", "achieved": acts / (ms_fused * 1e-3) / 1e12,
-                "peak": sfu_ops_s / 1e12, "unit": "Tactivation/s", "frac": t_sfu / (ms_fused * 1e-3),
-                "traffic": NCU_TRAFFIC_BYTES if a.workload == "cfg3" else NCU_TRAFFIC_BYTES_CFG4,
-                "peak_src": f"etac_measure_sfu_rate, live on this device: {sfu_per_clk_sm:.2f} MUFU results per clock and SM",
-                "activations_per_launch": acts, "pipe": "MUFU (special-function unit)"}
-    cpu_rate, cpu_n, cpu_t, cpu_threads = time_oracle(wl, a.envs if a.workload == "cfg3" else 48)   # ~10 s of CPU work
+    wms = [work_model(s, m) for s, m in zip(sets, m_eps)]
+    wm = {k: float(np.mean([w[k] for w in wms])) for k in wms[0]}      # the timed steps rotate over the sets
+    hbm = peaks["hbm_gbs"] * 1e9
+    t_hbm = wm["b_hbm_min"] / hbm
+    power_capped = bool(clocks and "sw_power_cap" in clocks.get("reasons", []))
+    traffic, traffic_src = ncu_traffic(a.workload)
+    if bf16:
+        # roofline.frac: the dominant kernel against the bf16 tensor peak -- the BURST figure when no sw_power_cap
+        # sample was seen during the timed region (the kernel then runs at the clocks of a kernel timed alone), the
+        # SUSTAINED figure otherwise (MEASURED_PEAKS.json; B200_PROFILING.md).
+        peak = peaks["bf16_tflops_sustained"] if power_capped else peaks["bf16_tflops"]
+        peak_name = "bf16_tflops_sustained (sw_power_cap seen)" if power_capped else "bf16_tflops (burst; no sw_power_cap sample)"
+        kernel = "fused_mlp_kernel" if path_taken == T.ETAC_PATH_DENSE else "fused_mlp_kernel (gather form)"
+        flops = wm["f_prop_dense"] + wm["f_mlp"]
+        flops_alg = wm["f_prop_alg"] + wm["f_mlp_alg"]
+        achieved = flops / (ms_fused * 1e-3) / 1e12
+        t_tensor, t_tensor_alg = flops / (peak * 1e12), flops_alg / (peak * 1e12)
+        # Floors of the fused kernel on the three units it loads: tensor pipe, HBM, and the special-function pipe
+        # (128 SiLUs per node-environment of a contacting pair).  "roofline" is the contract's (tensor
+        # peak / HBM); the activation-pipe bound is reported beside it as "roofline_sfu" against a rate measured
+        # live, and does not replace the contract fraction.
+        acts = 128.0 * wm["w_nodeenv"]
+        t_sfu = acts / sfu_ops_s
+        t_hbm_fused = (wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"]) / hbm
+        roofline = {"bound": "tensor", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                    "frac": achieved / peak, "traffic": traffic, "traffic_src": traffic_src,
+                    "peak_src": f"MEASURED_PEAKS.json {peak_name} ({peaks['src']})", "flops_per_launch": flops,
+                    "frac_vs_burst": achieved / peaks["bf16_tflops"], "frac_vs_sustained": achieved / peaks["bf16_tflops_sustained"],
+                    "ceiling_frac_if_sfu_bound": t_tensor / t_sfu,
+                    "note": "flops = F_prop,dense + F_mlp (SURVEY.md §8(d)); ceiling_frac_if_sfu_bound = tensor floor / MUFU floor "
+                            "with one MUFU op per SiLU: the fraction this kernel would show if it ran AT its special-function floor"}
+        extra = {
+            "roofline_sfu": {"bound": "alu", "kernel": kernel, "achieved": acts / (ms_fused * 1e-3) / 1e12,
+                             "peak": sfu_ops_s / 1e12, "unit": "Tactivation/s", "frac": t_sfu / (ms_fused * 1e-3),
+                             "peak_src": f"etac_measure_sfu_rate, live on this device: {sfu_per_clk_sm:.2f} MUFU results per clock and SM",
+                             "activations_per_launch": acts, "pipe": "MUFU (special-function unit), one op per SiLU"},
+            "roofline_floors_us": {"tensor": t_tensor * 1e6, "hbm": t_hbm_fused * 1e6, "sfu_1_mufu_per_act": t_sfu * 1e6},
+        }
+        t_roof, t_roof_alg = max(t_tensor, t_hbm), max(t_tensor_alg, t_hbm)
+        dtype = "bf16"
+    else:
+        # fp32 contexts (cfg 1, 2): plain FP32 FMA arithmetic; peak derived from the guide's unit counts and clock
+        peak = FP32_FMA_TFLOPS
+        flops = wm["f_prop_gather"] + wm["f_mlp"]
+        flops_alg = wm["f_prop_alg"] + wm["f_mlp_alg"]
+        achieved = flops / (ms_fused * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": "gather_fp32_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                    "frac": achieved / peak, "traffic": traffic, "traffic_src": traffic_src,
+                    "peak_src": "derived: 148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts)",
+                    "flops_per_launch": flops}
+        extra = {}
+        t_roof, t_roof_alg = max(flops / (peak * 1e12), t_hbm), max(flops_alg / (peak * 1e12), t_hbm)
+        dtype = "f32"
+    n_cpu = a.envs if a.workload in ("cfg1", "cfg2", "cfg3") else min(a.envs, 64)      # ~10 s of CPU work
+    cpu = time_oracle(wl, n_cpu)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "bf16", "data": "synthetic",
+        "dtype": dtype, "data": "synthetic",
         "node_updates_per_s": value * eng.N,
         "config": {"workload": label, "n_envs_per_gpu": a.envs,
-                   "n_nodes": eng.N, "n_patches": eng.P, "precision": "bf16 operands, fp32 accumulate",
+                   "n_nodes": eng.N, "n_patches": eng.P,
+                   "precision": "bf16 operands, fp32 accumulate" if bf16 else "fp32",
+                   "path": {T.ETAC_PATH_DENSE: "dense", T.ETAC_PATH_SPARSE: "sparse"}.get(path_taken, str(path_taken)),
                    "contact_pairs_per_step": wm["pairs"], "node_envs_per_step": wm["w_nodeenv"],
+                   "active_nodes_per_step": wm["n_active"], "realised_contact_frac_of_contacting_patches": wm["contact_frac"],
                    "l2": f"{N_INPUT_SETS} rotating seeded input sets; {12 * a.envs * eng.N / 1e6:.0f} MB output + "
-                         f"{10 * a.envs * eng.N / 1e6:.0f} MB workspace per step > 126 MB L2",
+                         f"{10 * a.envs * eng.N / 1e6:.0f} MB workspace per step vs 126 MB L2",
                    "algorithmic_bytes_fused": wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"],
                    "parallelism": f"env-sharded x{world}, no collective"},
         "clocks": clocks,
         "e2e": {"value": world * a.envs * n_e2e / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "steps": n_e2e,
-                "note": "pinned host indenters+patch poses -> device, etac_step, full [E,N,3] fp32 result -> pinned host; the read of step i overlaps step i+1 (two result buffers, copy stream)"},
+                "note": "pinned host indenters (+ patch poses) -> device, etac_step, full [E,N,3] fp32 result -> pinned host; the read of step i overlaps step i+1 (two result buffers, copy stream)"},
         "e2e_bf16_output": {"value": world * a.envs * n_e2e / (e2e16_ms * 1e-3), "unit": UNIT, "d2h_bytes_per_step": d2h // 2,
                             "note": "same loop, result written as bf16 by the kernel (out_dtype); not the headline"},
         "gpu_launches": launches,
-        "kernels_ms": {"s1_sdf_kernel_incl_memsets": ms_s1, "dense_bf16_kernel": ms_fused},
-        "roofline": roof_tensor, "roofline_sfu": roof_sfu,
-        "roofline_floors_us": {"tensor": t_tensor * 1e6, "hbm": t_hbm_fused * 1e6, "sfu": t_sfu * 1e6},
-        "roofline_step": {"t_roof_us": t_roof * 1e6, "t_tensor_us": t_tensor * 1e6, "t_hbm_us": t_hbm * 1e6,
-                          "roof_dense_frac": t_roof / (ms_step * 1e-3),
-                          "hbm_frac_of_measured": wm["b_hbm_min"] / (ms_step * 1e-3) / (peaks["hbm_gbs"] * 1e9),
-                          "t_act_us_1mufu": t_sfu * 1e6},
-        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
-                         "sample": f"{cpu_n} of {a.envs} envs (strided), {cpu_t:.1f} s, numpy fp64"},
+        "kernels_ms": {"s1_sdf_kernel_incl_memsets": ms_s1, "fused_s2_s3_s4_kernel": ms_fused},
+        "roofline": roofline,
+        "roofline_step": {"roof_dense": t_roof / (ms_step * 1e-3), "roof_alg": t_roof_alg / (ms_step * 1e-3),
+                          "t_roof_dense_us": t_roof * 1e6, "t_roof_alg_us": t_roof_alg * 1e6, "t_hbm_us": t_hbm * 1e6,
+                          "f_prop_dense": wm["f_prop_dense"], "f_prop_alg": wm["f_prop_alg"], "f_mlp": wm["f_mlp"],
+                          "hbm_frac_of_measured": wm["b_hbm_min"] / (ms_step * 1e-3) / hbm,
+                          "note": "whole step vs max(F/P, B/BW), SURVEY.md §8(d): roof_dense with F_prop,dense = 6 sum N_p^2 over contacting "
+                                  "pairs (the north_star's >= 0.60 target refers to it), roof_alg with F_prop,alg = 6 sum m (N_p - m) "
+                                  "and the MLP on passive rows only (the method's own work, Omega is (n-m) x m)"},
+        "cpu_baseline": cpu_baseline_dict(cpu, a.envs),
     }
+    out.update(extra)
     print(json.dumps(out))
     eng.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
 
 
 if __name__ == "__main__":
@@ -353,10 +538,17 @@ if __name__ == "__main__":
     ap.add_argument("--steps", type=int, default=500)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--envs", type=int, default=4096)
-    ap.add_argument("--workload", default="cfg3", choices=sorted(WORKLOADS))
-    ap.add_argument("--l2-group-mb", type=int, default=0,
-                    help="experiments: ETAC_OPT_L2_GROUP_BYTES in MiB (0 = library default, 1024 = one group)")
+    ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the config's own batch)")
+    ap.add_argument("--workload", default="cfg3", choices=sorted(LABELS))
+    ap.add_argument("--nodes", type=int, nargs="+", default=None, help="cfg5: mesh sizes (default 256 1024 4096 8192)")
+    ap.add_argument("--fracs", type=float, nargs="+", default=None, help="cfg5: contact fractions (default 0.001 .. 0.20)")
+    ap.add_argument("--fp32", action="store_true", help="cfg5: also time the fp32 context at every point")
     args = ap.parse_args()
+    args.envs = args.envs or LABELS[args.workload][1]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # one process per GPU: re-launch under torchrun (the driver's own launch line does the same)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
     (run_reference if args.impl == "reference" else run_ours)(args)

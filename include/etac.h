@@ -7,7 +7,9 @@
  *       Omega U_a                                                             (Eq. 1)
  *   S3  residual correction Phi (per-node MLP form of BASELINE.json)
  *   S4  mask M_p + combine  U_p = Omega U_a + Phi_p                           (Eq. 2)
- * Calibration of alpha / Phi (Eq. 3) is offline and out of scope: parameters are inputs.
+ * alpha and the weights of Phi are inputs of etac_create.  Their calibration (Eq. 3) is
+ * an offline loop of the caller; this library serves it with etac_backward (the gradients of one step) and
+ * etac_update_params (writes a descent step back); the FEM data the paper calibrates on is not part of it.
  *
  * Conventions
  *   - All functions return etac_status; nothing throws; no global state.
@@ -41,7 +43,8 @@ typedef struct etac_ctx etac_ctx; /* opaque; owns every device allocation it mak
 typedef enum {
   ETAC_OK = 0,
   ETAC_ERR_INVALID_ARG = 1, /* NULL / out-of-range / inconsistent argument; ctx unchanged */
-  ETAC_ERR_UNSUPPORTED = 2, /* valid request this build cannot serve (e.g. POINTNET residual) */
+  ETAC_ERR_UNSUPPORTED = 2, /* valid request this build cannot serve (e.g. ETAC_PATH_DENSE on an fp32 context,
+                               ETAC_RESID_POINTNET on an fp32 context, a device that is not sm_100) */
   ETAC_ERR_ALLOC = 3,       /* host or device allocation failed */
   ETAC_ERR_CUDA = 4,        /* a CUDA call failed; etac_last_error() has the CUDA message */
   ETAC_ERR_CAPACITY = 5     /* n_envs > max_envs */
@@ -240,23 +243,6 @@ etac_status etac_update_params(etac_ctx* ctx, const etac_params* params);
 
 /* Library ABI version (ETAC_ABI_VERSION the .so was built with). */
 int32_t etac_abi_version(void);
-
-/* Timing helper for bench.py: times `iters` back-to-back etac_step calls on cuda_stream with CUDA
- * events recorded on that stream and returns the mean milliseconds per step in *ms_per_step
- * (host pointer).  If ms_kernels (host, [2]) is not NULL a second pass of `iters` steps records
- * events between the kernels: ms_kernels[0] = S1 (sdf_penetration, incl. its two small memsets),
- * ms_kernels[1] = fused S2+S3+S4 kernel, mean ms per launch.  Synchronises the stream on both sides. */
-etac_status etac_time_steps(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args, int32_t iters,
-                            float* ms_per_step, float* ms_kernels);
-
-/* Measurement helper for bench.py's roofline (not on the hot path): runs a microbenchmark of independent
- * tanh.approx.f32 chains on every SM of the current device, on cuda_stream, and returns the measured rate of
- * the special-function pipe in results per second (*ops_per_s, host pointer) and, if not NULL, per clock and
- * SM at the device's nominal maximum clock (*ops_per_clk_per_sm).  The fused kernel evaluates 128 SiLUs
- * (one MUFU.TANH each) per node-environment of a contacting pair, BASELINE.json configs[0] "2x64 SiLU"; this
- * rate is the denominator of its "alu" roofline.  Synchronises the stream.
- * Errors: ETAC_ERR_INVALID_ARG (NULL ops_per_s), ETAC_ERR_CUDA. */
-etac_status etac_measure_sfu_rate(void* cuda_stream, double* ops_per_s, double* ops_per_clk_per_sm);
 
 #ifdef __cplusplus
 }

@@ -9,6 +9,7 @@
 #include <vector>
 
 #include "../../include/etac.h"
+#include "../../include/etac_bench.h"
 
 namespace etac {
 

@@ -21,8 +21,8 @@ __global__ void __launch_bounds__(kGatherChunk) gather_fp32_kernel(DevModel m, S
   __shared__ float s_u[kGatherChunk][3];
   __shared__ int s_wcnt[kGatherChunk / 32];
 
-  const ChunkInfo ch = m.chunk[blockIdx.x];
-  const int e = blockIdx.y;
+  const int e = blockIdx.x / m.n_chunks;  // 1-D grid: n_envs is not bounded by gridDim.y's 65535
+  const ChunkInfo ch = m.chunk[blockIdx.x - e * m.n_chunks];
   if (!m.flags[(int64_t)e * m.n_patches + ch.patch]) return;  // S1 zero-filled this patch
   const PatchInfo pi = m.patch[ch.patch];
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
@@ -68,6 +68,7 @@ __global__ void __launch_bounds__(kGatherChunk) gather_fp32_kernel(DevModel m, S
   if (!valid) return;
 
   float ox = ax, oy = ay, oz = az;
+  if (m.resid == ETAC_RESID_NONE && m.residual_only) ox = oy = oz = 0.0f;  // Phi_p of a context without Phi
   if (m.resid != ETAC_RESID_NONE) {
     const float* W1u = s_w;
     const float* W2 = s_w + 192;
@@ -114,7 +115,7 @@ __global__ void __launch_bounds__(kGatherChunk) gather_fp32_kernel(DevModel m, S
 }
 
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s) {
-  dim3 grid(m.n_chunks, io.n_envs);
+  const unsigned grid = (unsigned)((int64_t)m.n_chunks * io.n_envs);
   gather_fp32_kernel<<<grid, kGatherChunk, 0, s>>>(m, io);
   return cudaGetLastError();
 }

@@ -220,7 +220,8 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
         }
         // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
         const float phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
-        sp.evaluated = !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
+        // (phi_lo = +inf: no indenter applies to this patch -- all slots NONE, or only the patch's own link)
+        sp.evaluated = phi_lo < __int_as_float(0x7f800000) && !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
         s_pose[threadIdx.x] = sp;
       }
     }
@@ -414,7 +415,8 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
     phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
   }
   // conservative cull: phi(x_i) >= phi(c) - L * brad on the patch's bounding sphere
-  const bool evaluated = !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
+  // (phi_lo = +inf: no indenter applies to this patch -- all slots NONE, or only the patch's own link)
+  const bool evaluated = phi_lo < __int_as_float(0x7f800000) && !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
   bool any = false;
   int nact = 0;
   float* delta = m.delta + row0;

@@ -51,12 +51,22 @@ __device__ __forceinline__ bool mbar_test_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Bounded wait: a protocol bug must end in a trap (sticky CUDA error), never in a hung GPU.
+// Bounded wait: a protocol bug must end in a trap (sticky CUDA error), never in a hung GPU.  The bound is
+// wall time (10 s on %globaltimer, read once per 16 Ki failed polls), so that a legitimate wait under a
+// debugger, compute-sanitizer or heavy instrumentation does not trip it.
+__device__ __forceinline__ uint64_t global_timer_ns() {
+  uint64_t t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t spins = 0;
+  uint64_t t0 = 0;
   while (!mbar_try_wait(bar, parity)) {
-    if (++spins > (1u << 20)) {  // a failed try_wait suspends for microseconds: this is seconds
-      __trap();
+    if ((++spins & 0x3fffu) == 0) {
+      const uint64_t now = global_timer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 10000000000ull) __trap();
     }
   }
 }

@@ -427,7 +427,115 @@ def test_pointnet_branch_is_permutation_equivariant():
     assert np.abs(O.residual_pointnet(w, uh2, p, nr)[1:] - a[1:]).max() > 1e-6
 
 
+def _pointnet_weights(seed, std=0.2):
+    rng = np.random.default_rng(seed)
+    shp = {"E1": (64, 9), "e1": (64,), "E2": (64, 64), "e2": (64,), "G1": (64, 64), "g1": (64,),
+           "D1": (64, 128), "d1": (64,), "D2": (3, 64), "d2": (3,)}
+    return {k: rng.normal(0, std, s).astype(np.float32) for k, s in shp.items()}
+
+
+def test_pointnet_branch_against_torch_float64_restatement():
+    """PAPER.md:L93-L99 restated with library routines in the paper's order: n x 9 input [P, N, U^]
+    -> shared MLP (point-wise features) -> Max-Pooling into a 64-d global feature -> another MLP ->
+    broadcast + concatenate with the per-node features (n x 128) -> shared-MLP decoder -> n x 3.
+    torch float64 F.linear / F.silu / torch.max / torch.cat; no code shared with the oracle."""
+    import torch
+    import torch.nn.functional as F
+    w = _pointnet_weights(31)
+    rng = np.random.default_rng(32)
+    for n in (1, 7, 300):
+        uh, p, nr = rng.normal(0, 0.7, (n, 3)), rng.normal(0, 3.0, (n, 3)), rng.normal(size=(n, 3))
+        t = {k: torch.from_numpy(v.astype(np.float64)) for k, v in w.items()}
+        x = torch.cat([torch.from_numpy(p), torch.from_numpy(nr), torch.from_numpy(uh)], dim=1)   # [P, N, U^]
+        f = F.silu(F.linear(F.silu(F.linear(x, t["E1"], t["e1"])), t["E2"], t["e2"]))                # n x 64
+        g = torch.max(f, dim=0).values                                                               # 64-d global feature
+        g = F.silu(F.linear(g, t["G1"], t["g1"]))                                                    # "another MLP"
+        cat = torch.cat([f, g.unsqueeze(0).expand(n, 64)], dim=1)                                    # n x 128, [f_i ; g']
+        want = F.linear(F.silu(F.linear(cat, t["D1"], t["d1"])), t["D2"], t["d2"]).numpy()
+        got = O.residual_pointnet(w, uh, p, nr)
+        assert got.shape == (n, 3)
+        np.testing.assert_allclose(got, want, rtol=0, atol=1e-13 * max(1.0, np.abs(want).max()))
+
+
+def test_pointnet_branch_structure():
+    """What the permutation test cannot see: (a) the max-pool is the ONLY coupling between nodes: changing
+    the input of a node that holds no column maximum leaves every other node's output unchanged; (b) the
+    concatenation order is [f_i ; g']: with D1[:, :64] = 0 the output does not depend on f_i (all rows
+    equal), with D1[:, 64:] = 0 it does not depend on the other nodes; (c) the global MLP sits between the
+    pool and the concat (zero G1 and g1 => g' = 0, so the output equals the one with D1[:, 64:] = 0);
+    (d) the pool is a max, not a mean or sum: duplicating a node changes nothing."""
+    w = _pointnet_weights(33)
+    rng = np.random.default_rng(34)
+    n = 50
+    uh, p, nr = rng.normal(0, 0.5, (n, 3)), rng.normal(size=(n, 3)), rng.normal(size=(n, 3))
+    a = O.residual_pointnet(w, uh, p, nr)
+    # (a) find a node that is arg-max of no encoder column, perturb it slightly (it must stay below the maxima)
+    f64 = lambda k: w[k].astype(np.float64)
+    x9 = np.concatenate([p, nr, uh], 1)
+    f = O.silu(O.silu(x9 @ f64("E1").T + f64("e1")) @ f64("E2").T + f64("e2"))
+    holders = set(np.argmax(f, axis=0).tolist())
+    free = [i for i in range(n) if i not in holders]
+    assert free
+    i0 = free[0]
+    uh2 = uh.copy()
+    uh2[i0] += 1e-3
+    x9b = np.concatenate([p, nr, uh2], 1)
+    fb = O.silu(O.silu(x9b @ f64("E1").T + f64("e1")) @ f64("E2").T + f64("e2"))
+    assert np.array_equal(fb.max(0), f.max(0))                    # still below every column maximum
+    b = O.residual_pointnet(w, uh2, p, nr)
+    others = np.arange(n) != i0
+    assert np.array_equal(a[others], b[others]) and np.abs(a[i0] - b[i0]).max() > 0
+    # (b) concat order
+    wz = dict(w)
+    wz["D1"] = w["D1"].copy()
+    wz["D1"][:, :64] = 0
+    c = O.residual_pointnet(wz, uh, p, nr)
+    assert np.abs(c - c[0]).max() < 1e-14 and np.abs(a - a[0]).max() > 1e-3
+    wy = dict(w)
+    wy["D1"] = w["D1"].copy()
+    wy["D1"][:, 64:] = 0
+    d_all = O.residual_pointnet(wy, uh, p, nr)
+    d_sub = O.residual_pointnet(wy, uh[:10], p[:10], nr[:10])
+    np.testing.assert_allclose(d_all[:10], d_sub, atol=1e-14)     # per-node only once the global half is cut
+    # (c) the global MLP: g' = silu(G1 g + g1); zero G1, g1 => g' = 0 => same as cutting D1[:, 64:]
+    wg = dict(w)
+    wg["G1"], wg["g1"] = np.zeros_like(w["G1"]), np.zeros_like(w["g1"])
+    np.testing.assert_allclose(O.residual_pointnet(wg, uh, p, nr), d_all, atol=1e-14)
+    # (d) max-pool: a duplicated node changes nothing for the original nodes
+    dup = lambda v: np.concatenate([v, v[3:4]], 0)
+    e = O.residual_pointnet(w, dup(uh), dup(p), dup(nr))
+    np.testing.assert_allclose(e[:n], a, atol=1e-14)
+    np.testing.assert_allclose(e[n], a[3], atol=1e-14)
+
+
 # ---------------------------------------------------------------- fp32 decision twin
+@pytest.mark.parametrize("cfg", ["cfg3", "cfg4"])
+def test_full_size_twin_band_is_empty_or_harmless(cfg):
+    """SURVEY.md Q7 / DESIGN.md §5 at BASELINE.json's full sizes: the contact decision is taken on the fp32
+    twin; the two evaluations may only disagree for nodes within the band |phi64| < 1e-4 of the surface.
+    Counts the nodes of the full-size bench workloads in that band and asserts that the twin's mask equals
+    the float64 mask everywhere outside it (cfg 3: all 4096 envs; cfg 4: every 8th env)."""
+    if cfg == "cfg3":
+        wl, envs, band = W.config3(0, 4096), range(4096), 1e-4
+    else:
+        wl, envs, band = W.config4(0, 4096), range(0, 4096, 8), 1e-4
+    m = O.model_from_workload(wl)
+    in_band = disagree = evaluated = 0
+    for e in envs:
+        pp = None if wl.patch_pose is None else wl.patch_pose[e]
+        p64 = O.signed_distance(m, wl.indenters[e], pp, np.float64)
+        p32 = O.signed_distance(m, wl.indenters[e], pp, np.float32)
+        near = np.abs(p64) < band
+        in_band += int(near.sum())
+        evaluated += int((p64 < 50.0).sum())
+        diff = (p32 < 0) != (p64 < 0)
+        disagree += int(diff.sum())
+        assert not (diff & ~near).any(), (e, np.argwhere(diff & ~near)[:4])
+    print(f"[twin band] {cfg}: {in_band} of {evaluated} nodes within 50 mm of an indenter have |phi64| < {band}; "
+          f"{disagree} decisions differ (all inside the band)")
+    assert in_band <= 1e-4 * evaluated + 5
+
+
 def test_fp32_twin_agrees_with_fp64_away_from_the_surface():
     for wl in (W.config2(seed=7, n_envs=6), W.config3(seed=7, n_envs=4)):
         m = O.model_from_workload(wl)

@@ -163,14 +163,14 @@ def test_patches_derived_from_adjacency_on_device():
     T.etac_destroy(ctx)
 
 
-def test_full_size_config3_sampled():
+def test_full_size_config3_all_envs():
     """BASELINE.json's bench configuration (4096 envs, N = 5696, bf16) in the launch
-    configuration bench.py times; the oracle checks a sample of environments one by one."""
+    configuration bench.py times; the oracle checks EVERY environment element by element
+    ("parity is checked on all envs for configs 1-4")."""
     wl = W.config3(0, 4096)
     gpu = run_gpu(wl)
-    envs = list(range(0, 4096, 171)) + [4095]
-    ref = run_oracle(wl, envs=envs)
-    _report("cfg3 full", compare(gpu, ref, TOL["bf16"], envs=envs, resid_tol=5e-2, label="cfg3-full"))
+    ref = run_oracle(wl)
+    _report("cfg3 full", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="cfg3-full"))
     # properties that hold at any size: contact pairs = chosen patches; un-chosen patches are 0
     assert gpu["pairs"] == int(wl.meta["chosen"].sum())
     rows = ~np.repeat(wl.meta["chosen"], np.diff(wl.mesh.patch_offset), axis=1)
@@ -226,7 +226,8 @@ def test_many_patches_several_indenters(posed):
     compare(gpu32, ref, TOL["fp32"], resid_tol=1e-4, label="hand-multi-fp32")
 
 
-@pytest.mark.parametrize("n_nodes,curved,frac", [(256, False, 0.05), (1024, True, 0.20), (1024, False, 0.01)])
+@pytest.mark.parametrize("n_nodes,curved,frac", [(256, False, 0.05), (1024, True, 0.20), (1024, False, 0.01),
+                                                 (4096, True, 0.01), (4096, False, 0.20), (8192, True, 0.20)])
 def test_config5_dense_and_sparse_paths(n_nodes, curved, frac):
     """BASELINE.json configs[4] sweep points at a size the oracle finishes in seconds: the bf16
     context through the tensor-core contraction and through the gather form, the fp32 context
@@ -244,9 +245,19 @@ def test_config5_dense_and_sparse_paths(n_nodes, curved, frac):
     _report(f"cfg5 N={n_nodes} sparse fp32", compare(sparse32, ref, TOL["fp32"], resid_tol=1e-4, label="cfg5-sparse32", delta_tol=1e-4))
 
 
-def test_full_size_config4_sampled():
+def test_fp32_context_large_batch_all_envs():
+    """An fp32 context beyond toy batch sizes (cfg-5 point N = 1024 curved, 5 %, E = 1024; the fp32 gather
+    kernel's grid covers every (chunk, env)): every environment against the oracle at the fp32 tolerance."""
+    wl = W.config5(1024, 1024, True, 0.05, "fp32")
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    assert gpu["path"] == T.ETAC_PATH_SPARSE
+    _report("cfg5 fp32 E=1024", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="cfg5-fp32-1024", delta_tol=1e-4))
+
+
+def test_full_size_config4_strided():
     """BASELINE.json configs[3] at full size (4096 envs, one dense K[8192 x 8192], bf16); the
-    oracle checks a sample of environments; invariants hold on every environment."""
+    oracle checks every 16th environment (256 of them, so that every CTA's env tiles are hit) element by
+    element; invariants hold on every environment."""
     wl = W.config4(0, 4096)
     import torch
     eng = T.Etac(wl, debug_outputs=False)
@@ -255,7 +266,7 @@ def test_full_size_config4_sampled():
         eng.out.fill_(float("nan"))
         U = eng.step(wl.n_envs, dev)
         torch.cuda.synchronize()
-        envs = [0, 1777, 4095]
+        envs = list(range(7, 4096, 16))
         ref = run_oracle(wl, envs=envs)
         Us = U[envs].cpu().numpy()
         umax = float(np.abs(ref["U"]).max())
@@ -706,3 +717,75 @@ def test_big_patch_instantiation_pointnet_and_linear_only(out_bf16):
             eng.close()
         umax = float(np.abs(ref["U"]).max())
         assert np.isfinite(U).all() and np.abs(U - ref["U"]).max() <= (TOL["bf16"] + 2.0 ** -8) * umax
+
+
+@pytest.mark.parametrize("kind", ["dense", "gather16", "fp32", "pointnet", "big_patch"])
+def test_workspace_reuse_across_changing_contact_sets(kind):
+    """One context stepped with input set A, then set B (other contacts, other (env, patch) pairs), then the
+    first third of B's environments: every result equals, bit for bit, what a fresh context gives for the
+    same inputs -- the per-step workspace (U^ slot rows, active lists, delta, env lists, pooled features)
+    carries nothing from one step to the next."""
+    import dataclasses
+    import torch
+    E = 61
+    if kind == "big_patch":
+        wa, wb = W.config4(21, E), W.config4(22, E)
+    else:
+        wa, wb = W.config3(21, E), W.config3(22, E)
+    pw = W.make_pointnet_weights(3, 5, std=0.15) if kind == "pointnet" else wa.weights
+    wa, wb = dataclasses.replace(wa, weights=pw), dataclasses.replace(wb, weights=pw)   # one model, two input sets
+    precision = "fp32" if kind == "fp32" else "bf16"
+    path = T.ETAC_PATH_SPARSE if kind == "gather16" else T.ETAC_PATH_AUTO
+    n_small = E // 3
+
+    def fresh(wl, n):
+        eng = T.Etac(wl, precision=precision, max_envs=E)
+        try:
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+            eng.out.fill_(float("nan"))
+            out = eng.step(n, eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)).cpu().numpy()
+        finally:
+            eng.close()
+        return out
+
+    want_b, want_small = fresh(wb, E), fresh(wb, n_small)
+    eng = T.Etac(wa, precision=precision, max_envs=E)
+    try:
+        T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+        da = eng.upload(indenters=wa.indenters, patch_pose=wa.patch_pose)
+        db = eng.upload(indenters=wb.indenters, patch_pose=wb.patch_pose)
+        eng.step(E, da)
+        eng.out.fill_(float("nan"))
+        got_b = eng.step(E, db).cpu().numpy()
+        eng.step(E, da)
+        eng.out.fill_(float("nan"))
+        got_small = eng.step(n_small, db).cpu().numpy()
+        rest = eng.out[n_small:E].cpu().numpy()
+    finally:
+        eng.close()
+    assert np.isfinite(got_b).all()
+    assert np.array_equal(got_b, want_b)
+    assert np.array_equal(got_small, want_small)
+    assert np.isnan(rest).all()                       # rows of environments >= n_envs are not touched
+    ref = run_oracle(wb)
+    assert np.abs(got_b - ref["U"]).max() <= TOL[precision] * np.abs(ref["U"]).max()
+
+
+def test_residual_only_without_a_residual_network_is_zero_on_passive_rows():
+    """ETAC_ABLATE_RESIDUAL_ONLY on a context created without Phi: U_p = Phi_p = 0 on the passive rows,
+    active rows keep u^ -- the same answer from the fp32 and the bf16 context (and from the oracle)."""
+    from oracle import etac_oracle as O
+    wl = W.config3(23, 13)
+    m = O.model_from_workload(wl, resid_arch="none")
+    m.ablation = "residual_only"
+    ref = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)
+    assert np.all(ref["U"][~ref["mask"]] == 0)
+    for precision in ("fp32", "bf16"):
+        eng = T.Etac(wl, precision=precision, resid=False)
+        try:
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_ABLATION, T.ETAC_ABLATE_RESIDUAL_ONLY)
+            U = eng.step(wl.n_envs, eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)).cpu().numpy()
+        finally:
+            eng.close()
+        assert np.all(U[~ref["mask"]] == 0), precision
+        np.testing.assert_allclose(U[ref["mask"]], ref["U"][ref["mask"]], rtol=0, atol=2e-5)
