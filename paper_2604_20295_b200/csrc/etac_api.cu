@@ -17,7 +17,7 @@ struct etac_ctx {
   size_t bytes = 0;
   int device = 0, n_sm = 0, precision = 0, path_opt = ETAC_PATH_AUTO, n_alpha = 1;
   int last_path = ETAC_PATH_AUTO, last_launches = 0;
-  CUtensorMap tmA{}, tmB{};
+  CUtensorMap tmA{}, tmB16{}, tmB32{};
   bool have_tm = false;
   cudaStream_t last_stream = nullptr;
   std::string err;
@@ -187,11 +187,11 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
     if (abl == ETAC_ABLATE_LINEAR_ONLY) {  // "Linear Decay Only": the kernels compiled without Phi
       DevModel lin = ctx->m;
       lin.resid = ETAC_RESID_NONE;
-      e = launch_dense_bf16(lin, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s);
+      e = launch_fused_bf16(lin, io, ctx->tmA, ctx->tmB16, ctx->tmB32, ctx->n_sm, gather16, &n_launch, s);
     } else {
-      e = launch_dense_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s);
+      e = launch_fused_bf16(ctx->m, io, ctx->tmA, ctx->tmB16, ctx->tmB32, ctx->n_sm, gather16, &n_launch, s);
     }
-    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("dense_bf16_kernel", e));
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("fused_mlp_kernel", e));
     ctx->last_launches += n_launch - 1;
   } else {
     if (abl == ETAC_ABLATE_LINEAR_ONLY) {
@@ -388,6 +388,14 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   }
   CK(dev_upload(c, &m.pos4, pos4.data(), N), "upload pos");
   CK(dev_upload(c, &m.nrm4, nrm4.data(), N), "upload normal");
+  {
+    std::vector<uint4> a1c(N);
+    for (int i = 0; i < N; ++i) {
+      auto pk = [](float lo, float hi) { return (uint32_t)f2bf(lo) | ((uint32_t)f2bf(hi) << 16); };
+      a1c[i] = make_uint4(pk(pos4[i].x, 0.f), pk(pos4[i].y, pos4[i].z), pk(nrm4[i].x, nrm4[i].y), pk(nrm4[i].z, 1.0f));
+    }
+    CK(dev_upload(c, &m.a1c, a1c.data(), N), "upload layer-1 constants");
+  }
 
   std::vector<PatchInfo> hp(P);
   std::vector<ChunkInfo> chunks;
@@ -479,19 +487,21 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   }
 
   // ---- per-step workspace
-  const size_t urows = (size_t)((d->max_envs + kDenseTE - 1) / kDenseTE) * kDenseBN;
+  const size_t urows = (size_t)((d->max_envs + kMaxTE - 1) / kMaxTE) * kMaxTE * 3;
   CK(dev_alloc(c, &m.delta, (size_t)d->max_envs * N, true), "alloc delta");
   CK(dev_alloc(c, &m.count, (size_t)P, true), "alloc count");
   CK(dev_alloc(c, &m.envlist, (size_t)P * d->max_envs, true), "alloc envlist");
   CK(dev_alloc(c, &m.flags, (size_t)P * d->max_envs, true), "alloc flags");
   if (d->precision == ETAC_PREC_BF16) {
+    if (!fused_fits(P)) return bail(ETAC_ERR_UNSUPPORTED, "too many patches for the shared-memory tables of the tensor-core path");
     CK(dev_alloc(c, &m.uhat_t, urows * m.ldu, true), "alloc uhat");
     std::string why;
     if (!make_tmap(&c->tmA, m.k16, (uint64_t)N, (uint64_t)m.kw, (uint64_t)m.kw, 128, &why) ||
-        !make_tmap(&c->tmB, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, kDenseBN, &why))
+        !make_tmap(&c->tmB16, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 48, &why) ||
+        !make_tmap(&c->tmB32, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 96, &why))
       return bail(ETAC_ERR_CUDA, why);
     c->have_tm = true;
-    CK(dense_bf16_configure(), "cudaFuncSetAttribute(dense_bf16_kernel)");
+    CK(fused_configure(), "cudaFuncSetAttribute(fused_mlp_kernel)");
   }
   c->n_alpha = d->n_alpha;
   CK(backward_configure(), "cudaFuncSetAttribute(backward_kernel)");
@@ -540,7 +550,7 @@ etac_status etac_set_option(etac_ctx* ctx, int32_t key, int64_t value) {
     DeviceGuard guard(ctx->device);
     ActiveEntry* al = nullptr;
     int32_t* ac = nullptr;
-    const size_t rows = (size_t)((ctx->m.max_envs + kDenseTE - 1) / kDenseTE) * kDenseTE;
+    const size_t rows = (size_t)((ctx->m.max_envs + kMaxTE - 1) / kMaxTE) * kMaxTE;
     cudaError_t e = dev_alloc(ctx, &al, rows * ctx->m.ldu, false);
     if (e == cudaSuccess) e = dev_alloc(ctx, &ac, (size_t)ctx->m.n_patches * ctx->m.max_envs, true);
     if (e != cudaSuccess) return fail(ctx, e == cudaErrorMemoryAllocation ? ETAC_ERR_ALLOC : ETAC_ERR_CUDA, cuda_msg("alloc active lists", e));

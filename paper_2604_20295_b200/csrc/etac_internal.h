@@ -34,12 +34,12 @@ struct ChunkInfo {
 };
 constexpr int kGatherChunk = 128;
 
-// tensor-core path tiling: environments per work item and the GEMM N extent (3 columns per env)
-constexpr int kDenseTE = 16;
-constexpr int kDenseBN = kDenseTE * 3;
+// tensor-core path tiling: environments per work item (16, or 32 for large patches); the U^ operand and the
+// active lists are sized for whole tiles of the larger one
+constexpr int kMaxTE = 32;
 
 // Shared-memory image of the MLP weights for the tensor-core path (bf16, UMMA K-major
-// SWIZZLE_NONE core-matrix layout; see k_dense_bf16.cu).
+// SWIZZLE_NONE core-matrix layout; see k_fused.cu).
 constexpr int kW1ImgBytes = 64 * 16 * 2;   // N=64,  K=16   (9 inputs + bias column)
 constexpr int kW2ImgBytes = 64 * 80 * 2;   // N=64,  K=80   (64 + bias column, padded to 5 k-steps)
 // The output layer (3 x 64) is not an MMA: the epilogue applies it with FFMAs to the fp32 SiLU
@@ -79,6 +79,8 @@ struct DevModel {
   int32_t ablation;           // ETAC_ABLATE_* (LINEAR_ONLY / NO_PROPAGATION select other kernels on the host)
   const float4* pos4;         // [N] (x,y,z,0)
   const float4* nrm4;         // [N]
+  const uint4* a1c;           // [N] constant part of the layer-1 operand of the tensor-core MLP, bf16:
+                              //     .x = px (low half), .y = (py, pz), .z = (nx, ny), .w = (nz, 1.0)
   const PatchInfo* patch;     // [P]
   const ChunkInfo* chunk;     // [n_chunks]
   const float* k32;           // per patch [n x n]
@@ -165,8 +167,10 @@ cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_
 cudaError_t backward_configure();
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,
                             float* grad_w, float* grad_delta, int n_sm, cudaStream_t s);
-cudaError_t launch_dense_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB,
-                              int n_sm, bool gather, int* launches, cudaStream_t s);
-cudaError_t dense_bf16_configure();
+cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB16,
+                              const CUtensorMap& tmB32, int n_sm, bool gather, int* launches, cudaStream_t s);
+cudaError_t fused_configure();
+bool fused_uses_big_tile(const DevModel& m, int n_envs);
+bool fused_fits(int n_patches);
 
 }  // namespace etac
