@@ -82,7 +82,6 @@ __host__ __device__ constexpr int mode_layers(int mode) { return mode == 1 ? 2 :
 __host__ __device__ constexpr int mode_img_bytes(int mode) {
   return mode == 1 ? kWImgBytes : mode == 2 ? kW1ImgBytes + kW2ImgBytes : mode == 3 ? kPnImgBytes : 0;
 }
-__host__ __device__ constexpr int kPrefixInts(int n_patches) { return n_patches + 1; }
 
 // dynamic shared memory of one instantiation: TMA ring (dense propagation only), weight image, ones block, the
 // chains' operand regions, barriers, the item prefix table (+ 4 ints per patch for the grouped order) and the
@@ -92,18 +91,17 @@ template <int TE>
 __host__ __device__ constexpr size_t fused_smem_bytes(int n_patches, int mode, bool gather, bool grouped) {
   const bool prop = !gather && mode != 2;
   return 1024 /*align slack*/ + (prop ? (size_t)kStages * (A_STAGE + Tile<TE>::B_STAGE) : 0) + mode_img_bytes(mode) + kOnesBytes +
-         (size_t)Tile<TE>::NC * kAopBytes + sizeof(FusedBars<Tile<TE>::NC>) + (size_t)((grouped ? 5 : 1) * n_patches + 4) * 4 + 16 + 16 +
+         (size_t)Tile<TE>::NC * kAopBytes + sizeof(FusedBars<Tile<TE>::NC>) + (size_t)(7 * n_patches + 4) * 4 + 16 + 16 +
          (gather ? (size_t)Tile<TE>::NC * 4 * 32 * 16 : 0);
 }
-
-struct Item {
-  int p, mb, tile, cnt;
-};
 
 constexpr int kGatherDepth = 16;  // K loads in flight per thread in the gather form (divides 32)
 
 __device__ __forceinline__ void named_bar_sync(int id, int threads) {
   asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ void named_bar_arrive(int id, int threads) {
+  asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(threads) : "memory");
 }
 __device__ __forceinline__ void st_shared_v4(uint32_t saddr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
   asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(saddr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
@@ -153,35 +151,38 @@ struct ZeroFill {
   }
 };
 
-// prefix[0..P]: first work index of every patch.  kGrouped: four more ints per patch behind it (contacting
-// envs, env tiles, env tiles per group G, G x node blocks), written once by the prologue.
+// prefix[0..P]: first work index of every patch, followed by one PTab per patch, both written once by the
+// prologue into shared memory (an item decode on the epilogue's path must not wait for global memory).
 // Item order inside a patch.  Plain (kGrouped = false): node block mb = r / tiles, the env tile is the fast
 // index.  Grouped: env tiles in groups of G whose U^ operand tiles (BN x n bf16 each) stay resident in L2
 // together; a group sweeps all node blocks before the next group starts.  Without the groups a large single
 // patch (cfg 4: 201 MB of U^ tiles > L2) re-reads every U^ tile from HBM once per node block.
+struct PTab {
+  int cnt, tiles, off, n;  // contacting envs, env tiles, first node, nodes
+  int G, GN;               // grouped order: env tiles per group, G x node blocks
+};
+__host__ __device__ constexpr int kTabInts(int n_patches) { return n_patches + 1 + 6 * n_patches; }
+struct Item {
+  int p, mb, tile, cnt, off, n;  // patch, node block, env tile, units; first node and node count of the patch
+};
 template <bool kGrouped, int TE>
-__device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, const DevModel& m, int w, int& pcur,
-                                            Item& it) {
+__device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, int w, int& pcur, Item& it) {
   if (w >= prefix[n_patches]) return false;
   while (prefix[pcur + 1] <= w) ++pcur;
   const int r = w - prefix[pcur];
-  it.p = pcur;
+  const PTab t = reinterpret_cast<const PTab*>(prefix + n_patches + 1)[pcur];
+  it.p = pcur, it.off = t.off, it.n = t.n;
   if constexpr (!kGrouped) {
-    const int cnt = m.count[pcur];
-    const int tiles = (cnt + TE - 1) / TE;
-    it.mb = r / tiles;
-    it.tile = r - it.mb * tiles;
-    it.cnt = min(TE, cnt - it.tile * TE);
+    it.mb = r / t.tiles;
+    it.tile = r - it.mb * t.tiles;
   } else {
-    const int* pinfo = prefix + kPrefixInts(n_patches) + 4 * pcur;
-    const int cnt = pinfo[0], tiles = pinfo[1], G = pinfo[2], GN = pinfo[3];
-    const int g = r / GN;
-    const int rem = r - g * GN;
-    const int gsz = min(G, tiles - g * G);
+    const int g = r / t.GN;
+    const int rem = r - g * t.GN;
+    const int gsz = min(t.G, t.tiles - g * t.G);
     it.mb = rem / gsz;
-    it.tile = g * G + (rem - it.mb * gsz);
-    it.cnt = min(TE, cnt - it.tile * TE);
+    it.tile = g * t.G + (rem - it.mb * gsz);
   }
+  it.cnt = min(TE, t.cnt - it.tile * TE);
   return true;
 }
 
@@ -209,7 +210,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   uint8_t* sAop = sOnes + kOnesBytes;
   FusedBars<NC>* bars = reinterpret_cast<FusedBars<NC>*>(sAop + NC * kAopBytes);
   int* prefix = reinterpret_cast<int*>(bars + 1);
-  uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + kPrefixInts(m.n_patches) + (kGrouped ? 4 * m.n_patches : 0)) + 15) & ~uintptr_t(15));  // 4 NC warps x 32 entries
+  uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + kTabInts(m.n_patches)) + 15) & ~uintptr_t(15));  // 4 NC warps x 32 entries
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -229,14 +230,15 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       const int p = p0 + lane;
       int v = 0;
       if (p < m.n_patches) {
-        const int cnt = m.count[p], n = m.patch[p].n;
-        const int tiles = (cnt + TE - 1) / TE, nmb = (n + BM - 1) / BM;
-        if constexpr (kGrouped) {
-          const int G = max(1, min(tiles, m.group_bytes / (BN * 2 * max(n, 1))));
-          int* pinfo = prefix + kPrefixInts(m.n_patches) + 4 * p;
-          pinfo[0] = cnt, pinfo[1] = tiles, pinfo[2] = G, pinfo[3] = max(G * nmb, 1);
-        }
-        v = tiles * nmb;
+        const PatchInfo pi = m.patch[p];
+        PTab t;
+        t.cnt = m.count[p], t.off = pi.off, t.n = pi.n;
+        t.tiles = (t.cnt + TE - 1) / TE;
+        const int nmb = (pi.n + BM - 1) / BM;
+        t.G = max(1, min(t.tiles, m.group_bytes / (BN * 2 * max(pi.n, 1))));
+        t.GN = max(t.G * nmb, 1);
+        reinterpret_cast<PTab*>(prefix + m.n_patches + 1)[p] = t;
+        v = t.tiles * nmb;
       }
 #pragma unroll
       for (int d = 1; d < 32; d <<= 1) {
@@ -272,15 +274,14 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       int pcur = 0, stage = 0;
       uint32_t ph = 0;
       Item it;
-      for (int w = blockIdx.x; decode_item<kGrouped, TE>(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x) {
-        const PatchInfo pi = m.patch[it.p];
-        const int nkb = (pi.n + BK - 1) / BK;
+      for (int w = blockIdx.x; decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it); w += gridDim.x) {
+        const int nkb = (it.n + BK - 1) / BK;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(&bars->empty[stage], ph ^ 1);
           if (elect_one()) {
             mbar_arrive_expect_tx(&bars->full[stage], A_STAGE + B_STAGE);
-            tma_load_2d(sA + stage * A_STAGE, &tmA, &bars->full[stage], kb * BK, pi.off + it.mb * BM);
-            tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], pi.off + kb * BK, it.tile * BN);
+            tma_load_2d(sA + stage * A_STAGE, &tmA, &bars->full[stage], kb * BK, it.off + it.mb * BM);
+            tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], it.off + kb * BK, it.tile * BN);
           }
           __syncwarp();
           if (++stage == kStages) stage = 0, ph ^= 1;
@@ -297,8 +298,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       int pcur = 0, stage = 0, k_item = 0;
       uint32_t ph = 0;
       Item it;
-      for (int w = blockIdx.x; decode_item<kGrouped, TE>(prefix, m.n_patches, m, w, pcur, it); w += gridDim.x, ++k_item) {
-        const int nkb = (m.patch[it.p].n + BK - 1) / BK;
+      for (int w = blockIdx.x; decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it); w += gridDim.x, ++k_item) {
+        const int nkb = (it.n + BK - 1) / BK;
         const int b = k_item & 1;
         mbar_wait(&bars->acc_empty[b], ((k_item >> 1) & 1) ^ 1);  // the epilogue has fetched item k_item - 2
         tc_fence_after();
@@ -348,8 +349,13 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       if constexpr (kResid) {
         fence_proxy_async_smem();
         tc_fence_before();
-        named_bar_sync(1 + c, 128);
-        if (q == 0) {
+        // only the issuing warp has to wait for the chain; the other three arrive and go on (their next stop is the
+        // layer's d_ready).  The issue costs its warp a few hundred cycles (the MMAs queue behind the MUFU traffic of
+        // its sub-partition), so the role is spread over the sub-partitions: chain c issues from its warp c % 4.
+        if (q != (c & 3)) {
+          named_bar_arrive(1 + c, 128);
+        } else {
+          named_bar_sync(1 + c, 128);
           tc_fence_after();
           if (elect_one()) {
             constexpr uint32_t idesc_h = make_idesc_bf16(BM, 64);
@@ -374,7 +380,15 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     // ---- cursor over the units of this chain: unit q of the CTA's item stream belongs to chain q mod NC
     int cw = blockIdx.x, ck = 0, cel = c, pcur = 0;  // work index, item ordinal, unit within the item
     Item it;
-    bool live = decode_item<kGrouped, TE>(prefix, m.n_patches, m, cw, pcur, it);
+    bool live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, pcur, it);
+    int it_g = 0;           // this thread's node of the item (row clamped into the patch) and whether the row is inside
+    bool it_valid = false;
+    auto item_setup = [&]() {
+      const int li = it.mb * BM + row;
+      it_valid = li < it.n;
+      it_g = it.off + (it_valid ? li : 0);
+    };
+    if (live) item_setup();
     auto enter_item = [&]() {  // the propagation GEMM of item ck must have landed before its accumulator is touched
       if constexpr (kProp) {
         mbar_wait(&bars->acc_full[ck & 1], (ck >> 1) & 1);
@@ -393,8 +407,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
         cel -= it.cnt;
         leave_item();
         ++ck, cw += gridDim.x;
-        live = decode_item<kGrouped, TE>(prefix, m.n_patches, m, cw, pcur, it);
-        if (live) enter_item();
+        live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, pcur, it);
+        if (live) item_setup(), enter_item();
       }
     };
     if (live) enter_item();
@@ -408,10 +422,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     };
     // requests only; tc_wait_ld() follows.  delta is loaded later (load_delta) so that no load waits on `env`.
     auto fetch_unit = [&](Unit& u, uint32_t (&ur)[4]) {
-      const PatchInfo pi = m.patch[it.p];
-      const int li = it.mb * BM + row;
-      u.valid = li < pi.n;
-      u.g = pi.off + (u.valid ? li : 0);
+      u.valid = it_valid;
+      u.g = it_g;
       const int slot = it.tile * TE + cel;
       u.pslot = it.p * m.max_envs + slot;
       u.env = __ldg(m.envlist + u.pslot);
@@ -424,8 +436,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
         // Omega U_a: sum over the active nodes of this (env, patch); entry loads are warp-uniform
         // (broadcast), K row j is read coalesced over the rows i of the warp
         const int cnt = m.acount[u.pslot];
-        const ActiveEntry* __restrict__ al = m.alist + (int64_t)slot * m.ldu + pi.off;
-        const __nv_bfloat16* __restrict__ kcol = m.k16 + (int64_t)pi.off * m.kw + (u.valid ? li : 0);
+        const ActiveEntry* __restrict__ al = m.alist + (int64_t)slot * m.ldu + it.off;
+        const __nv_bfloat16* __restrict__ kcol = m.k16 + (int64_t)it.off * m.kw + (u.g - it.off);
         float ax = 0.f, ay = 0.f, az = 0.f;
         // 32 entries per sweep: lane l loads entry k0+l (one coalesced 512-byte read) into the
         // warp's shared-memory staging row; the entries are then read back as broadcasts while
@@ -557,6 +569,12 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
           for (int half = 0; half < 2; ++half) {
             tmem_ld32(tD + 32 * half, h);
             tc_wait_ld();
+            // D is in registers: the next unit's layer-1 operand and request go out now, its tensor-core round trip
+            // runs under the second half's SiLUs and the output layer
+            if (half == 1 && more) {
+              if constexpr (kPn) load_delta(nxt);
+              request_layer1(nxt, un);
+            }
 #pragma unroll
             for (int k4 = 0; k4 < 8; ++k4) {
               float4 c4 = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -585,7 +603,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       }
       // the next unit's layer-1 operand and request: D is free once all four warps have read the last layer
       // (the chain barrier inside the request)
-      if (more) {
+      if (more && (kMode == kModeNone || kMode == kModePnEncode)) {
         if constexpr (kPn) load_delta(nxt);
         request_layer1(nxt, un);
       }
