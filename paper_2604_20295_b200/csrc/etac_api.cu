@@ -166,7 +166,7 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   }
   if (io.nact_out && (e = cudaMemsetAsync(io.nact_out, 0, sizeof(int32_t) * a->n_envs, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset active count", e));
-  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess)
+  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 1), s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset count", e));
   // bf16 context: tensor-core MLP either way; DENSE = tcgen05 contraction K.U^, SPARSE = gather over the
   // active-node lists.  fp32 context: fp32 SIMT gather kernel (which needs S1 to zero-fill).
@@ -175,9 +175,10 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   const int abl = ctx->m.ablation;
   const int s1_flags = abl == ETAC_ABLATE_NO_PROPAGATION ? 0 : !bf16 ? kS1FillOut : (gather16 ? kS1WriteAlist : kS1WriteUhat);
   if (gather16 && !ctx->m.alist) return fail(ctx, ETAC_ERR_INVALID_ARG, "select ETAC_PATH_SPARSE with etac_set_option first");
-  if ((e = launch_sdf(ctx->m, io, s1_flags, s)) != cudaSuccess)
+  int n_s1 = 1;
+  if ((e = launch_sdf(ctx->m, io, s1_flags, &n_s1, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
-  ++ctx->last_launches;
+  ctx->last_launches += n_s1;
   if (ev) cudaEventRecord(ev[1], s);
   if (abl == ETAC_ABLATE_NO_PROPAGATION) {
     if ((e = launch_penalty_only(ctx->m, io, s)) != cudaSuccess)
@@ -489,7 +490,13 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   // ---- per-step workspace
   const size_t urows = (size_t)((d->max_envs + kMaxTE - 1) / kMaxTE) * kMaxTE * 3;
   CK(dev_alloc(c, &m.delta, (size_t)d->max_envs * N, true), "alloc delta");
-  CK(dev_alloc(c, &m.count, (size_t)P, true), "alloc count");
+  CK(dev_alloc(c, &m.count, (size_t)P + 1, true), "alloc count");
+  m.ntask = m.count + P;
+  if (d->max_indenters == 1 && P >= 4) {  // S1 as cull + evaluate kernels: 128-byte task records
+    void* tasks = nullptr;
+    CK(dev_alloc(c, reinterpret_cast<uint8_t**>(&tasks), (size_t)128 * P * d->max_envs, false), "alloc S1 tasks");
+    m.tasks = static_cast<PairTask*>(tasks);
+  }
   CK(dev_alloc(c, &m.envlist, (size_t)P * d->max_envs, true), "alloc envlist");
   CK(dev_alloc(c, &m.flags, (size_t)P * d->max_envs, true), "alloc flags");
   if (d->precision == ETAC_PREC_BF16) {
@@ -675,17 +682,18 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
   io.n_envs = a->n_envs, io.input_mode = a->input_mode;
   io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
   cudaError_t e;
-  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * ctx->m.n_patches, s)) != cudaSuccess ||
+  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 1), s)) != cudaSuccess ||
       (e = cudaMemsetAsync(a->d_grad_alpha, 0, sizeof(float) * ctx->n_alpha, s)) != cudaSuccess ||
       (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * ETAC_GRAD_WEIGHTS_LEN, s)) != cudaSuccess) ||
       (a->d_grad_penetration &&
        (e = cudaMemsetAsync(a->d_grad_penetration, 0, sizeof(float) * (size_t)a->n_envs * ctx->m.n_nodes, s)) != cudaSuccess))
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset", e));
-  if ((e = launch_sdf(ctx->m, io, 0, s)) != cudaSuccess)  // S1: delta and the pair flags only
+  int n_s1 = 1;
+  if ((e = launch_sdf(ctx->m, io, 0, &n_s1, s)) != cudaSuccess)  // S1: delta and the pair flags only
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
   if ((e = launch_backward(ctx->m, io, a->d_grad_out, a->d_grad_alpha, ctx->n_alpha, a->d_grad_weights, a->d_grad_penetration, ctx->n_sm, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("backward_kernel", e));
-  ctx->last_launches = 2;
+  ctx->last_launches = 1 + n_s1;
   return ETAC_OK;
 }
 

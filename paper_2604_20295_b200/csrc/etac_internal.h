@@ -67,6 +67,7 @@ struct GridDesc {
   float h, inv_h;  // inv_h = 1.0f / h (IEEE fp32 division)
 };
 
+struct PairTask;
 struct DevModel {
   int32_t n_nodes, n_patches, n_chunks;
   int32_t max_patch_nodes;    // largest patch
@@ -99,6 +100,8 @@ struct DevModel {
   int32_t* count;             // [P] contacting envs per patch (this step)
   int32_t* envlist;           // [P x max_envs]
   uint8_t* flags;             // [max_envs x P]
+  struct PairTask* tasks;     // [max_envs x P] S1 task list of the cull / evaluate kernel pair (many patches, one indenter)
+  int32_t* ntask;             // [1], behind count[P] (zeroed with it)
   GridDesc grid[kMaxGrids];   // sampled-SDF objects (etac_set_sdf_grid)
   ActiveEntry* alist;         // [max_envs (slots) x ldu]: the active nodes of (slot, patch p) start at
                               // slot * ldu + off_p, in node order (allocated when the bf16 gather path is first selected)
@@ -161,7 +164,7 @@ __device__ __forceinline__ void store_out3(const StepIO& io, int env, int g, flo
 // kernel launchers (each returns cudaGetLastError())
 cudaError_t launch_build_k(const DevModel& m, float* k32, __nv_bfloat16* k16, cudaStream_t s);
 cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1, float* c1t, cudaStream_t s);
-cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s);
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* launches, cudaStream_t s);
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t backward_configure();

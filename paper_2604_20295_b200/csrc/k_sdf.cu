@@ -24,6 +24,17 @@ struct SInd {
   float R[9];
 };
 
+// Task of the two-kernel S1 (sdf_cull_kernel -> sdf_eval_kernel): a pair that survived the cull, with the rotations
+// the cull computed
+struct __align__(16) PairTask {
+  float R[9], t[3];  // patch pose
+  SInd ind;          // the environment's indenter (type NONE if it is this patch's own link)
+  int pair;
+  int evaluated;     // 0: culled -- only the contact-free outputs remain to be written
+  int pad;
+};
+static_assert(sizeof(PairTask) == 128, "PairTask");
+
 __device__ __forceinline__ void quat_to_rot(const float* q, float* R) {
   const float x = q[0], y = q[1], z = q[2], w = q[3];
   const float xx = __fmul_rn(x, x), yy = __fmul_rn(y, y), zz = __fmul_rn(z, z);
@@ -498,6 +509,208 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// S1 for meshes of many small patches with ONE indenter slot per environment (the dexterous hand of
+// BASELINE.json configs[2]), as two kernels:
+//   sdf_cull_kernel  one THREAD per (env, patch) pair: pose -> rotation, indenter -> rotation, conservative
+//                    bounding-sphere cull.  Two thirds of the pairs of the hand workload end here after ~200
+//                    instructions of one thread (in sdf_pairs_kernel every lane of a warp repeats them, 28 % of
+//                    that kernel's instructions).  Survivors are appended, with their rotations, to a task list.
+//   sdf_eval_kernel  one WARP per task: nodes -> phi, delta (workspace), warp vote -> contact flag, slot in the
+//                    patch's compact environment list, then the U^ operand rows / active list / optional outputs.
+//                    The grid is sized for the worst case (every pair a task); warps beyond the list exit at once.
+// Same single-rounded arithmetic in the same order as the other S1 kernels.
+constexpr int kCullThreads = 128, kEvalWarps = 2;
+
+template <bool kGrid>
+__global__ void __launch_bounds__(kCullThreads) sdf_cull_kernel(DevModel m, StepIO io, int s1_flags) {
+  const bool fill_out = s1_flags & kS1FillOut;
+  const int lane = threadIdx.x & 31;
+  const int P = m.n_patches;
+  const int64_t n_pairs = (int64_t)io.n_envs * P;
+  const bool posed = io.patch_pose != nullptr;
+  // a culled pair needs a warp only if rows have to be zero-filled for it
+  const bool culled_needs_warp = fill_out || io.pen_out != nullptr;
+  const int64_t pair = (int64_t)blockIdx.x * kCullThreads + threadIdx.x;
+  bool task = false;
+  PairTask tk;
+  if (pair < n_pairs) {
+    const int e = (int)(pair / P), p = (int)(pair - (int64_t)e * P);
+    const PatchInfo pi = m.patch[p];
+    tk.R[0] = tk.R[4] = tk.R[8] = 1.f, tk.R[1] = tk.R[2] = tk.R[3] = tk.R[5] = tk.R[6] = tk.R[7] = 0.f;
+    tk.t[0] = tk.t[1] = tk.t[2] = 0.f;
+    float C0 = pi.bc[0], C1 = pi.bc[1], C2 = pi.bc[2];
+    if (posed) {
+      const float* pp = io.patch_pose + pair * 7;
+      const float q[4] = {pp[3], pp[4], pp[5], pp[6]};
+      tk.t[0] = pp[0], tk.t[1] = pp[1], tk.t[2] = pp[2];
+      quat_to_rot(q, tk.R);
+      to_world(tk.R, tk.t, pi.bc[0], pi.bc[1], pi.bc[2], C0, C1, C2);
+    }
+    tk.ind = load_indenter(io.ind + e);
+    if (tk.ind.skip1 == p + 1) tk.ind.type = ETAC_IND_NONE;  // the shape of this patch's own link
+    const float phi_lo = union_sdf_lower<kGrid>(&tk.ind, 1, C0, C1, C2, pi.brad, m.grid, p + 1);
+    // conservative cull: phi(x_i) >= phi(c) - L * brad on the patch's bounding sphere
+    // (phi_lo = +inf: no indenter applies to this patch)
+    tk.evaluated = phi_lo < __int_as_float(0x7f800000) && !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
+    tk.pair = (int)pair;
+    task = tk.evaluated || culled_needs_warp;
+    if (!task) {
+      m.flags[pair] = 0;
+      if (io.contact_out) io.contact_out[pair] = 0;
+    }
+  }
+  const uint32_t bal = __ballot_sync(0xffffffffu, task);
+  int base = 0;
+  if (lane == 0 && bal) base = atomicAdd(m.ntask, __popc(bal));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (task) m.tasks[base + __popc(bal & ((1u << lane) - 1u))] = tk;
+}
+
+template <bool kGrid>
+__global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel m, StepIO io, int s1_flags) {
+  const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
+  const int lane = threadIdx.x & 31;
+  const int k = blockIdx.x * kEvalWarps + (threadIdx.x >> 5);
+  if (k >= *m.ntask) return;
+  const int P = m.n_patches;
+  const bool posed = io.patch_pose != nullptr;
+  const PairTask* __restrict__ tk = m.tasks + k;  // every lane reads the same words: broadcast loads
+  const int64_t pair = tk->pair;
+  const int e = (int)(pair / P), p = (int)(pair - (int64_t)e * P);
+  const PatchInfo pi = m.patch[p];
+  const int off = pi.off, n = pi.n;
+  const int64_t row0 = (int64_t)e * m.n_nodes + off;
+  float* delta = m.delta + row0;
+  bool any = false;
+  int nact = 0;
+  if (tk->evaluated) {
+    float R[9], t[3];
+#pragma unroll
+    for (int a = 0; a < 9; ++a) R[a] = tk->R[a];
+    t[0] = tk->t[0], t[1] = tk->t[1], t[2] = tk->t[2];
+    const SInd one = tk->ind;
+#pragma unroll 2
+    for (int i = lane; i < n; i += 32) {
+      const float4 pos = m.pos4[off + i];
+      float X0 = pos.x, X1 = pos.y, X2 = pos.z;
+      if (posed) to_world(R, t, pos.x, pos.y, pos.z, X0, X1, X2);
+      const float phi = fminf(__int_as_float(0x7f800000), sdf_one<kGrid>(one, X0, X1, X2, m.grid));
+      const float d = phi < 0.0f ? -phi : 0.0f;
+      delta[i] = d;
+      any |= d > 0.0f;
+      nact += d > 0.0f;
+    }
+    any = __any_sync(0xffffffffu, any);
+  }
+  if (io.nact_out && any) {
+    nact = __reduce_add_sync(0xffffffffu, nact);
+    if (lane == 0) atomicAdd(&io.nact_out[e], nact);
+  }
+  int slot = 0;
+  if (lane == 0) {
+    m.flags[pair] = (uint8_t)any;
+    if (io.contact_out) io.contact_out[pair] = (uint8_t)any;
+    if (any) {
+      slot = atomicAdd(&m.count[p], 1);
+      m.envlist[(int64_t)p * m.max_envs + slot] = e;
+    }
+  }
+  if (any) {
+    slot = __shfl_sync(0xffffffffu, slot, 0);
+    const int words = (m.n_nodes + 31) >> 5;
+    if (write_alist) {  // compact list of the patch's active nodes, in node order
+      ActiveEntry* al = m.alist + (int64_t)slot * m.ldu + off;
+      int base = 0;
+      for (int i0 = 0; i0 < n; i0 += 32) {
+        const int i = i0 + lane;
+        const float d = i < n ? delta[i] : 0.0f;
+        const uint32_t bal = __ballot_sync(0xffffffffu, d > 0.0f);
+        if (d > 0.0f) {
+          const float4 nn = m.nrm4[off + i];
+          ActiveEntry en;
+          en.ux = -d * nn.x, en.uy = -d * nn.y, en.uz = -d * nn.z, en.j = i;
+          al[base + __popc(bal & ((1u << lane) - 1u))] = en;
+        }
+        base += __popc(bal);
+      }
+      if (lane == 0) m.acount[(int64_t)p * m.max_envs + slot] = base;
+    }
+    // second sweep: the U^ operand rows (bf16, all n columns: the rows are reused from step to step) and the
+    // optional outputs.  A lane takes EIGHT consecutive nodes: delta comes back from L2 as two 16-byte loads
+    // (written by this warp above), a group without an active node -- most of them: a tenth of the nodes of a
+    // contacting patch is active -- costs three 16-byte zero stores, and normals are only loaded for active nodes.
+    __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off;
+    const bool vec = ((off | m.ldu) & 7) == 0 && ((row0 & 3) == 0);  // 16-byte aligned groups (else node by node)
+    __syncwarp();  // the lanes read delta values that other lanes of the warp wrote
+    if (write_uhat && vec) {
+      for (int i0 = lane * 8; i0 < n; i0 += 256) {
+        float d[8];
+        if (i0 + 8 <= n) {
+          const float4 a = *reinterpret_cast<const float4*>(delta + i0), b = *reinterpret_cast<const float4*>(delta + i0 + 4);
+          d[0] = a.x, d[1] = a.y, d[2] = a.z, d[3] = a.w, d[4] = b.x, d[5] = b.y, d[6] = b.z, d[7] = b.w;
+        } else {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) d[c] = i0 + c < n ? delta[i0 + c] : 0.0f;
+        }
+        uint32_t w[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+        bool some = false;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) some |= d[c] > 0.0f;
+        if (some) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            if (d[c] > 0.0f) {
+              const float4 nn = m.nrm4[off + i0 + c];
+              const uint32_t sh = (c & 1) * 16;
+              w[0][c >> 1] |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(-d[c] * nn.x)) << sh;
+              w[1][c >> 1] |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(-d[c] * nn.y)) << sh;
+              w[2][c >> 1] |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(-d[c] * nn.z)) << sh;
+            }
+          }
+        }
+        // (columns past the patch end inside the last group belong to the padding / the next patch's columns of
+        //  this slot row, which only that patch's own contacting environments ever write: do not touch them)
+        if (i0 + 8 <= n) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
+            *reinterpret_cast<uint4*>(u0 + (int64_t)c * m.ldu + i0) = make_uint4(w[c][0], w[c][1], w[c][2], w[c][3]);
+        } else {
+          for (int c = 0; i0 + c < n; ++c)
+            for (int a = 0; a < 3; ++a)
+              u0[(int64_t)a * m.ldu + i0 + c] = __ushort_as_bfloat16((unsigned short)(w[a][c >> 1] >> ((c & 1) * 16)));
+        }
+      }
+    }
+    if ((write_uhat && !vec) || io.pen_out || io.mask_out) {
+      for (int i = lane; i < n; i += 32) {
+        const float d = delta[i];
+        if (io.pen_out) io.pen_out[row0 + i] = d;
+        if (io.mask_out && d > 0.0f) {
+          const int g = off + i;
+          atomicOr(&io.mask_out[(int64_t)e * words + (g >> 5)], 1u << (g & 31));
+        }
+        if (write_uhat && !vec) {
+          const float4 nn = m.nrm4[off + i];
+          u0[i] = __float2bfloat16_rn(-d * nn.x);
+          u0[m.ldu + i] = __float2bfloat16_rn(-d * nn.y);
+          u0[2 * (int64_t)m.ldu + i] = __float2bfloat16_rn(-d * nn.z);
+        }
+      }
+    }
+  } else {
+    // contact-free pair: optional outputs are zero; for the fp32 gather kernel the output rows too
+    // (the tensor-core kernel zero-fills them itself)
+    if (fill_out) {
+      zero_out_rows(io, e, off, n, lane, 32);
+      if (io.analytic_out)
+        for (int i = lane; i < n * 3; i += 32) io.analytic_out[row0 * 3 + i] = 0.0f;
+    }
+    if (io.pen_out)
+      for (int i = lane; i < n; i += 32) io.pen_out[row0 + i] = 0.0f;
+  }
+}
+
 // ETAC_ABLATE_NO_PROPAGATION: U = U^, the penalty displacement -delta * n of the nodes in contact and 0
 // elsewhere (no K, no Phi).  Reads S1's delta (valid for the contacting pairs) and pair flags.
 __global__ void __launch_bounds__(256) penalty_only_kernel(DevModel m, StepIO io) {
@@ -523,7 +736,8 @@ cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_
   return cudaGetLastError();
 }
 
-cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaStream_t s) {
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* launches, cudaStream_t s) {
+  *launches = 1;
   const unsigned grid = (unsigned)io.n_envs;
   bool grids = false;  // the sampled-SDF code is only in the variants launched once a grid is registered
   for (int k = 0; k < kMaxGrids; ++k) grids |= m.grid[k].v != nullptr;
@@ -532,8 +746,13 @@ cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, cudaSt
     const int64_t pairs = (int64_t)io.n_envs * m.n_patches;
     const unsigned pgrid = (unsigned)((pairs + kPairWarps - 1) / kPairWarps);
     const size_t smem = m.max_ind == 1 ? 0 : sizeof(SInd) * (size_t)m.max_ind * kPairWarps;
-    if (m.max_ind == 1 && !grids) sdf_pairs_kernel<true, false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
-    if (m.max_ind == 1 && grids) sdf_pairs_kernel<true, true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
+    if (m.max_ind == 1) {  // cull by threads, evaluate by warps (m.ntask is zeroed with the other per-step counters)
+      const unsigned gc = (unsigned)((pairs + kCullThreads - 1) / kCullThreads), ge = (unsigned)((pairs + kEvalWarps - 1) / kEvalWarps);
+      if (grids) sdf_cull_kernel<true><<<gc, kCullThreads, 0, s>>>(m, io, s1_flags), sdf_eval_kernel<true><<<ge, kEvalWarps * 32, 0, s>>>(m, io, s1_flags);
+      else sdf_cull_kernel<false><<<gc, kCullThreads, 0, s>>>(m, io, s1_flags), sdf_eval_kernel<false><<<ge, kEvalWarps * 32, 0, s>>>(m, io, s1_flags);
+      *launches = 2;
+      return cudaGetLastError();
+    }
     if (m.max_ind != 1 && !grids) sdf_pairs_kernel<false, false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
     if (m.max_ind != 1 && grids) sdf_pairs_kernel<false, true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
     return cudaGetLastError();

@@ -52,7 +52,7 @@ def test_config3_sparse_paths():
     _report("cfg3 sparse fp32", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="cfg3-sparse"))
     wl = W.config3(2, 97)          # several env tiles per patch + a ragged one
     gpu = run_gpu(wl, path=T.ETAC_PATH_SPARSE)
-    assert gpu["path"] == T.ETAC_PATH_SPARSE and gpu["launches"] == 2
+    assert gpu["path"] == T.ETAC_PATH_SPARSE and gpu["launches"] == 3      # S1 (cull, evaluate), fused
     _report("cfg3 sparse bf16", compare(gpu, run_oracle(wl), TOL["bf16"], resid_tol=5e-2, label="cfg3-sparse16"))
 
 
@@ -290,7 +290,7 @@ def test_pointnet_residual_bf16(n_envs, path):
     import dataclasses
     wl = dataclasses.replace(W.config3(4, n_envs), weights=W.make_pointnet_weights(3, 1, std=0.15))
     gpu, ref = run_gpu(wl, path=path), run_oracle(wl)
-    assert gpu["launches"] == 4                      # S1, encode + pool, global MLP, decode
+    assert gpu["launches"] == 5                      # S1 (cull, evaluate), encode + pool, global MLP, decode
     st = compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="pointnet")
     _report(f"pointnet E={n_envs}", st)
     # the global feature matters: with g' removed (per-node part only) the residual is different
