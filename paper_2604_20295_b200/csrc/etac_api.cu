@@ -173,7 +173,8 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   const bool bf16 = ctx->precision == ETAC_PREC_BF16;
   const bool gather16 = bf16 && path == ETAC_PATH_SPARSE;
   const int abl = ctx->m.ablation;
-  const int s1_flags = abl == ETAC_ABLATE_NO_PROPAGATION ? 0 : !bf16 ? kS1FillOut : (gather16 ? kS1WriteAlist : kS1WriteUhat);
+  int s1_flags = abl == ETAC_ABLATE_NO_PROPAGATION ? 0 : !bf16 ? kS1FillOut : (gather16 ? kS1WriteAlist : kS1WriteUhat);
+  if ((s1_flags & kS1WriteUhat) && ctx->m.khist && fused_uses_big_tile(ctx->m, a->n_envs)) s1_flags |= kS1Bucket;
   if (gather16 && !ctx->m.alist) return fail(ctx, ETAC_ERR_INVALID_ARG, "select ETAC_PATH_SPARSE with etac_set_option first");
   int n_s1 = 1;
   if ((e = launch_sdf(ctx->m, io, s1_flags, &n_s1, s)) != cudaSuccess)
@@ -502,6 +503,14 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   if (d->precision == ETAC_PREC_BF16) {
     if (!fused_fits(P)) return bail(ETAC_ERR_UNSUPPORTED, "too many patches for the shared-memory tables of the tensor-core path");
     CK(dev_alloc(c, &m.uhat_t, urows * m.ldu, true), "alloc uhat");
+    CK(dev_alloc(c, &m.kbmap, (size_t)P * ((size_t)(d->max_envs + kMaxTE - 1) / kMaxTE * kMaxTE) * kKbWords, true), "alloc k-block bitmaps");
+    m.kbtile_stride = (d->max_envs + kMaxTE - 1) / kMaxTE;
+    CK(dev_alloc(c, &m.kbtile, (size_t)P * m.kbtile_stride * kKbWords, true), "alloc tile k-block masks");
+    if (P <= 64 && max_np >= 1024) {  // bucketing of the environments by contact position (large patches)
+      CK(dev_alloc(c, &m.khist, (size_t)P * 512, true), "alloc bucket histogram");
+      m.kcursor = m.khist + (size_t)P * 256;
+      CK(dev_alloc(c, &m.keybuf, (size_t)P * d->max_envs, true), "alloc bucket keys");
+    }
     std::string why;
     if (!make_tmap(&c->tmA, m.k16, (uint64_t)N, (uint64_t)m.kw, (uint64_t)m.kw, 128, &why) ||
         !make_tmap(&c->tmB16, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 48, &why) ||

@@ -37,6 +37,9 @@ constexpr int kGatherChunk = 128;
 // tensor-core path tiling: environments per work item (16, or 32 for large patches); the U^ operand and the
 // active lists are sized for whole tiles of the larger one
 constexpr int kMaxTE = 32;
+// Block-sparse contraction: S1 records, per contacting (patch, slot), which 64-node k-blocks of the patch hold an
+// active node (kKbWords x 32 bits; k-blocks beyond that are always contracted)
+constexpr int kKbWords = 8;
 
 // Shared-memory image of the MLP weights for the tensor-core path (bf16, UMMA K-major
 // SWIZZLE_NONE core-matrix layout; see k_fused.cu).
@@ -56,7 +59,7 @@ struct __align__(16) ActiveEntry {
 };
 
 // what S1 writes besides delta / flags / env lists
-enum : int { kS1WriteUhat = 1, kS1WriteAlist = 2, kS1FillOut = 4 };
+enum : int { kS1WriteUhat = 1, kS1WriteAlist = 2, kS1FillOut = 4, kS1Bucket = 8 };
 
 // Sampled SDF of an object (ETAC_IND_GRID): values[(iz*ny + iy)*nx + ix] at origin + h*(ix, iy, iz).
 constexpr int kMaxGrids = 8;
@@ -100,6 +103,14 @@ struct DevModel {
   int32_t* count;             // [P] contacting envs per patch (this step)
   int32_t* envlist;           // [P x max_envs]
   uint8_t* flags;             // [max_envs x P]
+  uint32_t* kbmap;            // [P x max_envs x kKbWords] active k-block bitmaps of the contacting pairs (bf16 contexts)
+  uint32_t* kbtile;           // [P x kbtile_stride x kKbWords] union of the bitmaps per tile of 32 slots (kbtile_kernel)
+  int32_t kbtile_stride;      // tiles per patch in kbtile
+  // S1 bucketing of the contacting environments of a large patch by the position of their contact (first active
+  // k-block), so that the environments of a tile share their active k-blocks: counting sort
+  int32_t* khist;             // [P x 256] environments per key (zeroed per step), NULL = no bucketing on this context
+  int32_t* kcursor;           // [P x 256] running rank inside a key (zeroed per step)
+  uint8_t* keybuf;            // [max_envs x P] key of every contacting pair
   struct PairTask* tasks;     // [max_envs x P] S1 task list of the cull / evaluate kernel pair (many patches, one indenter)
   int32_t* ntask;             // [1], behind count[P] (zeroed with it)
   GridDesc grid[kMaxGrids];   // sampled-SDF objects (etac_set_sdf_grid)

@@ -186,6 +186,54 @@ __device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, in
   return true;
 }
 
+// Block-sparse contraction (Omega is (n - m) x m, not n x n): a k-block of 64 nodes in which none of
+// the item's environments has an active node contributes exact zeros to the accumulator and is skipped by the
+// TMA and MMA warps alike (large patches only: the kGrouped instantiation).  S1 wrote one bitmap per contacting
+// (patch, slot), kbtile_kernel ORs them per tile of TE slots, and the two warps read their item's 8 words one item
+// ahead, so that the load is never waited for.
+template <int TE>
+__global__ void __launch_bounds__(32) kbtile_kernel(DevModel m) {
+  const int p = blockIdx.y, tile = blockIdx.x, lane = threadIdx.x;
+  const int cnt = min(TE, m.count[p] - tile * TE);
+  if (cnt <= 0) return;
+  const uint32_t* __restrict__ b = m.kbmap + ((int64_t)p * m.max_envs + tile * TE) * kKbWords + (lane & (kKbWords - 1));
+  uint32_t v = 0;
+#pragma unroll
+  for (int s0 = 0; s0 < TE; s0 += 32 / kKbWords) {
+    const int sidx = s0 + lane / kKbWords;
+    if (sidx < cnt) v |= b[sidx * kKbWords];
+  }
+#pragma unroll
+  for (int d = kKbWords; d < 32; d <<= 1) v |= __shfl_xor_sync(0xffffffffu, v, d);
+  if (lane < kKbWords) m.kbtile[((int64_t)p * m.kbtile_stride + tile) * kKbWords + lane] = v;
+}
+__device__ __forceinline__ uint32_t load_tile_kbmask(const DevModel& m, const Item& it, int lane) {
+  return lane < kKbWords ? __ldg(m.kbtile + ((int64_t)it.p * m.kbtile_stride + it.tile) * kKbWords + lane) : 0u;
+}
+
+// Walks the active k-blocks of an item in ascending order: next() returns the next k-block index or -1.  All lanes
+// hold the same state (the words come from the lanes' union by shuffle); k-blocks beyond the bitmap are all active.
+struct KbIter {
+  uint32_t lane_word, bits;
+  int word, nkb, tail;
+  __device__ __forceinline__ void init(uint32_t mask_lane, int nkb_) {
+    lane_word = mask_lane, nkb = nkb_, word = 0, tail = 32 * kKbWords;
+    bits = __shfl_sync(0xffffffffu, lane_word, 0);
+  }
+  __device__ __forceinline__ int next() {
+    while (word < kKbWords) {
+      if (bits) {
+        const int kb = word * 32 + __ffs(bits) - 1;
+        bits &= bits - 1;
+        if (kb < nkb) return kb;
+        bits = 0;
+      }
+      if (++word < kKbWords) bits = __shfl_sync(0xffffffffu, lane_word, word);
+    }
+    return tail < nkb ? tail++ : -1;
+  }
+};
+
 // kGather: the propagation is not the dense tensor-core contraction but Omega U_a literally
 // (PAPER.md:L87): every epilogue thread sums K[i][j] u^_j over the ACTIVE nodes j of its unit,
 // read from the compact lists S1 wrote (bf16 K row j, coalesced over i because K is symmetric;
@@ -273,10 +321,19 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     {
       int pcur = 0, stage = 0;
       uint32_t ph = 0;
-      Item it;
-      for (int w = blockIdx.x; decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it); w += gridDim.x) {
+      Item it, nx;
+      int w = blockIdx.x;
+      bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it);
+      uint32_t km = 0;
+      if constexpr (kGrouped) km = have ? load_tile_kbmask(m, it, lane) : 0u;
+      while (have) {
+        // the next item and (large patches) its k-block mask, requested before this item's k-blocks are streamed
+        const int wn = w + gridDim.x;
+        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, pcur, nx);
+        uint32_t kmn = 0;
+        if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
         const int nkb = (it.n + BK - 1) / BK;
-        for (int kb = 0; kb < nkb; ++kb) {
+        auto load_kb = [&](const int kb) {
           mbar_wait(&bars->empty[stage], ph ^ 1);
           if (elect_one()) {
             mbar_arrive_expect_tx(&bars->full[stage], A_STAGE + B_STAGE);
@@ -285,7 +342,15 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
           }
           __syncwarp();
           if (++stage == kStages) stage = 0, ph ^= 1;
+        };
+        if constexpr (kGrouped) {
+          KbIter ki;
+          ki.init(km, nkb);
+          for (int kb = ki.next(); kb >= 0; kb = ki.next()) load_kb(kb);
+        } else {
+          for (int kb = 0; kb < nkb; ++kb) load_kb(kb);
         }
+        it = nx, km = kmn, have = have_n, w = wn;
       }
     }
   } else if (warp == 1) {
@@ -297,13 +362,22 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       constexpr uint32_t idesc_prop = make_idesc_bf16(BM, BN);
       int pcur = 0, stage = 0, k_item = 0;
       uint32_t ph = 0;
-      Item it;
-      for (int w = blockIdx.x; decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it); w += gridDim.x, ++k_item) {
+      Item it, nx;
+      int w = blockIdx.x;
+      bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it);
+      uint32_t km = 0;
+      if constexpr (kGrouped) km = have ? load_tile_kbmask(m, it, lane) : 0u;
+      while (have) {
+        const int wn = w + gridDim.x;
+        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, pcur, nx);
+        uint32_t kmn = 0;
+        if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
         const int nkb = (it.n + BK - 1) / BK;
         const int b = k_item & 1;
         mbar_wait(&bars->acc_empty[b], ((k_item >> 1) & 1) ^ 1);  // the epilogue has fetched item k_item - 2
         tc_fence_after();
-        for (int kb = 0; kb < nkb; ++kb) {
+        bool first = true;
+        auto mma_kb = [&](const bool last) {
           mbar_wait(&bars->full[stage], ph);
           tc_fence_after();
           const uint64_t dA = make_desc(smem_u32(sA + stage * A_STAGE), 16, 1024, kLayoutSw128);
@@ -311,13 +385,25 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
           if (elect_one()) {
 #pragma unroll
             for (int k = 0; k < BK / 16; ++k)
-              mma_ss(tmem + b * BN, dA + 2 * k, dB + 2 * k, idesc_prop, (kb | k) != 0);
+              mma_ss(tmem + b * BN, dA + 2 * k, dB + 2 * k, idesc_prop, (!first || k != 0) ? 1u : 0u);
             tc_commit(&bars->empty[stage]);
-            if (kb == nkb - 1) tc_commit(&bars->acc_full[b]);
+            if (last) tc_commit(&bars->acc_full[b]);
           }
           __syncwarp();
+          first = false;
           if (++stage == kStages) stage = 0, ph ^= 1;
+        };
+        if constexpr (kGrouped) {
+          KbIter ki;  // (every slot of an item is a contacting pair: at least one k-block is active)
+          ki.init(km, nkb);
+          for (int kb = ki.next(), kb_next; kb >= 0; kb = kb_next) {
+            kb_next = ki.next();
+            mma_kb(kb_next < 0);
+          }
+        } else {
+          for (int kb = 0; kb < nkb; ++kb) mma_kb(kb == nkb - 1);
         }
+        it = nx, km = kmn, have = have_n, w = wn, ++k_item;
       }
     }
   } else if (warp < 4) {
@@ -716,6 +802,7 @@ static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& t
     if (io.out_bf16) fused_mlp_kernel<kMode, true, true, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
     else fused_mlp_kernel<kMode, true, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
   } else if (big) {
+    kbtile_kernel<32><<<dim3((unsigned)((io.n_envs + 31) / 32), (unsigned)m.n_patches), 32, 0, s>>>(m);
     if (io.out_bf16) fused_mlp_kernel<kMode, false, true, true, 32><<<grid, T32, smem32, s>>>(m, io, tmA, tmB32);
     else fused_mlp_kernel<kMode, false, false, true, 32><<<grid, T32, smem32, s>>>(m, io, tmA, tmB32);
   } else {
@@ -728,7 +815,8 @@ static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& t
 cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB16,
                               const CUtensorMap& tmB32, int n_sm, bool gather, int* launches, cudaStream_t s) {
   const int grid = n_sm;
-  *launches = 1;
+  const int n_big = (!gather && fused_uses_big_tile(m, io.n_envs)) ? 1 : 0;  // + kbtile_kernel
+  *launches = 1 + n_big;
   if (m.resid == ETAC_RESID_NONE) {
     launch_one<kModeNone>(m, io, tmA, tmB16, tmB32, grid, gather, s);
   } else if (m.resid == ETAC_RESID_PERNODE_MLP) {
@@ -739,7 +827,7 @@ cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtenso
     launch_one<kModePnEncode>(m, io, tmA, tmB16, tmB32, grid, false, s);
     pn_global_kernel<<<dim3((unsigned)((io.n_envs + kPnSlots - 1) / kPnSlots), (unsigned)m.n_patches), 64, 0, s>>>(m);
     launch_one<kModePnDecode>(m, io, tmA, tmB16, tmB32, grid, gather, s);
-    *launches = 3;
+    *launches = 3 + n_big;
   }
   return cudaGetLastError();
 }

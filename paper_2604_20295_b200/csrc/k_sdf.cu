@@ -185,14 +185,19 @@ struct SPose {
 //      U^ operand rows (bf16), optional delta / mask outputs
 template <bool kIndenters, bool kGrid>
 __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int s1_flags) {
-  const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
+  // kS1Bucket: the slot of a contacting pair and its U^ rows are left to sdf_scatter_kernel (counting sort of the
+  // environments by contact position); this kernel records the key and counts the environments per key
+  const bool bucket = s1_flags & kS1Bucket;
+  const bool write_uhat = (s1_flags & kS1WriteUhat) && !bucket, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
   __shared__ int s_wcnt[8];
+  __shared__ int s_key[kPoseChunk];  // first active node of the patch
   extern __shared__ uint8_t smem_raw[];
   SInd* sind = reinterpret_cast<SInd*>(smem_raw);
   __shared__ SPose s_pose[kPoseChunk];
   __shared__ int s_any[kPoseChunk];
   __shared__ int s_slot[kPoseChunk];
   __shared__ int s_off[kPoseChunk + 1];  // node offsets of the chunk's patches (+ end)
+  __shared__ uint32_t s_kb[kKbWords];
 
   const int e = blockIdx.x;
   const int lane = threadIdx.x & 31;
@@ -210,6 +215,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
     if ((int)threadIdx.x < np) {
       const int p = p0 + threadIdx.x;
       s_any[threadIdx.x] = 0;
+      s_key[threadIdx.x] = 0x7fffffff;
       {
         const PatchInfo pi0 = m.patch[p];
         s_off[threadIdx.x] = pi0.off;
@@ -247,7 +253,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       const int64_t row0 = (int64_t)e * m.n_nodes + pi.off;
       float* delta = m.delta + row0;
       bool any = false;
-      int nact = 0;
+      int nact = 0, first_act = 0x7fffffff;
       if constexpr (kIndenters) {
         const SPose& sp = s_pose[q];
         // kNodeChunk nodes per thread at a time with the indenter loop outside: an indenter's 17 words are
@@ -281,6 +287,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
               delta[i] = d;
               any |= d > 0.0f;
               nact += d > 0.0f;
+              if (d > 0.0f) first_act = min(first_act, i);
             }
           }
         }
@@ -290,9 +297,14 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           delta[i] = d;
           any |= d > 0.0f;
           nact += d > 0.0f;
+          if (d > 0.0f) first_act = min(first_act, i);
         }
       }
       if (__any_sync(0xffffffffu, any) && lane == 0) atomicOr(&s_any[q], 1);
+      if (bucket) {
+        first_act = __reduce_min_sync(0xffffffffu, first_act);
+        if (lane == 0 && first_act != 0x7fffffff) atomicMin(&s_key[q], first_act);
+      }
       if (io.nact_out) {
         nact = __reduce_add_sync(0xffffffffu, nact);
         if (lane == 0 && nact) atomicAdd(&io.nact_out[e], nact);
@@ -305,7 +317,13 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
       const int hit = s_any[threadIdx.x];
       m.flags[(int64_t)e * m.n_patches + p] = (uint8_t)hit;
       if (io.contact_out) io.contact_out[(int64_t)e * m.n_patches + p] = (uint8_t)hit;
-      if (hit) {
+      if (hit && bucket) {
+        const int n_p = s_off[threadIdx.x + 1] - s_off[threadIdx.x];
+        const int key = (int)(((int64_t)s_key[threadIdx.x] << 8) / n_p);  // 0..255: position of the first active node
+        m.keybuf[(int64_t)e * m.n_patches + p] = (uint8_t)key;
+        atomicAdd(&m.khist[p * 256 + key], 1);
+        s_slot[threadIdx.x] = 0;
+      } else if (hit) {
         const int slot = atomicAdd(&m.count[p], 1);
         m.envlist[(int64_t)p * m.max_envs + slot] = e;
         s_slot[threadIdx.x] = slot;
@@ -361,6 +379,10 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
         }
         if (threadIdx.x == 0) m.acount[(int64_t)(p0 + q) * m.max_envs + slot] = base;
       }
+      if (write_uhat) {  // bitmap of the 64-node k-blocks that hold an active node (the contraction skips the others)
+        if (threadIdx.x < kKbWords) s_kb[threadIdx.x] = 0;
+        __syncthreads();
+      }
       for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const float d = delta[i];
         if (io.pen_out) io.pen_out[row0 + i] = d;
@@ -374,7 +396,13 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
           u[0] = __float2bfloat16_rn(-d * nn.x);
           u[m.ldu] = __float2bfloat16_rn(-d * nn.y);
           u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * nn.z);
+          const int kb = i >> 6;
+          if (d > 0.0f && kb < 32 * kKbWords) atomicOr(&s_kb[kb >> 5], 1u << (kb & 31));
         }
+      }
+      if (write_uhat) {
+        __syncthreads();
+        if (threadIdx.x < kKbWords) m.kbmap[((int64_t)(p0 + q) * m.max_envs + slot) * kKbWords + threadIdx.x] = s_kb[threadIdx.x];
       }
     }
   }
@@ -480,6 +508,7 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       }
       if (lane == 0) m.acount[(int64_t)p * m.max_envs + slot] = base;
     }
+    uint32_t kb0 = 0;  // bitmap of the 64-node k-blocks with an active node (n <= 2048: one word)
 #pragma unroll 2
     for (int i = lane; i < n; i += 32) {
       const float d = delta[i];  // written by this thread above
@@ -494,7 +523,12 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
         u[0] = __float2bfloat16_rn(-d * nn.x);
         u[m.ldu] = __float2bfloat16_rn(-d * nn.y);
         u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * nn.z);
+        if (d > 0.0f) kb0 |= 1u << ((i >> 6) & 31);
       }
+    }
+    if (write_uhat) {
+      kb0 = __reduce_or_sync(0xffffffffu, kb0);
+      if (lane < kKbWords) m.kbmap[((int64_t)p * m.max_envs + slot) * kKbWords + lane] = lane == 0 ? kb0 : 0u;
     }
   } else {
     // contact-free pair: optional outputs are zero; for the fp32 gather kernel the output rows too
@@ -643,6 +677,7 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel 
     __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off;
     const bool vec = ((off | m.ldu) & 7) == 0 && ((row0 & 3) == 0);  // 16-byte aligned groups (else node by node)
     __syncwarp();  // the lanes read delta values that other lanes of the warp wrote
+    uint32_t kb0 = 0;  // bitmap of the 64-node k-blocks with an active node (n <= 2048: one word)
     if (write_uhat && vec) {
       for (int i0 = lane * 8; i0 < n; i0 += 256) {
         float d[8];
@@ -657,6 +692,7 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel 
         bool some = false;
 #pragma unroll
         for (int c = 0; c < 8; ++c) some |= d[c] > 0.0f;
+        if (some) kb0 |= 1u << ((i0 >> 6) & 31);
         if (some) {
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
@@ -695,8 +731,13 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel 
           u0[i] = __float2bfloat16_rn(-d * nn.x);
           u0[m.ldu + i] = __float2bfloat16_rn(-d * nn.y);
           u0[2 * (int64_t)m.ldu + i] = __float2bfloat16_rn(-d * nn.z);
+          if (d > 0.0f) kb0 |= 1u << ((i >> 6) & 31);
         }
       }
+    }
+    if (write_uhat) {
+      kb0 = __reduce_or_sync(0xffffffffu, kb0);
+      if (lane < kKbWords) m.kbmap[((int64_t)p * m.max_envs + slot) * kKbWords + lane] = lane == 0 ? kb0 : 0u;
     }
   } else {
     // contact-free pair: optional outputs are zero; for the fp32 gather kernel the output rows too
@@ -708,6 +749,94 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel 
     }
     if (io.pen_out)
       for (int i = lane; i < n; i += 32) io.pen_out[row0 + i] = 0.0f;
+  }
+}
+
+// Second half of S1 with bucketing (kS1Bucket, large patches): one CTA per environment.  The slot of a contacting
+// (env, patch) in the patch's environment list is its position in the counting sort by key (position of the first
+// active node): environments of one tile of the contraction then share most of their active k-blocks, and the
+// others are skipped (k_fused.cu).  Writes the list entry, the U^ operand rows and the k-block bitmap from delta.
+__global__ void __launch_bounds__(256) sdf_scatter_kernel(DevModel m, StepIO io) {
+  __shared__ int s_part[2][8];
+  __shared__ int s_slot;
+  __shared__ uint32_t s_kb[kKbWords];
+  const int e = blockIdx.x, t = threadIdx.x, lane = t & 31;
+  for (int p = 0; p < m.n_patches; ++p) {
+    if (!m.flags[(int64_t)e * m.n_patches + p]) continue;  // (uniform over the CTA)
+    const int key = m.keybuf[(int64_t)e * m.n_patches + p];
+    const int h = m.khist[p * 256 + t];
+    int below = __reduce_add_sync(0xffffffffu, t < key ? h : 0), total = __reduce_add_sync(0xffffffffu, h);
+    __syncthreads();  // previous patch done with the shared words
+    if (lane == 0) s_part[0][t >> 5] = below, s_part[1][t >> 5] = total;
+    if (t < kKbWords) s_kb[t] = 0;
+    __syncthreads();
+    if (t == 0) {
+      below = 0, total = 0;
+      for (int w = 0; w < 8; ++w) below += s_part[0][w], total += s_part[1][w];
+      const int slot = below + atomicAdd(&m.kcursor[p * 256 + key], 1);
+      m.envlist[(int64_t)p * m.max_envs + slot] = e;
+      m.count[p] = total;  // (every contacting environment writes the same value)
+      s_slot = slot;
+    }
+    __syncthreads();
+    const int slot = s_slot;
+    const PatchInfo pi = m.patch[p];
+    const int off = pi.off, n = pi.n;
+    const int64_t row0 = (int64_t)e * m.n_nodes + off;
+    const float* __restrict__ delta = m.delta + row0;
+    __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off;
+    const bool vec = ((off | m.ldu) & 7) == 0 && ((row0 & 3) == 0);  // 16-byte aligned groups of eight nodes
+    if (vec) {
+      for (int i0 = t * 8; i0 < n; i0 += 2048) {
+        float d[8];
+        if (i0 + 8 <= n) {
+          const float4 a = *reinterpret_cast<const float4*>(delta + i0), b = *reinterpret_cast<const float4*>(delta + i0 + 4);
+          d[0] = a.x, d[1] = a.y, d[2] = a.z, d[3] = a.w, d[4] = b.x, d[5] = b.y, d[6] = b.z, d[7] = b.w;
+        } else {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) d[c] = i0 + c < n ? delta[i0 + c] : 0.0f;
+        }
+        uint32_t w[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
+        bool some = false;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) some |= d[c] > 0.0f;
+        if (some) {
+          const int kb = i0 >> 6;
+          if (kb < 32 * kKbWords) atomicOr(&s_kb[kb >> 5], 1u << (kb & 31));
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            if (d[c] > 0.0f) {
+              const float4 nn = m.nrm4[off + i0 + c];
+              const uint32_t sh = (c & 1) * 16;
+              w[0][c >> 1] |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(-d[c] * nn.x)) << sh;
+              w[1][c >> 1] |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(-d[c] * nn.y)) << sh;
+              w[2][c >> 1] |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(-d[c] * nn.z)) << sh;
+            }
+          }
+        }
+        if (i0 + 8 <= n) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
+            *reinterpret_cast<uint4*>(u0 + (int64_t)c * m.ldu + i0) = make_uint4(w[c][0], w[c][1], w[c][2], w[c][3]);
+        } else {
+          for (int c = 0; i0 + c < n; ++c)
+            for (int a = 0; a < 3; ++a)
+              u0[(int64_t)a * m.ldu + i0 + c] = __ushort_as_bfloat16((unsigned short)(w[a][c >> 1] >> ((c & 1) * 16)));
+        }
+      }
+    } else {
+      for (int i = t; i < n; i += 256) {
+        const float d = delta[i];
+        const float4 nn = m.nrm4[off + i];
+        u0[i] = __float2bfloat16_rn(-d * nn.x);
+        u0[m.ldu + i] = __float2bfloat16_rn(-d * nn.y);
+        u0[2 * (int64_t)m.ldu + i] = __float2bfloat16_rn(-d * nn.z);
+        const int kb = i >> 6;
+        if (d > 0.0f && kb < 32 * kKbWords) atomicOr(&s_kb[kb >> 5], 1u << (kb & 31));
+      }
+    }
+    __syncthreads();
+    if (t < kKbWords) m.kbmap[((int64_t)p * m.max_envs + slot) * kKbWords + t] = s_kb[t];
   }
 }
 
@@ -736,13 +865,15 @@ cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_
   return cudaGetLastError();
 }
 
-cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* launches, cudaStream_t s) {
+cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags_in, int* launches, cudaStream_t s) {
+  int s1_flags = s1_flags_in;
   *launches = 1;
   const unsigned grid = (unsigned)io.n_envs;
   bool grids = false;  // the sampled-SDF code is only in the variants launched once a grid is registered
   for (int k = 0; k < kMaxGrids; ++k) grids |= m.grid[k].v != nullptr;
   // many small patches with indenters: one warp per (env, patch) pair; otherwise one CTA per environment
   if (io.input_mode == ETAC_IN_INDENTERS && m.max_ind >= 1 && m.n_patches >= 4 && m.max_patch_nodes <= 2048) {
+    s1_flags &= ~kS1Bucket;  // (slots are taken in arrival order by the pair kernels)
     const int64_t pairs = (int64_t)io.n_envs * m.n_patches;
     const unsigned pgrid = (unsigned)((pairs + kPairWarps - 1) / kPairWarps);
     const size_t smem = m.max_ind == 1 ? 0 : sizeof(SInd) * (size_t)m.max_ind * kPairWarps;
@@ -757,12 +888,20 @@ cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* l
     if (m.max_ind != 1 && grids) sdf_pairs_kernel<false, true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
     return cudaGetLastError();
   }
+  if (s1_flags & kS1Bucket) {
+    cudaError_t e = cudaMemsetAsync(m.khist, 0, sizeof(int32_t) * 512 * (size_t)m.n_patches, s);  // histogram + cursors
+    if (e != cudaSuccess) return e;
+  }
   if (io.input_mode == ETAC_IN_INDENTERS) {
     const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
     if (grids) sdf_penetration_kernel<true, true><<<grid, 256, smem, s>>>(m, io, s1_flags);
     else sdf_penetration_kernel<true, false><<<grid, 256, smem, s>>>(m, io, s1_flags);
   } else {
     sdf_penetration_kernel<false, false><<<grid, 256, 0, s>>>(m, io, s1_flags);
+  }
+  if (s1_flags & kS1Bucket) {
+    sdf_scatter_kernel<<<grid, 256, 0, s>>>(m, io);
+    *launches = 2;
   }
   return cudaGetLastError();
 }

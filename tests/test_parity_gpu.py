@@ -699,7 +699,7 @@ def test_big_patch_instantiation_pointnet_and_linear_only(out_bf16):
     ref = run_oracle(wl)
     if not out_bf16:
         gpu = run_gpu(wl)
-        assert gpu["launches"] == 4
+        assert gpu["launches"] == 6      # S1 (evaluate, bucket scatter), encode + pool, global MLP, tile k-block masks, decode
         _report("big-patch pointnet", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="big-pointnet", delta_tol=1e-4))
         lin, ref_lin = run_gpu(base, resid=False), run_oracle(base, resid=False)
         _report("big-patch linear", compare(lin, ref_lin, TOL["bf16"], label="big-linear", delta_tol=1e-4))
@@ -789,3 +789,35 @@ def test_residual_only_without_a_residual_network_is_zero_on_passive_rows():
             eng.close()
         assert np.all(U[~ref["mask"]] == 0), precision
         np.testing.assert_allclose(U[ref["mask"]], ref["U"][ref["mask"]], rtol=0, atol=2e-5)
+
+
+@pytest.mark.parametrize("pattern", ["disjoint", "clustered", "spread"])
+def test_block_sparse_contraction_on_a_large_patch(pattern):
+    """Large patches take the block-sparse form of the dense contraction (Omega is (n-m) x m): S1
+    records which 64-node k-blocks hold an active node, buckets the environments by contact position, and the
+    TMA / MMA warps skip the k-blocks no environment of a 32-env tile touches.  Penetration input on a 64 x 64 pad
+    (N = 4096, 64 k-blocks), 77 environments = three tiles, the last ragged: "disjoint" = every environment touches
+    ONE k-block of its own (no two environments of a tile share one: the union has as many blocks as the tile has
+    environments), "clustered" = all contacts inside four neighbouring k-blocks (almost everything is skipped),
+    "spread" = nodes in contact all over the pad (nothing can be skipped).  Against the oracle on every env."""
+    mesh = W.assemble([W.flat_pad(64, 64, 1.0)])
+    E, N = 77, mesh.n_nodes
+    rng = np.random.default_rng({"disjoint": 1, "clustered": 2, "spread": 3}[pattern])
+    pen = np.zeros((E, N), np.float32)
+    for e in range(E):
+        if pattern == "disjoint":
+            blk = (e * 29) % 64
+            idx = blk * 64 + rng.choice(64, size=rng.integers(1, 9), replace=False)
+        elif pattern == "clustered":
+            idx = 20 * 64 + rng.choice(256, size=rng.integers(3, 40), replace=False)
+        else:
+            idx = rng.choice(N, size=rng.integers(30, 300), replace=False)
+        pen[e, idx] = rng.uniform(0.05, 1.0, len(idx))
+    pen[5] = 0.0                                    # an environment without contact in the middle of a tile
+    wl = W.Workload("block_sparse", mesh, np.float32([0.5]), W.make_weights(8, 3, std=0.1), E, 0,
+                    np.zeros((E, 0), dtype=W.INDENTER_DTYPE), None, "bf16")
+    ref = run_oracle(wl, penetration=pen)
+    gpu = run_gpu(wl, penetration=pen)
+    assert gpu["path"] == T.ETAC_PATH_DENSE and gpu["pairs"] == E - 1
+    _report(f"block-sparse {pattern}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="block-sparse"))
+    assert np.all(gpu["U"][5] == 0)
