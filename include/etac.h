@@ -149,12 +149,17 @@ etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* ar
 /* Options / introspection. */
 enum { ETAC_OPT_PATH = 1, ETAC_OPT_ABLATION = 2, ETAC_OPT_L2_GROUP_BYTES = 3 };
 enum { ETAC_PATH_AUTO = 0, ETAC_PATH_DENSE = 1, ETAC_PATH_SPARSE = 2 };
-/* DENSE : tcgen05 tensor-core contraction K_p . U^ (needs ETAC_PREC_BF16);
+/* DENSE : tcgen05 tensor-core contraction K_p . U^ (needs ETAC_PREC_BF16).  For patches of >= 2048 nodes (or when
+ *         the U^ operand of a patch exceeds ETAC_OPT_L2_GROUP_BYTES) it is block-sparse: S1 records which 64-node
+ *         k-blocks of a contacting (env, patch) hold an active node and sorts the environments of a patch by the
+ *         position of their contact, and the contraction skips the k-blocks that no environment of a 32-env tile
+ *         touches (Omega is (n-m) x m).  Skipped blocks contribute exact zeros: same result;
  * SPARSE: gather over the active nodes only (Omega U_a literally).  FP32 context: fp32 SIMT kernel,
  *         fp32 MLP.  BF16 context: bf16 K, fp32 u^ and accumulation, tensor-core MLP as in DENSE;
  *         selecting it allocates the active-node lists (16 bytes x max_envs x N), which is why the
  *         choice is made with etac_set_option and never inside etac_step;
- * AUTO  : DENSE for BF16 contexts, SPARSE for FP32 contexts. */
+ * AUTO  : DENSE for BF16 contexts, SPARSE for FP32 contexts.  (On a BF16 context the block-sparse DENSE form is
+ *         faster than SPARSE at every contact fraction measured, 0.1 % .. 20 %, N = 256 .. 8192: BASELINE.md §4.) */
 /* ETAC_OPT_ABLATION: the rows of Table II as run-time modes.  FULL (default):
  * U_p = M_p (Omega U_a + Phi_p) + active part.  RESIDUAL_ONLY: Phi_p without the linear term ("Residual
  * Network Only").  LINEAR_ONLY: Omega U_a without Phi_p ("Linear Decay Only"; same result as a context

@@ -20,19 +20,24 @@
 // gives the control warps 24 registers and the epilogue warps the rest of the pool.
 //
 // NC units are in flight per SM (6 for the 16-env tile, 5 for the 32-env tile): the kernel is bound by the
-// special-function pipe (128 SiLUs per node-env), and a unit spends more time waiting for its tcgen05.mma
-// round trips (operand store -> barrier -> mma -> commit -> mbarrier -> TMEM load) than in its SiLUs, so the
+// special-function pipe (128 SiLUs per node-env), and a unit spends as much time in its two tcgen05.mma
+// round trips (operand store -> chain barrier -> mma -> commit -> mbarrier -> TMEM load) as in its SiLUs, so the
 // pipe only stays busy if enough independent units overlap.  A chain owns a 64-column D region of TMEM and
 // 20 KB of shared memory for its layer operands; the units of the CTA's item stream are dealt to the chains
-// round robin (unit q goes to chain q mod NC), independent of item boundaries.  The chain's own four warps
-// issue its MLP MMAs (named barrier over the chain's 128 threads, then one elected lane of its first
-// warp): there is no issuer warp in between.  The propagation accumulator is double-buffered, so the GEMM
-// of item k+1 runs under the MLP of item k.
+// round robin (unit q goes to chain q mod NC), independent of item boundaries.  The chain's own warps issue
+// its MLP MMAs: three warps arrive on the chain's named barrier and go on, the fourth (warp c % 4 of chain c)
+// waits on it and one of its lanes issues -- there is no issuer warp in between.  The next unit's layer 1 is
+// requested as soon as the last layer's D is in registers.  The propagation accumulator is double-buffered,
+// so the GEMM of item k+1 runs under the MLP of item k.
+//
+// Large patches (kGrouped, 32-env tile): the item order keeps the U^ tiles of a group of env tiles resident in
+// L2, and the contraction is block-sparse -- the TMA and MMA warps skip the 64-node k-blocks in which no
+// environment of the tile has an active node (S1 wrote the bitmaps and bucketed the environments by contact
+// position; Omega is (n - m) x m).
 //
 // Template variants (one source, see kMode / kGather / TE below): per-node MLP or none; the PointNet form
 // of Phi as an encoder pass with max-pool and a decoder pass; the gather form of the propagation
-// (Omega U_a over the active-node lists) instead of the dense contraction; and the 32-env tile with the
-// L2-grouped item order for large patches.
+// (Omega U_a over the active-node lists) instead of the dense contraction.
 //
 // TMEM columns (fp32 lanes = nodes): [0, BN) and [BN, 2 BN): u_lin accumulators, column 3*env+c;
 //                                    chain c at 2 BN + 64 c: D, the pre-activations of its current layer.

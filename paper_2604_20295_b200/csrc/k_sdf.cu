@@ -409,21 +409,22 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
 }
 
 // ---------------------------------------------------------------------------------------------
-// S1 for meshes of many small patches (dexterous hand): one WARP per (env, patch) pair.
-// All lanes build the patch rotation and do the conservative bounding-sphere cull against the
-// environment's indenters (warp-uniform, no divergence); a culled warp exits at once.  Otherwise
-// the warp evaluates the nodes -> phi, delta (workspace), warp vote -> contact flag; on contact
-// lane 0 takes a slot in the patch's compact environment list and the warp writes the U^ operand
-// rows.  No block barrier; the indenter lives in registers when there is one slot per environment.
+// S1 for meshes of many small patches with SEVERAL indenter slots per environment (self-contact: the other
+// links' shapes): one WARP per (env, patch) pair.  All lanes build the patch rotation and do the conservative
+// bounding-sphere cull against the environment's indenters (warp-uniform, no divergence; the indenters are
+// staged per warp in shared memory); a culled warp exits at once.  Otherwise the warp evaluates the nodes ->
+// phi, delta (workspace), warp vote -> contact flag; on contact lane 0 takes a slot in the patch's compact
+// environment list and the warp writes the U^ operand rows.  No block barrier.  (One slot per environment:
+// sdf_cull_kernel / sdf_eval_kernel below.)
 // Same single-rounded arithmetic in the same order as sdf_penetration_kernel.
 constexpr int kPairWarps = 2;
 
-template <bool kOne, bool kGrid>
+template <bool kGrid>
 __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel m, StepIO io, int s1_flags) {
   const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
   extern __shared__ uint8_t smem_raw[];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  SInd* sind = reinterpret_cast<SInd*>(smem_raw) + (size_t)wib * (kOne ? 0 : m.max_ind);  // per-warp staging (M > 1)
+  SInd* sind = reinterpret_cast<SInd*>(smem_raw) + (size_t)wib * m.max_ind;  // per-warp staging
   const int P = m.n_patches;
   const int64_t pair = (int64_t)blockIdx.x * kPairWarps + wib;
   if (pair >= (int64_t)io.n_envs * P) return;
@@ -442,17 +443,9 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
     quat_to_rot(q, R);
     to_world(R, t, pi.bc[0], pi.bc[1], pi.bc[2], C0, C1, C2);
   }
-  SInd one;
-  float phi_lo;
-  if constexpr (kOne) {
-    one = load_indenter(io.ind + e);
-    if (one.skip1 == p + 1) one.type = ETAC_IND_NONE;  // the shape of this patch's own link
-    phi_lo = union_sdf_lower<kGrid>(&one, 1, C0, C1, C2, pi.brad, m.grid, p + 1);
-  } else {
-    for (int k = lane; k < m.max_ind; k += 32) sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
-    __syncwarp();
-    phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
-  }
+  for (int k = lane; k < m.max_ind; k += 32) sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
+  __syncwarp();
+  const float phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
   // conservative cull: phi(x_i) >= phi(c) - L * brad on the patch's bounding sphere
   // (phi_lo = +inf: no indenter applies to this patch -- all slots NONE, or only the patch's own link)
   const bool evaluated = phi_lo < __int_as_float(0x7f800000) && !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
@@ -465,9 +458,7 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       const float4 pos = m.pos4[off + i];
       float X0 = pos.x, X1 = pos.y, X2 = pos.z;
       if (posed) to_world(R, t, pos.x, pos.y, pos.z, X0, X1, X2);
-      float phi;
-      if constexpr (kOne) phi = fminf(__int_as_float(0x7f800000), sdf_one<kGrid>(one, X0, X1, X2, m.grid));
-      else phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid, p + 1);
+      const float phi = union_sdf<kGrid>(sind, m.max_ind, X0, X1, X2, m.grid, p + 1);
       const float d = phi < 0.0f ? -phi : 0.0f;
       delta[i] = d;
       any |= d > 0.0f;
@@ -884,8 +875,8 @@ cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags_in, int
       *launches = 2;
       return cudaGetLastError();
     }
-    if (m.max_ind != 1 && !grids) sdf_pairs_kernel<false, false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
-    if (m.max_ind != 1 && grids) sdf_pairs_kernel<false, true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
+    if (m.max_ind != 1 && !grids) sdf_pairs_kernel<false><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
+    if (m.max_ind != 1 && grids) sdf_pairs_kernel<true><<<pgrid, kPairWarps * 32, smem, s>>>(m, io, s1_flags);
     return cudaGetLastError();
   }
   if (s1_flags & kS1Bucket) {
