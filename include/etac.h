@@ -44,7 +44,7 @@ typedef enum {
   ETAC_OK = 0,
   ETAC_ERR_INVALID_ARG = 1, /* NULL / out-of-range / inconsistent argument; ctx unchanged */
   ETAC_ERR_UNSUPPORTED = 2, /* valid request this build cannot serve (e.g. ETAC_PATH_DENSE on an fp32 context,
-                               ETAC_RESID_POINTNET on an fp32 context, a device that is not sm_100) */
+                               etac_backward on a PointNet context, a device that is not sm_100) */
   ETAC_ERR_ALLOC = 3,       /* host or device allocation failed */
   ETAC_ERR_CUDA = 4,        /* a CUDA call failed; etac_last_error() has the CUDA message */
   ETAC_ERR_CAPACITY = 5     /* n_envs > max_envs */
@@ -67,7 +67,7 @@ typedef struct {
 } etac_indenter; /* 48 bytes */
 
 enum { ETAC_KERNEL_EXP_L2 = 0 };                                  /* Eq. (1): exp(-alpha*|p_j-p_i|_2) */
-enum { ETAC_RESID_NONE = 0, ETAC_RESID_PERNODE_MLP = 1, ETAC_RESID_POINTNET = 2 /* ETAC_PREC_BF16 contexts only */ };
+enum { ETAC_RESID_NONE = 0, ETAC_RESID_PERNODE_MLP = 1, ETAC_RESID_POINTNET = 2 };
 enum { ETAC_PREC_FP32 = 0, ETAC_PREC_BF16 = 1 };                  /* BF16: 16-bit tensor-core operands, fp32 accumulate */
 enum { ETAC_ACTIVE_PASSTHROUGH = 0, ETAC_ACTIVE_PROPAGATE = 1 };  /* PASSTHROUGH: active rows keep u^ (mask M_p, L99) */
 enum { ETAC_IN_INDENTERS = 0, ETAC_IN_PENETRATION = 1 };

@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libetac.so")
-SOURCES = ["etac_api.cu", "k_build.cu", "k_sdf.cu", "k_gather_fp32.cu", "k_fused.cu", "k_backward.cu", "k_peaks.cu"]
+SOURCES = ["etac_api.cu", "k_build.cu", "k_sdf.cu", "k_gather_fp32.cu", "k_pointnet_fp32.cu", "k_fused.cu", "k_backward.cu", "k_peaks.cu"]
 HEADERS = ["etac_internal.h", "sm100_prims.cuh", os.path.join("..", "..", "include", "etac.h"),
            os.path.join("..", "..", "include", "etac_bench.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -200,6 +200,10 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
       DevModel lin = ctx->m;
       lin.resid = ETAC_RESID_NONE;
       e = launch_gather_fp32(lin, io, s);
+    } else if (ctx->m.resid == ETAC_RESID_POINTNET) {
+      int n_launch = 1;
+      e = launch_pointnet_fp32(ctx->m, io, &n_launch, s);
+      ctx->last_launches += n_launch - 1;
     } else {
       e = launch_gather_fp32(ctx->m, io, s);
     }
@@ -303,7 +307,6 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   if (d->resid_arch != ETAC_RESID_NONE && d->resid_arch != ETAC_RESID_PERNODE_MLP && d->resid_arch != ETAC_RESID_POINTNET)
     return fail(nullptr, ETAC_ERR_INVALID_ARG, "bad resid_arch");
   if (d->resid_arch == ETAC_RESID_POINTNET) {
-    if (d->precision != ETAC_PREC_BF16) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "ETAC_RESID_POINTNET needs an ETAC_PREC_BF16 context");
     if (d->resid_hidden != kHidden) return fail(nullptr, ETAC_ERR_UNSUPPORTED, "only resid_hidden == 64 is built");
     if (!d->E1 || !d->e1 || !d->E2 || !d->e2 || !d->G1 || !d->g1 || !d->D1 || !d->d1 || !d->D2 || !d->d2)
       return fail(nullptr, ETAC_ERR_INVALID_ARG, "PointNet weights missing");
@@ -484,6 +487,15 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
     memcpy(pf.data() + 4096, d->g1, 64 * 4);
     memcpy(pf.data() + 4160 + 4096, d->d1, 64 * 4);
     CK(dev_upload(c, &m.pn_f32, pf.data(), pf.size()), "upload PointNet global MLP");
+    if (d->precision == ETAC_PREC_FP32) {  // fp32 SIMT form (k_pointnet_fp32.cu)
+      std::vector<float> w32;
+      w32.insert(w32.end(), d->E1, d->E1 + 576), w32.insert(w32.end(), d->e1, d->e1 + 64);
+      w32.insert(w32.end(), d->E2, d->E2 + 4096), w32.insert(w32.end(), d->e2, d->e2 + 64);
+      for (int n = 0; n < 64; ++n) w32.insert(w32.end(), d->D1 + n * 128, d->D1 + n * 128 + 64);
+      w32.insert(w32.end(), d->D2, d->D2 + 192), w32.insert(w32.end(), d->d2, d->d2 + 3);
+      CK(dev_upload(c, &m.pn_w32, w32.data(), w32.size()), "upload PointNet fp32 weights");
+      CK(pointnet_fp32_configure(), "cudaFuncSetAttribute(pn_decode_fp32_kernel)");
+    }
     CK(dev_alloc(c, &m.gmax, (size_t)64 * P * d->max_envs, true), "alloc gmax");
     CK(dev_alloc(c, &m.cvec, (size_t)64 * P * d->max_envs, true), "alloc cvec");
   }

@@ -94,6 +94,7 @@ struct DevModel {
   const uint8_t* wimg;        // kWImgBytes
   const uint8_t* wimg_pn;     // kPnImgBytes (ETAC_RESID_POINTNET)
   const float* pn_f32;        // G1^T [in][out] g1[64] D1[:,64:128]^T [in][out] d1[64] (fp32, pn_global_kernel)
+  const float* pn_w32;        // fp32 contexts: E1[64x9] e1 E2[64x64] e2 D1[:, :64] D2[3x64] d2 (k_pointnet_fp32.cu)
   uint32_t* gmax;             // [P x max_envs x 64] max-pooled encoder features as order-preserving keys
   float* cvec;                // [P x max_envs x 64] c_(e,p) / 2
   float wout[196];            // output layer of Phi in fp32: W3 (or D2) [3 x 64] row-major, then b3 (d2) at 192..194
@@ -177,6 +178,8 @@ cudaError_t launch_build_k(const DevModel& m, float* k32, __nv_bfloat16* k16, cu
 cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1, float* c1t, cudaStream_t s);
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* launches, cudaStream_t s);
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
+cudaError_t launch_pointnet_fp32(const DevModel& m, const StepIO& io, int* launches, cudaStream_t s);
+cudaError_t pointnet_fp32_configure();
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t backward_configure();
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,

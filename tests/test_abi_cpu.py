@@ -62,10 +62,6 @@ def test_create_validates_before_cuda(lib):
                       resid_arch=T.ETAC_RESID_POINTNET, precision=T.ETAC_PREC_BF16)
     assert ei.value.status == T.ETAC_ERR_INVALID_ARG and "PointNet" in str(ei.value)     # per-node weights only
     with pytest.raises(T.EtacError) as ei:
-        T.etac_create(m.pos, m.normal, [0.5], patch_offset=m.patch_offset, weights=W.make_pointnet_weights(1),
-                      precision=T.ETAC_PREC_FP32)
-    assert ei.value.status == T.ETAC_ERR_UNSUPPORTED                                     # bf16 contexts only
-    with pytest.raises(T.EtacError) as ei:
         T.etac_create(m.pos, m.normal, [0.5], patch_offset=m.patch_offset, max_envs=0)
     assert ei.value.status == T.ETAC_ERR_INVALID_ARG
     # an edge crossing a declared patch boundary is rejected

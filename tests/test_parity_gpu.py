@@ -297,6 +297,32 @@ def test_pointnet_residual_bf16(n_envs, path):
     assert float(np.abs(ref["U"] - ref["analytic"]).max()) > 1e-2 * float(np.abs(ref["U"]).max())
 
 
+@pytest.mark.parametrize("mesh_kind,n_envs", [("hand", 29), ("cap", 12)])
+def test_pointnet_residual_fp32(mesh_kind, n_envs):
+    """The paper's form of Phi on an fp32 context (k_pointnet_fp32.cu: fp32 SIMT, exact expf) at the fp32
+    tolerance, on the hand mesh (16 patches) and on a single cap; N(0, 0.15) weights so that the residual and its
+    global part matter; also its "Residual Network Only" and "Linear Decay Only" modes."""
+    import dataclasses
+    from oracle import etac_oracle as O
+    base = W.config3(4, n_envs) if mesh_kind == "hand" else W.config2(4, n_envs)
+    wl = dataclasses.replace(base, weights=W.make_pointnet_weights(3, 1, std=0.15))
+    gpu, ref = run_gpu(wl, precision="fp32"), run_oracle(wl)
+    assert gpu["launches"] == (5 if mesh_kind == "hand" else 4)     # S1 (hand: cull + evaluate), encode, global MLP, decode
+    _report(f"pointnet fp32 {mesh_kind}", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="pointnet-fp32"))
+    assert float(np.abs(ref["U"] - ref["analytic"]).max()) > 1e-2 * float(np.abs(ref["U"]).max())
+    for mode, code in (("residual_only", T.ETAC_ABLATE_RESIDUAL_ONLY), ("linear_only", T.ETAC_ABLATE_LINEAR_ONLY)):
+        m = O.model_from_workload(wl, resid_arch="pointnet")
+        m.ablation = mode
+        want = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)["U"]
+        eng = T.Etac(wl, precision="fp32")
+        try:
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_ABLATION, code)
+            U = eng.step(wl.n_envs, eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)).cpu().numpy()
+        finally:
+            eng.close()
+        assert np.abs(U - want).max() <= 1e-4 * np.abs(ref["U"]).max(), mode
+
+
 def test_two_contexts_on_two_streams_are_independent():
     """include/etac.h: one in-flight stream per ctx, different ctxs are independent, a step only
     enqueues.  Two contexts (different meshes, precisions) stepped alternately on two streams
