@@ -545,7 +545,7 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
 //                    patch's compact environment list, then the U^ operand rows / active list / optional outputs.
 //                    The grid is sized for the worst case (every pair a task); warps beyond the list exit at once.
 // Same single-rounded arithmetic in the same order as the other S1 kernels.
-constexpr int kCullThreads = 128, kEvalWarps = 2;
+constexpr int kCullThreads = 128, kEvalWarps = 4;
 
 template <bool kGrid>
 __global__ void __launch_bounds__(kCullThreads) sdf_cull_kernel(DevModel m, StepIO io, int s1_flags) {
@@ -593,7 +593,7 @@ __global__ void __launch_bounds__(kCullThreads) sdf_cull_kernel(DevModel m, Step
 }
 
 template <bool kGrid>
-__global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel m, StepIO io, int s1_flags) {
+__global__ void __launch_bounds__(kEvalWarps * 32, 8) sdf_eval_kernel(DevModel m, StepIO io, int s1_flags) {
   const bool write_uhat = s1_flags & kS1WriteUhat, write_alist = s1_flags & kS1WriteAlist, fill_out = s1_flags & kS1FillOut;
   const int lane = threadIdx.x & 31;
   const int k = blockIdx.x * kEvalWarps + (threadIdx.x >> 5);
@@ -671,20 +671,25 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel 
     uint32_t kb0 = 0;  // bitmap of the 64-node k-blocks with an active node (n <= 2048: one word)
     if (write_uhat && vec) {
       for (int i0 = lane * 8; i0 < n; i0 += 256) {
-        float d[8];
-        if (i0 + 8 <= n) {
-          const float4 a = *reinterpret_cast<const float4*>(delta + i0), b = *reinterpret_cast<const float4*>(delta + i0 + 4);
-          d[0] = a.x, d[1] = a.y, d[2] = a.z, d[3] = a.w, d[4] = b.x, d[5] = b.y, d[6] = b.z, d[7] = b.w;
-        } else {
-#pragma unroll
-          for (int c = 0; c < 8; ++c) d[c] = i0 + c < n ? delta[i0 + c] : 0.0f;
+        if (i0 + 8 > n) {  // ragged last group: node by node
+          for (int i = i0; i < n; ++i) {
+            const float dd = delta[i];
+            const float4 nn = m.nrm4[off + i];
+            u0[i] = __float2bfloat16_rn(-dd * nn.x);
+            u0[m.ldu + i] = __float2bfloat16_rn(-dd * nn.y);
+            u0[2 * (int64_t)m.ldu + i] = __float2bfloat16_rn(-dd * nn.z);
+            if (dd > 0.0f) kb0 |= 1u << ((i >> 6) & 31);
+          }
+          continue;
         }
+        const float4 da = *reinterpret_cast<const float4*>(delta + i0), db = *reinterpret_cast<const float4*>(delta + i0 + 4);
+        const float d[8] = {da.x, da.y, da.z, da.w, db.x, db.y, db.z, db.w};
         uint32_t w[3][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}, {0, 0, 0, 0}};
         bool some = false;
 #pragma unroll
         for (int c = 0; c < 8; ++c) some |= d[c] > 0.0f;
-        if (some) kb0 |= 1u << ((i0 >> 6) & 31);
         if (some) {
+          kb0 |= 1u << ((i0 >> 6) & 31);
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
             if (d[c] > 0.0f) {
@@ -696,17 +701,11 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 16) sdf_eval_kernel(DevModel 
             }
           }
         }
-        // (columns past the patch end inside the last group belong to the padding / the next patch's columns of
-        //  this slot row, which only that patch's own contacting environments ever write: do not touch them)
-        if (i0 + 8 <= n) {
+        // (columns past the patch end belong to the padding / the next patch's columns of this slot row, which
+        //  only that patch's own contacting environments ever write: whole groups inside the patch only)
 #pragma unroll
-          for (int c = 0; c < 3; ++c)
-            *reinterpret_cast<uint4*>(u0 + (int64_t)c * m.ldu + i0) = make_uint4(w[c][0], w[c][1], w[c][2], w[c][3]);
-        } else {
-          for (int c = 0; i0 + c < n; ++c)
-            for (int a = 0; a < 3; ++a)
-              u0[(int64_t)a * m.ldu + i0 + c] = __ushort_as_bfloat16((unsigned short)(w[a][c >> 1] >> ((c & 1) * 16)));
-        }
+        for (int c = 0; c < 3; ++c)
+          *reinterpret_cast<uint4*>(u0 + (int64_t)c * m.ldu + i0) = make_uint4(w[c][0], w[c][1], w[c][2], w[c][3]);
       }
     }
     if ((write_uhat && !vec) || io.pen_out || io.mask_out) {
