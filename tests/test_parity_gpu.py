@@ -847,3 +847,31 @@ def test_block_sparse_contraction_on_a_large_patch(pattern):
     assert gpu["path"] == T.ETAC_PATH_DENSE and gpu["pairs"] == E - 1
     _report(f"block-sparse {pattern}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="block-sparse"))
     assert np.all(gpu["U"][5] == 0)
+
+
+@pytest.mark.parametrize("n_envs", [1, 70])
+def test_two_large_patches_bucketed(n_envs):
+    """Two patches of 2048 nodes (a flat pad and a curved sheet, own alpha each) with sphere indenters: the per-env S1
+    kernel in bucket mode + scatter over SEVERAL patches, the 32-env tile with a ragged last tile (and a single
+    environment), an environment that touches only one of the two patches."""
+    mesh = W.assemble([W.flat_pad(32, 64, 1.0), W.cyl_sheet(40.0, 32.0 / 40.0, 32, 64, 1.0)])
+    rng = np.random.default_rng(77 + n_envs)
+    ind = W._blank_indenters(n_envs, 2)
+    off = np.asarray(mesh.patch_offset)
+    pose = np.zeros((n_envs, 2, 7), np.float32)
+    pose[:, :, 6] = 1.0
+    pose[:, 1, 0] = 500.0                                              # the sheet sits 0.5 m away from the pad
+    for k in range(2):
+        c = rng.integers(off[k], off[k + 1], size=n_envs)
+        size = rng.uniform(3.0, 12.0, n_envs)
+        centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, rng.uniform(0.1, 1.2, n_envs), np.zeros(n_envs))
+        ind["type"][:, k] = W.IND_SPHERE
+        ind["param"][:, k, 0] = size
+        ind["pose"][:, k, 0:3] = centre + pose[:, k, 0:3]
+        ind["pose"][:, k, 3:7] = q
+    if n_envs > 3:
+        ind["type"][3, 1] = W.IND_NONE                                 # env 3 touches the pad only
+    wl = W.Workload("two_large", mesh, np.float32([0.5, 0.35]), W.make_weights(8, 5, std=0.1), n_envs, 2, ind, pose, "bf16")
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    _report(f"two large patches E={n_envs}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="two-large", delta_tol=1e-4))
+    assert gpu["pairs"] == int(ref["contact"].sum()) and gpu["launches"] == 4      # S1 evaluate + scatter, tile masks, fused
