@@ -17,7 +17,7 @@ struct etac_ctx {
   size_t bytes = 0;
   int device = 0, n_sm = 0, precision = 0, path_opt = ETAC_PATH_AUTO, n_alpha = 1;
   int last_path = ETAC_PATH_AUTO, last_launches = 0;
-  CUtensorMap tmA{}, tmB16{}, tmB32{};
+  CUtensorMap tmA{}, tmB{};  // K rows [128 x 64]; U^ rows [48 x 64]: the 16-env tile, half of the 32-env tile
   bool have_tm = false;
   cudaStream_t last_stream = nullptr;
   std::string err;
@@ -189,9 +189,9 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
     if (abl == ETAC_ABLATE_LINEAR_ONLY) {  // "Linear Decay Only": the kernels compiled without Phi
       DevModel lin = ctx->m;
       lin.resid = ETAC_RESID_NONE;
-      e = launch_fused_bf16(lin, io, ctx->tmA, ctx->tmB16, ctx->tmB32, ctx->n_sm, gather16, &n_launch, s);
+      e = launch_fused_bf16(lin, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s);
     } else {
-      e = launch_fused_bf16(ctx->m, io, ctx->tmA, ctx->tmB16, ctx->tmB32, ctx->n_sm, gather16, &n_launch, s);
+      e = launch_fused_bf16(ctx->m, io, ctx->tmA, ctx->tmB, ctx->n_sm, gather16, &n_launch, s);
     }
     if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("fused_mlp_kernel", e));
     ctx->last_launches += n_launch - 1;
@@ -405,10 +405,12 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   std::vector<PatchInfo> hp(P);
   std::vector<ChunkInfo> chunks;
   int64_t k32_total = 0;
-  int max_np = 0;
+  int max_np = 0, ucols = 0;
   for (int p = 0; p < P; ++p) {
     PatchInfo& pi = hp[p];
     pi.off = off[p], pi.n = off[p + 1] - off[p];
+    pi.uoff = ucols;
+    ucols += (pi.n + 7) / 8 * 8;
     pi.k32_off = k32_total;
     k32_total += (int64_t)pi.n * pi.n;
     pi.alpha = d->alpha[d->n_alpha == 1 ? 0 : p];
@@ -429,7 +431,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   m.n_chunks = (int)chunks.size();
   m.max_patch_nodes = max_np;
   m.kw = (max_np + 63) / 64 * 64;
-  m.ldu = (N + 63) / 64 * 64;
+  m.ldu = (ucols + 63) / 64 * 64;
   CK(dev_upload(c, &m.patch, hp.data(), P), "upload patches");
   CK(dev_upload(c, &m.chunk, chunks.data(), chunks.size()), "upload chunks");
 
@@ -525,8 +527,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
     }
     std::string why;
     if (!make_tmap(&c->tmA, m.k16, (uint64_t)N, (uint64_t)m.kw, (uint64_t)m.kw, 128, &why) ||
-        !make_tmap(&c->tmB16, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 48, &why) ||
-        !make_tmap(&c->tmB32, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 96, &why))
+        !make_tmap(&c->tmB, m.uhat_t, (uint64_t)urows, (uint64_t)m.ldu, (uint64_t)m.ldu, 48, &why))
       return bail(ETAC_ERR_CUDA, why);
     c->have_tm = true;
     CK(fused_configure(), "cudaFuncSetAttribute(fused_mlp_kernel)");

@@ -20,6 +20,7 @@ constexpr int kMaxPatches = 1024;
 struct PatchInfo {
   int32_t off;        // first node
   int32_t n;          // nodes in the patch
+  int32_t uoff;       // first column of the patch in the U^ operand rows (a multiple of 8: TMA wants 16-byte aligned boxes)
   int64_t k32_off;    // element offset of K_p (fp32, [n x n] row-major) in k32
   float alpha;
   float bc[3];        // bounding-sphere centre (patch-local frame)
@@ -184,8 +185,8 @@ cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_
 cudaError_t backward_configure();
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,
                             float* grad_w, float* grad_delta, int n_sm, cudaStream_t s);
-cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB16,
-                              const CUtensorMap& tmB32, int n_sm, bool gather, int* launches, cudaStream_t s);
+cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int n_sm, bool gather,
+                              int* launches, cudaStream_t s);
 cudaError_t fused_configure();
 bool fused_uses_big_tile(const DevModel& m, int n_envs);
 bool fused_fits(int n_patches);

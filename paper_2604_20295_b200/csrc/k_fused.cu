@@ -23,7 +23,7 @@
 // special-function pipe (128 SiLUs per node-env), and a unit spends as much time in its two tcgen05.mma
 // round trips (operand store -> chain barrier -> mma -> commit -> mbarrier -> TMEM load) as in its SiLUs, so the
 // pipe only stays busy if enough independent units overlap.  A chain owns a 64-column D region of TMEM and
-// 20 KB of shared memory for its layer operands; the units of the CTA's item stream are dealt to the chains
+// 16 KB of shared memory for its layer operands; the units of the CTA's item stream are dealt to the chains
 // round robin (unit q goes to chain q mod NC), independent of item boundaries.  The chain's own warps issue
 // its MLP MMAs: three warps arrive on the chain's named barrier and go on, the fourth (warp c % 4 of chain c)
 // waits on it and one of its lanes issues -- there is no issuer warp in between.  The next unit's layer 1 is
@@ -33,7 +33,9 @@
 // Large patches (kGrouped, 32-env tile): the item order keeps the U^ tiles of a group of env tiles resident in
 // L2, and the contraction is block-sparse -- the TMA and MMA warps skip the 64-node k-blocks in which no
 // environment of the tile has an active node (S1 wrote the bitmaps and bucketed the environments by contact
-// position; Omega is (n - m) x m).
+// position; Omega is (n - m) x m).  The grid runs as clusters of two CTAs that take the two node
+// blocks of a pair for the same env tile: each fetches half of the U^ tile and multicasts it into both shared
+// memories, and a ring stage is released by the commits of both CTAs' MMAs.
 //
 // Template variants (one source, see kMode / kGather / TE below): per-node MLP or none; the PointNet form
 // of Phi as an encoder pass with max-pool and a decoder pass; the gather form of the propagation
@@ -46,30 +48,35 @@
 
 namespace etac {
 
-constexpr int BM = 128, BK = 64, kStages = 3;
+constexpr int BM = 128, BK = 64, kMaxStages = 4;
 constexpr int A_STAGE = BM * BK * 2;
 constexpr int kAop1Bytes = 128 * 16 * 2;   // layer-1 operand of a chain: [128 x 16] bf16, K-major core matrices
 constexpr int kAop2Bytes = 128 * 64 * 2;   // hidden-layer operand: [128 x 64]
-constexpr int kAopBytes = kAop1Bytes + kAop2Bytes;
+// The two share one region: the next unit's layer-1 operand is written when the last hidden layer's MMA, the last
+// reader of the hidden operand, has completed (its D is in registers), and the hidden operand is written when the
+// layer-1 MMA has completed.
+constexpr int kAopBytes = kAop2Bytes;
+static_assert(kAop1Bytes <= kAop2Bytes, "layer-1 operand inside the hidden operand");
 constexpr int kOnesBytes = 128 * 16 * 2;   // [128 x 16]: column 0 = 1.0, the A operand of the bias k-step
 constexpr uint32_t kAopLBO = 2048, kAopSBO = 128;   // 16 row groups x 128 B per k-octet
-constexpr int kRegsCtrl = 24;
 
 template <int TE>
 struct Tile {
   static constexpr int BN = 3 * TE;
   static constexpr int NC = TE == 16 ? 6 : 5;                 // chains: 2 BN + 64 NC <= 512 TMEM columns
+  static constexpr int kStages = TE == 16 ? 3 : 4;            // TMA ring (the pair's ring turns around more slowly)
   static constexpr int kThreads = 128 * (NC + 1);
   static constexpr int B_STAGE = BN * BK * 2;
   static constexpr uint32_t COL_D0 = 2 * BN;
-  // register pool: kThreads x (65536 / kThreads rounded down to 8) = 4 warps x 24 + 4 NC warps x kRegsEpi
+  // register pool: kThreads x (65536 / kThreads rounded down to 8) = 4 warps x kRegsCtrl + 4 NC warps x kRegsEpi
+  static constexpr int kRegsCtrl = TE == 16 ? 24 : 40;  // control warps (the 32-env tile's walk the k-block bitmaps)
   static constexpr int kRegsEpi = TE == 16 ? 80 : 88;
   static_assert(2 * BN + 64 * NC <= 512, "TMEM columns");
 };
 
 template <int NC>
 struct __align__(8) FusedBars {
-  uint64_t full[kStages], empty[kStages];
+  uint64_t full[kMaxStages], empty[kMaxStages];
   uint64_t acc_full[2], acc_empty[2], d_ready[NC];
   uint32_t tmem_base;
   uint32_t pad;
@@ -95,8 +102,8 @@ constexpr int kMaxDynSmem = 232448;  // 227 KB opt-in limit of sm_100
 template <int TE>
 __host__ __device__ constexpr size_t fused_smem_bytes(int n_patches, int mode, bool gather, bool grouped) {
   const bool prop = !gather && mode != 2;
-  return 1024 /*align slack*/ + (prop ? (size_t)kStages * (A_STAGE + Tile<TE>::B_STAGE) : 0) + mode_img_bytes(mode) + kOnesBytes +
-         (size_t)Tile<TE>::NC * kAopBytes + sizeof(FusedBars<Tile<TE>::NC>) + (size_t)(7 * n_patches + 4) * 4 + 16 + 16 +
+  return 1024 /*align slack*/ + (prop ? (size_t)Tile<TE>::kStages * (A_STAGE + Tile<TE>::B_STAGE) : 0) + mode_img_bytes(mode) + kOnesBytes +
+         (size_t)Tile<TE>::NC * kAopBytes + sizeof(FusedBars<Tile<TE>::NC>) + (size_t)(8 * n_patches + 4) * 4 + 16 + 16 +
          (gather ? (size_t)Tile<TE>::NC * 4 * 32 * 16 : 0);
 }
 
@@ -165,18 +172,23 @@ struct ZeroFill {
 struct PTab {
   int cnt, tiles, off, n;  // contacting envs, env tiles, first node, nodes
   int G, GN;               // grouped order: env tiles per group, G x node blocks
+  int uoff;                // first column of the patch in the U^ operand rows
 };
-__host__ __device__ constexpr int kTabInts(int n_patches) { return n_patches + 1 + 6 * n_patches; }
+__host__ __device__ constexpr int kTabInts(int n_patches) { return n_patches + 1 + 7 * n_patches; }
 struct Item {
-  int p, mb, tile, cnt, off, n;  // patch, node block, env tile, units; first node and node count of the patch
+  int p, mb, tile, cnt, off, n, uoff;  // patch, node block, env tile, units; first node, node count, first U^ column of the patch
 };
+// Grouped order: the two CTAs of a cluster walk the same stream of (env tile, PAIR of node blocks) and CTA `rank`
+// takes node block 2 mbp + rank, so that both want the same U^ tiles at the same time (TMA multicast, see the
+// producer).  A patch with an odd number of node blocks leaves one CTA a block beyond the patch: it streams and
+// multiplies along (the ring is shared) but has no units (cnt = 0).
 template <bool kGrouped, int TE>
-__device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, int w, int& pcur, Item& it) {
+__device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, int w, int rank, int& pcur, Item& it) {
   if (w >= prefix[n_patches]) return false;
   while (prefix[pcur + 1] <= w) ++pcur;
   const int r = w - prefix[pcur];
   const PTab t = reinterpret_cast<const PTab*>(prefix + n_patches + 1)[pcur];
-  it.p = pcur, it.off = t.off, it.n = t.n;
+  it.p = pcur, it.off = t.off, it.n = t.n, it.uoff = t.uoff;
   if constexpr (!kGrouped) {
     it.mb = r / t.tiles;
     it.tile = r - it.mb * t.tiles;
@@ -184,10 +196,12 @@ __device__ __forceinline__ bool decode_item(const int* prefix, int n_patches, in
     const int g = r / t.GN;
     const int rem = r - g * t.GN;
     const int gsz = min(t.G, t.tiles - g * t.G);
-    it.mb = rem / gsz;
-    it.tile = g * t.G + (rem - it.mb * gsz);
+    const int mbp = rem / gsz;
+    it.mb = 2 * mbp + rank;
+    it.tile = g * t.G + (rem - mbp * gsz);
   }
   it.cnt = min(TE, t.cnt - it.tile * TE);
+  if (kGrouped && it.mb * BM >= it.n) it.cnt = 0;
   return true;
 }
 
@@ -248,12 +262,18 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     fused_mlp_kernel(DevModel m, StepIO io, const __grid_constant__ CUtensorMap tmA,
                      const __grid_constant__ CUtensorMap tmB) {
   using TL = Tile<TE>;
-  constexpr int BN = TL::BN, NC = TL::NC, B_STAGE = TL::B_STAGE, kThreads = TL::kThreads;
+  constexpr int BN = TL::BN, NC = TL::NC, B_STAGE = TL::B_STAGE, kThreads = TL::kThreads, kStages = TL::kStages;
   constexpr bool kResid = kMode != kModeNone;
   constexpr bool kPn = kMode == kModePnEncode || kMode == kModePnDecode;
   constexpr bool kProp = !kGather && kMode != kModePnEncode;  // TMA + propagation GEMM run
   constexpr bool kFill = kMode != kModePnEncode;              // the decode pass zero-fills
   constexpr int kLayers = mode_layers(kMode), kImgBytes = mode_img_bytes(kMode);
+  // Large patches run as clusters of two CTAs on the same env tile and adjacent node blocks: each CTA fetches half
+  // of the U^ tile and multicasts it into both shared memories, which takes a fifth off the L2 -> SM traffic that
+  // bounds the contraction (K tile 16 KB + 6 instead of 12 KB per k-block and SM).  A ring stage is refilled when
+  // the MMAs of BOTH CTAs have read it: `empty` counts two commits, each CTA's commit arrives in both.
+  constexpr bool kPair = kGrouped;
+  constexpr uint16_t kPairMask = 3;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sA = smem;
@@ -266,9 +286,11 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   uint8_t* sGather = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(prefix + kTabInts(m.n_patches)) + 15) & ~uintptr_t(15));  // 4 NC warps x 32 entries
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = kPair ? (int)cluster_ctarank() : 0;
+  const int w_first = kPair ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, w_step = kPair ? (int)(gridDim.x >> 1) : (int)gridDim.x;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], 1);
+    for (int s = 0; s < kStages; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], kPair ? 2 : 1);
     for (int b = 0; b < 2; ++b) mbar_init(&bars->acc_full[b], 1), mbar_init(&bars->acc_empty[b], 4 * NC);
     for (int c = 0; c < NC; ++c) mbar_init(&bars->d_ready[c], 1);
     fence_barrier_init();
@@ -285,9 +307,10 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       if (p < m.n_patches) {
         const PatchInfo pi = m.patch[p];
         PTab t;
-        t.cnt = m.count[p], t.off = pi.off, t.n = pi.n;
+        t.cnt = m.count[p], t.off = pi.off, t.n = pi.n, t.uoff = pi.uoff;
         t.tiles = (t.cnt + TE - 1) / TE;
-        const int nmb = (pi.n + BM - 1) / BM;
+        int nmb = (pi.n + BM - 1) / BM;
+        if constexpr (kPair) nmb = (nmb + 1) / 2;  // pairs of node blocks
         t.G = max(1, min(t.tiles, m.group_bytes / (BN * 2 * max(pi.n, 1))));
         t.GN = max(t.G * nmb, 1);
         reinterpret_cast<PTab*>(prefix + m.n_patches + 1)[p] = t;
@@ -315,11 +338,12 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   }
   tc_fence_before();
   __syncthreads();
+  if constexpr (kPair) cluster_sync();  // the peer's barriers are initialised before anything is sent to them
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
   if (warp == 0) {
-    reg_dealloc<kRegsCtrl>();
+    reg_dealloc<TL::kRegsCtrl>();
     if constexpr (kProp)
     // ------------------------------------------------------------------ TMA producer
     // (the whole warp runs the loop so that every operand stays warp-uniform; one elected lane issues)
@@ -327,14 +351,14 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       int pcur = 0, stage = 0;
       uint32_t ph = 0;
       Item it, nx;
-      int w = blockIdx.x;
-      bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it);
+      int w = w_first;
+      bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, rank, pcur, it);
       uint32_t km = 0;
       if constexpr (kGrouped) km = have ? load_tile_kbmask(m, it, lane) : 0u;
       while (have) {
         // the next item and (large patches) its k-block mask, requested before this item's k-blocks are streamed
-        const int wn = w + gridDim.x;
-        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, pcur, nx);
+        const int wn = w + w_step;
+        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
         uint32_t kmn = 0;
         if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
         const int nkb = (it.n + BK - 1) / BK;
@@ -343,7 +367,11 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
           if (elect_one()) {
             mbar_arrive_expect_tx(&bars->full[stage], A_STAGE + B_STAGE);
             tma_load_2d(sA + stage * A_STAGE, &tmA, &bars->full[stage], kb * BK, it.off + it.mb * BM);
-            tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], it.off + kb * BK, it.tile * BN);
+            if constexpr (kPair)  // tmB's box is half a tile: rows [rank BN/2, +BN/2) of the tile, into both CTAs
+              tma_load_2d_multicast(sB + stage * B_STAGE + rank * (B_STAGE / 2), &tmB, &bars->full[stage], it.uoff + kb * BK,
+                                    it.tile * BN + rank * (BN / 2), kPairMask);
+            else
+              tma_load_2d(sB + stage * B_STAGE, &tmB, &bars->full[stage], it.uoff + kb * BK, it.tile * BN);
           }
           __syncwarp();
           if (++stage == kStages) stage = 0, ph ^= 1;
@@ -359,7 +387,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       }
     }
   } else if (warp == 1) {
-    reg_dealloc<kRegsCtrl>();
+    reg_dealloc<TL::kRegsCtrl>();
     if constexpr (kProp)
     // ------------------------------------------------------------------ MMA issuer
     // Warp-uniform control flow; tcgen05.mma / tcgen05.commit are issued by one elected lane.
@@ -368,13 +396,13 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       int pcur = 0, stage = 0, k_item = 0;
       uint32_t ph = 0;
       Item it, nx;
-      int w = blockIdx.x;
-      bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, pcur, it);
+      int w = w_first;
+      bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, rank, pcur, it);
       uint32_t km = 0;
       if constexpr (kGrouped) km = have ? load_tile_kbmask(m, it, lane) : 0u;
       while (have) {
-        const int wn = w + gridDim.x;
-        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, pcur, nx);
+        const int wn = w + w_step;
+        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
         uint32_t kmn = 0;
         if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
         const int nkb = (it.n + BK - 1) / BK;
@@ -391,7 +419,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
 #pragma unroll
             for (int k = 0; k < BK / 16; ++k)
               mma_ss(tmem + b * BN, dA + 2 * k, dB + 2 * k, idesc_prop, (!first || k != 0) ? 1u : 0u);
-            tc_commit(&bars->empty[stage]);
+            if constexpr (kPair) tc_commit_multicast(&bars->empty[stage], kPairMask);
+            else tc_commit(&bars->empty[stage]);
             if (last) tc_commit(&bars->acc_full[b]);
           }
           __syncwarp();
@@ -412,7 +441,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       }
     }
   } else if (warp < 4) {
-    reg_dealloc<kRegsCtrl>();
+    reg_dealloc<TL::kRegsCtrl>();
     // ------------------------------------------------------------------ zero-fill of the contact-free rows
     // Two warps per CTA walk the (env, patch) flags and zero-fill one run of contact-free patches at a time,
     // with a pause in between: 190 MB of stores (cfg 3) trickle out next to the MUFU-bound work instead of
@@ -431,7 +460,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     const uint32_t tD = trow + TL::COL_D0 + 64 * c;
     const int row = lane_base + lane;
     uint64_t* d_ready = &bars->d_ready[c];
-    const uint32_t sA1 = smem_u32(sAop + c * kAopBytes), sA2 = sA1 + kAop1Bytes;
+    const uint32_t sA1 = smem_u32(sAop + c * kAopBytes), sA2 = sA1;  // (one region, see kAopBytes)
     const uint32_t sRow1 = sA1 + row * 16, sRow2 = sA2 + row * 16;  // this thread's 16-byte slot in k-octet 0
     uint32_t d_ph = 0;
 
@@ -469,9 +498,9 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     };
 
     // ---- cursor over the units of this chain: unit q of the CTA's item stream belongs to chain q mod NC
-    int cw = blockIdx.x, ck = 0, cel = c, pcur = 0;  // work index, item ordinal, unit within the item
+    int cw = w_first, ck = 0, cel = c, pcur = 0;  // work index, item ordinal, unit within the item
     Item it;
-    bool live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, pcur, it);
+    bool live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, rank, pcur, it);
     int it_g = 0;           // this thread's node of the item (row clamped into the patch) and whether the row is inside
     bool it_valid = false;
     auto item_setup = [&]() {
@@ -497,8 +526,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       while (live && cel >= it.cnt) {
         cel -= it.cnt;
         leave_item();
-        ++ck, cw += gridDim.x;
-        live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, pcur, it);
+        ++ck, cw += w_step;
+        live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, rank, pcur, it);
         if (live) item_setup(), enter_item();
       }
     };
@@ -718,6 +747,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   }
   tc_fence_before();
   __syncthreads();
+  if constexpr (kPair) cluster_sync();  // the peer's last commits arrive on this CTA's barriers
   if (warp == 1) {
     tc_fence_after();
     tmem_dealloc<512>(tmem);
@@ -795,46 +825,60 @@ bool fused_uses_big_tile(const DevModel& m, int n_envs) {
   return (size_t)n_envs * (size_t)m.max_patch_nodes * 6 > (size_t)m.group_bytes || m.max_patch_nodes >= 2048;
 }
 
+// the 32-env instantiation: clusters of two CTAs (an even grid); tmB is the map with the half-tile box (48 rows)
+template <int kMode, bool kOutBf16>
+static cudaError_t launch_pairs(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int grid, size_t smem,
+                                cudaStream_t s) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)(grid & ~1)), cfg.blockDim = dim3(Tile<32>::kThreads), cfg.dynamicSmemBytes = smem, cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 2, at[0].val.clusterDim.y = 1, at[0].val.clusterDim.z = 1;
+  cfg.attrs = at, cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, fused_mlp_kernel<kMode, false, kOutBf16, true, 32>, m, io, tmA, tmB);
+}
+
 template <int kMode>
-static void launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB16,
-                       const CUtensorMap& tmB32, int grid, bool gather, cudaStream_t s) {
+static cudaError_t launch_one(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int grid, bool gather,
+                              cudaStream_t s) {
   const size_t smem16 = fused_smem_bytes<16>(m.n_patches, kMode, gather, false), smem32 = fused_smem_bytes<32>(m.n_patches, kMode, false, true);
-  constexpr int T16 = Tile<16>::kThreads, T32 = Tile<32>::kThreads;
+  constexpr int T16 = Tile<16>::kThreads;
   const bool big = !gather && fused_uses_big_tile(m, io.n_envs);
   if constexpr (kMode == kModePnEncode) {
-    fused_mlp_kernel<kMode, false, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
+    fused_mlp_kernel<kMode, false, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB);
   } else if (gather) {
-    if (io.out_bf16) fused_mlp_kernel<kMode, true, true, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
-    else fused_mlp_kernel<kMode, true, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
+    if (io.out_bf16) fused_mlp_kernel<kMode, true, true, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB);
+    else fused_mlp_kernel<kMode, true, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB);
   } else if (big) {
     kbtile_kernel<32><<<dim3((unsigned)((io.n_envs + 31) / 32), (unsigned)m.n_patches), 32, 0, s>>>(m);
-    if (io.out_bf16) fused_mlp_kernel<kMode, false, true, true, 32><<<grid, T32, smem32, s>>>(m, io, tmA, tmB32);
-    else fused_mlp_kernel<kMode, false, false, true, 32><<<grid, T32, smem32, s>>>(m, io, tmA, tmB32);
+    return io.out_bf16 ? launch_pairs<kMode, true>(m, io, tmA, tmB, grid, smem32, s) : launch_pairs<kMode, false>(m, io, tmA, tmB, grid, smem32, s);
   } else {
-    if (io.out_bf16) fused_mlp_kernel<kMode, false, true, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
-    else fused_mlp_kernel<kMode, false, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB16);
+    if (io.out_bf16) fused_mlp_kernel<kMode, false, true, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB);
+    else fused_mlp_kernel<kMode, false, false, false, 16><<<grid, T16, smem16, s>>>(m, io, tmA, tmB);
   }
+  return cudaSuccess;
 }
 
 // Launches S2-S4 for the context's residual form; *launches receives the number of kernels.
-cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB16,
-                              const CUtensorMap& tmB32, int n_sm, bool gather, int* launches, cudaStream_t s) {
+cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtensorMap& tmA, const CUtensorMap& tmB, int n_sm, bool gather,
+                              int* launches, cudaStream_t s) {
   const int grid = n_sm;
   const int n_big = (!gather && fused_uses_big_tile(m, io.n_envs)) ? 1 : 0;  // + kbtile_kernel
   *launches = 1 + n_big;
+  cudaError_t e = cudaSuccess;
   if (m.resid == ETAC_RESID_NONE) {
-    launch_one<kModeNone>(m, io, tmA, tmB16, tmB32, grid, gather, s);
+    e = launch_one<kModeNone>(m, io, tmA, tmB, grid, gather, s);
   } else if (m.resid == ETAC_RESID_PERNODE_MLP) {
-    launch_one<kModePerNode>(m, io, tmA, tmB16, tmB32, grid, gather, s);
+    e = launch_one<kModePerNode>(m, io, tmA, tmB, grid, gather, s);
   } else {  // ETAC_RESID_POINTNET: encode + max-pool, per-(env, patch) vector, decode
-    cudaError_t e = cudaMemsetAsync(m.gmax, 0, sizeof(uint32_t) * 64 * (size_t)m.n_patches * m.max_envs, s);
+    e = cudaMemsetAsync(m.gmax, 0, sizeof(uint32_t) * 64 * (size_t)m.n_patches * m.max_envs, s);
     if (e != cudaSuccess) return e;
-    launch_one<kModePnEncode>(m, io, tmA, tmB16, tmB32, grid, false, s);
+    launch_one<kModePnEncode>(m, io, tmA, tmB, grid, false, s);
     pn_global_kernel<<<dim3((unsigned)((io.n_envs + kPnSlots - 1) / kPnSlots), (unsigned)m.n_patches), 64, 0, s>>>(m);
-    launch_one<kModePnDecode>(m, io, tmA, tmB16, tmB32, grid, gather, s);
+    e = launch_one<kModePnDecode>(m, io, tmA, tmB, grid, gather, s);
     *launches = 3 + n_big;
   }
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace etac

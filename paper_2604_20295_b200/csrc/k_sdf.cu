@@ -349,7 +349,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
         run0 = -1;
       }
       if (q == np) break;
-      const int off = s_off[q], n = s_off[q + 1] - off;
+      const int off = s_off[q], n = s_off[q + 1] - off, uoff = m.patch[p0 + q].uoff;
       const int64_t row0 = (int64_t)e * m.n_nodes + off;
       const int slot = s_slot[q];
       const float* delta = m.delta + row0;
@@ -392,7 +392,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
         }
         if (write_uhat) {
           const float4 nn = m.nrm4[off + i];
-          __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off + i;
+          __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + uoff + i;
           u[0] = __float2bfloat16_rn(-d * nn.x);
           u[m.ldu] = __float2bfloat16_rn(-d * nn.y);
           u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * nn.z);
@@ -510,7 +510,7 @@ __global__ void __launch_bounds__(kPairWarps * 32, 24) sdf_pairs_kernel(DevModel
       }
       if (write_uhat) {
         const float4 nn = m.nrm4[off + i];
-        __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off + i;
+        __nv_bfloat16* u = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.uoff + i;
         u[0] = __float2bfloat16_rn(-d * nn.x);
         u[m.ldu] = __float2bfloat16_rn(-d * nn.y);
         u[2 * (int64_t)m.ldu] = __float2bfloat16_rn(-d * nn.z);
@@ -665,8 +665,8 @@ __global__ void __launch_bounds__(kEvalWarps * 32, 8) sdf_eval_kernel(DevModel m
     // optional outputs.  A lane takes EIGHT consecutive nodes: delta comes back from L2 as two 16-byte loads
     // (written by this warp above), a group without an active node -- most of them: a tenth of the nodes of a
     // contacting patch is active -- costs three 16-byte zero stores, and normals are only loaded for active nodes.
-    __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off;
-    const bool vec = ((off | m.ldu) & 7) == 0 && ((row0 & 3) == 0);  // 16-byte aligned groups (else node by node)
+    __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.uoff;
+    const bool vec = (row0 & 3) == 0;  // 16-byte aligned groups (else node by node)
     __syncwarp();  // the lanes read delta values that other lanes of the warp wrote
     uint32_t kb0 = 0;  // bitmap of the 64-node k-blocks with an active node (n <= 2048: one word)
     if (write_uhat && vec) {
@@ -774,8 +774,8 @@ __global__ void __launch_bounds__(256) sdf_scatter_kernel(DevModel m, StepIO io)
     const int off = pi.off, n = pi.n;
     const int64_t row0 = (int64_t)e * m.n_nodes + off;
     const float* __restrict__ delta = m.delta + row0;
-    __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + off;
-    const bool vec = ((off | m.ldu) & 7) == 0 && ((row0 & 3) == 0);  // 16-byte aligned groups of eight nodes
+    __nv_bfloat16* u0 = m.uhat_t + (int64_t)(slot * 3) * m.ldu + pi.uoff;
+    const bool vec = (row0 & 3) == 0;  // 16-byte aligned groups of eight nodes
     if (vec) {
       for (int i0 = t * 8; i0 < n; i0 += 2048) {
         float d[8];

@@ -875,3 +875,39 @@ def test_two_large_patches_bucketed(n_envs):
     gpu, ref = run_gpu(wl), run_oracle(wl)
     _report(f"two large patches E={n_envs}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="two-large", delta_tol=1e-4))
     assert gpu["pairs"] == int(ref["contact"].sum()) and gpu["launches"] == 4      # S1 evaluate + scatter, tile masks, fused
+
+
+@pytest.mark.parametrize("kind,n_envs", [("pair", 40), ("pair", 1), ("tile16", 40)])
+def test_patch_sizes_that_are_not_multiples_of_eight(kind, n_envs):
+    """Patches whose node counts are odd: every patch after the first starts at an odd node index, while TMA boxes of
+    the U^ operand have to start on 16-byte boundaries (the operand rows are padded per patch).
+    "pair": the 32-env instantiation runs as clusters of two CTAs that share the U^ tile of a PAIR of node blocks; a
+    patch of 2139 nodes (17 blocks of 128, the last one ragged: the pair's second CTA has a block beyond the patch)
+    beside a patch of 100 nodes (one block: the second CTA has no block at all) and one of 384 (three blocks).
+    "tile16": the 16-env instantiation on patches of 35, 2015 and 81 nodes."""
+    if kind == "pair":
+        parts = [W.flat_pad(31, 69, 1.0), W.flat_pad(10, 10, 1.0), W.cyl_sheet(40.0, 16.0 / 40.0, 16, 24, 1.0)]
+    else:
+        parts = [W.flat_pad(5, 7, 1.0), W.flat_pad(31, 65, 1.0), W.flat_pad(9, 9, 1.0)]
+    mesh = W.assemble(parts)
+    rng = np.random.default_rng(99 + n_envs)
+    ind = W._blank_indenters(n_envs, 3)
+    off = np.asarray(mesh.patch_offset)
+    pose = np.zeros((n_envs, 3, 7), np.float32)
+    pose[:, :, 6] = 1.0
+    pose[:, 1, 0], pose[:, 2, 0] = 400.0, 800.0
+    for k in range(3):
+        c = rng.integers(off[k], off[k + 1], size=n_envs)
+        size = rng.uniform(2.0, 9.0, n_envs)
+        centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, rng.uniform(0.1, 1.0, n_envs), np.zeros(n_envs))
+        ind["type"][:, k] = W.IND_SPHERE
+        ind["param"][:, k, 0] = size
+        ind["pose"][:, k, 0:3] = centre + pose[:, k, 0:3]
+        ind["pose"][:, k, 3:7] = q
+    if n_envs > 5:
+        ind["type"][5, 1 if kind == "tile16" else 0] = W.IND_NONE      # env 5 does not touch the large patch
+    wl = W.Workload("odd_sizes", mesh, np.float32([0.5, 0.4, 0.3]), W.make_weights(8, 6, std=0.1), n_envs, 3, ind, pose, "bf16")
+    gpu, ref = run_gpu(wl), run_oracle(wl)
+    _report(f"odd patch sizes ({kind}) E={n_envs}", compare(gpu, ref, TOL["bf16"], resid_tol=5e-2, label="odd-sizes", delta_tol=1e-4))
+    assert gpu["pairs"] == int(ref["contact"].sum())
+    assert gpu["launches"] == (4 if kind == "pair" else 2)             # the 32-env tile: S1 evaluate + scatter, tile masks, fused
