@@ -16,6 +16,12 @@ with the CUDA path).  It differentiates exactly what ``etac_oracle.step`` comput
   DESIGN.md R5): dL/ddelta_j = -n_j . (sum_i K_ij dL/du_i + G_j if row j is u^_j itself); 0 for the other nodes.
   The contact set is held fixed (it does not depend on alpha or Phi).
 
+  PointNet form of Phi (the network Eq. (3) calibrates): its input is [P, N, U^], so Phi does
+  not depend on alpha (dL/dalpha comes from u_i alone) and dL/ddelta_j gains -n_j . dL/du^_j through the encoder
+  input of the nodes in contact.  The chain rule runs backwards through the decoder, the broadcast of the global
+  feature (sum of the decoder-input gradients over the rows), the global MLP, the max-pool (the gradient of
+  column k goes to the row that attains the maximum) and the shared encoder.
+
 float64 numpy, one (env, patch) at a time, no fusion.  Pins (tests/test_oracle_pins.py): central
 finite differences of ``etac_oracle.step`` (itself pinned) with respect to alpha, to sampled weights
 of every layer and (penetration input mode) to the penetration of sampled contact nodes.
@@ -34,18 +40,20 @@ def silu_prime(z):
 
 def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetration=None, envs=None):
     """G: dL/dU [E', N, 3] for the listed envs (default all).  Returns float64 gradients
-    {"alpha": [n_alpha], "delta": [E', N], "W1": [64, 9], "b1", "W2", "b2", "W3", "b3"} (weights only for the
-    per-node form)."""
-    if model.resid_arch not in ("none", "pernode") or model.ablation != "full":
-        raise ValueError("backward oracle: per-node / no residual, full pipeline only")
+    {"alpha": [n_alpha], "delta": [E', N]} and, per residual form, "W1": [64, 9], "b1", "W2", "b2", "W3", "b3"
+    (per-node) or "E1", "e1", "E2", "e2", "G1", "g1", "D1", "d1", "D2", "d2" (PointNet)."""
+    if model.resid_arch not in ("none", "pernode", "pointnet") or model.ablation != "full":
+        raise ValueError("backward oracle: full pipeline only")
     G = np.asarray(G, dtype=np.float64)
     fwd = O.step(model, indenters=indenters, patch_pose=patch_pose, penetration=penetration, envs=envs)
     alpha = np.atleast_1d(np.asarray(model.alpha, dtype=np.float64))
     grads = {"alpha": np.zeros(alpha.shape[0]), "delta": np.zeros((G.shape[0], model.n_nodes))}
     mlp = model.resid_arch == "pernode"
-    if mlp:
+    pnet = model.resid_arch == "pointnet"
+    if mlp or pnet:
         w = {k: np.asarray(v, dtype=np.float64) for k, v in model.weights.items()}
-        for k in ("W1", "b1", "W2", "b2", "W3", "b3"):
+        names = ("W1", "b1", "W2", "b2", "W3", "b3") if mlp else ("E1", "e1", "E2", "e2", "G1", "g1", "D1", "d1", "D2", "d2")
+        for k in names:
             grads[k] = np.zeros_like(w[k])
     pos = model.pos.astype(np.float64)
     nrm = model.normal.astype(np.float64)
@@ -82,9 +90,43 @@ def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetrati
                 grads["W1"] += gz1.T @ x9
                 grads["b1"] += gz1.sum(0)
                 glin += (gz1 @ w["W1"])[:, 0:3]
+            guhat = 0.0                                           # dL/du^ through the input of Phi (PointNet only)
+            if pnet:
+                x9 = np.concatenate([P, nrm[lo:hi], uhat[lo:hi]], axis=1)     # [P, N, U^]
+                z1 = x9 @ w["E1"].T + w["e1"]
+                f1 = O.silu(z1)
+                z2 = f1 @ w["E2"].T + w["e2"]
+                f = O.silu(z2)                                    # n x 64 point-wise features
+                arg = f.argmax(axis=0)                            # max-pool: the row that gives column k
+                gmax = f[arg, np.arange(f.shape[1])]
+                zg = gmax @ w["G1"].T + w["g1"]
+                gp = O.silu(zg)                                   # global feature after its MLP
+                cat = np.concatenate([f, np.broadcast_to(gp, f.shape)], axis=1)
+                zc = cat @ w["D1"].T + w["d1"]
+                h = O.silu(zc)
+                grads["D2"] += g.T @ h
+                grads["d2"] += g.sum(0)
+                gzc = (g @ w["D2"]) * silu_prime(zc)
+                grads["D1"] += gzc.T @ cat
+                grads["d1"] += gzc.sum(0)
+                gcat = gzc @ w["D1"]
+                gf = gcat[:, :64].copy()
+                ggp = gcat[:, 64:].sum(0)                         # the broadcast global feature collects every row
+                gzg = ggp * silu_prime(zg)
+                grads["G1"] += np.outer(gzg, gmax)
+                grads["g1"] += gzg
+                np.add.at(gf, (arg, np.arange(64)), gzg @ w["G1"])            # max-pool routes to the arg-max rows
+                gz2 = gf * silu_prime(z2)
+                grads["E2"] += gz2.T @ f1
+                grads["e2"] += gz2.sum(0)
+                gz1 = (gz2 @ w["E2"]) * silu_prime(z1)
+                grads["E1"] += gz1.T @ x9
+                grads["e1"] += gz1.sum(0)
+                guhat = (gz1 @ w["E1"])[:, 6:9][act]
             grads["alpha"][p if alpha.shape[0] > 1 else 0] += float((glin * v).sum())
-            # u^_j = -delta_j n_j: dL/ddelta_j = -n_j . (sum_i K_ij dL/du_i + G_j if row j is u^_j itself)
-            back = K[:, act].T @ glin
+            # u^_j = -delta_j n_j: dL/ddelta_j = -n_j . (sum_i K_ij dL/du_i + G_j if row j is u^_j itself
+            #                                            + dL/du^_j through the input of Phi)
+            back = K[:, act].T @ glin + guhat
             if model.active_mode == "passthrough":
                 back = back + G[oi, lo:hi][act]
             grads["delta"][oi, lo:hi][act] = -(nrm[lo:hi][act] * back).sum(1)

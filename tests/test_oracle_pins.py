@@ -347,7 +347,10 @@ def _grad_case(n_alpha_per_patch, active_mode="passthrough", resid_arch="pernode
         ind["type"][:, k], ind["param"][:, k, 0] = W.IND_SPHERE, size
         ind["pose"][:, k, 0:3], ind["pose"][:, k, 3:7] = centre, q
     alpha = np.asarray([0.45, 0.7] if n_alpha_per_patch else [0.5], np.float32)
-    wl = W.Workload("grad_case", mesh, alpha, W.make_weights(9, 1, std=0.3), E, 2, ind, None, "fp32")
+    weights = W.make_weights(9, 1, std=0.3)
+    if resid_arch == "pointnet":
+        weights = {**weights, **W.make_pointnet_weights(9, 1, std=0.3)}
+    wl = W.Workload("grad_case", mesh, alpha, weights, E, 2, ind, None, "fp32")
     target = rng.normal(0, 0.2, (E, mesh.n_nodes, 3))
 
     def loss(wl_):
@@ -357,7 +360,8 @@ def _grad_case(n_alpha_per_patch, active_mode="passthrough", resid_arch="pernode
 
 
 @pytest.mark.parametrize("per_patch,active_mode,resid_arch", [(True, "passthrough", "pernode"), (False, "propagate", "pernode"),
-                                                               (True, "passthrough", "none")])
+                                                               (True, "passthrough", "none"), (True, "passthrough", "pointnet"),
+                                                               (False, "propagate", "pointnet")])
 def test_backward_oracle_matches_finite_differences(per_patch, active_mode, resid_arch):
     """The gradient oracle against its definition: central differences of the (pinned) forward oracle's
     loss 0.5*||U - U*||^2 (Eq. 3) in alpha and in sampled weights of every layer."""
@@ -395,17 +399,25 @@ def test_backward_oracle_matches_finite_differences(per_patch, active_mode, resi
     if resid_arch == "none":
         return
     rng = np.random.default_rng(5)
-    for name in ("W1", "b1", "W2", "b2", "W3", "b3"):
+    names = ("W1", "b1", "W2", "b2", "W3", "b3") if resid_arch == "pernode" else ("E1", "e1", "E2", "e2", "G1", "g1", "D1", "d1", "D2", "d2")
+    noise = 8 * np.finfo(np.float64).eps * abs(loss(wl)[0]) / eps       # rounding of the two losses in the difference quotient
+    for name in names:
         base = wl.weights[name].astype(np.float64)
-        for _ in range(3):
+        tested = 0
+        for _ in range(200):
             idx = tuple(rng.integers(0, s) for s in base.shape)
+            if abs(g[name][idx]) < 100 * noise:                       # the quotient's rounding would hide a mistake
+                continue
+            tested += 1
             wp, wm = base.copy(), base.copy()
             wp[idx] += eps
             wm[idx] -= eps
             fd = (loss(dataclasses.replace(wl, weights={**wl.weights, name: wp}))[0]
                   - loss(dataclasses.replace(wl, weights={**wl.weights, name: wm}))[0]) / (2 * eps)
-            assert abs(fd - g[name][idx]) <= 2e-6 * max(1.0, abs(fd)), (name, idx, fd, g[name][idx])
-        assert np.abs(g[name]).max() > 1e-4
+            assert abs(fd - g[name][idx]) <= 2e-6 * max(1.0, abs(fd)) + noise, (name, idx, fd, g[name][idx], noise)
+            if tested == 3:
+                break
+        assert tested == 3 and np.abs(g[name]).max() > 1e-4
 
 
 # ---------------------------------------------------------------- P12
