@@ -44,10 +44,10 @@ FP32_FMA_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12              # 74.4: 148 SMs x 
 # capture named beside it; "src_sha" = sha1 (first 12 hex digits) of the kernel's source file at capture time.
 # bench.py prints the figure only while the source still has that hash -- a changed kernel gives traffic: null.
 NCU_TRAFFIC = {
-    "cfg3": {"bytes": 311.59e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
-             "src_sha": "c58bdba42f6d"},
-    "cfg4": {"bytes": 1571.35e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
-             "src_sha": "c58bdba42f6d"},
+    "cfg3": {"bytes": 312.11e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
+             "src_sha": "bfc7a631b422"},
+    "cfg4": {"bytes": 1693.28e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
+             "src_sha": "bfc7a631b422"},
 }
 
 CFG5_NODES = (256, 1024, 4096, 8192)

@@ -44,7 +44,7 @@ typedef enum {
   ETAC_OK = 0,
   ETAC_ERR_INVALID_ARG = 1, /* NULL / out-of-range / inconsistent argument; ctx unchanged */
   ETAC_ERR_UNSUPPORTED = 2, /* valid request this build cannot serve (e.g. ETAC_PATH_DENSE on an fp32 context,
-                               etac_backward on a PointNet context, a device that is not sm_100) */
+                               etac_backward with an ablation mode, a device that is not sm_100) */
   ETAC_ERR_ALLOC = 3,       /* host or device allocation failed */
   ETAC_ERR_CUDA = 4,        /* a CUDA call failed; etac_last_error() has the CUDA message */
   ETAC_ERR_CAPACITY = 5     /* n_envs > max_envs */
@@ -212,8 +212,10 @@ etac_status etac_patches_from_adjacency(int32_t n_nodes, const int32_t* adj_rowp
  * ETAC_ACTIVE_PASSTHROUGH) and rows of contact-free (env, patch) pairs carry no gradient to them.  Optionally
  * also dL/d(penetration); gradients with respect to poses are not computed.  Arithmetic: fp32 on the fp32 copies of
  * K and the weights, whatever the context's precision; sums over environments use fp32 atomics, so
- * repeated calls agree to rounding, not bit for bit.  Contexts with ETAC_RESID_POINTNET and ablation
- * modes other than FULL: ETAC_ERR_UNSUPPORTED.  Enqueues on cuda_stream, no host synchronisation. */
+ * repeated calls agree to rounding, not bit for bit.  With ETAC_RESID_POINTNET (the network of PAPER.md:L91-L99,
+ * whose input is [P, N, U^]) Phi does not depend on alpha, the weight gradients are those of its five layers and
+ * dL/d(penetration) includes the path through the encoder input; the max-pool passes its gradient to the arg-max
+ * row of every feature column.  Ablation modes other than FULL: ETAC_ERR_UNSUPPORTED.  Enqueues on cuda_stream, no host synchronisation. */
 typedef struct {
   uint32_t struct_size;               /* = sizeof(etac_backward_args) */
   int32_t n_envs;                     /* 1..max_envs (0 is a no-op) */
@@ -224,13 +226,16 @@ typedef struct {
   const float* d_grad_out;            /* device [E x N x 3] fp32: dL/dU, REQUIRED */
   float* d_grad_alpha;                /* device [n_alpha] fp32, REQUIRED, overwritten: dL/dalpha (per patch if the
                                          context was created with n_alpha = P) */
-  float* d_grad_weights;              /* device [4995] fp32, overwritten, or NULL: dL/d W1[64x9] b1[64] W2[64x64]
-                                         b2[64] W3[3x64] b3[3], in this order; must be NULL for ETAC_RESID_NONE */
+  float* d_grad_weights;              /* device fp32, overwritten, or NULL; must be NULL for ETAC_RESID_NONE.
+                                         ETAC_RESID_PERNODE_MLP: [4995] = dL/d W1[64x9] b1[64] W2[64x64] b2[64]
+                                         W3[3x64] b3[3], in this order.  ETAC_RESID_POINTNET: [17411] = dL/d E1[64x9]
+                                         e1[64] E2[64x64] e2[64] G1[64x64] g1[64] D1[64x128] d1[64] D2[3x64] d2[3] */
   float* d_grad_penetration;          /* device [E x N] fp32, overwritten, or NULL: dL/ddelta for the nodes in contact
                                          (u^ = -delta n, L77; the contact set is held fixed, 0 for the other nodes).
                                          The caller chains it to object / link poses through its SDF gradients */
 } etac_backward_args;
 #define ETAC_GRAD_WEIGHTS_LEN 4995
+#define ETAC_GRAD_WEIGHTS_POINTNET_LEN 17411
 etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* args);
 
 /* Replaces the calibrated parameters of a context in place (one gradient-descent step of Eq. (3)):

@@ -489,7 +489,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
     memcpy(pf.data() + 4096, d->g1, 64 * 4);
     memcpy(pf.data() + 4160 + 4096, d->d1, 64 * 4);
     CK(dev_upload(c, &m.pn_f32, pf.data(), pf.size()), "upload PointNet global MLP");
-    if (d->precision == ETAC_PREC_FP32) {  // fp32 SIMT form (k_pointnet_fp32.cu)
+    {  // fp32 copies for the fp32 SIMT forward (k_pointnet_fp32.cu) and the backward (k_backward_pointnet.cu)
       std::vector<float> w32;
       w32.insert(w32.end(), d->E1, d->E1 + 576), w32.insert(w32.end(), d->e1, d->e1 + 64);
       w32.insert(w32.end(), d->E2, d->E2 + 4096), w32.insert(w32.end(), d->e2, d->e2 + 64);
@@ -497,7 +497,11 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
       w32.insert(w32.end(), d->D2, d->D2 + 192), w32.insert(w32.end(), d->d2, d->d2 + 3);
       CK(dev_upload(c, &m.pn_w32, w32.data(), w32.size()), "upload PointNet fp32 weights");
       CK(pointnet_fp32_configure(), "cudaFuncSetAttribute(pn_decode_fp32_kernel)");
+      CK(backward_pointnet_configure(), "cudaFuncSetAttribute(pn_bwd_node_kernel)");
     }
+    CK(dev_alloc(c, &m.pn_gkey, (size_t)64 * P * d->max_envs, true), "alloc PointNet arg-max keys");
+    CK(dev_alloc(c, &m.pn_ssum, (size_t)64 * P * d->max_envs, true), "alloc PointNet backward sums");
+    CK(dev_alloc(c, &m.pn_ggmax, (size_t)64 * P * d->max_envs, true), "alloc PointNet backward dL/dgmax");
     CK(dev_alloc(c, &m.gmax, (size_t)64 * P * d->max_envs, true), "alloc gmax");
     CK(dev_alloc(c, &m.cvec, (size_t)64 * P * d->max_envs, true), "alloc cvec");
   }
@@ -692,7 +696,6 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
     return fail(ctx, ETAC_ERR_INVALID_ARG, "d_indenters is NULL");
   if (a->input_mode == ETAC_IN_PENETRATION && !a->d_penetration)
     return fail(ctx, ETAC_ERR_INVALID_ARG, "d_penetration is NULL");
-  if (ctx->m.resid == ETAC_RESID_POINTNET) return fail(ctx, ETAC_ERR_UNSUPPORTED, "etac_backward: per-node residual only");
   if (ctx->m.ablation != ETAC_ABLATE_FULL) return fail(ctx, ETAC_ERR_UNSUPPORTED, "etac_backward: ETAC_ABLATE_FULL only");
   if (ctx->m.resid == ETAC_RESID_NONE && a->d_grad_weights)
     return fail(ctx, ETAC_ERR_INVALID_ARG, "d_grad_weights given for a context without a residual network");
@@ -704,18 +707,26 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
   io.n_envs = a->n_envs, io.input_mode = a->input_mode;
   io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
   cudaError_t e;
+  const bool pointnet = ctx->m.resid == ETAC_RESID_POINTNET;
   if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 1), s)) != cudaSuccess ||
       (e = cudaMemsetAsync(a->d_grad_alpha, 0, sizeof(float) * ctx->n_alpha, s)) != cudaSuccess ||
-      (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * ETAC_GRAD_WEIGHTS_LEN, s)) != cudaSuccess) ||
+      (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * (pointnet ? ETAC_GRAD_WEIGHTS_POINTNET_LEN : ETAC_GRAD_WEIGHTS_LEN), s)) != cudaSuccess) ||
       (a->d_grad_penetration &&
        (e = cudaMemsetAsync(a->d_grad_penetration, 0, sizeof(float) * (size_t)a->n_envs * ctx->m.n_nodes, s)) != cudaSuccess))
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset", e));
   int n_s1 = 1;
   if ((e = launch_sdf(ctx->m, io, 0, &n_s1, s)) != cudaSuccess)  // S1: delta and the pair flags only
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("sdf_penetration_kernel", e));
-  if ((e = launch_backward(ctx->m, io, a->d_grad_out, a->d_grad_alpha, ctx->n_alpha, a->d_grad_weights, a->d_grad_penetration, ctx->n_sm, s)) != cudaSuccess)
+  // (PointNet: Phi does not see u_i, so backward_kernel runs without a residual -- dL/dalpha and the K part of
+  //  dL/ddelta -- and k_backward_pointnet.cu adds the weight gradients and the encoder-input part of dL/ddelta)
+  if ((e = launch_backward(ctx->m, io, a->d_grad_out, a->d_grad_alpha, ctx->n_alpha, pointnet ? nullptr : a->d_grad_weights,
+                           a->d_grad_penetration, ctx->n_sm, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("backward_kernel", e));
-  ctx->last_launches = 1 + n_s1;
+  int n_pn = 0;
+  if (pointnet && (a->d_grad_weights || a->d_grad_penetration) &&
+      (e = launch_backward_pointnet(ctx->m, io, a->d_grad_out, a->d_grad_weights, a->d_grad_penetration, ctx->n_sm, &n_pn, s)) != cudaSuccess)
+    return fail(ctx, ETAC_ERR_CUDA, cuda_msg("pn_bwd_node_kernel", e));
+  ctx->last_launches = 1 + n_s1 + n_pn;
   return ETAC_OK;
 }
 

@@ -95,9 +95,13 @@ struct DevModel {
   const uint8_t* wimg;        // kWImgBytes
   const uint8_t* wimg_pn;     // kPnImgBytes (ETAC_RESID_POINTNET)
   const float* pn_f32;        // G1^T [in][out] g1[64] D1[:,64:128]^T [in][out] d1[64] (fp32, pn_global_kernel)
-  const float* pn_w32;        // fp32 contexts: E1[64x9] e1 E2[64x64] e2 D1[:, :64] D2[3x64] d2 (k_pointnet_fp32.cu)
+  const float* pn_w32;        // E1[64x9] e1 E2[64x64] e2 D1[:, :64] D2[3x64] d2 (fp32: k_pointnet_fp32.cu, k_backward_pointnet.cu)
   uint32_t* gmax;             // [P x max_envs x 64] max-pooled encoder features as order-preserving keys
   float* cvec;                // [P x max_envs x 64] c_(e,p) / 2
+  // workspaces of the PointNet backward, [P x max_envs x 64] each (indexed by the environment)
+  unsigned long long* pn_gkey;  // column max with its arg-max node: key of the value << 32 | ~node
+  float* pn_ssum;               // sum over the rows of dL/d(decoder hidden pre-activation)
+  float* pn_ggmax;              // dL/d(max-pooled feature)
   float wout[196];            // output layer of Phi in fp32: W3 (or D2) [3 x 64] row-major, then b3 (d2) at 192..194
   // per-step workspace
   float* delta;               // [max_envs x N]
@@ -181,6 +185,10 @@ cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* l
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t launch_pointnet_fp32(const DevModel& m, const StepIO& io, int* launches, cudaStream_t s);
 cudaError_t pointnet_fp32_configure();
+void launch_pointnet_global_env(const DevModel& m, int n_envs, cudaStream_t s);
+cudaError_t backward_pointnet_configure();
+cudaError_t launch_backward_pointnet(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_w, float* grad_delta,
+                                     int n_sm, int* launches, cudaStream_t s);
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t backward_configure();
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,

@@ -8,43 +8,9 @@
 //                          mask + combine (Eq. 2)
 // gmax / cvec are the arrays of the bf16 path, indexed by the environment instead of the contact-list slot.
 #include "etac_internal.h"
+#include "pointnet_fp32.cuh"
 
 namespace etac {
-
-constexpr int kPnW32Floats = 64 * 9 + 64 + 64 * 64 + 64 + 64 * 64 + 3 * 64 + 3;  // E1 e1 E2 e2 D1[:, :64] D2 d2
-
-__device__ __forceinline__ float silu_exact(float x) { return x / (1.0f + expf(-x)); }
-// monotone map float -> uint32 (max of keys = key of the max); 0 is below every float's key
-__device__ __forceinline__ uint32_t float_key(float f) {
-  const uint32_t b = __float_as_uint(f);
-  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
-}
-__device__ __forceinline__ float key_float(uint32_t k) {
-  return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
-}
-
-// point-wise features of one node: x9 = [p(3), n(3), u^(3)], weights in shared memory
-__device__ __forceinline__ void pn_features(const float* __restrict__ sw, const float (&x9)[9], float (&f)[64]) {
-  const float *E1 = sw, *e1 = E1 + 576, *E2 = e1 + 64, *e2 = E2 + 4096;
-  float h1[64];
-#pragma unroll
-  for (int k = 0; k < 64; ++k) {
-    float s = e1[k];
-#pragma unroll
-    for (int c = 0; c < 9; ++c) s = fmaf(E1[k * 9 + c], x9[c], s);
-    h1[k] = silu_exact(s);
-  }
-  for (int k2 = 0; k2 < 64; ++k2) {
-    float s = e2[k2];
-    const float4* w = reinterpret_cast<const float4*>(E2 + k2 * 64);
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const float4 wv = w[k];
-      s = fmaf(wv.x, h1[4 * k], s), s = fmaf(wv.y, h1[4 * k + 1], s), s = fmaf(wv.z, h1[4 * k + 2], s), s = fmaf(wv.w, h1[4 * k + 3], s);
-    }
-    f[k2] = silu_exact(s);
-  }
-}
 
 __global__ void __launch_bounds__(kGatherChunk) pn_encode_fp32_kernel(DevModel m, StepIO io) {
   extern __shared__ float s_w[];
@@ -181,6 +147,11 @@ __global__ void __launch_bounds__(kGatherChunk) pn_decode_fp32_kernel(DevModel m
   }
 }
 
+// c_(e,p) for every contacting (env, patch) from gmax (also the first half of the backward's global pass)
+void launch_pointnet_global_env(const DevModel& m, int n_envs, cudaStream_t s) {
+  pn_global_env_kernel<<<dim3((unsigned)((n_envs + 15) / 16), (unsigned)m.n_patches), 64, 0, s>>>(m, n_envs);
+}
+
 cudaError_t pointnet_fp32_configure() {
   return cudaFuncSetAttribute(pn_decode_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPnW32Floats * 4);
 }
@@ -191,7 +162,7 @@ cudaError_t launch_pointnet_fp32(const DevModel& m, const StepIO& io, int* launc
   if (e != cudaSuccess) return e;
   const unsigned grid = (unsigned)((int64_t)m.n_chunks * io.n_envs);
   pn_encode_fp32_kernel<<<grid, kGatherChunk, (576 + 64 + 4096 + 64) * 4, s>>>(m, io);
-  pn_global_env_kernel<<<dim3((unsigned)((io.n_envs + 15) / 16), (unsigned)m.n_patches), 64, 0, s>>>(m, io.n_envs);
+  launch_pointnet_global_env(m, io.n_envs, s);
   pn_decode_fp32_kernel<<<grid, kGatherChunk, kPnW32Floats * 4, s>>>(m, io);
   *launches = 3;
   return cudaGetLastError();

@@ -75,6 +75,9 @@ class etac_params(C.Structure):
 
 ETAC_GRAD_WEIGHTS_LEN = 4995
 GRAD_WEIGHTS_LAYOUT = (("W1", (64, 9)), ("b1", (64,)), ("W2", (64, 64)), ("b2", (64,)), ("W3", (3, 64)), ("b3", (3,)))
+ETAC_GRAD_WEIGHTS_POINTNET_LEN = 17411
+GRAD_WEIGHTS_POINTNET_LAYOUT = (("E1", (64, 9)), ("e1", (64,)), ("E2", (64, 64)), ("e2", (64,)), ("G1", (64, 64)), ("g1", (64,)),
+                                ("D1", (64, 128)), ("d1", (64,)), ("D2", (3, 64)), ("d2", (3,)))
 
 _lib = None
 
@@ -261,9 +264,10 @@ def etac_update_params(ctx, alpha=None, weights=None) -> None:
 
 
 def split_grad_weights(flat):
-    """[4995] -> {"W1": [64, 9], "b1": [64], ...} views in the order of etac_backward_args.d_grad_weights."""
+    """[4995] -> {"W1": [64, 9], "b1": [64], ...} or [17411] -> {"E1": [64, 9], ...} (PointNet): views in the order
+    of etac_backward_args.d_grad_weights."""
     out, o = {}, 0
-    for name, shape in GRAD_WEIGHTS_LAYOUT:
+    for name, shape in (GRAD_WEIGHTS_POINTNET_LAYOUT if flat.shape[0] == ETAC_GRAD_WEIGHTS_POINTNET_LEN else GRAD_WEIGHTS_LAYOUT):
         n = int(np.prod(shape))
         out[name] = flat[o:o + n].reshape(shape)
         o += n

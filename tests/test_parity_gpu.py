@@ -516,6 +516,9 @@ def _backward_case(kind):
     if kind == "hand_bf16":
         wl = dataclasses.replace(W.config3(15, 19), weights=W.make_weights(3, 4, std=0.2))
         return wl, "bf16", T.ETAC_ACTIVE_PASSTHROUGH, True
+    if kind == "pointnet_hand_bf16":
+        wl = dataclasses.replace(W.config3(15, 19), weights=W.make_pointnet_weights(3, 4, std=0.12))
+        return wl, "bf16", T.ETAC_ACTIVE_PASSTHROUGH, True
     mesh = W.assemble([W.fib_cap(6.0, 72), W.flat_pad(10, 20, 1.0), W.half_cylinder(5.0, 12.0, 9, 15)])   # ragged: 72, 200, 135
     rng = np.random.default_rng(31)
     E = 9
@@ -527,20 +530,24 @@ def _backward_case(kind):
         ind["type"][:, k], ind["param"][:, k, 0] = W.IND_SPHERE, size
         ind["pose"][:, k, 0:3], ind["pose"][:, k, 3:7] = centre, q
     alpha = np.asarray([0.45, 0.7, 0.55], np.float32)
-    wl = W.Workload("grad_case", mesh, alpha, W.make_weights(9, 1, std=0.3), E, 2, ind, None, "fp32")
-    mode = T.ETAC_ACTIVE_PROPAGATE if kind == "propagate" else T.ETAC_ACTIVE_PASSTHROUGH
+    weights = W.make_pointnet_weights(9, 1, std=0.15) if kind.startswith("pointnet") else W.make_weights(9, 1, std=0.3)
+    wl = W.Workload("grad_case", mesh, alpha, weights, E, 2, ind, None, "fp32")
+    mode = T.ETAC_ACTIVE_PROPAGATE if kind.endswith("propagate") else T.ETAC_ACTIVE_PASSTHROUGH
     return wl, "fp32", mode, kind != "no_resid"
 
 
-@pytest.mark.parametrize("kind", ["per_patch_alpha", "propagate", "no_resid", "hand_bf16"])
+@pytest.mark.parametrize("kind", ["per_patch_alpha", "propagate", "no_resid", "hand_bf16", "pointnet", "pointnet_propagate",
+                                  "pointnet_hand_bf16"])
 def test_backward_against_the_gradient_oracle(kind):
     """etac_backward (calibration gradients of Eq. 3) against oracle/etac_oracle_grad.py
-    (itself pinned by finite differences): dL/dalpha and dL/d(MLP weights) for L = 0.5*||U - U*||^2.
+    (itself pinned by finite differences): dL/dalpha, dL/ddelta and dL/d(weights of Phi) -- the per-node MLP or the
+    paper's PointNet -- for L = 0.5*||U - U*||^2.
     fp32 arithmetic, fp32 atomics across CTAs: 2e-5 of the largest entry of each tensor (measured: 1e-8 .. 6e-7)."""
     import torch
     from oracle import etac_oracle as O, etac_oracle_grad as OG
     wl, precision, mode, resid = _backward_case(kind)
-    m = O.model_from_workload(wl, resid_arch="pernode" if resid else "none",
+    pointnet = "E1" in wl.weights
+    m = O.model_from_workload(wl, resid_arch=("pointnet" if pointnet else "pernode") if resid else "none",
                               active_mode="propagate" if mode == T.ETAC_ACTIVE_PROPAGATE else "passthrough")
     U = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)["U"]
     G = U - np.random.default_rng(3).normal(0, 0.2, U.shape)
@@ -550,7 +557,8 @@ def test_backward_against_the_gradient_oracle(kind):
         dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
         d_G = torch.from_numpy(G.astype(np.float32)).to(eng.device)
         g_alpha = torch.full((len(wl.alpha),), 7.0, device=eng.device)
-        g_w = torch.full((T.ETAC_GRAD_WEIGHTS_LEN,), 7.0, device=eng.device) if resid else None
+        n_w = T.ETAC_GRAD_WEIGHTS_POINTNET_LEN if pointnet else T.ETAC_GRAD_WEIGHTS_LEN
+        g_w = torch.full((n_w,), 7.0, device=eng.device) if resid else None
         g_pen = torch.full((wl.n_envs, eng.N), 7.0, device=eng.device)
         stream = torch.cuda.current_stream().cuda_stream
         for _ in range(2):                                                # the outputs are overwritten, not accumulated
