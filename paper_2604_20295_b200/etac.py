@@ -31,7 +31,8 @@ ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
 
 EXPORTS = ["etac_create", "etac_destroy", "etac_step", "etac_set_option", "etac_get_info", "etac_last_error",
            "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward", "etac_update_params",
-           "etac_measure_sfu_rate"]
+           "etac_measure_sfu_rate", "etac_propagate_noalloc"]
+ETAC_NOALLOC_MAX_ENTRIES, ETAC_NOALLOC_MAX_ENVS = 262144, 4096
 
 _fp = C.POINTER(C.c_float)
 _ip = C.POINTER(C.c_int32)
@@ -104,6 +105,8 @@ def load() -> C.CDLL:
         lib.etac_backward.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(etac_backward_args)]
         lib.etac_measure_sfu_rate.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         lib.etac_set_sdf_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
+        lib.etac_propagate_noalloc.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p,
+                                               C.c_void_p, C.c_char_p, C.c_int32]
         for name in EXPORTS:
             getattr(lib, name)
         _lib = lib
@@ -261,6 +264,15 @@ def etac_update_params(ctx, alpha=None, weights=None) -> None:
             keep.append(w)
             setattr(p, k, w.ctypes.data_as(_fp))
     _check(ctx, load().etac_update_params(ctx, C.byref(p)))
+
+
+def etac_propagate_noalloc(stream, n_envs, n_nodes, alpha, pos, normal, penetration, out) -> None:
+    """include/etac_noalloc.h: analytic propagation + mask of one patch, no allocation (device fp32 tensors)."""
+    err = C.create_string_buffer(256)
+    st = load().etac_propagate_noalloc(stream, n_envs, n_nodes, alpha, _dptr(pos), _dptr(normal), _dptr(penetration), _dptr(out),
+                                       err, len(err))
+    if st != ETAC_OK:
+        raise EtacError(st, err.value.decode())
 
 
 def split_grad_weights(flat):
