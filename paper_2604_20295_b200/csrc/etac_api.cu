@@ -199,13 +199,13 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
     if (abl == ETAC_ABLATE_LINEAR_ONLY) {
       DevModel lin = ctx->m;
       lin.resid = ETAC_RESID_NONE;
-      e = launch_gather_fp32(lin, io, s);
+      e = launch_gather_fp32(lin, io, ctx->n_sm, s);
     } else if (ctx->m.resid == ETAC_RESID_POINTNET) {
       int n_launch = 1;
       e = launch_pointnet_fp32(ctx->m, io, &n_launch, s);
       ctx->last_launches += n_launch - 1;
     } else {
-      e = launch_gather_fp32(ctx->m, io, s);
+      e = launch_gather_fp32(ctx->m, io, ctx->n_sm, s);
     }
     if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("gather_fp32_kernel", e));
   }
@@ -225,7 +225,9 @@ struct PerNodeStage {
 };
 void stage_pernode(const float* W1, const float* b1, const float* W2, const float* b2, const float* W3, const float* b3,
                    PerNodeStage* st) {
-  st->wf.assign(64 * 3 + 64 * 64 + 64 + 3 * 64 + 3, 0.f);
+  st->wf.assign(kWf32W2t + 64 * 64, 0.f);  // W1u | W2 | b2 | W3 | b3 | pad | W2^T (for gather_fp32_kernel)
+  for (int k2 = 0; k2 < 64; ++k2)
+    for (int k = 0; k < 64; ++k) st->wf[kWf32W2t + k * 64 + k2] = W2[k2 * 64 + k];
   float* q = st->wf.data();
   for (int k = 0; k < 64; ++k)
     for (int cc = 0; cc < 3; ++cc) *q++ = W1[k * 9 + cc];
@@ -538,6 +540,7 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   }
   c->n_alpha = d->n_alpha;
   CK(backward_configure(), "cudaFuncSetAttribute(backward_kernel)");
+  CK(gather_fp32_configure(), "cudaFuncSetAttribute(gather_fp32_kernel)");
   CK(cudaDeviceSynchronize(), "create-time kernels");
 #undef CK
   *out = c;

@@ -17,6 +17,8 @@ constexpr int kHidden = 64;
 constexpr int kMaxPatches = 1024;
 
 // One sensor patch (contiguous node range; K is zero across patches, R9).
+constexpr int kWf32W2t = 4548;  // offset of W2^T in DevModel::wf32 (16-byte aligned, behind the 4547 floats of the blob)
+
 struct PatchInfo {
   int32_t off;        // first node
   int32_t n;          // nodes in the patch
@@ -91,6 +93,7 @@ struct DevModel {
   const float* k32;           // per patch [n x n]
   const __nv_bfloat16* k16;   // [N x kw], row i holds K_p[i - off_p][0..n_p) then zeros
   const float* wf32;          // fp32 weights blob: W1u[64x3] | c1t[64 x N] is separate | W2[64x64] b2[64] W3[3x64] b3[3]
+                              // | pad | W2^T[64x64] at kWf32W2t
   const float* c1t;           // [64 x N]: W1[:,3:9].[p;n] + b1, transposed for coalescing
   const uint8_t* wimg;        // kWImgBytes
   const uint8_t* wimg_pn;     // kPnImgBytes (ETAC_RESID_POINTNET)
@@ -182,7 +185,8 @@ __device__ __forceinline__ void store_out3(const StepIO& io, int env, int g, flo
 cudaError_t launch_build_k(const DevModel& m, float* k32, __nv_bfloat16* k16, cudaStream_t s);
 cudaError_t launch_build_c1(const DevModel& m, const float* W1, const float* b1, float* c1t, cudaStream_t s);
 cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags, int* launches, cudaStream_t s);
-cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, cudaStream_t s);
+cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, int n_sm, cudaStream_t s);
+cudaError_t gather_fp32_configure();
 cudaError_t launch_pointnet_fp32(const DevModel& m, const StepIO& io, int* launches, cudaStream_t s);
 cudaError_t pointnet_fp32_configure();
 void launch_pointnet_global_env(const DevModel& m, int n_envs, cudaStream_t s);
