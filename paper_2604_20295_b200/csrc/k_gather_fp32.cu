@@ -25,9 +25,10 @@ __device__ __forceinline__ float silu_f32(float x) { return __fdividef(x, 1.0f +
 //   layer 3  thread = (node, half of the hidden units), partial sums combined through shared memory
 // The grid is persistent: the weights (W2 transposed, so that a thread's four outputs are one 16-byte load) are
 // staged once per CTA, not once per 128 nodes.
-constexpr int kCtasPerSm = 3;            // 80 registers, 57 KB of shared memory: the phases of three items overlap on an SM
+constexpr int kCtasPerSm = 3;            // 80 registers, 73 KB of shared memory: the phases of three items overlap on an SM
 constexpr int kGT = 2 * kGatherChunk;   // threads per CTA
 constexpr int kSub = 4, kSweep = kSub * kGT;  // nodes of a patch scanned per sweep: kSub per thread
+constexpr int kCache = 1024;             // entries of the cached active-node list
 constexpr int kDepth = 16;              // K loads in flight per thread in the gather
 constexpr int kHld = kGatherChunk + 4;  // row pitch of the [64][128] activation arrays (rows stay 16-byte aligned)
 struct GatherSmem {
@@ -43,13 +44,79 @@ struct GatherSmem {
   float ulin[3][kGatherChunk];
   float part[2][3][kGatherChunk];  // per-half partial sums (gather: upper half; layer 3: upper half)
   int wcnt[kSub * (kGT / 32)];
+  // (last: the one-chunk-per-item instantiation is launched without them)
+  float cu[kCache][3];             // cached list of a patch's active nodes, shared by the chunks of an item
+  int cj[kCache];
 };
+constexpr size_t kGatherSmemNoCache = offsetof(GatherSmem, cu);
 static_assert(sizeof(float) * (kSweep * 3 + kSweep) <= sizeof(float) * 64 * kHld, "sweep arrays inside H");
 
-__global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m, StepIO io) {
+// Ordered compaction of the active nodes (delta > 0) among the nodes [base, base + kSweep) of a patch: entries
+// (u^_j, j) are appended in node order at u[slot0 ..], jl[slot0 ..] as far as they fit below `cap`; returns the number
+// of active nodes of the sweep.  Four delta loads in flight per thread: a sweep costs one L2 round trip and two barriers.
+__device__ __forceinline__ int compact_sweep(GatherSmem& S, const DevModel& m, const PatchInfo& pi, const float* __restrict__ delta,
+                                             int base, float (*u)[3], int* jl, int slot0, int cap) {
+  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  float d[kSub];
+  unsigned bal[kSub];
+#pragma unroll
+  for (int q = 0; q < kSub; ++q) {
+    const int j = base + q * kGT + t;
+    d[q] = j < pi.n ? delta[j] : 0.0f;
+  }
+#pragma unroll
+  for (int q = 0; q < kSub; ++q) {
+    bal[q] = __ballot_sync(0xffffffffu, d[q] > 0.0f);
+    if (lane == 0) S.wcnt[q * (kGT / 32) + warp] = __popc(bal[q]);
+  }
+  __syncthreads();
+  int pre[kSub] = {0, 0, 0, 0}, total = 0;
+#pragma unroll
+  for (int w = 0; w < kSub * (kGT / 32); ++w) {
+    const int c = S.wcnt[w];
+#pragma unroll
+    for (int q = 0; q < kSub; ++q) pre[q] += w < q * (kGT / 32) + warp ? c : 0;
+    total += c;
+  }
+#pragma unroll
+  for (int q = 0; q < kSub; ++q)
+    if (d[q] > 0.0f) {
+      const int j = base + q * kGT + t;
+      const int slot = slot0 + pre[q] + __popc(bal[q] & ((1u << lane) - 1u));
+      if (slot < cap) {
+        const float4 n = m.nrm4[pi.off + j];
+        jl[slot] = j;
+        u[slot][0] = -d[q] * n.x, u[slot][1] = -d[q] * n.y, u[slot][2] = -d[q] * n.z;
+      }
+    }
+  __syncthreads();  // entries visible; wcnt free for the next sweep
+  return total;
+}
+
+// a += sum over the list of K[j][li] u^_j: the two halves of the CTA take alternating groups of kDepth entries for
+// their node, kDepth loads of K in flight per thread (the loop is bound by their latency); fixed order: deterministic
+__device__ __forceinline__ void gather_list(const float (*u)[3], const int* jl, int total, const float* __restrict__ K, int n, int li,
+                                            int half, float& ax, float& ay, float& az) {
+  for (int a0 = half * kDepth; a0 < total; a0 += 2 * kDepth) {
+    float kv[kDepth];
+#pragma unroll
+    for (int q = 0; q < kDepth; ++q) kv[q] = a0 + q < total ? K[(int64_t)jl[a0 + q] * n + li] : 0.0f;
+#pragma unroll
+    for (int q = 0; q < kDepth; ++q) {
+      const int a = min(a0 + q, total - 1);  // (kv = 0 beyond the list)
+      ax = fmaf(kv[q], u[a][0], ax);
+      ay = fmaf(kv[q], u[a][1], ay);
+      az = fmaf(kv[q], u[a][2], az);
+    }
+  }
+}
+
+// kShare: work items of several chunks with the shared list (cpg > 1); false: one chunk per item, no cache code
+template <bool kShare>
+__global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m, StepIO io, int cpg) {
   extern __shared__ __align__(16) uint8_t smem_raw[];
   GatherSmem& S = *reinterpret_cast<GatherSmem*>(smem_raw);
-  const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
+  const int t = threadIdx.x;
   const int node = t & (kGatherChunk - 1), half = t >> 7;  // (warp-uniform)
   const bool mlp = m.resid != ETAC_RESID_NONE;
   if (mlp) {
@@ -62,10 +129,17 @@ __global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m
   }
   __syncthreads();
 
-  const int64_t n_items = (int64_t)m.n_chunks * io.n_envs;
+  // Work item = `cpg` consecutive chunks of one environment (the host sizes cpg so that every CTA still gets several
+  // items).  The chunks of one patch in an item share the patch's compacted active-node list if it fits the cache:
+  // without it every chunk scans all delta of its patch, N / 128 scans per environment and patch.
+  const int gpe = (m.n_chunks + cpg - 1) / cpg;  // items per environment
+  const int64_t n_items = (int64_t)gpe * io.n_envs;
   for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
-    const int e = (int)(item / m.n_chunks);
-    const ChunkInfo ch = m.chunk[item - (int64_t)e * m.n_chunks];
+   const int e = (int)(item / gpe);
+   const int c0 = (int)(item - (int64_t)e * gpe) * cpg, c1 = min(c0 + cpg, m.n_chunks);
+   int cache_patch = -1, cache_total = -1;  // cache_total < 0: the list of cache_patch did not fit
+   for (int c = c0; c < c1; ++c) {
+    const ChunkInfo ch = m.chunk[c];
     if (!m.flags[(int64_t)e * m.n_patches + ch.patch]) continue;  // S1 zero-filled this patch (uniform over the CTA)
     const PatchInfo pi = m.patch[ch.patch];
     const bool valid = node < ch.count;
@@ -74,56 +148,21 @@ __global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m
     const float* __restrict__ delta = m.delta + (int64_t)e * m.n_nodes + pi.off;
     const float* __restrict__ K = m.k32 + pi.k32_off;
 
-    // ---- Omega U_a: the patch's active nodes compacted in node order, kSweep = 1024 per sweep (four delta loads
-    // in flight per thread: a sweep costs one L2 round trip and three barriers); the two halves of the CTA
-    // sum alternating groups of kDepth entries of a sweep for their node (fixed order: deterministic)
+    // ---- Omega U_a over the patch's active nodes in node order
     float ax = 0.f, ay = 0.f, az = 0.f;
-    for (int base = 0; base < pi.n; base += kSweep) {
-      float d[kSub];
-      unsigned bal[kSub];
-#pragma unroll
-      for (int q = 0; q < kSub; ++q) {
-        const int j = base + q * kGT + t;
-        d[q] = j < pi.n ? delta[j] : 0.0f;
+    if (kShare && ch.patch != cache_patch && c + 1 < c1 && m.chunk[c + 1].patch == ch.patch) {  // more chunks of this patch follow
+      int total = 0;
+      for (int base = 0; base < pi.n; base += kSweep) total += compact_sweep(S, m, pi, delta, base, S.cu, S.cj, total, kCache);
+      cache_patch = ch.patch, cache_total = total <= kCache ? total : -1;
+    }
+    if (kShare && ch.patch == cache_patch && cache_total >= 0) {
+      gather_list(S.cu, S.cj, cache_total, K, pi.n, li, half, ax, ay, az);
+    } else {
+      for (int base = 0; base < pi.n; base += kSweep) {  // (sweep arrays inside H: the previous chunk's MLP is over)
+        const int total = compact_sweep(S, m, pi, delta, base, S.u, S.j, 0, kSweep);
+        gather_list(S.u, S.j, total, K, pi.n, li, half, ax, ay, az);
+        __syncthreads();
       }
-#pragma unroll
-      for (int q = 0; q < kSub; ++q) {
-        bal[q] = __ballot_sync(0xffffffffu, d[q] > 0.0f);
-        if (lane == 0) S.wcnt[q * (kGT / 32) + warp] = __popc(bal[q]);
-      }
-      __syncthreads();
-      int pre[kSub] = {0, 0, 0, 0}, total = 0;
-#pragma unroll
-      for (int w = 0; w < kSub * (kGT / 32); ++w) {
-        const int c = S.wcnt[w];
-#pragma unroll
-        for (int q = 0; q < kSub; ++q) pre[q] += w < q * (kGT / 32) + warp ? c : 0;
-        total += c;
-      }
-#pragma unroll
-      for (int q = 0; q < kSub; ++q)
-        if (d[q] > 0.0f) {
-          const int j = base + q * kGT + t;
-          const int slot = pre[q] + __popc(bal[q] & ((1u << lane) - 1u));
-          const float4 n = m.nrm4[pi.off + j];
-          S.j[slot] = j;
-          S.u[slot][0] = -d[q] * n.x, S.u[slot][1] = -d[q] * n.y, S.u[slot][2] = -d[q] * n.z;
-        }
-      __syncthreads();
-      // kDepth loads of K in flight per thread (the loop is bound by their latency); the halves alternate groups
-      for (int a0 = half * kDepth; a0 < total; a0 += 2 * kDepth) {
-        float kv[kDepth];
-#pragma unroll
-        for (int q = 0; q < kDepth; ++q) kv[q] = a0 + q < total ? K[(int64_t)S.j[a0 + q] * pi.n + li] : 0.0f;
-#pragma unroll
-        for (int q = 0; q < kDepth; ++q) {
-          const int a = min(a0 + q, total - 1);  // (kv = 0 beyond the list)
-          ax = fmaf(kv[q], S.u[a][0], ax);
-          ay = fmaf(kv[q], S.u[a][1], ay);
-          az = fmaf(kv[q], S.u[a][2], az);
-        }
-      }
-      __syncthreads();
     }
     if (half) S.part[0][0][node] = ax, S.part[0][1][node] = ay, S.part[0][2][node] = az;
     __syncthreads();
@@ -215,17 +254,24 @@ __global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m
     const int64_t o = ((int64_t)e * m.n_nodes + g) * 3;
     store_out3(io, e, g, ox, oy, oz);
     if (io.analytic_out) io.analytic_out[o] = ax, io.analytic_out[o + 1] = ay, io.analytic_out[o + 2] = az;
+   }
   }
 }
 
 cudaError_t gather_fp32_configure() {
-  return cudaFuncSetAttribute(gather_fp32_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GatherSmem));
+  cudaError_t e = cudaFuncSetAttribute(gather_fp32_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GatherSmem));
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(gather_fp32_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GatherSmem));
+  return e;
 }
 
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, int n_sm, cudaStream_t s) {
-  const int64_t n_items = (int64_t)m.n_chunks * io.n_envs;
-  const unsigned grid = (unsigned)(n_items < kCtasPerSm * (int64_t)n_sm ? n_items : kCtasPerSm * (int64_t)n_sm);
-  gather_fp32_kernel<<<grid, kGT, sizeof(GatherSmem), s>>>(m, io);
+  const int64_t slots = (int64_t)kCtasPerSm * n_sm, n_chunk_items = (int64_t)m.n_chunks * io.n_envs;
+  // chunks per item: as many as leave every resident CTA about eight items (load balance), at most 16
+  const int cpg = (int)(n_chunk_items / (8 * slots) < 1 ? 1 : (n_chunk_items / (8 * slots) > 16 ? 16 : n_chunk_items / (8 * slots)));
+  const int64_t n_items = (int64_t)((m.n_chunks + cpg - 1) / cpg) * io.n_envs;
+  const unsigned grid = (unsigned)(n_items < slots ? n_items : slots);
+  if (cpg > 1) gather_fp32_kernel<true><<<grid, kGT, sizeof(GatherSmem), s>>>(m, io, cpg);
+  else gather_fp32_kernel<false><<<grid, kGT, kGatherSmemNoCache, s>>>(m, io, 1);
   return cudaGetLastError();
 }
 

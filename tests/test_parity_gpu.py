@@ -254,6 +254,21 @@ def test_fp32_context_large_batch_all_envs():
     _report("cfg5 fp32 E=1024", compare(gpu, ref, TOL["fp32"], resid_tol=1e-4, label="cfg5-fp32-1024", delta_tol=1e-4))
 
 
+@pytest.mark.parametrize("frac", [0.01, 0.2])
+def test_fp32_large_patch_shared_and_overflowing_active_lists(frac):
+    """fp32 context, one patch of 8192 nodes, enough environments for the gather kernel to take several chunks of a
+    patch per work item: at 1 % contact the chunks of an item share ONE compacted list of the patch's active nodes,
+    at 20 % (about 1300 active nodes per environment) the list exceeds the cache and every chunk scans for itself.
+    Sampled environments against the oracle at the fp32 tolerance; every row of every environment finite."""
+    wl = W.config5(192, 8192, True, frac, "fp32")
+    envs = [0, 1, 95, 191]
+    gpu, ref = run_gpu(wl), run_oracle(wl, envs=envs)
+    n_act = ref["mask"].sum(1)
+    assert (n_act.max() > 1024) == (frac == 0.2) and n_act.min() > 0
+    _report(f"cfg5 N=8192 fp32 frac={frac}", compare(gpu, ref, TOL["fp32"], envs=envs, resid_tol=1e-4, label="fp32-lists", delta_tol=1e-4))
+    assert np.isfinite(gpu["U"]).all()
+
+
 def test_full_size_config4_strided():
     """BASELINE.json configs[3] at full size (4096 envs, one dense K[8192 x 8192], bf16); the
     oracle checks every 16th environment (256 of them, so that every CTA's env tiles are hit) element by
