@@ -54,15 +54,15 @@ static_assert(sizeof(float) * (kSweep * 3 + kSweep) <= sizeof(float) * 64 * kHld
 // Ordered compaction of the active nodes (delta > 0) among the nodes [base, base + kSweep) of a patch: entries
 // (u^_j, j) are appended in node order at u[slot0 ..], jl[slot0 ..] as far as they fit below `cap`; returns the number
 // of active nodes of the sweep.  Four delta loads in flight per thread: a sweep costs one L2 round trip and two barriers.
-__device__ __forceinline__ int compact_sweep(GatherSmem& S, const DevModel& m, const PatchInfo& pi, const float* __restrict__ delta,
-                                             int base, float (*u)[3], int* jl, int slot0, int cap) {
+__device__ __forceinline__ int compact_sweep(GatherSmem& S, const float4* __restrict__ nrm4, int pn, const float* __restrict__ delta,
+                                             int base, float (*__restrict__ u)[3], int* __restrict__ jl, int slot0, int cap) {
   const int t = threadIdx.x, lane = t & 31, warp = t >> 5;
   float d[kSub];
   unsigned bal[kSub];
 #pragma unroll
   for (int q = 0; q < kSub; ++q) {
     const int j = base + q * kGT + t;
-    d[q] = j < pi.n ? delta[j] : 0.0f;
+    d[q] = j < pn ? delta[j] : 0.0f;
   }
 #pragma unroll
   for (int q = 0; q < kSub; ++q) {
@@ -84,7 +84,7 @@ __device__ __forceinline__ int compact_sweep(GatherSmem& S, const DevModel& m, c
       const int j = base + q * kGT + t;
       const int slot = slot0 + pre[q] + __popc(bal[q] & ((1u << lane) - 1u));
       if (slot < cap) {
-        const float4 n = m.nrm4[pi.off + j];
+        const float4 n = nrm4[j];
         jl[slot] = j;
         u[slot][0] = -d[q] * n.x, u[slot][1] = -d[q] * n.y, u[slot][2] = -d[q] * n.z;
       }
@@ -95,7 +95,7 @@ __device__ __forceinline__ int compact_sweep(GatherSmem& S, const DevModel& m, c
 
 // a += sum over the list of K[j][li] u^_j: the two halves of the CTA take alternating groups of kDepth entries for
 // their node, kDepth loads of K in flight per thread (the loop is bound by their latency); fixed order: deterministic
-__device__ __forceinline__ void gather_list(const float (*u)[3], const int* jl, int total, const float* __restrict__ K, int n, int li,
+__device__ __forceinline__ void gather_list(const float (*__restrict__ u)[3], const int* __restrict__ jl, int total, const float* __restrict__ K, int n, int li,
                                             int half, float& ax, float& ay, float& az) {
   for (int a0 = half * kDepth; a0 < total; a0 += 2 * kDepth) {
     float kv[kDepth];
@@ -152,14 +152,14 @@ __global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m
     float ax = 0.f, ay = 0.f, az = 0.f;
     if (kShare && ch.patch != cache_patch && c + 1 < c1 && m.chunk[c + 1].patch == ch.patch) {  // more chunks of this patch follow
       int total = 0;
-      for (int base = 0; base < pi.n; base += kSweep) total += compact_sweep(S, m, pi, delta, base, S.cu, S.cj, total, kCache);
+      for (int base = 0; base < pi.n; base += kSweep) total += compact_sweep(S, m.nrm4 + pi.off, pi.n, delta, base, S.cu, S.cj, total, kCache);
       cache_patch = ch.patch, cache_total = total <= kCache ? total : -1;
     }
     if (kShare && ch.patch == cache_patch && cache_total >= 0) {
       gather_list(S.cu, S.cj, cache_total, K, pi.n, li, half, ax, ay, az);
     } else {
       for (int base = 0; base < pi.n; base += kSweep) {  // (sweep arrays inside H: the previous chunk's MLP is over)
-        const int total = compact_sweep(S, m, pi, delta, base, S.u, S.j, 0, kSweep);
+        const int total = compact_sweep(S, m.nrm4 + pi.off, pi.n, delta, base, S.u, S.j, 0, kSweep);
         gather_list(S.u, S.j, total, K, pi.n, li, half, ax, ay, az);
         __syncthreads();
       }
@@ -267,7 +267,9 @@ cudaError_t gather_fp32_configure() {
 cudaError_t launch_gather_fp32(const DevModel& m, const StepIO& io, int n_sm, cudaStream_t s) {
   const int64_t slots = (int64_t)kCtasPerSm * n_sm, n_chunk_items = (int64_t)m.n_chunks * io.n_envs;
   // chunks per item: as many as leave every resident CTA about eight items (load balance), at most 16
-  const int cpg = (int)(n_chunk_items / (8 * slots) < 1 ? 1 : (n_chunk_items / (8 * slots) > 16 ? 16 : n_chunk_items / (8 * slots)));
+  // (only for meshes with a patch of >= 8 chunks: on small patches the shared list saves less than the larger items cost)
+  int cpg = (int)(n_chunk_items / (8 * slots) < 1 ? 1 : (n_chunk_items / (8 * slots) > 16 ? 16 : n_chunk_items / (8 * slots)));
+  if (m.max_patch_nodes < 8 * kGatherChunk) cpg = 1;
   const int64_t n_items = (int64_t)((m.n_chunks + cpg - 1) / cpg) * io.n_envs;
   const unsigned grid = (unsigned)(n_items < slots ? n_items : slots);
   if (cpg > 1) gather_fp32_kernel<true><<<grid, kGT, sizeof(GatherSmem), s>>>(m, io, cpg);
