@@ -227,6 +227,50 @@ def make_pointnet_weights(cfg: int, seed: int = 0, std: float = 0.1):
 
 
 # --------------------------------------------------------------------------------------
+# closed triangle meshes of objects (inputs of etac_mesh_to_sdf_grid; geometry only)
+# --------------------------------------------------------------------------------------
+def box_mesh(hx, hy, hz):
+    """Axis-aligned box with half extents (hx, hy, hz): 8 vertices, 12 outward-oriented triangles."""
+    v = np.array([[sx * hx, sy * hy, sz * hz] for sx in (-1, 1) for sy in (-1, 1) for sz in (-1, 1)], np.float64)
+    quads = [(0, 1, 3, 2), (4, 6, 7, 5), (0, 4, 5, 1), (2, 3, 7, 6), (0, 2, 6, 4), (1, 5, 7, 3)]
+    t = [tri for a, b, c, d in quads for tri in ((a, b, c), (a, c, d))]
+    return v, np.asarray(t, np.int32)
+
+
+def tetra_mesh(scale=1.0):
+    """Regular tetrahedron centred at the origin, outward-oriented."""
+    v = scale * np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], np.float64)
+    t = np.array([[0, 1, 2], [0, 3, 1], [0, 2, 3], [1, 3, 2]], np.int32)
+    return v, t
+
+
+def icosphere(radius, subdivisions):
+    """Icosahedron subdivided `subdivisions` times, vertices on the sphere of `radius` (20 * 4^s triangles)."""
+    g = (1.0 + math.sqrt(5.0)) / 2.0
+    v = [(-1, g, 0), (1, g, 0), (-1, -g, 0), (1, -g, 0), (0, -1, g), (0, 1, g), (0, -1, -g), (0, 1, -g),
+         (g, 0, -1), (g, 0, 1), (-g, 0, -1), (-g, 0, 1)]
+    v = [np.asarray(x, np.float64) / np.linalg.norm(x) for x in v]
+    t = [(0, 11, 5), (0, 5, 1), (0, 1, 7), (0, 7, 10), (0, 10, 11), (1, 5, 9), (5, 11, 4), (11, 10, 2), (10, 7, 6),
+         (7, 1, 8), (3, 9, 4), (3, 4, 2), (3, 2, 6), (3, 6, 8), (3, 8, 9), (4, 9, 5), (2, 4, 11), (6, 2, 10), (8, 6, 7),
+         (9, 8, 1)]
+    for _ in range(subdivisions):
+        mid, t2 = {}, []
+
+        def m(i, j):
+            key = (min(i, j), max(i, j))
+            if key not in mid:
+                x = v[i] + v[j]
+                v.append(x / np.linalg.norm(x))
+                mid[key] = len(v) - 1
+            return mid[key]
+        for a, b, c in t:
+            ab, bc, ca = m(a, b), m(b, c), m(c, a)
+            t2 += [(a, ab, ca), (b, bc, ab), (c, ca, bc), (ab, bc, ca)]
+        t = t2
+    return radius * np.asarray(v), np.asarray(t, np.int32)
+
+
+# --------------------------------------------------------------------------------------
 # workload container
 # --------------------------------------------------------------------------------------
 @dataclass

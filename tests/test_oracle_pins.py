@@ -612,3 +612,72 @@ def test_grid_sdf_of_a_sphere_obeys_the_interpolation_bound():
     # fp32 twin: same formula, every op in float32, agrees to rounding
     got32 = O.sdf_grid(vals, (-3.0, -3.0, -3.0), h, q[keep, 0], q[keep, 1], q[keep, 2], np.float32)
     assert got32.dtype == np.float32 and np.abs(got32 - got).max() < 5e-6
+
+
+# ---------------------------------------------------------------- P13: signed distance to a closed triangle mesh
+def _ray_parity_inside(V, T, P, direction):
+    """Brute force: a point is inside a closed surface iff a ray from it crosses the surface an odd number of times
+    (Moeller-Trumbore ray/triangle test, written out here; random direction, so no edge is hit exactly)."""
+    inside = np.zeros(len(P), dtype=bool)
+    for a, b, c in V[T]:
+        e1, e2 = b - a, c - a
+        h = np.cross(direction, e2)
+        det = e1 @ h
+        s = P - a
+        u = (s @ h) / det
+        qv = np.cross(s, e1)
+        v = (qv @ direction) / det
+        t = (qv @ e2) / det
+        inside ^= (u >= 0) & (v >= 0) & (u + v <= 1) & (t > 0)
+    return inside
+
+
+def test_mesh_sdf_oracle_against_closed_forms_and_ray_parity():
+    """oracle/etac_oracle_mesh.py (the SDF of an object mesh) against what the mathematics fixes:
+    a box mesh = the closed-form box SDF everywhere; inside a tetrahedron = minus the smallest face-plane distance;
+    an icosphere within its sagitta of |x| - r with the right sign; the sign against brute-force ray parity; the
+    result does not depend on the order or the (consistent) orientation of the triangles."""
+    from oracle import etac_oracle_mesh as M
+    rng = np.random.default_rng(11)
+    # (1) box: exact closed form, inside and outside, faces / edges / corners regions
+    V, T = W.box_mesh(1.0, 2.0, 0.5)
+    P = rng.uniform(-3.0, 3.0, (3000, 3))
+    phi = M.mesh_signed_distance(V, T, P)
+    ref = O.sdf_local(O.IND_BOX, [1.0, 2.0, 0.5], P[:, 0], P[:, 1], P[:, 2])
+    assert (ref < 0).sum() > 50 and np.abs(phi - ref).max() <= 1e-12
+    # (2) convex polyhedron, interior points: phi = -min_f distance to the plane of face f
+    V, T = W.tetra_mesh(1.5)
+    Q = rng.uniform(-0.4, 0.4, (500, 3))
+    n = np.cross(V[T[:, 1]] - V[T[:, 0]], V[T[:, 2]] - V[T[:, 0]])
+    n /= np.linalg.norm(n, axis=1, keepdims=True)
+    plane = np.einsum("fj,nfj->nf", n, V[T[:, 0]][None] - Q[:, None])           # > 0 inside (outward normals)
+    assert (plane > 0).all()
+    assert np.abs(M.mesh_signed_distance(V, T, Q) + plane.min(1)).max() <= 1e-12
+    # (3) icosphere: polyhedron inscribed in the sphere of radius r; its faces stay within the sagitta of the sphere
+    r = 2.0
+    V, T = W.icosphere(r, 2)
+    inradius = np.abs(np.einsum("fj,fj->f", np.cross(V[T[:, 1]] - V[T[:, 0]], V[T[:, 2]] - V[T[:, 0]]) /
+                                np.linalg.norm(np.cross(V[T[:, 1]] - V[T[:, 0]], V[T[:, 2]] - V[T[:, 0]]), axis=1, keepdims=True),
+                                V[T[:, 0]])).min()
+    sag = r - inradius
+    assert 0 < sag < 0.05 * r
+    P = rng.uniform(-3.0, 3.0, (2000, 3))
+    phi = M.mesh_signed_distance(V, T, P)
+    rad = np.linalg.norm(P, axis=1)
+    assert (np.abs(phi - (rad - r)) <= sag + 1e-12).all()
+    assert (phi[rad < inradius] < 0).all() and (phi[rad > r] > 0).all()
+    # (4) sign = ray parity (brute force), on the icosphere and on the box
+    d = rng.normal(size=3)
+    d /= np.linalg.norm(d)
+    assert np.array_equal(phi < 0, _ray_parity_inside(V, T, P, d))
+    Vb, Tb = W.box_mesh(1.0, 2.0, 0.5)
+    Pb = rng.uniform(-2.5, 2.5, (2000, 3))
+    assert np.array_equal(M.mesh_signed_distance(Vb, Tb, Pb) < 0, _ray_parity_inside(Vb, Tb, Pb, d))
+    # (5) triangle order and orientation do not matter
+    perm = rng.permutation(len(T))
+    assert np.abs(M.mesh_signed_distance(V, T[perm], P[:300]) - phi[:300]).max() <= 1e-12
+    assert np.abs(M.mesh_signed_distance(V, T[:, ::-1], P[:300]) - phi[:300]).max() <= 1e-12
+    # (6) the grid layout of etac_set_sdf_grid: values[iz, iy, ix] at origin + h (ix, iy, iz)
+    g = M.mesh_sdf_grid(Vb, Tb, (4, 5, 3), (-1.5, -2.0, -1.0), 1.0)
+    assert g.shape == (3, 5, 4)
+    assert abs(g[2, 1, 3] - O.sdf_local(O.IND_BOX, [1.0, 2.0, 0.5], np.float64(1.5), np.float64(-1.0), np.float64(1.0))) <= 1e-12
