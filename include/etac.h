@@ -195,6 +195,19 @@ etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value);
 etac_status etac_set_sdf_grid(etac_ctx* ctx, int32_t grid_id, int32_t nx, int32_t ny, int32_t nz,
                               const float* origin, float spacing, const float* values);
 
+/* Set-up helper for objects given as triangle meshes ("SDFs between nodes and object meshes"): samples
+ * the signed distance field of a CLOSED, consistently oriented triangle mesh on the grid origin + spacing*(ix, iy, iz),
+ * values_out[(iz*ny + iy)*nx + ix] -- the layout etac_set_sdf_grid takes, so that the object can be used as an
+ * ETAC_IND_GRID indenter.  distance = min over the triangles of the distance to the triangle; negative where the
+ * winding number of the surface around the point is >= 1/2 in magnitude (inside; either orientation).  Brute force on
+ * `device` (one thread per grid point over all triangles, fp32), host pointers in and out (vertices [n_vertices x 3],
+ * triangles [n_triangles x 3] vertex indices, origin [3]); allocates temporaries and synchronises: not for the step
+ * loop.  ETAC_ERR_INVALID_ARG: NULL, fewer than 4 vertices / triangles, index out of range, non-finite vertex, grid
+ * dimension < 2, spacing <= 0.  The message of a failure is etac_last_error(NULL). */
+etac_status etac_mesh_to_sdf_grid(int32_t device, int32_t n_vertices, const float* vertices, int32_t n_triangles,
+                                  const int32_t* triangles, int32_t nx, int32_t ny, int32_t nz, const float* origin,
+                                  float spacing, float* values_out);
+
 /* Message of the last failure on this ctx ("" if none); ctx-owned, valid until the next call.
  * With ctx == NULL returns the message of the last failed etac_create on this thread. */
 const char* etac_last_error(const etac_ctx* ctx);

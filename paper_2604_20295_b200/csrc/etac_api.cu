@@ -624,6 +624,38 @@ etac_status etac_set_sdf_grid(etac_ctx* ctx, int32_t grid_id, int32_t nx, int32_
   return ETAC_OK;
 }
 
+etac_status etac_mesh_to_sdf_grid(int32_t device, int32_t n_vertices, const float* vertices, int32_t n_triangles,
+                                  const int32_t* triangles, int32_t nx, int32_t ny, int32_t nz, const float* origin, float spacing,
+                                  float* values_out) {
+  if (n_vertices < 4 || n_triangles < 4 || !vertices || !triangles || !origin || !values_out)
+    return fail(nullptr, ETAC_ERR_INVALID_ARG, "etac_mesh_to_sdf_grid: NULL pointer or fewer than 4 vertices / triangles");
+  if (nx < 2 || ny < 2 || nz < 2 || !(spacing > 0.0f) || !isfinite(spacing))
+    return fail(nullptr, ETAC_ERR_INVALID_ARG, "etac_mesh_to_sdf_grid: bad grid");
+  std::vector<float> tri((size_t)n_triangles * 9);
+  for (int t = 0; t < n_triangles; ++t)
+    for (int k = 0; k < 3; ++k) {
+      const int v = triangles[3 * t + k];
+      if (v < 0 || v >= n_vertices) return fail(nullptr, ETAC_ERR_INVALID_ARG, "etac_mesh_to_sdf_grid: vertex index out of range");
+      for (int a = 0; a < 3; ++a) {
+        if (!isfinite(vertices[3 * v + a])) return fail(nullptr, ETAC_ERR_INVALID_ARG, "etac_mesh_to_sdf_grid: vertex is not finite");
+        tri[(size_t)t * 9 + 3 * k + a] = vertices[3 * v + a];
+      }
+    }
+  DeviceGuard guard(device);
+  if (!guard.ok) return fail(nullptr, ETAC_ERR_CUDA, "cudaSetDevice failed");
+  const size_t count = (size_t)nx * ny * nz;
+  float *d_tri = nullptr, *d_val = nullptr;
+  cudaError_t e = cudaMalloc(&d_tri, tri.size() * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc(&d_val, count * sizeof(float));
+  if (e == cudaSuccess) e = cudaMemcpy(d_tri, tri.data(), tri.size() * sizeof(float), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = launch_mesh_sdf_grid(d_tri, n_triangles, nx, ny, nz, origin, spacing, d_val, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(values_out, d_val, count * sizeof(float), cudaMemcpyDeviceToHost);
+  cudaFree(d_tri), cudaFree(d_val);
+  if (e != cudaSuccess)
+    return fail(nullptr, e == cudaErrorMemoryAllocation ? ETAC_ERR_ALLOC : ETAC_ERR_CUDA, cuda_msg("etac_mesh_to_sdf_grid", e));
+  return ETAC_OK;
+}
+
 etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value) {
   if (!ctx || !value) return ETAC_ERR_INVALID_ARG;
   switch (key) {

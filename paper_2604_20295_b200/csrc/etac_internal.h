@@ -193,6 +193,8 @@ void launch_pointnet_global_env(const DevModel& m, int n_envs, cudaStream_t s);
 cudaError_t backward_pointnet_configure();
 cudaError_t launch_backward_pointnet(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_w, float* grad_delta,
                                      int n_sm, int* launches, cudaStream_t s);
+cudaError_t launch_mesh_sdf_grid(const float* tri, int n_tri, int nx, int ny, int nz, const float* origin, float h, float* values,
+                                 cudaStream_t s);
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);
 cudaError_t backward_configure();
 cudaError_t launch_backward(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_alpha, int n_alpha,

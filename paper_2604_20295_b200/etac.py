@@ -31,7 +31,7 @@ ETAC_PATH_AUTO, ETAC_PATH_DENSE, ETAC_PATH_SPARSE = 0, 1, 2
 
 EXPORTS = ["etac_create", "etac_destroy", "etac_step", "etac_set_option", "etac_get_info", "etac_last_error",
            "etac_patches_from_adjacency", "etac_abi_version", "etac_time_steps", "etac_set_sdf_grid", "etac_backward", "etac_update_params",
-           "etac_measure_sfu_rate", "etac_propagate_noalloc"]
+           "etac_measure_sfu_rate", "etac_propagate_noalloc", "etac_mesh_to_sdf_grid"]
 ETAC_NOALLOC_MAX_ENTRIES, ETAC_NOALLOC_MAX_ENVS = 262144, 4096
 
 _fp = C.POINTER(C.c_float)
@@ -107,6 +107,7 @@ def load() -> C.CDLL:
         lib.etac_set_sdf_grid.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
         lib.etac_propagate_noalloc.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p,
                                                C.c_void_p, C.c_char_p, C.c_int32]
+        lib.etac_mesh_to_sdf_grid.argtypes = [C.c_int32, C.c_int32, _fp, C.c_int32, _ip, C.c_int32, C.c_int32, C.c_int32, _fp, C.c_float, _fp]
         for name in EXPORTS:
             getattr(lib, name)
         _lib = lib
@@ -264,6 +265,18 @@ def etac_update_params(ctx, alpha=None, weights=None) -> None:
             keep.append(w)
             setattr(p, k, w.ctypes.data_as(_fp))
     _check(ctx, load().etac_update_params(ctx, C.byref(p)))
+
+
+def etac_mesh_to_sdf_grid(vertices, triangles, shape, origin, spacing, device=0):
+    """Closed triangle mesh -> sampled SDF values [nz, ny, nx] fp32 (the layout of etac_set_sdf_grid); shape = (nx, ny, nz)."""
+    v, t, o = _f32(vertices), _i32(triangles), _f32(origin)
+    nx, ny, nz = (int(x) for x in shape)
+    out = np.empty((nz, ny, nx), np.float32)
+    st = load().etac_mesh_to_sdf_grid(int(device), v.shape[0], _p(v, _fp), t.shape[0], _p(t, _ip), nx, ny, nz, _p(o, _fp),
+                                      C.c_float(float(spacing)), _p(out, _fp))
+    if st != ETAC_OK:
+        raise EtacError(st, load().etac_last_error(None).decode())
+    return out
 
 
 def etac_propagate_noalloc(stream, n_envs, n_nodes, alpha, pos, normal, penetration, out) -> None:

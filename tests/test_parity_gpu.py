@@ -407,6 +407,67 @@ def test_sampled_sdf_grid_indenters(mesh_kind, n_envs):
     assert float(np.abs(ref["delta"]).max()) > 0.2
 
 
+@pytest.mark.parametrize("shape_kind", ["box", "icosphere", "tetra"])
+def test_mesh_to_sdf_grid_against_the_mesh_oracle(shape_kind):
+    """etac_mesh_to_sdf_grid (objects given as triangle meshes) against oracle/etac_oracle_mesh.py on
+    grids that are not cubes, with points inside, outside and close to the surface: fp32 brute force against float64,
+    1e-5 of the scene's diagonal; the sign agrees wherever the point is further than that from the surface."""
+    from oracle import etac_oracle_mesh as M
+    V, Tr = {"box": lambda: W.box_mesh(4.0, 3.0, 5.0), "icosphere": lambda: W.icosphere(4.5, 2), "tetra": lambda: W.tetra_mesh(4.0)}[shape_kind]()
+    shape, origin, h = (23, 19, 27), (-7.1, -6.3, -8.2), 0.61
+    ref = M.mesh_sdf_grid(V, Tr, shape, origin, h)
+    got = T.etac_mesh_to_sdf_grid(V, Tr, shape, origin, h).astype(np.float64)
+    assert got.shape == ref.shape == (27, 19, 23) and (ref < 0).sum() > 200 and (ref > 0).sum() > 200
+    diag = float(np.linalg.norm(np.asarray(shape) * h))
+    err = float(np.abs(got - ref).max())
+    print(f"[mesh grid {shape_kind}] {len(Tr)} triangles, {ref.size} points: max err {err:.3g} ({err / diag:.2e} of the diagonal)")
+    assert err <= 1e-5 * diag
+    far = np.abs(ref) > 1e-5 * diag
+    assert np.array_equal(got[far] < 0, ref[far] < 0)
+    with pytest.raises(T.EtacError):
+        T.etac_mesh_to_sdf_grid(V, Tr + len(V), shape, origin, h)                    # vertex index out of range
+
+
+def test_mesh_object_as_indenter_end_to_end():
+    """A triangle-mesh object pressed on the fingertip cap: the GPU samples its SDF (etac_mesh_to_sdf_grid), the grid
+    is registered as an ETAC_IND_GRID indenter and stepped; the oracle samples the same mesh with its own routine.
+    The two grids differ by fp32 rounding (checked above), so masks may differ only where the oracle's penetration is
+    below 1e-4 mm; displacements at the fp32 tolerance."""
+    from oracle import etac_oracle_mesh as M
+    import dataclasses
+    rng = np.random.default_rng(77)
+    base = W.config2(5, 10)
+    mesh = base.mesh
+    V, Tr = W.icosphere(5.0, 2)
+    V = V * np.array([1.0, 0.8, 1.2])                                                 # an ellipsoid-like polyhedron
+    shape, origin, h = (33, 29, 37), (-8.0, -7.0, -9.0), 0.5
+    vals_ref = M.mesh_sdf_grid(V, Tr, shape, origin, h).astype(np.float32)
+    n_envs = base.n_envs
+    ind = W._blank_indenters(n_envs, 1)
+    c = rng.integers(0, mesh.n_nodes, n_envs)
+    centre, quat = W._press_on_node(mesh.pos, mesh.normal, c, None, np.full(n_envs, 4.0), rng.uniform(0.3, 1.2, n_envs),
+                                    rng.uniform(0, 6.28, n_envs))
+    ind["type"][:, 0], ind["param"][:, 0, 0] = T.ETAC_IND_GRID, 1.0
+    ind["pose"][:, 0, 0:3], ind["pose"][:, 0, 3:7] = centre, quat
+    wl = dataclasses.replace(base, indenters=ind, max_indenters=1, meta={"grids": {1: (vals_ref, origin, h)}})
+    ref = run_oracle(wl)
+    assert ref["mask"].sum() > 100
+    eng = T.Etac(wl, debug_outputs=True)
+    try:
+        T.etac_set_sdf_grid(eng.ctx, 1, T.etac_mesh_to_sdf_grid(V, Tr, shape, origin, h), origin, h)   # the GPU-sampled field
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        U = eng.step(n_envs, dev).cpu().numpy()
+        mask = eng.mask_bool(n_envs)
+    finally:
+        eng.close()
+    differ = mask != ref["mask"]
+    assert (ref["delta"][differ] < 1e-4).all() and differ.sum() <= 5
+    umax = float(np.abs(ref["U"]).max())
+    err = float(np.abs(U - ref["U"]).max())
+    print(f"[mesh object] active nodes {int(ref['mask'].sum())}, masks differ at {int(differ.sum())}, max err {err:.3g} / {umax:.3g}")
+    assert err <= 2 * TOL["fp32"] * umax                                              # two fp32 paths to the penetration
+
+
 @pytest.mark.parametrize("precision", ["fp32", "bf16"])
 def test_ablation_residual_only(precision):
     """Table II's "Residual Network Only" row as a run-time mode: passive rows get Phi_p alone."""
