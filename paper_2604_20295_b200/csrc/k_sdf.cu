@@ -22,6 +22,7 @@ struct SInd {
   float prm[3];
   float t[3];
   float R[9];
+  float rb2;  // square of a radius around t beyond which the shape's SDF is > 0.05 (conservative; +inf: unknown, -1: no shape)
 };
 
 // Task of the two-kernel S1 (sdf_cull_kernel -> sdf_eval_kernel): a pair that survived the cull, with the rotations
@@ -31,7 +32,6 @@ struct __align__(16) PairTask {
   SInd ind;          // the environment's indenter (type NONE if it is this patch's own link)
   int pair;
   int evaluated;     // 0: culled -- only the contact-free outputs remain to be written
-  int pad;
 };
 static_assert(sizeof(PairTask) == 128, "PairTask");
 
@@ -146,6 +146,13 @@ __device__ __forceinline__ SInd load_indenter(const etac_indenter* __restrict__ 
   s.prm[0] = p->param[0], s.prm[1] = p->param[1], s.prm[2] = p->param[2];
   s.t[0] = p->pose[0], s.t[1] = p->pose[1], s.t[2] = p->pose[2];
   quat_to_rot(p->pose + 3, s.R);
+  // bounding radius of the shape around its origin: sphere r, box |half extents|, capsule r + L; sampled grids: unknown
+  const float b = s.type == ETAC_IND_SPHERE  ? s.prm[0]
+                  : s.type == ETAC_IND_BOX   ? sqrtf(s.prm[0] * s.prm[0] + s.prm[1] * s.prm[1] + s.prm[2] * s.prm[2])
+                  : s.type == ETAC_IND_CAPSULE ? s.prm[0] + s.prm[1]
+                                               : __int_as_float(0x7f800000);
+  const float rb = fmaf(fabsf(b), 1.001f, 0.05f);
+  s.rb2 = s.type == ETAC_IND_NONE ? -1.0f : rb * rb;
   return s;
 }
 
@@ -193,6 +200,7 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
   __shared__ int s_key[kPoseChunk];  // first active node of the patch
   extern __shared__ uint8_t smem_raw[];
   SInd* sind = reinterpret_cast<SInd*>(smem_raw);
+  float4* s_tb = reinterpret_cast<float4*>(smem_raw + (((size_t)(m.max_ind > 0 ? m.max_ind : 1) * sizeof(SInd) + 15) & ~(size_t)15));  // (t, rb2)
   __shared__ SPose s_pose[kPoseChunk];
   __shared__ int s_any[kPoseChunk];
   __shared__ int s_slot[kPoseChunk];
@@ -205,7 +213,9 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
   const bool posed = io.patch_pose != nullptr;
   if constexpr (kIndenters) {
     for (int k = threadIdx.x; k < m.max_ind; k += blockDim.x) {
-      sind[k] = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
+      const SInd s = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
+      sind[k] = s;
+      s_tb[k] = make_float4(s.t[0], s.t[1], s.t[2], s.rb2);
     }
   }
   for (int p0 = 0; p0 < m.n_patches; p0 += kPoseChunk) {
@@ -274,10 +284,24 @@ __global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO
             phi[c] = __int_as_float(0x7f800000);
           }
           for (int k = 0; k < m.max_ind; ++k) {
+            // A node further than the shape's bounding radius (+ margin) from its origin has phi > 0.05 whatever the
+            // rounding: it stays passive (delta = 0) without the exact, single-rounded evaluation.  On a large patch
+            // most nodes are far from every indenter (one 16-byte load and 7 instructions per slot and node instead
+            // of the 18-word record and the two transforms).
+            const float4 tb = s_tb[k];
+            bool near[kNodeChunk], any_near = false;
+#pragma unroll
+            for (int c = 0; c < kNodeChunk; ++c) {
+              const float dx = X[c][0] - tb.x, dy = X[c][1] - tb.y, dz = X[c][2] - tb.z;
+              near[c] = !(fmaf(dx, dx, fmaf(dy, dy, dz * dz)) > tb.w);
+              any_near |= near[c];
+            }
+            if (!any_near) continue;
             if (sind[k].skip1 == p0 + q + 1) continue;
             const SInd s = sind[k];
 #pragma unroll
-            for (int c = 0; c < kNodeChunk; ++c) phi[c] = fminf(phi[c], sdf_one<kGrid>(s, X[c][0], X[c][1], X[c][2], m.grid));
+            for (int c = 0; c < kNodeChunk; ++c)
+              if (near[c]) phi[c] = fminf(phi[c], sdf_one<kGrid>(s, X[c][0], X[c][1], X[c][2], m.grid));
           }
 #pragma unroll
           for (int c = 0; c < kNodeChunk; ++c) {
@@ -883,7 +907,7 @@ cudaError_t launch_sdf(const DevModel& m, const StepIO& io, int s1_flags_in, int
     if (e != cudaSuccess) return e;
   }
   if (io.input_mode == ETAC_IN_INDENTERS) {
-    const size_t smem = sizeof(SInd) * (size_t)(m.max_ind > 0 ? m.max_ind : 1);
+    const size_t smem = (sizeof(SInd) + sizeof(float4)) * (size_t)(m.max_ind > 0 ? m.max_ind : 1) + 16;  // + (t, rb2) per slot, aligned
     if (grids) sdf_penetration_kernel<true, true><<<grid, 256, smem, s>>>(m, io, s1_flags);
     else sdf_penetration_kernel<true, false><<<grid, 256, smem, s>>>(m, io, s1_flags);
   } else {
