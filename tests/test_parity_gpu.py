@@ -723,7 +723,7 @@ def test_step_is_capturable_in_a_cuda_graph():
     """etac_step only enqueues (no sync, no allocation, no host copy): it can be captured in a
     CUDA graph and replayed; the replays give the eager result bit for bit."""
     import torch
-    for wl in (W.config2(13, 16), W.config3(13, 40)):
+    for wl in (W.config2(13, 16), W.config3(13, 40), W.config4(13, 40)):      # fp32; 16-env tile; clusters + bucketed S1
         eng = T.Etac(wl)
         try:
             dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
