@@ -252,8 +252,9 @@ typedef struct {
 etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* args);
 
 /* Replaces the calibrated parameters of a context in place (one gradient-descent step of Eq. (3)):
- * alpha ([n_alpha], same n_alpha as at create; NULL = keep; K is rebuilt on the device) and / or the six
- * arrays of the per-node MLP (all six or none; layouts as in etac_model_desc).  Host pointers, copied.
+ * alpha ([n_alpha], same n_alpha as at create; NULL = keep; K is rebuilt on the device) and / or the
+ * weights of the context's residual network: the six arrays of the per-node MLP or the ten of the PointNet form (all
+ * or none; layouts as in etac_model_desc).  Host pointers, copied.
  * Synchronises the device before and after; not to be called concurrently with etac_step /
  * etac_backward on the same ctx.  The result is the same as a context created with these parameters. */
 typedef struct {
@@ -261,6 +262,9 @@ typedef struct {
   int32_t n_alpha;
   const float* alpha;
   const float *W1, *b1, *W2, *b2, *W3, *b3;
+  const float *E1, *e1, *E2, *e2, *G1, *g1, *D1, *d1, *D2, *d2; /* ETAC_RESID_POINTNET contexts: all ten or none (layouts as
+                                                                   in etac_model_desc); a struct_size that ends before E1
+                                                                   is accepted (no PointNet arrays) */
 } etac_params;
 etac_status etac_update_params(etac_ctx* ctx, const etac_params* params);
 

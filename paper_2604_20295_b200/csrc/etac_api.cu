@@ -251,6 +251,49 @@ void stage_pernode(const float* W1, const float* b1, const float* W2, const floa
   st->wout[195] = 0.0f;
 }
 
+// The PointNet form of Phi staged for the device: the bf16 shared-memory image of the tensor-core
+// passes, the global MLP (fp32, both matrices transposed), the fp32 copies of the node layers, the output layer.
+struct PointNetStage {
+  std::vector<uint8_t> img;
+  std::vector<float> pf, w32;
+  float wout[196];
+};
+void stage_pointnet(const float* E1, const float* e1, const float* E2, const float* e2, const float* G1, const float* g1,
+                    const float* D1, const float* d1, const float* D2, const float* d2, PointNetStage* st) {
+  // bf16 image; the 0.5 of silu(x) = h + h*tanh(h), h = x/2, is folded into every layer that feeds a SiLU.
+  // Layer-1 operand columns are [u^(3), p(3), n(3), 1]; E1's inputs are [p, n, u^].
+  st->img.assign(kPnImgBytes, 0);
+  auto put = [&](size_t base, int n, int k, int rows, float v) {
+    const uint16_t b = f2bf(v);
+    memcpy(&st->img[base + wimg_off(n, k, rows)], &b, 2);
+  };
+  const size_t o1 = kW1ImgBytes, o2 = o1 + kW2ImgBytes;
+  for (int n = 0; n < 64; ++n) {
+    for (int k = 0; k < 3; ++k) {
+      put(0, n, k, 64, 0.5f * E1[n * 9 + 6 + k]);      // u^
+      put(0, n, 3 + k, 64, 0.5f * E1[n * 9 + k]);      // p
+      put(0, n, 6 + k, 64, 0.5f * E1[n * 9 + 3 + k]);  // n
+    }
+    put(0, n, 9, 64, 0.5f * e1[n]);
+    for (int k = 0; k < 64; ++k) put(o1, n, k, 64, 0.5f * E2[n * 64 + k]);
+    put(o1, n, 64, 64, 0.5f * e2[n]);
+    for (int k = 0; k < 64; ++k) put(o2, n, k, 64, 0.5f * D1[n * 128 + k]);  // bias column stays 0: c_(e,p) is added in the epilogue
+  }
+  memcpy(st->wout, D2, 192 * 4);
+  memcpy(st->wout + 192, d2, 3 * 4);
+  st->wout[195] = 0.0f;
+  st->pf.assign(4096 + 64 + 4096 + 64, 0.f);
+  for (int n = 0; n < 64; ++n)  // both 64 x 64 matrices transposed to [in][out] (coalesced over the outputs)
+    for (int j = 0; j < 64; ++j) st->pf[j * 64 + n] = G1[n * 64 + j], st->pf[4160 + j * 64 + n] = D1[n * 128 + 64 + j];
+  memcpy(st->pf.data() + 4096, g1, 64 * 4);
+  memcpy(st->pf.data() + 4160 + 4096, d1, 64 * 4);
+  st->w32.clear();  // fp32 SIMT forward (k_pointnet_fp32.cu) and backward (k_backward_pointnet.cu)
+  st->w32.insert(st->w32.end(), E1, E1 + 576), st->w32.insert(st->w32.end(), e1, e1 + 64);
+  st->w32.insert(st->w32.end(), E2, E2 + 4096), st->w32.insert(st->w32.end(), e2, e2 + 64);
+  for (int n = 0; n < 64; ++n) st->w32.insert(st->w32.end(), D1 + n * 128, D1 + n * 128 + 64);
+  st->w32.insert(st->w32.end(), D2, D2 + 192), st->w32.insert(st->w32.end(), d2, d2 + 3);
+}
+
 }  // namespace
 
 extern "C" {
@@ -462,45 +505,14 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   }
 
   if (d->resid_arch == ETAC_RESID_POINTNET) {
-    // bf16 shared-memory image; the 0.5 of silu(x) = h + h*tanh(h), h = x/2, is folded into every layer
-    // that feeds a SiLU.  Layer-1 operand columns are [u^(3), p(3), n(3), 1]; E1's inputs are [p, n, u^].
-    std::vector<uint8_t> img(kPnImgBytes, 0);
-    auto put = [&](size_t base, int n, int k, int rows, float v) {
-      const uint16_t b = f2bf(v);
-      memcpy(&img[base + wimg_off(n, k, rows)], &b, 2);
-    };
-    const size_t o1 = kW1ImgBytes, o2 = o1 + kW2ImgBytes;
-    for (int n = 0; n < 64; ++n) {
-      for (int k = 0; k < 3; ++k) {
-        put(0, n, k, 64, 0.5f * d->E1[n * 9 + 6 + k]);      // u^
-        put(0, n, 3 + k, 64, 0.5f * d->E1[n * 9 + k]);      // p
-        put(0, n, 6 + k, 64, 0.5f * d->E1[n * 9 + 3 + k]);  // n
-      }
-      put(0, n, 9, 64, 0.5f * d->e1[n]);
-      for (int k = 0; k < 64; ++k) put(o1, n, k, 64, 0.5f * d->E2[n * 64 + k]);
-      put(o1, n, 64, 64, 0.5f * d->e2[n]);
-      for (int k = 0; k < 64; ++k) put(o2, n, k, 64, 0.5f * d->D1[n * 128 + k]);  // bias column stays 0: c_(e,p) is added in the epilogue
-    }
-    memcpy(m.wout, d->D2, 192 * 4);
-    memcpy(m.wout + 192, d->d2, 3 * 4);
-    m.wout[195] = 0.0f;
-    CK(dev_upload(c, &m.wimg_pn, img.data(), img.size()), "upload PointNet weight image");
-    std::vector<float> pf(4096 + 64 + 4096 + 64);
-    for (int n = 0; n < 64; ++n)      // both 64 x 64 matrices transposed to [in][out] (coalesced over the outputs)
-      for (int j = 0; j < 64; ++j) pf[j * 64 + n] = d->G1[n * 64 + j], pf[4160 + j * 64 + n] = d->D1[n * 128 + 64 + j];
-    memcpy(pf.data() + 4096, d->g1, 64 * 4);
-    memcpy(pf.data() + 4160 + 4096, d->d1, 64 * 4);
-    CK(dev_upload(c, &m.pn_f32, pf.data(), pf.size()), "upload PointNet global MLP");
-    {  // fp32 copies for the fp32 SIMT forward (k_pointnet_fp32.cu) and the backward (k_backward_pointnet.cu)
-      std::vector<float> w32;
-      w32.insert(w32.end(), d->E1, d->E1 + 576), w32.insert(w32.end(), d->e1, d->e1 + 64);
-      w32.insert(w32.end(), d->E2, d->E2 + 4096), w32.insert(w32.end(), d->e2, d->e2 + 64);
-      for (int n = 0; n < 64; ++n) w32.insert(w32.end(), d->D1 + n * 128, d->D1 + n * 128 + 64);
-      w32.insert(w32.end(), d->D2, d->D2 + 192), w32.insert(w32.end(), d->d2, d->d2 + 3);
-      CK(dev_upload(c, &m.pn_w32, w32.data(), w32.size()), "upload PointNet fp32 weights");
-      CK(pointnet_fp32_configure(), "cudaFuncSetAttribute(pn_decode_fp32_kernel)");
-      CK(backward_pointnet_configure(), "cudaFuncSetAttribute(pn_bwd_node_kernel)");
-    }
+    PointNetStage st;
+    stage_pointnet(d->E1, d->e1, d->E2, d->e2, d->G1, d->g1, d->D1, d->d1, d->D2, d->d2, &st);
+    memcpy(m.wout, st.wout, sizeof(m.wout));
+    CK(dev_upload(c, &m.wimg_pn, st.img.data(), st.img.size()), "upload PointNet weight image");
+    CK(dev_upload(c, &m.pn_f32, st.pf.data(), st.pf.size()), "upload PointNet global MLP");
+    CK(dev_upload(c, &m.pn_w32, st.w32.data(), st.w32.size()), "upload PointNet fp32 weights");
+    CK(pointnet_fp32_configure(), "cudaFuncSetAttribute(pn_decode_fp32_kernel)");
+    CK(backward_pointnet_configure(), "cudaFuncSetAttribute(pn_bwd_node_kernel)");
     CK(dev_alloc(c, &m.pn_gkey, (size_t)64 * P * d->max_envs, true), "alloc PointNet arg-max keys");
     CK(dev_alloc(c, &m.pn_ssum, (size_t)64 * P * d->max_envs, true), "alloc PointNet backward sums");
     CK(dev_alloc(c, &m.pn_ggmax, (size_t)64 * P * d->max_envs, true), "alloc PointNet backward dL/dgmax");
@@ -680,13 +692,23 @@ etac_status etac_get_info(const etac_ctx* ctx, int32_t key, int64_t* value) {
 
 etac_status etac_update_params(etac_ctx* ctx, const etac_params* p) {
   if (!ctx) return ETAC_ERR_INVALID_ARG;
-  if (!p || p->struct_size != sizeof(etac_params)) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_params");
+  // (a caller built against the header before the PointNet arrays were added passes the shorter struct)
+  if (!p || (p->struct_size != sizeof(etac_params) && p->struct_size != offsetof(etac_params, E1)))
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_params");
   const float* w[6] = {p->W1, p->b1, p->W2, p->b2, p->W3, p->b3};
-  int n_w = 0;
+  int n_w = 0, n_pn = 0;
   for (const float* q : w) n_w += q != nullptr;
   if (n_w != 0 && n_w != 6) return fail(ctx, ETAC_ERR_INVALID_ARG, "give all six weight arrays or none");
   if (n_w && ctx->m.resid != ETAC_RESID_PERNODE_MLP)
-    return fail(ctx, ETAC_ERR_UNSUPPORTED, "weights can be replaced on ETAC_RESID_PERNODE_MLP contexts only");
+    return fail(ctx, ETAC_ERR_UNSUPPORTED, "W1 .. b3 can be replaced on ETAC_RESID_PERNODE_MLP contexts only");
+  const float* pn[10] = {};
+  if (p->struct_size == sizeof(etac_params)) {
+    const float* q[10] = {p->E1, p->e1, p->E2, p->e2, p->G1, p->g1, p->D1, p->d1, p->D2, p->d2};
+    for (int k = 0; k < 10; ++k) pn[k] = q[k], n_pn += q[k] != nullptr;
+  }
+  if (n_pn != 0 && n_pn != 10) return fail(ctx, ETAC_ERR_INVALID_ARG, "give all ten PointNet arrays or none");
+  if (n_pn && ctx->m.resid != ETAC_RESID_POINTNET)
+    return fail(ctx, ETAC_ERR_UNSUPPORTED, "E1 .. d2 can be replaced on ETAC_RESID_POINTNET contexts only");
   if (p->alpha) {
     if (p->n_alpha != ctx->n_alpha) return fail(ctx, ETAC_ERR_INVALID_ARG, "n_alpha differs from the context's");
     for (int k = 0; k < p->n_alpha; ++k)
@@ -712,6 +734,15 @@ etac_status etac_update_params(etac_ctx* ctx, const etac_params* p) {
     if (e == cudaSuccess) e = launch_build_c1(m, ctx->dW1_w, ctx->db1_w, const_cast<float*>(m.c1t), 0);
     if (e == cudaSuccess) e = cudaMemcpy(const_cast<uint8_t*>(m.wimg), st.img.data(), st.img.size(), cudaMemcpyHostToDevice);
     if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("restage weights", e));
+    memcpy(m.wout, st.wout, sizeof(m.wout));
+  }
+  if (n_pn) {
+    PointNetStage st;
+    stage_pointnet(pn[0], pn[1], pn[2], pn[3], pn[4], pn[5], pn[6], pn[7], pn[8], pn[9], &st);
+    e = cudaMemcpy(const_cast<uint8_t*>(m.wimg_pn), st.img.data(), st.img.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(const_cast<float*>(m.pn_f32), st.pf.data(), st.pf.size() * 4, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(const_cast<float*>(m.pn_w32), st.w32.data(), st.w32.size() * 4, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("restage PointNet weights", e));
     memcpy(m.wout, st.wout, sizeof(m.wout));
   }
   if ((e = cudaDeviceSynchronize()) != cudaSuccess) return fail(ctx, ETAC_ERR_CUDA, cuda_msg("update kernels", e));

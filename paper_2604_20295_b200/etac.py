@@ -71,7 +71,9 @@ class etac_backward_args(C.Structure):
 
 class etac_params(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_alpha", C.c_int32), ("alpha", _fp),
-                ("W1", _fp), ("b1", _fp), ("W2", _fp), ("b2", _fp), ("W3", _fp), ("b3", _fp)]
+                ("W1", _fp), ("b1", _fp), ("W2", _fp), ("b2", _fp), ("W3", _fp), ("b3", _fp),
+                ("E1", _fp), ("e1", _fp), ("E2", _fp), ("e2", _fp), ("G1", _fp), ("g1", _fp),
+                ("D1", _fp), ("d1", _fp), ("D2", _fp), ("d2", _fp)]
 
 
 ETAC_GRAD_WEIGHTS_LEN = 4995
@@ -251,7 +253,8 @@ def etac_backward(ctx, stream, n_envs, grad_out, grad_alpha, grad_weights=None, 
 
 
 def etac_update_params(ctx, alpha=None, weights=None) -> None:
-    """Replace alpha and / or the per-node MLP weights ({"W1": ..., ..., "b3": ...}) of a context in place."""
+    """Replace alpha and / or the weights of the context's residual network in place: {"W1": ..., ..., "b3": ...} on a
+    per-node MLP context, {"E1": ..., ..., "d2": ...} on a PointNet context."""
     p = etac_params()
     p.struct_size = C.sizeof(etac_params)
     keep = []
@@ -260,7 +263,8 @@ def etac_update_params(ctx, alpha=None, weights=None) -> None:
         keep.append(a)
         p.n_alpha, p.alpha = a.size, a.ctypes.data_as(_fp)
     if weights is not None:
-        for k in ("W1", "b1", "W2", "b2", "W3", "b3"):
+        names = ("E1", "e1", "E2", "e2", "G1", "g1", "D1", "d1", "D2", "d2") if "E1" in weights else ("W1", "b1", "W2", "b2", "W3", "b3")
+        for k in names:
             w = np.ascontiguousarray(weights[k], dtype=np.float32)
             keep.append(w)
             setattr(p, k, w.ctypes.data_as(_fp))

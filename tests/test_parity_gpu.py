@@ -5,6 +5,8 @@ the same seeded inputs.  Tolerances are BASELINE.json's:
    bf16 tensor-core path     : max|u_gpu - u_ref| <= 2e-2 * max|u_ref|   (fp32 accumulation)
 The residual MLP is ~1 % of max|u| with the N(0, 0.02) weights of the configs, so it is also
 checked on its own (r = U - u_lin on passive nodes) and with larger weights."""
+import ctypes as C
+
 import numpy as np
 import pytest
 
@@ -684,6 +686,100 @@ def test_update_params_equals_a_fresh_context(precision):
         eng.close()
     assert np.abs(U_a - U_b).max() > 1e-2
     assert np.array_equal(U_ab, U_b) and np.array_equal(U_aa, U_a)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "bf16"])
+def test_update_params_pointnet_equals_a_fresh_context(precision):
+    """etac_update_params on an ETAC_RESID_POINTNET context: all ten arrays of the paper's Phi
+    restaged in place (bf16 image, fp32 copies, global MLP, output layer) give bit for bit the step of a context
+    created with them; the per-node arrays are refused there, and the PointNet arrays on a per-node context."""
+    import dataclasses
+    base = W.config3(17, 11) if precision == "bf16" else W.config2(17, 11)
+    wl_a = dataclasses.replace(base, weights=W.make_pointnet_weights(3, 6, std=0.15))
+    wl_b = dataclasses.replace(wl_a, alpha=(base.alpha * 1.3).astype(np.float32), weights=W.make_pointnet_weights(3, 7, std=0.12))
+    dev_kw = dict(indenters=wl_a.indenters, patch_pose=wl_a.patch_pose)
+    eng_b = T.Etac(wl_b, precision=precision)
+    U_b = eng_b.step(wl_b.n_envs, eng_b.upload(**dev_kw)).cpu().numpy()
+    eng_b.close()
+    eng = T.Etac(wl_a, precision=precision)
+    try:
+        dev = eng.upload(**dev_kw)
+        U_a = eng.step(wl_a.n_envs, dev).cpu().numpy()
+        T.etac_update_params(eng.ctx, alpha=wl_b.alpha, weights=wl_b.weights)
+        U_ab = eng.step(wl_a.n_envs, dev).cpu().numpy()
+        T.etac_update_params(eng.ctx, weights=wl_a.weights)
+        T.etac_update_params(eng.ctx, alpha=wl_a.alpha)
+        U_aa = eng.step(wl_a.n_envs, dev).cpu().numpy()
+        with pytest.raises(T.EtacError) as ei:
+            T.etac_update_params(eng.ctx, weights=W.make_weights(3, 9))      # per-node arrays on a PointNet context
+        assert ei.value.status == T.ETAC_ERR_UNSUPPORTED
+        part = dict(wl_b.weights)
+        p = T.etac_params()
+        p.struct_size = C.sizeof(T.etac_params)
+        e1 = np.ascontiguousarray(part["E1"])
+        p.E1 = e1.ctypes.data_as(C.POINTER(C.c_float))                       # one of ten
+        assert T.load().etac_update_params(eng.ctx, C.byref(p)) == T.ETAC_ERR_INVALID_ARG
+        p = T.etac_params()                                                  # a caller built before the PointNet arrays
+        p.struct_size = T.etac_params.E1.offset
+        assert T.load().etac_update_params(eng.ctx, C.byref(p)) == T.ETAC_OK
+        assert np.array_equal(eng.step(wl_a.n_envs, dev).cpu().numpy(), U_a)
+    finally:
+        eng.close()
+    eng = T.Etac(base, precision=precision)                                  # per-node context
+    try:
+        with pytest.raises(T.EtacError) as ei:
+            T.etac_update_params(eng.ctx, weights=wl_b.weights)
+        assert ei.value.status == T.ETAC_ERR_UNSUPPORTED
+    finally:
+        eng.close()
+    assert np.abs(U_a - U_b).max() > 1e-2
+    assert np.array_equal(U_ab, U_b) and np.array_equal(U_aa, U_a)
+
+
+def test_calibration_of_the_pointnet_residual_lowers_the_loss():
+    """Eq. (3) with the paper's Phi end to end on synthetic data: targets from a teacher with its own PointNet weights
+    and alpha; Adam on all ten weight arrays and alpha (gradients from etac_backward, written back with
+    etac_update_params) from another random start lowers 1/2 ||U - U*||^2 by more than 100x in 150 steps."""
+    import dataclasses
+    import torch
+    base = W.config2(18, 12)
+    wl_t = dataclasses.replace(base, weights=W.make_pointnet_weights(3, 8, std=0.15))
+    dev_kw = dict(indenters=wl_t.indenters, patch_pose=wl_t.patch_pose)
+    teacher = T.Etac(wl_t, precision="fp32")
+    target = teacher.step(wl_t.n_envs, teacher.upload(**dev_kw)).clone()
+    teacher.close()
+    w = {k: v.astype(np.float64) for k, v in W.make_pointnet_weights(3, 9, std=0.1).items()}
+    a = wl_t.alpha.astype(np.float64) * 0.8
+    eng = T.Etac(dataclasses.replace(wl_t, alpha=a.astype(np.float32), weights={k: v.astype(np.float32) for k, v in w.items()}),
+                 precision="fp32")
+    try:
+        dev = eng.upload(**dev_kw)
+        stream = torch.cuda.current_stream().cuda_stream
+        g_alpha = torch.empty(a.size, device=eng.device)
+        g_w = torch.empty(T.ETAC_GRAD_WEIGHTS_POINTNET_LEN, device=eng.device)
+        theta = {"alpha": a, **w}
+        m1 = {k: np.zeros_like(v) for k, v in theta.items()}
+        m2 = {k: np.zeros_like(v) for k, v in theta.items()}
+        lr = {k: 3e-3 for k in theta}
+        lr["alpha"] = 0.01
+        losses = []
+        for it in range(1, 151):
+            G = eng.step(wl_t.n_envs, dev) - target
+            losses.append(0.5 * float((G * G).sum()))
+            T.etac_backward(eng.ctx, stream, wl_t.n_envs, G.contiguous(), g_alpha, g_w, **dev)
+            grads = {k: v.astype(np.float64) for k, v in T.split_grad_weights(g_w.cpu().numpy()).items()}
+            grads["alpha"] = g_alpha.cpu().numpy().astype(np.float64)
+            for k in theta:
+                m1[k] = 0.9 * m1[k] + 0.1 * grads[k]
+                m2[k] = 0.999 * m2[k] + 0.001 * grads[k] ** 2
+                theta[k] = theta[k] - lr[k] * (m1[k] / (1 - 0.9 ** it)) / (np.sqrt(m2[k] / (1 - 0.999 ** it)) + 1e-12)
+            theta["alpha"] = np.maximum(theta["alpha"], 0.05)
+            T.etac_update_params(eng.ctx, alpha=theta["alpha"].astype(np.float32),
+                                 weights={k: v.astype(np.float32) for k, v in theta.items() if k != "alpha"})
+    finally:
+        eng.close()
+    print(f"[calibration pointnet] alpha {theta['alpha']} vs {wl_t.alpha}; loss {losses[0]:.4g} -> {min(losses):.4g} (last {losses[-1]:.4g})")
+    assert losses[-1] < 0.01 * losses[0]
 
 
 def test_calibration_recovers_alpha_of_a_synthetic_teacher():
