@@ -245,7 +245,16 @@ typedef struct {
                                          e1[64] E2[64x64] e2[64] G1[64x64] g1[64] D1[64x128] d1[64] D2[3x64] d2[3] */
   float* d_grad_penetration;          /* device [E x N] fp32, overwritten, or NULL: dL/ddelta for the nodes in contact
                                          (u^ = -delta n, L77; the contact set is held fixed, 0 for the other nodes).
-                                         The caller chains it to object / link poses through its SDF gradients */
+                                         The caller chains it to object / link poses through its SDF gradients, or
+                                         asks for the two arrays below */
+  /* dL/d(poses) (Table I: differentiability; delta comes from the SDFs of L77): dL/ddelta chained through the SDF
+     gradient of the indenter that attains the union's min at each node in contact (contact set held fixed).  Both
+     optional; ETAC_IN_INDENTERS mode only; need d_grad_penetration (read back by the kernel) and max_indenters <= 256.
+     A row is (dL/dt[3], dL/dtheta[3]): t the pose's translation, theta a rotation applied on the LEFT in the world
+     frame, R <- exp([theta]x) R (the torque about the body's own origin t, up to sign conventions of the caller).
+     A struct_size that ends before these two fields is accepted (no pose gradients). */
+  float* d_grad_indenter_pose;        /* device [E x max_indenters x 6] fp32, overwritten, or NULL; 0 for empty slots */
+  float* d_grad_patch_pose;           /* device [E x P x 6] fp32, overwritten, or NULL; 0 if d_patch_pose is NULL */
 } etac_backward_args;
 #define ETAC_GRAD_WEIGHTS_LEN 4995
 #define ETAC_GRAD_WEIGHTS_POINTNET_LEN 17411

@@ -24,7 +24,9 @@ with the CUDA path).  It differentiates exactly what ``etac_oracle.step`` comput
 
 float64 numpy, one (env, patch) at a time, no fusion.  Pins (tests/test_oracle_pins.py): central
 finite differences of ``etac_oracle.step`` (itself pinned) with respect to alpha, to sampled weights
-of every layer and (penetration input mode) to the penetration of sampled contact nodes.
+of every layer and (penetration input mode) to the penetration of sampled contact nodes; ``pose_gradients``
+(dL/ddelta chained to indenter and patch poses) by central differences of ``etac_oracle.step`` under translations
+and small left rotations of the poses, for every indenter type.
 """
 from __future__ import annotations
 
@@ -131,3 +133,128 @@ def backward(model: O.OracleModel, G, indenters=None, patch_pose=None, penetrati
                 back = back + G[oi, lo:hi][act]
             grads["delta"][oi, lo:hi][act] = -(nrm[lo:hi][act] * back).sum(1)
     return grads
+
+
+# ------------------------------------------------------------------ dL/d(poses) from dL/ddelta
+def sdf_local_gradient(itype, param, y):
+    """Gradient [n, 3] of ``etac_oracle.sdf_local`` with respect to the local point y [n, 3] (closed forms):
+    sphere y/|y|; box outside sign(y) max(q, 0)/|max(q, 0)|, q = |y| - b, inside the unit vector of the axis with the
+    largest q, signed like y; capsule (y0, y1, y2 - clamp(y2, -L, L)) / |.|."""
+    y = np.asarray(y, dtype=np.float64)
+    if itype == O.IND_SPHERE:
+        return y / np.linalg.norm(y, axis=1, keepdims=True)
+    if itype == O.IND_BOX:
+        b = np.asarray(param[:3], dtype=np.float64)
+        q = np.abs(y) - b
+        o = np.maximum(q, 0.0)
+        no = np.linalg.norm(o, axis=1, keepdims=True)
+        sgn = np.where(y < 0, -1.0, 1.0)
+        with np.errstate(invalid="ignore", divide="ignore"):
+            g_out = sgn * o / no
+        g_in = np.zeros_like(y)
+        a = q.argmax(axis=1)
+        g_in[np.arange(y.shape[0]), a] = sgn[np.arange(y.shape[0]), a]
+        return np.where(no > 0, g_out, g_in)
+    if itype == O.IND_CAPSULE:
+        L = float(param[1])
+        v = y.copy()
+        v[:, 2] = y[:, 2] - np.clip(y[:, 2], -L, L)
+        return v / np.linalg.norm(v, axis=1, keepdims=True)
+    raise ValueError(f"bad indenter type {itype}")
+
+
+def sdf_grid_gradient(values, origin, spacing, y):
+    """Gradient [n, 3] of ``etac_oracle.sdf_grid`` with respect to y [n, 3]: along an axis on which y lies inside the
+    grid's box the derivative of the trilinear interpolant (difference of the two faces of the cell along that
+    axis, interpolated bilinearly on the other two, over the spacing); along an axis on which y was clamped the
+    interpolant is constant and the distance term gives (y - clamp(y)) / |y - clamp(y)|."""
+    v = np.asarray(values, dtype=np.float64)
+    y = np.asarray(y, dtype=np.float64)
+    nz, ny, nx = v.shape
+    n = np.array([nx, ny, nz])
+    h = float(spacing)
+    lo = np.asarray(origin, dtype=np.float64)
+    hi = lo + h * (n - 1)
+    yc = np.clip(y, lo, hi)
+    t = (yc - lo) / h
+    i = np.minimum(np.floor(t), n - 2).astype(np.int64)
+    f = t - i
+    g = np.zeros_like(y)
+    for r in range(y.shape[0]):
+        c = v[i[r, 2]:i[r, 2] + 2, i[r, 1]:i[r, 1] + 2, i[r, 0]:i[r, 0] + 2]      # [z, y, x] corner samples of the cell
+        wx = np.array([1 - f[r, 0], f[r, 0]])
+        wy = np.array([1 - f[r, 1], f[r, 1]])
+        wz = np.array([1 - f[r, 2], f[r, 2]])
+        dx = np.einsum("zy,z,y->", c[:, :, 1] - c[:, :, 0], wz, wy) / h
+        dy = np.einsum("zx,z,x->", c[:, 1, :] - c[:, 0, :], wz, wx) / h
+        dz = np.einsum("yx,y,x->", c[1, :, :] - c[0, :, :], wy, wx) / h
+        inside = y[r] == yc[r]
+        g[r] = np.where(inside, [dx, dy, dz], 0.0)
+        off = y[r] - yc[r]
+        dist = np.linalg.norm(off)
+        if dist > 0:
+            g[r] += off / dist
+    return g
+
+
+def pose_gradients(model: O.OracleModel, g_delta, indenters, patch_pose=None, envs=None):
+    """Chains dL/ddelta [E', N] (``backward(...)["delta"]``) to the poses the penetration came from
+    (delta from SDFs between nodes and objects; Table I: differentiability).
+
+    For a node in contact  delta_i = -phi_k*(y),  y = R_k^T (x_i - t_k),  x_i = R_p p_i + t_p,  k* the indenter that
+    attains the min of the union (the contact set and k* are held fixed).  With n_w = R_k grad phi_k(y) (the SDF's
+    gradient in the world frame), d = x_i - t_k, r = x_i - t_p, and rotations perturbed on the LEFT in the world
+    frame, R <- exp([theta]x) R:
+        d delta/d t_k = +n_w          d delta/d theta_k = -(n_w x d)
+        d delta/d t_p = -n_w          d delta/d theta_p = -(r x n_w)
+    Returns float64 {"indenter": [E', max_ind, 6], "patch": [E', P, 6]}, each row (dL/dt, dL/dtheta); the patch part
+    is zero if there are no patch poses."""
+    g_delta = np.asarray(g_delta, dtype=np.float64)
+    E_all = indenters.shape[0]
+    envs = list(range(E_all)) if envs is None else list(envs)
+    pos = model.pos.astype(np.float64)
+    out = {"indenter": np.zeros((len(envs), indenters.shape[1], 6)), "patch": np.zeros((len(envs), model.n_patches, 6))}
+    for oi, e in enumerate(envs):
+        X = pos.copy()
+        tp = np.zeros((model.n_patches, 3))
+        if patch_pose is not None:
+            for p in range(model.n_patches):
+                lo, hi = int(model.patch_offset[p]), int(model.patch_offset[p + 1])
+                tp[p] = np.asarray(patch_pose[e][p, 0:3], dtype=np.float64)
+                X[lo:hi] = pos[lo:hi] @ O.quat_to_rot(patch_pose[e][p, 3:7]).T + tp[p]
+        phi = np.full((indenters.shape[1], model.n_nodes), np.inf)
+        grad_w = np.zeros((indenters.shape[1], model.n_nodes, 3))
+        for k, ind in enumerate(indenters[e]):
+            itype = int(ind["type"])
+            if itype == O.IND_NONE:
+                continue
+            R = O.quat_to_rot(ind["pose"][3:7])
+            y = (X - np.asarray(ind["pose"][0:3], dtype=np.float64)) @ R          # rows R^T d
+            if itype == O.IND_GRID:
+                values, origin, spacing = model.grids[int(ind["param"][0])]
+                phi[k] = O.sdf_grid(values, origin, spacing, y[:, 0], y[:, 1], y[:, 2])
+                gl = sdf_grid_gradient(values, origin, spacing, y)
+            else:
+                phi[k] = O.sdf_local(itype, ind["param"], y[:, 0], y[:, 1], y[:, 2])
+                gl = sdf_local_gradient(itype, ind["param"], y)
+            grad_w[k] = gl @ R.T
+            skip = int(ind["skip_patch1"]) - 1 if "skip_patch1" in ind.dtype.names else -1
+            if 0 <= skip < model.n_patches:
+                phi[k, int(model.patch_offset[skip]):int(model.patch_offset[skip + 1])] = np.inf
+        kstar = phi.argmin(axis=0)
+        for p in range(model.n_patches):
+            lo, hi = int(model.patch_offset[p]), int(model.patch_offset[p + 1])
+            for i in range(lo, hi):
+                g = g_delta[oi, i]
+                if g == 0.0:
+                    continue
+                k = int(kstar[i])
+                nw = grad_w[k, i]
+                d = X[i] - np.asarray(indenters[e][k]["pose"][0:3], dtype=np.float64)
+                r = X[i] - tp[p]
+                out["indenter"][oi, k, 0:3] += g * nw
+                out["indenter"][oi, k, 3:6] += -g * np.cross(nw, d)
+                if patch_pose is not None:
+                    out["patch"][oi, p, 0:3] += -g * nw
+                    out["patch"][oi, p, 3:6] += -g * np.cross(r, nw)
+    return out

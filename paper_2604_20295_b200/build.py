@@ -13,8 +13,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libetac.so")
-SOURCES = ["etac_api.cu", "k_build.cu", "k_sdf.cu", "k_gather_fp32.cu", "k_pointnet_fp32.cu", "k_fused.cu", "k_backward.cu", "k_backward_pointnet.cu", "k_peaks.cu", "k_noalloc.cu", "k_mesh.cu"]
-HEADERS = ["etac_internal.h", "sm100_prims.cuh", "pointnet_fp32.cuh", os.path.join("..", "..", "include", "etac.h"),
+SOURCES = ["etac_api.cu", "k_build.cu", "k_sdf.cu", "k_gather_fp32.cu", "k_pointnet_fp32.cu", "k_fused.cu", "k_backward.cu", "k_backward_pointnet.cu", "k_backward_pose.cu", "k_peaks.cu", "k_noalloc.cu", "k_mesh.cu"]
+HEADERS = ["etac_internal.h", "sm100_prims.cuh", "pointnet_fp32.cuh", "sdf_device.cuh", os.path.join("..", "..", "include", "etac.h"),
            os.path.join("..", "..", "include", "etac_bench.h"), os.path.join("..", "..", "include", "etac_noalloc.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

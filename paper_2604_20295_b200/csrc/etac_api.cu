@@ -752,7 +752,12 @@ etac_status etac_update_params(etac_ctx* ctx, const etac_params* p) {
 etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_args* a) {
   if (!ctx) return ETAC_ERR_INVALID_ARG;
   cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
-  if (!a || a->struct_size != sizeof(etac_backward_args)) return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_backward_args");
+  // (a caller built against the header before the pose gradients were added passes the shorter struct)
+  if (!a || (a->struct_size != sizeof(etac_backward_args) && a->struct_size != offsetof(etac_backward_args, d_grad_indenter_pose)))
+    return fail(ctx, ETAC_ERR_INVALID_ARG, "bad etac_backward_args");
+  const bool has_pose_fields = a->struct_size == sizeof(etac_backward_args);
+  float* const g_ind_pose = has_pose_fields ? a->d_grad_indenter_pose : nullptr;
+  float* const g_patch_pose = has_pose_fields ? a->d_grad_patch_pose : nullptr;
   if (a->n_envs < 0) return fail(ctx, ETAC_ERR_INVALID_ARG, "n_envs < 0");
   if (a->n_envs > ctx->m.max_envs) return fail(ctx, ETAC_ERR_CAPACITY, "n_envs > max_envs");
   if (a->input_mode != ETAC_IN_INDENTERS && a->input_mode != ETAC_IN_PENETRATION)
@@ -765,6 +770,12 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
   if (ctx->m.ablation != ETAC_ABLATE_FULL) return fail(ctx, ETAC_ERR_UNSUPPORTED, "etac_backward: ETAC_ABLATE_FULL only");
   if (ctx->m.resid == ETAC_RESID_NONE && a->d_grad_weights)
     return fail(ctx, ETAC_ERR_INVALID_ARG, "d_grad_weights given for a context without a residual network");
+  if (g_ind_pose || g_patch_pose) {
+    if (a->input_mode != ETAC_IN_INDENTERS)
+      return fail(ctx, ETAC_ERR_INVALID_ARG, "pose gradients exist in ETAC_IN_INDENTERS mode only");
+    if (!a->d_grad_penetration) return fail(ctx, ETAC_ERR_INVALID_ARG, "pose gradients need d_grad_penetration");
+    if (ctx->m.max_ind > kMaxPoseGradIndenters) return fail(ctx, ETAC_ERR_UNSUPPORTED, "pose gradients: max_indenters > 256");
+  }
   ctx->last_stream = s;
   if (a->n_envs == 0) return ETAC_OK;
   DeviceGuard guard(ctx->device);
@@ -792,7 +803,16 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
   if (pointnet && (a->d_grad_weights || a->d_grad_penetration) &&
       (e = launch_backward_pointnet(ctx->m, io, a->d_grad_out, a->d_grad_weights, a->d_grad_penetration, ctx->n_sm, &n_pn, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("pn_bwd_node_kernel", e));
-  ctx->last_launches = 1 + n_s1 + n_pn;
+  int n_pose = 0;
+  if (g_ind_pose || g_patch_pose) {
+    if (g_ind_pose && ctx->m.max_ind > 0 &&
+        (e = cudaMemsetAsync(g_ind_pose, 0, sizeof(float) * 6 * (size_t)a->n_envs * ctx->m.max_ind, s)) != cudaSuccess)
+      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset", e));
+    if ((e = launch_backward_pose(ctx->m, io, a->d_grad_penetration, g_ind_pose, g_patch_pose, s)) != cudaSuccess)
+      return fail(ctx, ETAC_ERR_CUDA, cuda_msg("pose_grad_kernel", e));
+    n_pose = 1;
+  }
+  ctx->last_launches = 1 + n_s1 + n_pn + n_pose;
   return ETAC_OK;
 }
 

@@ -193,6 +193,11 @@ void launch_pointnet_global_env(const DevModel& m, int n_envs, cudaStream_t s);
 cudaError_t backward_pointnet_configure();
 cudaError_t launch_backward_pointnet(const DevModel& m, const StepIO& io, const float* grad_out, float* grad_w, float* grad_delta,
                                      int n_sm, int* launches, cudaStream_t s);
+// etac_backward, pose part (k_backward_pose.cu): dL/ddelta chained to the indenter poses ([E x max_ind x 6], zero on
+// entry, may be NULL) and the patch poses ([E x P x 6], overwritten, may be NULL); rows are (dL/dt, dL/dtheta)
+constexpr int kMaxPoseGradIndenters = 256;
+cudaError_t launch_backward_pose(const DevModel& m, const StepIO& io, const float* g_delta, float* grad_ind, float* grad_patch,
+                                 cudaStream_t s);
 cudaError_t launch_mesh_sdf_grid(const float* tri, int n_tri, int nx, int ny, int nz, const float* origin, float h, float* values,
                                  cudaStream_t s);
 cudaError_t launch_penalty_only(const DevModel& m, const StepIO& io, cudaStream_t s);

@@ -66,7 +66,7 @@ class etac_backward_args(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("n_envs", C.c_int32), ("input_mode", C.c_int32),
                 ("d_indenters", C.c_void_p), ("d_patch_pose", C.c_void_p), ("d_penetration", C.c_void_p),
                 ("d_grad_out", C.c_void_p), ("d_grad_alpha", C.c_void_p), ("d_grad_weights", C.c_void_p),
-                ("d_grad_penetration", C.c_void_p)]
+                ("d_grad_penetration", C.c_void_p), ("d_grad_indenter_pose", C.c_void_p), ("d_grad_patch_pose", C.c_void_p)]
 
 
 class etac_params(C.Structure):
@@ -240,8 +240,9 @@ def etac_patches_from_adjacency(n_nodes, adj_rowptr, adj_col):
 
 
 def etac_backward(ctx, stream, n_envs, grad_out, grad_alpha, grad_weights=None, *, indenters=None, patch_pose=None,
-                  penetration=None, grad_penetration=None) -> None:
-    """dL/dalpha and dL/d(MLP weights) of one step from dL/dU (device tensors / addresses; marshalling only)."""
+                  penetration=None, grad_penetration=None, grad_indenter_pose=None, grad_patch_pose=None) -> None:
+    """dL/dalpha, dL/d(weights of Phi) and optionally dL/ddelta, dL/d(indenter poses) [E, M, 6], dL/d(patch poses)
+    [E, P, 6] of one step from dL/dU (device tensors / addresses; marshalling only)."""
     a = etac_backward_args()
     a.struct_size = C.sizeof(etac_backward_args)
     a.n_envs = n_envs
@@ -249,6 +250,7 @@ def etac_backward(ctx, stream, n_envs, grad_out, grad_alpha, grad_weights=None, 
     a.d_indenters, a.d_patch_pose, a.d_penetration = _dptr(indenters), _dptr(patch_pose), _dptr(penetration)
     a.d_grad_out, a.d_grad_alpha, a.d_grad_weights = _dptr(grad_out), _dptr(grad_alpha), _dptr(grad_weights)
     a.d_grad_penetration = _dptr(grad_penetration)
+    a.d_grad_indenter_pose, a.d_grad_patch_pose = _dptr(grad_indenter_pose), _dptr(grad_patch_pose)
     _check(ctx, load().etac_backward(ctx, stream, C.byref(a)))
 
 

@@ -681,3 +681,160 @@ def test_mesh_sdf_oracle_against_closed_forms_and_ray_parity():
     g = M.mesh_sdf_grid(Vb, Tb, (4, 5, 3), (-1.5, -2.0, -1.0), 1.0)
     assert g.shape == (3, 5, 4)
     assert abs(g[2, 1, 3] - O.sdf_local(O.IND_BOX, [1.0, 2.0, 0.5], np.float64(1.5), np.float64(-1.0), np.float64(1.0))) <= 1e-12
+
+
+# ---------------------------------------------------------------- pose gradients (dL/ddelta chained to the poses)
+IND64 = np.dtype([("type", "<i4"), ("param", "<f8", (3,)), ("pose", "<f8", (7,)), ("skip_patch1", "<i4")])
+
+
+def _quat_mul(a, b):
+    """Hamilton product a (x) b of quaternions stored (x, y, z, w): the rotation b followed by the rotation a."""
+    ax, ay, az, aw = a
+    bx, by, bz, bw = b
+    return np.array([aw * bx + ax * bw + ay * bz - az * by, aw * by - ax * bz + ay * bw + az * bx,
+                     aw * bz + ax * by - ay * bx + az * bw, aw * bw - ax * bx - ay * by - az * bz])
+
+
+def _perturb_pose(pose7, dof, eps):
+    """pose (t, q) with t[dof] += eps (dof 0-2) or rotated on the left by eps about world axis dof - 3."""
+    out = np.array(pose7, dtype=np.float64)
+    if dof < 3:
+        out[dof] += eps
+    else:
+        dq = np.zeros(4)
+        dq[dof - 3], dq[3] = math.sin(eps / 2), math.cos(eps / 2)
+        out[3:7] = _quat_mul(dq, out[3:7])
+    return out
+
+
+def pose_grad_case(seed=91, n_envs=2):
+    """Two patches under their own rigid poses; four indenter slots per env -- sphere, box (tilted), capsule (pressed
+    with its rounded end and its side), sampled grid (an ellipsoid-like field) -- each pressed into a node of one of
+    the patches.  Poses are fp32-representable float64 (the fp32 decision twin sees the same numbers)."""
+    mesh = W.assemble([W.fib_cap(6.0, 260), W.flat_pad(14, 16, 0.7)])
+    rng = np.random.default_rng(seed)
+    E, M = n_envs, 4
+    off = mesh.patch_offset
+    ppose = np.zeros((E, 2, 7))
+    ind = np.zeros((E, M), dtype=IND64)
+    Rp = W.random_rotations(rng, E * 2).reshape(E, 2, 3, 3)
+    gvals, _ = _grid_of(lambda X, Y, Z: np.sqrt((X / 1.2) ** 2 + Y ** 2 + (Z / 1.5) ** 2) * 1.2 - 2.0, n=(17, 17, 21),
+                        origin=(-4.13, -3.87, -5.06), h=0.5)   # no grid plane through the local z axis,
+    # on which the pressed node lies: the interpolant has kinks on the planes and a central difference would straddle one
+    for e in range(E):
+        for p in range(2):
+            ppose[e, p, 0:3] = rng.uniform(-20, 20, 3) + (40.0 * p, 0, 0)
+            ppose[e, p, 3:7] = W.quat_from_matrix(Rp[e, p])
+        for k, itype in enumerate((O.IND_SPHERE, O.IND_BOX, O.IND_CAPSULE, O.IND_GRID)):
+            p = (k + e) % 2
+            cand = np.arange(off[p], off[p + 1])
+            cand = cand[mesh.normal[cand, 2] > 0.6]
+            c = rng.choice(cand, size=1)
+            size = rng.uniform(2.0, 3.0, 1)
+            prm = [size[0], 0.0, 0.0]
+            if itype == O.IND_BOX:
+                prm = [rng.uniform(2, 4), rng.uniform(2, 4), size[0]]
+            if itype == O.IND_CAPSULE:
+                prm = [size[0] * 0.6, size[0] * 0.4, 0.0]           # r + L = size: pressed with its rounded end
+            if itype == O.IND_GRID:
+                prm, size = [0.0, 0.0, 0.0], np.asarray([2.0 * 1.5 / 1.2])   # zero level set on local z: 1.2 |z|/1.5 = 2
+            centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, rng.uniform(0.6, 1.0, 1), rng.uniform(0, 6.28, 1))
+            Rk = O.quat_to_rot(np.asarray(q[0], dtype=np.float64))
+            if itype in (O.IND_BOX, O.IND_CAPSULE):                 # tilt by ~0.1 / 0.5 rad about a local x
+                a = 0.1 if itype == O.IND_BOX else 0.5
+                Rk = Rk @ np.array([[1, 0, 0], [0, math.cos(a), -math.sin(a)], [0, math.sin(a), math.cos(a)]])
+            R = Rp[e, p] @ Rk                                       # carried along by the patch's pose
+            t = Rp[e, p] @ centre[0] + ppose[e, p, 0:3]
+            ind[e, k]["type"], ind[e, k]["param"] = itype, prm
+            ind[e, k]["pose"][0:3], ind[e, k]["pose"][3:7] = t, W.quat_from_matrix(R)
+    ind["pose"] = ind["pose"].astype(np.float32).astype(np.float64)
+    ppose = ppose.astype(np.float32).astype(np.float64)
+    wl = W.Workload("pose_grad_case", mesh, np.asarray([0.45, 0.7], np.float32), W.make_weights(9, 1, std=0.3), E, M, ind, ppose, "fp32",
+                    {"grids": {0: (gvals, (-4.13, -3.87, -5.06), 0.5)}})
+    return wl, rng.normal(0, 0.2, (E, mesh.n_nodes, 3))
+
+
+def test_sdf_gradients_against_central_differences_of_the_sdfs():
+    """grad phi of every indenter type (the building block of the pose gradients), inside, outside and -- capsule,
+    grid -- beyond the ends / the box: central differences of the pinned SDFs; |grad| = 1 for the exact ones."""
+    from oracle import etac_oracle_grad as OG
+    rng = np.random.default_rng(3)
+    y = rng.uniform(-5, 5, (400, 3))
+    h = 1e-6
+    cases = [(O.IND_SPHERE, [2.5, 0, 0]), (O.IND_BOX, [2.0, 3.0, 1.5]), (O.IND_CAPSULE, [1.5, 2.0, 0])]
+    for itype, prm in cases:
+        g = OG.sdf_local_gradient(itype, np.asarray(prm), y)
+        for a in range(3):
+            e = np.zeros(3)
+            e[a] = h
+            fd = (O.sdf_local(itype, prm, *(y + e).T) - O.sdf_local(itype, prm, *(y - e).T)) / (2 * h)
+            assert np.abs(fd - g[:, a]).max() < 1e-8, (itype, a)
+        np.testing.assert_allclose(np.linalg.norm(g, axis=1), 1.0, atol=1e-12)
+        assert (O.sdf_local(itype, prm, *y.T) < 0).sum() > 10       # the sample has points inside (where contact is)
+    vals, _ = _grid_of(lambda X, Y, Z: np.sqrt(X ** 2 + (Y / 1.5) ** 2 + Z ** 2) - 1.5)
+    origin, sp = (-2.0, -2.5, -3.0), 0.5
+    g = OG.sdf_grid_gradient(vals, origin, sp, y)                   # many of these points are outside the grid's box
+    for a in range(3):
+        e = np.zeros(3)
+        e[a] = h
+        fd = (O.sdf_grid(vals, origin, sp, *(y + e).T) - O.sdf_grid(vals, origin, sp, *(y - e).T)) / (2 * h)
+        cell = ((y[:, a] - origin[a]) / sp) % 1.0                   # away from the interpolant's kinks along this axis
+        hi = origin[a] + sp * (vals.shape[2 - a] - 1)
+        ok = (np.minimum(cell, 1 - cell) > 1e-4) & (np.abs(y[:, a] - origin[a]) > 1e-4) & (np.abs(y[:, a] - hi) > 1e-4)
+        assert ok.sum() > 350 and np.abs(fd - g[:, a])[ok].max() < 1e-7, a
+
+
+def test_pose_gradient_oracle_matches_finite_differences():
+    """pose_gradients against its definition: central differences of the (pinned) forward oracle's loss under a
+    translation of / a small left rotation about each world axis of every indenter's and every patch's pose, with
+    all four indenter types in contact (the contact set must not change under the perturbation: checked)."""
+    import dataclasses
+    from oracle import etac_oracle_grad as OG
+    wl, target = pose_grad_case()
+    m = O.model_from_workload(wl, resid_arch="pernode")
+
+    def loss(ind, ppose):
+        r = O.step(m, indenters=ind, patch_pose=ppose)
+        return 0.5 * float(((r["U"] - target) ** 2).sum()), r
+    l0, r0 = loss(wl.indenters, wl.patch_pose)
+    g_delta = OG.backward(m, r0["U"] - target, indenters=wl.indenters, patch_pose=wl.patch_pose)["delta"]
+    pg = OG.pose_gradients(m, g_delta, wl.indenters, wl.patch_pose)
+    # every indenter type is in contact in every env, on its own nodes
+    for e in range(wl.n_envs):
+        for k in range(4):
+            solo = wl.indenters[e:e + 1].copy()
+            solo["type"][0, [j for j in range(4) if j != k]] = O.IND_NONE
+            assert O.step(m, indenters=solo, patch_pose=wl.patch_pose[e:e + 1])["mask"].sum() >= 3, (e, k)
+    eps = 1e-6
+    noise = 8 * np.finfo(np.float64).eps * abs(l0) / eps
+    worst = 0.0
+    for e in range(wl.n_envs):
+        for kind, count in (("indenter", 4), ("patch", 2)):
+            for k in range(count):
+                for dof in range(6):
+                    vals = []
+                    for s in (+1, -1):
+                        ind, pp = wl.indenters.copy(), wl.patch_pose.copy()
+                        if kind == "indenter":
+                            ind[e, k]["pose"] = _perturb_pose(ind[e, k]["pose"], dof, s * eps)
+                        else:
+                            pp[e, k] = _perturb_pose(pp[e, k], dof, s * eps)
+                        l, r = loss(ind, pp)
+                        assert np.array_equal(r["mask"], r0["mask"])
+                        vals.append(l)
+                    fd = (vals[0] - vals[1]) / (2 * eps)
+                    got = pg[kind][e, k, dof]
+                    worst = max(worst, abs(fd - got) / max(1.0, abs(fd)))
+                    assert abs(fd - got) <= 2e-6 * max(1.0, abs(fd)) + noise, (e, kind, k, dof, fd, got)
+    assert np.abs(pg["indenter"]).min(axis=(0, 2)).max() > 0 and (np.abs(pg["indenter"]).max(axis=2) > 1e-2).all()
+    assert (np.abs(pg["patch"]).max(axis=2) > 1e-2).all()
+    # a rigid motion of the whole scene changes nothing: the gradients of an env sum to zero force, and to zero torque
+    # about the world origin (torques are about each body's own origin: shift them by t x force)
+    for e in range(wl.n_envs):
+        f = pg["indenter"][e, :, 0:3].sum(0) + pg["patch"][e, :, 0:3].sum(0)
+        tq = pg["indenter"][e, :, 3:6].sum(0) + pg["patch"][e, :, 3:6].sum(0)
+        tq = tq + sum(np.cross(wl.indenters[e, k]["pose"][0:3], pg["indenter"][e, k, 0:3]) for k in range(4))
+        tq = tq + sum(np.cross(wl.patch_pose[e, p, 0:3], pg["patch"][e, p, 0:3]) for p in range(2))
+        scale = np.abs(pg["indenter"][e]).max()
+        assert np.abs(f).max() < 1e-9 * scale and np.abs(tq).max() < 1e-7 * scale, (f, tq)
+    print(f"[pose grad pin] worst relative FD mismatch {worst:.2e}")

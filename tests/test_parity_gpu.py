@@ -658,6 +658,64 @@ def test_backward_against_the_gradient_oracle(kind):
     assert np.abs(U_fwd - U).max() <= (2e-2 if precision == "bf16" else 1e-4) * np.abs(U).max()
 
 
+@pytest.mark.parametrize("resid_arch", ["pernode", "pointnet"])
+def test_backward_pose_gradients_against_the_oracle(resid_arch):
+    """etac_backward's dL/d(indenter poses) and dL/d(patch poses) (k_backward_pose.cu) against
+    oracle/etac_oracle_grad.pose_gradients (pinned by central differences of the forward oracle): two patches under
+    their own poses, sphere + tilted box + capsule + sampled grid in contact in every env; rows (dL/dt, dL/dtheta).
+    fp32 with atomics: 2e-5 of the largest entry of each tensor, forces and torques apart (measured 7e-8 .. 6e-7)."""
+    import dataclasses
+    import torch
+    from oracle import etac_oracle as O, etac_oracle_grad as OG
+    from test_oracle_pins import pose_grad_case
+    wl64, target = pose_grad_case(seed=92, n_envs=5)
+    if resid_arch == "pointnet":
+        wl64 = dataclasses.replace(wl64, weights=W.make_pointnet_weights(9, 1, std=0.2))
+    m = O.model_from_workload(wl64, resid_arch=resid_arch)
+    U = O.step(m, indenters=wl64.indenters, patch_pose=wl64.patch_pose)["U"]
+    G = U - target
+    g_delta = OG.backward(m, G, indenters=wl64.indenters, patch_pose=wl64.patch_pose)["delta"]
+    ref = OG.pose_gradients(m, g_delta, wl64.indenters, wl64.patch_pose)
+    ind = np.zeros(wl64.indenters.shape, dtype=W.INDENTER_DTYPE)             # the same numbers (fp32-representable) in the ABI's layout
+    for f in ("type", "param", "pose", "skip_patch1"):
+        ind[f] = wl64.indenters[f]
+    wl = dataclasses.replace(wl64, indenters=ind, patch_pose=wl64.patch_pose.astype(np.float32))
+    eng = T.Etac(wl, precision="fp32")
+    try:
+        dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+        d_G = torch.from_numpy(G.astype(np.float32)).to(eng.device)
+        g_alpha = torch.empty(len(wl.alpha), device=eng.device)
+        g_pen = torch.empty((wl.n_envs, eng.N), device=eng.device)
+        g_ind = torch.full((wl.n_envs, wl.max_indenters, 6), 7.0, device=eng.device)
+        g_patch = torch.full((wl.n_envs, eng.P, 6), 7.0, device=eng.device)
+        stream = torch.cuda.current_stream().cuda_stream
+        for _ in range(2):                                                    # overwritten, not accumulated
+            T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, None, grad_penetration=g_pen, grad_indenter_pose=g_ind,
+                            grad_patch_pose=g_patch, **dev)
+        torch.cuda.synchronize()
+        got = {"indenter": g_ind.cpu().numpy().astype(np.float64), "patch": g_patch.cpu().numpy().astype(np.float64)}
+        with pytest.raises(T.EtacError):                                      # needs dL/ddelta
+            T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, None, grad_indenter_pose=g_ind, **dev)
+        with pytest.raises(T.EtacError):                                      # no poses in penetration input mode
+            T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, None, grad_penetration=g_pen, grad_patch_pose=g_patch,
+                            penetration=g_pen)
+        # without patch poses: the patch part is zero, the indenter part is that of identity poses
+        ind_only = eng.upload(indenters=wl.indenters)
+        T.etac_backward(eng.ctx, stream, wl.n_envs, d_G, g_alpha, None, grad_penetration=g_pen, grad_indenter_pose=g_ind,
+                        grad_patch_pose=g_patch, **ind_only)
+        torch.cuda.synchronize()
+        assert not g_patch.any()
+    finally:
+        eng.close()
+    for k in ("indenter", "patch"):
+        for part, sl in (("force", slice(0, 3)), ("torque", slice(3, 6))):
+            scale = np.abs(ref[k][..., sl]).max()
+            err = np.abs(got[k][..., sl] - ref[k][..., sl]).max()
+            print(f"[backward pose {resid_arch}] {k} {part}: max|ref| {scale:.4g} max err {err:.3g} ({err / scale:.2e} rel)")
+            assert scale > 1e-2 and err <= 2e-5 * scale, (k, part, err, scale)
+    assert ((np.abs(ref["indenter"]).max(axis=2) > 0).sum(axis=0) >= 4).all()  # every indenter type is in contact in >= 4 of 5 envs
+
+
 @pytest.mark.parametrize("precision", ["fp32", "bf16"])
 def test_update_params_equals_a_fresh_context(precision):
     """etac_update_params (a gradient-descent step of Eq. 3 writes alpha and Phi back): the context then
