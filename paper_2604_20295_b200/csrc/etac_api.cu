@@ -166,7 +166,7 @@ etac_status step_impl(etac_ctx* ctx, cudaStream_t s, const etac_step_args* a, cu
   }
   if (io.nact_out && (e = cudaMemsetAsync(io.nact_out, 0, sizeof(int32_t) * a->n_envs, s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset active count", e));
-  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 1), s)) != cudaSuccess)
+  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 3), s)) != cudaSuccess)
     return fail(ctx, ETAC_ERR_CUDA, cuda_msg("memset count", e));
   // bf16 context: tensor-core MLP either way; DENSE = tcgen05 contraction K.U^, SPARSE = gather over the
   // active-node lists.  fp32 context: fp32 SIMT gather kernel (which needs S1 to zero-fill).
@@ -523,8 +523,9 @@ etac_status etac_create(const etac_model_desc* d, etac_ctx** out) {
   // ---- per-step workspace
   const size_t urows = (size_t)((d->max_envs + kMaxTE - 1) / kMaxTE) * kMaxTE * 3;
   CK(dev_alloc(c, &m.delta, (size_t)d->max_envs * N, true), "alloc delta");
-  CK(dev_alloc(c, &m.count, (size_t)P + 1, true), "alloc count");
+  CK(dev_alloc(c, &m.count, (size_t)P + 3, true), "alloc count");
   m.ntask = m.count + P;
+  m.wq = m.count + P + 1;
   if (d->max_indenters == 1 && P >= 4) {  // S1 as cull + evaluate kernels: 128-byte task records
     void* tasks = nullptr;
     CK(dev_alloc(c, reinterpret_cast<uint8_t**>(&tasks), (size_t)128 * P * d->max_envs, false), "alloc S1 tasks");
@@ -785,7 +786,7 @@ etac_status etac_backward(etac_ctx* ctx, void* cuda_stream, const etac_backward_
   io.ind = a->d_indenters, io.patch_pose = a->d_patch_pose, io.pen_in = a->d_penetration;
   cudaError_t e;
   const bool pointnet = ctx->m.resid == ETAC_RESID_POINTNET;
-  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 1), s)) != cudaSuccess ||
+  if ((e = cudaMemsetAsync(ctx->m.count, 0, sizeof(int32_t) * (ctx->m.n_patches + 3), s)) != cudaSuccess ||
       (e = cudaMemsetAsync(a->d_grad_alpha, 0, sizeof(float) * ctx->n_alpha, s)) != cudaSuccess ||
       (a->d_grad_weights && (e = cudaMemsetAsync(a->d_grad_weights, 0, sizeof(float) * (pointnet ? ETAC_GRAD_WEIGHTS_POINTNET_LEN : ETAC_GRAD_WEIGHTS_LEN), s)) != cudaSuccess) ||
       (a->d_grad_penetration &&

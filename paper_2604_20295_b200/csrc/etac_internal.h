@@ -122,6 +122,8 @@ struct DevModel {
   uint8_t* keybuf;            // [max_envs x P] key of every contacting pair
   struct PairTask* tasks;     // [max_envs x P] S1 task list of the cull / evaluate kernel pair (many patches, one indenter)
   int32_t* ntask;             // [1], behind count[P] (zeroed with it)
+  int32_t* wq;                // [2], behind ntask: item counter of the fused kernel's dynamic item order and the
+                              // number of CTAs that are done with it (zeroed with count; the kernel leaves them at zero)
   GridDesc grid[kMaxGrids];   // sampled-SDF objects (etac_set_sdf_grid)
   ActiveEntry* alist;         // [max_envs (slots) x ldu]: the active nodes of (slot, patch p) start at
                               // slot * ldu + off_p, in node order (allocated when the bf16 gather path is first selected)

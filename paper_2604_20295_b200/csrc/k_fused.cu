@@ -74,12 +74,24 @@ struct Tile {
   static_assert(2 * BN + 64 * NC <= 512, "TMEM columns");
 };
 
+// The CTA's item stream.  Small patches (one CTA per item stream, dense propagation): the n-th item of a CTA is
+// claimed from a global counter (DevModel::wq) instead of being blockIdx.x + n gridDim.x -- the SMs do not run at the
+// same speed (end times of the static order spread over 9 % of the kernel), and a CTA that is ahead takes more
+// items.  The TMA warp claims the next item when it has streamed the current one and publishes the sequence in
+// shared memory.  The ring is longer than the pipeline is deep: the TMA warp is less than one item ahead of the
+// MMA warp, which is at most two items (the two accumulators) ahead of the slowest chain.
+constexpr int kSeqRing = 16;
+constexpr int kNoWork = 0x7fffffff;
+
 template <int NC>
 struct __align__(8) FusedBars {
   uint64_t full[kMaxStages], empty[kMaxStages];
   uint64_t acc_full[2], acc_empty[2], d_ready[NC];
   uint32_t tmem_base;
   uint32_t pad;
+  // dynamic item order (kDyn): entry n & (kSeqRing - 1) = (n << 32 | work index of the CTA's n-th item), written by
+  // the TMA warp, read by the MMA warp and the chains
+  unsigned long long seq[kSeqRing];
 };
 
 // Residual variants of the fused kernel (template parameter kMode).  The PointNet form of Phi
@@ -274,6 +286,7 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   // the MMAs of BOTH CTAs have read it: `empty` counts two commits, each CTA's commit arrives in both.
   constexpr bool kPair = kGrouped;
   constexpr uint16_t kPairMask = 3;
+  constexpr bool kDyn = kProp && !kPair;  // item order claimed from DevModel::wq (see kSeqRing)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sA = smem;
@@ -288,14 +301,32 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rank = kPair ? (int)cluster_ctarank() : 0;
   const int w_first = kPair ? (int)(blockIdx.x >> 1) : (int)blockIdx.x, w_step = kPair ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+  // kDyn: work index of the CTA's n-th item, n >= 1 (item 0 is w_first); waits until the TMA warp has published it
+  auto seq_w = [&](const int n) -> int {
+    volatile unsigned long long* slot = &bars->seq[n & (kSeqRing - 1)];
+    unsigned long long v;
+    do v = *slot; while ((int)(v >> 32) != n);
+    return (int)(uint32_t)v;
+  };
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < kStages; ++s) mbar_init(&bars->full[s], 1), mbar_init(&bars->empty[s], kPair ? 2 : 1);
     for (int b = 0; b < 2; ++b) mbar_init(&bars->acc_full[b], 1), mbar_init(&bars->acc_empty[b], 4 * NC);
     for (int c = 0; c < NC; ++c) mbar_init(&bars->d_ready[c], 1);
+    for (int k = 0; k < kSeqRing; ++k) bars->seq[k] = ~0ull;
     fence_barrier_init();
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB);
+  }
+  if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+  if constexpr (kResid) {
+    const uint4* src = reinterpret_cast<const uint4*>(kPn ? m.wimg_pn : m.wimg);
+    uint4* dst = reinterpret_cast<uint4*>(sW);
+    for (int k = threadIdx.x; k < kImgBytes / 16; k += kThreads) dst[k] = src[k];
+    // "ones" operand of the bias k-step: row r, k-octet 0 = (1, 0, ..., 0); k-octet 1 = 0
+    uint4* ones = reinterpret_cast<uint4*>(sOnes);
+    for (int k = threadIdx.x; k < kOnesBytes / 16; k += kThreads) ones[k] = make_uint4(k < 128 ? 0x00003F80u : 0u, 0u, 0u, 0u);
+    fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor-core (async) proxy
   }
   if (warp == 2) {
     // prefix[p] = first work index of patch p: warp scan, 32 patches per sweep (the per-patch counts
@@ -326,16 +357,6 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
     }
     if (lane == 0) prefix[0] = 0;
   }
-  if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
-  if constexpr (kResid) {
-    const uint4* src = reinterpret_cast<const uint4*>(kPn ? m.wimg_pn : m.wimg);
-    uint4* dst = reinterpret_cast<uint4*>(sW);
-    for (int k = threadIdx.x; k < kImgBytes / 16; k += kThreads) dst[k] = src[k];
-    // "ones" operand of the bias k-step: row r, k-octet 0 = (1, 0, ..., 0); k-octet 1 = 0
-    uint4* ones = reinterpret_cast<uint4*>(sOnes);
-    for (int k = threadIdx.x; k < kOnesBytes / 16; k += kThreads) ones[k] = make_uint4(k < 128 ? 0x00003F80u : 0u, 0u, 0u, 0u);
-    fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor-core (async) proxy
-  }
   tc_fence_before();
   __syncthreads();
   if constexpr (kPair) cluster_sync();  // the peer's barriers are initialised before anything is sent to them
@@ -351,16 +372,20 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       int pcur = 0, stage = 0;
       uint32_t ph = 0;
       Item it, nx;
-      int w = w_first;
+      int w = w_first, n_item = 0;
       bool have = decode_item<kGrouped, TE>(prefix, m.n_patches, w, rank, pcur, it);
       uint32_t km = 0;
       if constexpr (kGrouped) km = have ? load_tile_kbmask(m, it, lane) : 0u;
       while (have) {
-        // the next item and (large patches) its k-block mask, requested before this item's k-blocks are streamed
-        const int wn = w + w_step;
-        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
+        // static order: the next item and (large patches) its k-block mask, requested before this item's k-blocks
+        // are streamed
+        int wn = w + w_step;
+        bool have_n = false;
         uint32_t kmn = 0;
-        if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
+        if constexpr (!kDyn) {
+          have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
+          if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
+        }
         const int nkb = (it.n + BK - 1) / BK;
         auto load_kb = [&](const int kb) {
           mbar_wait(&bars->empty[stage], ph ^ 1);
@@ -383,7 +408,19 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
         } else {
           for (int kb = 0; kb < nkb; ++kb) load_kb(kb);
         }
-        it = nx, km = kmn, have = have_n, w = wn;
+        if constexpr (kDyn) {
+          // dynamic order: the next item is claimed as late as possible -- when this one is streamed -- so that few
+          // items are bound to a CTA when the counter runs out; this warp is an item ahead of the chains and can wait
+          int claimed = 0;
+          if (lane == 0) {
+            claimed = (int)gridDim.x + atomicAdd(m.wq, 1);
+            *reinterpret_cast<volatile unsigned long long*>(&bars->seq[(n_item + 1) & (kSeqRing - 1)]) =
+                ((unsigned long long)(uint32_t)(n_item + 1) << 32) | (uint32_t)claimed;
+          }
+          wn = __shfl_sync(0xffffffffu, claimed, 0);
+          have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
+        }
+        it = nx, km = kmn, have = have_n, w = wn, ++n_item;
       }
     }
   } else if (warp == 1) {
@@ -401,10 +438,13 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       uint32_t km = 0;
       if constexpr (kGrouped) km = have ? load_tile_kbmask(m, it, lane) : 0u;
       while (have) {
-        const int wn = w + w_step;
-        const bool have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
+        int wn = w + w_step;
+        bool have_n = false;
         uint32_t kmn = 0;
-        if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
+        if constexpr (!kDyn) {
+          have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
+          if constexpr (kGrouped) kmn = have_n ? load_tile_kbmask(m, nx, lane) : 0u;
+        }
         const int nkb = (it.n + BK - 1) / BK;
         const int b = k_item & 1;
         mbar_wait(&bars->acc_empty[b], ((k_item >> 1) & 1) ^ 1);  // the epilogue has fetched item k_item - 2
@@ -436,6 +476,10 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
           }
         } else {
           for (int kb = 0; kb < nkb; ++kb) mma_kb(kb == nkb - 1);
+        }
+        if constexpr (kDyn) {  // (published once the TMA warp has streamed this item: not before the k-blocks are consumed)
+          wn = seq_w(k_item + 1);
+          have_n = decode_item<kGrouped, TE>(prefix, m.n_patches, wn, rank, pcur, nx);
         }
         it = nx, km = kmn, have = have_n, w = wn, ++k_item;
       }
@@ -526,7 +570,8 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
       while (live && cel >= it.cnt) {
         cel -= it.cnt;
         leave_item();
-        ++ck, cw += w_step;
+        ++ck;
+        cw = kDyn ? seq_w(ck) : cw + w_step;
         live = decode_item<kGrouped, TE>(prefix, m.n_patches, cw, rank, pcur, it);
         if (live) item_setup(), enter_item();
       }
@@ -747,6 +792,10 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   }
   tc_fence_before();
   __syncthreads();
+  if constexpr (kDyn) {
+    // every claim of this CTA has returned; the last CTA to get here leaves the counters at zero for the next launch
+    if (threadIdx.x == 0 && atomicAdd(m.wq + 1, 1) == (int)gridDim.x - 1) m.wq[0] = 0, m.wq[1] = 0;
+  }
   if constexpr (kPair) cluster_sync();  // the peer's last commits arrive on this CTA's barriers
   if (warp == 1) {
     tc_fence_after();
