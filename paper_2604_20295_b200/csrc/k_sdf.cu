@@ -56,7 +56,7 @@ struct SPose {
 //   E  all threads: contact-free patches -> zero-fill of the output rows; contacting patches ->
 //      U^ operand rows (bf16), optional delta / mask outputs
 template <bool kIndenters, bool kGrid>
-__global__ void __launch_bounds__(256) sdf_penetration_kernel(DevModel m, StepIO io, int s1_flags) {
+__global__ void __launch_bounds__(256, 4) sdf_penetration_kernel(DevModel m, StepIO io, int s1_flags) {
   // kS1Bucket: the slot of a contacting pair and its U^ rows are left to sdf_scatter_kernel (counting sort of the
   // environments by contact position); this kernel records the key and counts the environments per key
   const bool bucket = s1_flags & kS1Bucket;
