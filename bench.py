@@ -44,10 +44,10 @@ FP32_FMA_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12              # 74.4: 148 SMs x 
 # capture named beside it; "src_sha" = sha1 (first 12 hex digits) of the kernel's source file at capture time.
 # bench.py prints the figure only while the source still has that hash -- a changed kernel gives traffic: null.
 NCU_TRAFFIC = {
-    "cfg3": {"bytes": 311.51e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
-             "src_sha": "081a50676469"},
-    "cfg4": {"bytes": 1642.39e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
-             "src_sha": "081a50676469"},
+    "cfg3": {"bytes": 314.73e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
+             "src_sha": "24fcb9e5ec90"},
+    "cfg4": {"bytes": 1686.36e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
+             "src_sha": "24fcb9e5ec90"},
 }
 
 CFG5_NODES = (256, 1024, 4096, 8192)

@@ -304,8 +304,17 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
   // kDyn: work index of the CTA's n-th item, n >= 1 (item 0 is w_first); waits until the TMA warp has published it
   auto seq_w = [&](const int n) -> int {
     volatile unsigned long long* slot = &bars->seq[n & (kSeqRing - 1)];
-    unsigned long long v;
-    do v = *slot; while ((int)(v >> 32) != n);
+    unsigned long long v = *slot;
+    uint32_t spins = 0;
+    uint64_t t0 = 0;
+    while ((int)(v >> 32) != n) {  // (bounded like mbar_wait: a protocol bug ends in a trap, not in a hung GPU)
+      if ((++spins & 0x3fffu) == 0) {
+        const uint64_t now = global_timer_ns();
+        if (t0 == 0) t0 = now;
+        else if (now - t0 > 10000000000ull) __trap();
+      }
+      v = *slot;
+    }
     return (int)(uint32_t)v;
   };
 
