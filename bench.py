@@ -38,16 +38,25 @@ METRIC = "tactile_env_steps_per_s"
 UNIT = "env-steps/s"
 N_INPUT_SETS = 4
 MLP_FLOP_PER_NODE_ENV = 2 * (9 * 64 + 64 * 64 + 64 * 3)      # 9,728
+# --phi: the residual network of the timed context.  "pernode" = BASELINE.json's per-node MLP (the metric's config);
+# "pointnet" = the paper's own form of Phi (widths = DESIGN.md R10).  Algorithmic flop and SiLU
+# count per node-environment of a contacting pair: encoder 9->64->64, decoder 128->64->3 (the kernels run the
+# encoder twice -- once for the max-pool, once in the decoder pass -- which these figures do not count), + the
+# global MLP 64->64 once per pair.
+PHI = {"pernode": {"flop_node": MLP_FLOP_PER_NODE_ENV, "act_node": 128.0, "flop_pair": 0.0, "act_pair": 0.0},
+       "pointnet": {"flop_node": 2 * (9 * 64 + 64 * 64 + 128 * 64 + 64 * 3), "act_node": 192.0,
+                    "flop_pair": 2 * 64 * 64, "act_pair": 64.0}}
+PHI_SEL = "pernode"
 FP32_FMA_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12              # 74.4: 148 SMs x 128 fp32 lanes x 2 flop at 1965 MHz
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the `ncu --set full`
 # capture named beside it; "src_sha" = sha1 (first 12 hex digits) of the kernel's source file at capture time.
 # bench.py prints the figure only while the source still has that hash -- a changed kernel gives traffic: null.
 NCU_TRAFFIC = {
-    "cfg3": {"bytes": 314.73e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
-             "src_sha": "24fcb9e5ec90"},
-    "cfg4": {"bytes": 1686.36e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
-             "src_sha": "24fcb9e5ec90"},
+    "cfg3": {"bytes": 312.55e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
+             "src_sha": "bf720de59a78"},
+    "cfg4": {"bytes": 1700.55e6, "profile": "profiles/r02_fused_ncu_full.md", "src": "k_fused.cu",
+             "src_sha": "bf720de59a78"},
 }
 
 CFG5_NODES = (256, 1024, 4096, 8192)
@@ -55,6 +64,14 @@ CFG5_FRACS = (0.001, 0.003, 0.01, 0.05, 0.20)
 
 
 def make_workload(name, seed, envs, **kw):
+    wl = _make_workload(name, seed, envs, **kw)
+    if PHI_SEL == "pointnet":      # same geometry and contact, the paper's form of Phi (N(0, 0.02) weights like the configs')
+        import dataclasses
+        wl = dataclasses.replace(wl, weights=W.make_pointnet_weights(int(name[3:]), 0, std=0.02))
+    return wl
+
+
+def _make_workload(name, seed, envs, **kw):
     if name == "cfg1":
         return W.config1(seed, envs)
     if name == "cfg2":
@@ -113,8 +130,9 @@ def work_model(wl, m_ep):
         "f_prop_dense": 6.0 * float((hit * npat * npat).sum()),          # what a dense K_p . U^ executes
         "f_prop_alg": 6.0 * float((m * (npat - m)).sum()),               # the method: Omega is (n - m) x m (L87)
         "f_prop_gather": 6.0 * float((m * npat).sum()),                  # gather over the active nodes, all rows
-        "f_mlp": MLP_FLOP_PER_NODE_ENV * w_nodeenv,                      # Phi on every row of a contacting pair
-        "f_mlp_alg": MLP_FLOP_PER_NODE_ENV * (w_nodeenv - n_active),     # passive rows only
+        "f_mlp": PHI[PHI_SEL]["flop_node"] * w_nodeenv + PHI[PHI_SEL]["flop_pair"] * float(hit.sum()),   # Phi on every row of a contacting pair
+        "f_mlp_alg": PHI[PHI_SEL]["flop_node"] * (w_nodeenv - n_active) + PHI[PHI_SEL]["flop_pair"] * float(hit.sum()),  # passive rows only
+        "acts": PHI[PHI_SEL]["act_node"] * w_nodeenv + PHI[PHI_SEL]["act_pair"] * float(hit.sum()),
         "b_hbm_min": 12.0 * E * N + 48.0 * E * wl.max_indenters + (28.0 * E * P if wl.patch_pose is not None else 0.0)
                      + 2.0 * float((npat * npat).sum()) + 20e3,
         "contact_frac": n_active / max(1.0, w_nodeenv),
@@ -161,7 +179,7 @@ def time_oracle(wl, n_sample):
     threads it kept busy (process CPU time / wall time)."""
     from oracle import etac_oracle as O
     from threadpoolctl import threadpool_info
-    m = O.model_from_workload(wl)
+    m = O.model_from_workload(wl, resid_arch="pointnet" if "E1" in wl.weights else "pernode")
     envs = list(range(0, wl.n_envs, max(1, wl.n_envs // n_sample)))[:n_sample]
     for p in range(m.n_patches):
         O.kernel_block(m, p)                       # K is create-time work on both sides
@@ -208,7 +226,7 @@ def run_reference(a):
         "warmup": a.warmup, "ms_per_step": 1e3 * dt / a.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "node_updates_per_s": v * wl.mesh.n_nodes,
-        "config": {"workload": label, "n_envs": a.envs,
+        "config": {"workload": label, "n_envs": a.envs, "phi": PHI_SEL,
                    "n_nodes": wl.mesh.n_nodes, "n_patches": wl.mesh.n_patches},
         "cpu_baseline": cb,
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -436,7 +454,7 @@ def run_ours(a):
     hbm = peaks["hbm_gbs"] * 1e9
     t_hbm = wm["b_hbm_min"] / hbm
     power_capped = bool(clocks and "sw_power_cap" in clocks.get("reasons", []))
-    traffic, traffic_src = ncu_traffic(a.workload)
+    traffic, traffic_src = ncu_traffic(a.workload) if PHI_SEL == "pernode" else (None, "no ncu capture for --phi pointnet")
     if bf16:
         # roofline.frac: the dominant kernel against the bf16 tensor peak -- the BURST figure when no sw_power_cap
         # sample was seen during the timed region (the kernel then runs at the clocks of a kernel timed alone), the
@@ -444,6 +462,8 @@ def run_ours(a):
         peak = peaks["bf16_tflops_sustained"] if power_capped else peaks["bf16_tflops"]
         peak_name = "bf16_tflops_sustained (sw_power_cap seen)" if power_capped else "bf16_tflops (burst; no sw_power_cap sample)"
         kernel = "fused_mlp_kernel" if path_taken == T.ETAC_PATH_DENSE else "fused_mlp_kernel (gather form)"
+        if PHI_SEL == "pointnet":
+            kernel += " x 2 (PointNet: encoder + max-pool pass, pn_global_kernel, decoder pass; timed together)"
         flops = wm["f_prop_dense"] + wm["f_mlp"]
         flops_alg = wm["f_prop_alg"] + wm["f_mlp_alg"]
         achieved = flops / (ms_fused * 1e-3) / 1e12
@@ -452,7 +472,7 @@ def run_ours(a):
         # (128 SiLUs per node-environment of a contacting pair).  "roofline" is the contract's (tensor
         # peak / HBM); the activation-pipe bound is reported beside it as "roofline_sfu" against a rate measured
         # live, and does not replace the contract fraction.
-        acts = 128.0 * wm["w_nodeenv"]
+        acts = wm["acts"]
         t_sfu = acts / sfu_ops_s
         t_hbm_fused = (wm["b_hbm_min"] + 4.0 * wm["w_nodeenv"]) / hbm
         roofline = {"bound": "tensor", "kernel": kernel, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
@@ -477,7 +497,8 @@ def run_ours(a):
         flops = wm["f_prop_gather"] + wm["f_mlp"]
         flops_alg = wm["f_prop_alg"] + wm["f_mlp_alg"]
         achieved = flops / (ms_fused * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": "gather_fp32_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+        kernel32 = "gather_fp32_kernel" if PHI_SEL == "pernode" else "fp32 PointNet kernels (propagation + encode, global, decode; timed together)"
+        roofline = {"bound": "alu", "kernel": kernel32, "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                     "frac": achieved / peak, "traffic": traffic, "traffic_src": traffic_src,
                     "peak_src": "derived: 148 SMs x 128 fp32 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts)",
                     "flops_per_launch": flops}
@@ -485,13 +506,15 @@ def run_ours(a):
         t_roof, t_roof_alg = max(flops / (peak * 1e12), t_hbm), max(flops_alg / (peak * 1e12), t_hbm)
         dtype = "f32"
     n_cpu = a.envs if a.workload in ("cfg1", "cfg2", "cfg3") else min(a.envs, 64)      # ~10 s of CPU work
+    if PHI_SEL != "pernode":                                                            # slower oracle branch: size the sample from a probe
+        n_cpu = int(min(n_cpu, max(8, 10.0 * time_oracle(wl, min(a.envs, 8))["rate"])))
     cpu = time_oracle(wl, n_cpu)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": dtype, "data": "synthetic",
         "node_updates_per_s": value * eng.N,
-        "config": {"workload": label, "n_envs_per_gpu": a.envs,
+        "config": {"workload": label, "n_envs_per_gpu": a.envs, "phi": PHI_SEL,
                    "n_nodes": eng.N, "n_patches": eng.P,
                    "precision": "bf16 operands, fp32 accumulate" if bf16 else "fp32",
                    "path": {T.ETAC_PATH_DENSE: "dense", T.ETAC_PATH_SPARSE: "sparse"}.get(path_taken, str(path_taken)),
@@ -540,10 +563,15 @@ if __name__ == "__main__":
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--envs", type=int, default=0, help="environments per GPU (default: the config's own batch)")
     ap.add_argument("--workload", default="cfg3", choices=sorted(LABELS))
+    ap.add_argument("--phi", default="pernode", choices=sorted(PHI),
+                    help="residual network: pernode = BASELINE.json's MLP (the metric's config), pointnet = the paper's form of Phi")
     ap.add_argument("--nodes", type=int, nargs="+", default=None, help="cfg5: mesh sizes (default 256 1024 4096 8192)")
     ap.add_argument("--fracs", type=float, nargs="+", default=None, help="cfg5: contact fractions (default 0.001 .. 0.20)")
     ap.add_argument("--fp32", action="store_true", help="cfg5: also time the fp32 context at every point")
     args = ap.parse_args()
+    PHI_SEL = args.phi
+    if args.phi != "pernode" and args.workload == "cfg5":
+        raise SystemExit("--phi pointnet: cfg1 .. cfg4 only")
     args.envs = args.envs or LABELS[args.workload][1]
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:

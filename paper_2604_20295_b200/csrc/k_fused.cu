@@ -816,32 +816,56 @@ __global__ void __launch_bounds__(Tile<TE>::kThreads, 1)
 // ("further encoded by another MLP"), c = D1[:, 64:128] g' + d1, stored halved like
 // the decoder weights.  A 64-thread CTA stages the two transposed 64 x 64 matrices in shared
 // memory once and walks kPnSlots contact-list slots of one patch.
-constexpr int kPnSlots = 16;
-__global__ void __launch_bounds__(64) pn_global_kernel(DevModel m) {
-  const int p = blockIdx.y, k = threadIdx.x;
+constexpr int kPnSlots = 32, kPnGroups = 4, kPnPer = kPnSlots / kPnGroups;  // slots per CTA; groups of 64 threads; slots per group
+__global__ void __launch_bounds__(64 * kPnGroups) pn_global_kernel(DevModel m) {
+  // thread = output k of kPnPer slots held in registers: a weight read from shared memory serves kPnPer FMAs (one
+  // output of one slot per thread would be bound by two shared-memory loads per FMA)
+  const int p = blockIdx.y, k = threadIdx.x & 63, grp = threadIdx.x >> 6;
   const int slot0 = blockIdx.x * kPnSlots, cnt = m.count[p];
   if (slot0 >= cnt) return;
-  __shared__ float sG1[64 * 64], sD1[64 * 64], g[64], g2[64];
+  __shared__ float sG1[64 * 64], sD1[64 * 64];
+  __shared__ __align__(16) float g[64][kPnSlots], g2[64][kPnSlots];  // [input j][slot of the CTA]
   const float* G1t = m.pn_f32, *g1 = G1t + 4096, *D1gt = g1 + 64, *d1 = D1gt + 4096;  // both matrices [in][out]
-  for (int i = k; i < 4096; i += 64) sG1[i] = G1t[i], sD1[i] = D1gt[i];
+#pragma unroll
+  for (int i = 0; i < kPnPer; ++i) {
+    const int sl = grp * kPnPer + i, slot = slot0 + sl;
+    const uint32_t key = slot < cnt ? m.gmax[((int64_t)p * m.max_envs + slot) * 64 + k] : 0x3f800000u;
+    g[k][sl] = __uint_as_float(key) - 1.0f;  // keys are the bit patterns of 1 + f
+  }
+  for (int i = threadIdx.x; i < 4096; i += 64 * kPnGroups) sG1[i] = G1t[i], sD1[i] = D1gt[i];
   const float bg = g1[k], bd = d1[k];
-  for (int slot = slot0; slot < min(cnt, slot0 + kPnSlots); ++slot) {
-    const int64_t base = ((int64_t)p * m.max_envs + slot) * 64;
-    const uint32_t key = m.gmax[base + k];
-    __syncthreads();  // previous slot done with g / g2; first pass: weights staged
-    g[k] = __uint_as_float(key) - 1.0f;  // keys are the bit patterns of 1 + f
-    __syncthreads();
-    float a = bg;
-#pragma unroll 8
-    for (int j = 0; j < 64; ++j) a = fmaf(sG1[j * 64 + k], g[j], a);
-    g2[k] = a / (1.0f + expf(-a));
-    __syncthreads();
-    float c = bd;
-#pragma unroll 8
-    for (int j = 0; j < 64; ++j) c = fmaf(sD1[j * 64 + k], g2[j], c);
-    m.cvec[base + k] = 0.5f * c;
+  __syncthreads();
+  float acc[kPnPer];
+#pragma unroll
+  for (int i = 0; i < kPnPer; ++i) acc[i] = bg;
+#pragma unroll 4
+  for (int j = 0; j < 64; ++j) {
+    const float w = sG1[j * 64 + k];
+    const float4 x0 = *reinterpret_cast<const float4*>(&g[j][grp * kPnPer]), x1 = *reinterpret_cast<const float4*>(&g[j][grp * kPnPer + 4]);
+    const float x[kPnPer] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+#pragma unroll
+    for (int i = 0; i < kPnPer; ++i) acc[i] = fmaf(w, x[i], acc[i]);
+  }
+#pragma unroll
+  for (int i = 0; i < kPnPer; ++i) g2[k][grp * kPnPer + i] = acc[i] / (1.0f + expf(-acc[i]));
+  __syncthreads();
+#pragma unroll
+  for (int i = 0; i < kPnPer; ++i) acc[i] = bd;
+#pragma unroll 4
+  for (int j = 0; j < 64; ++j) {
+    const float w = sD1[j * 64 + k];
+    const float4 x0 = *reinterpret_cast<const float4*>(&g2[j][grp * kPnPer]), x1 = *reinterpret_cast<const float4*>(&g2[j][grp * kPnPer + 4]);
+    const float x[kPnPer] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+#pragma unroll
+    for (int i = 0; i < kPnPer; ++i) acc[i] = fmaf(w, x[i], acc[i]);
+  }
+#pragma unroll
+  for (int i = 0; i < kPnPer; ++i) {
+    const int slot = slot0 + grp * kPnPer + i;
+    if (slot < cnt) m.cvec[((int64_t)p * m.max_envs + slot) * 64 + k] = 0.5f * acc[i];
   }
 }
+static_assert(kPnPer == 8, "pn_global_kernel reads a group's inputs as two float4");
 
 template <int kMode, bool kGather, bool kOutBf16, bool kGrouped, int TE>
 static cudaError_t set_smem() {
@@ -932,7 +956,7 @@ cudaError_t launch_fused_bf16(const DevModel& m, const StepIO& io, const CUtenso
     e = cudaMemsetAsync(m.gmax, 0, sizeof(uint32_t) * 64 * (size_t)m.n_patches * m.max_envs, s);
     if (e != cudaSuccess) return e;
     launch_one<kModePnEncode>(m, io, tmA, tmB, grid, false, s);
-    pn_global_kernel<<<dim3((unsigned)((io.n_envs + kPnSlots - 1) / kPnSlots), (unsigned)m.n_patches), 64, 0, s>>>(m);
+    pn_global_kernel<<<dim3((unsigned)((io.n_envs + kPnSlots - 1) / kPnSlots), (unsigned)m.n_patches), 64 * kPnGroups, 0, s>>>(m);
     e = launch_one<kModePnDecode>(m, io, tmA, tmB, grid, gather, s);
     *launches = 3 + n_big;
   }
