@@ -71,21 +71,36 @@ __global__ void __launch_bounds__(256, 4) sdf_penetration_kernel(DevModel m, Ste
   __shared__ int s_slot[kPoseChunk];
   __shared__ int s_off[kPoseChunk + 1];  // node offsets of the chunk's patches (+ end)
   __shared__ uint32_t s_kb[kKbWords];
+  __shared__ int s_nind;  // indenters of the environment that are not empty slots
 
   const int e = blockIdx.x;
   const int lane = threadIdx.x & 31;
   const int words = (m.n_nodes + 31) >> 5;
   const bool posed = io.patch_pose != nullptr;
   if constexpr (kIndenters) {
-    for (int k = threadIdx.x; k < m.max_ind; k += blockDim.x) {
-      const SInd s = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
-      sind[k] = s;
-      s_tb[k] = make_float4(s.t[0], s.t[1], s.t[2], s.rb2);
+    // the environment's indenters, empty slots dropped (slot order kept): every node pays a pre-test per entry
+    if (threadIdx.x < 32) {
+      int n_act = 0;
+      for (int k0 = 0; k0 < m.max_ind; k0 += 32) {
+        const int k = k0 + lane;
+        SInd s;
+        s.type = ETAC_IND_NONE;
+        if (k < m.max_ind) s = load_indenter(io.ind + (int64_t)e * m.max_ind + k);
+        const uint32_t bal = __ballot_sync(0xffffffffu, s.type != ETAC_IND_NONE);
+        if (s.type != ETAC_IND_NONE) {
+          const int pos = n_act + __popc(bal & ((1u << lane) - 1u));
+          sind[pos] = s;
+          s_tb[pos] = make_float4(s.t[0], s.t[1], s.t[2], s.rb2);
+        }
+        n_act += __popc(bal);
+      }
+      if (lane == 0) s_nind = n_act;
     }
   }
   for (int p0 = 0; p0 < m.n_patches; p0 += kPoseChunk) {
     const int np = min(kPoseChunk, m.n_patches - p0);
     __syncthreads();  // sind ready / previous chunk fully consumed
+    const int n_ind = kIndenters ? s_nind : 0;
     // ---- phase B
     if ((int)threadIdx.x < np) {
       const int p = p0 + threadIdx.x;
@@ -111,7 +126,7 @@ __global__ void __launch_bounds__(256, 4) sdf_penetration_kernel(DevModel m, Ste
           C2 = __fadd_rn(__fadd_rn(__fadd_rn(__fmul_rn(sp.R[6], x), __fmul_rn(sp.R[7], y)), __fmul_rn(sp.R[8], z)), sp.t[2]);
         }
         // conservative cull: exact SDFs are 1-Lipschitz, so phi(x_i) >= phi(c) - brad
-        const float phi_lo = union_sdf_lower<kGrid>(sind, m.max_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
+        const float phi_lo = union_sdf_lower<kGrid>(sind, n_ind, C0, C1, C2, pi.brad, m.grid, p + 1);
         // (phi_lo = +inf: no indenter applies to this patch -- all slots NONE, or only the patch's own link)
         sp.evaluated = phi_lo < __int_as_float(0x7f800000) && !(phi_lo > 0.01f + 1e-5f * (fabsf(phi_lo) + 3.0f * pi.brad));
         s_pose[threadIdx.x] = sp;
@@ -148,7 +163,7 @@ __global__ void __launch_bounds__(256, 4) sdf_penetration_kernel(DevModel m, Ste
             }
             phi[c] = __int_as_float(0x7f800000);
           }
-          for (int k = 0; k < m.max_ind; ++k) {
+          for (int k = 0; k < n_ind; ++k) {
             // A node further than the shape's bounding radius (+ margin) from its origin has phi > 0.05 whatever the
             // rounding: it stays passive (delta = 0) without the exact, single-rounded evaluation.  On a large patch
             // most nodes are far from every indenter (one 16-byte load and 7 instructions per slot and node instead
