@@ -716,6 +716,51 @@ def test_backward_pose_gradients_against_the_oracle(resid_arch):
     assert ((np.abs(ref["indenter"]).max(axis=2) > 0).sum(axis=0) >= 4).all()  # every indenter type is in contact in >= 4 of 5 envs
 
 
+def test_pose_gradients_recover_an_indenter_pose_from_a_tactile_target():
+    """Differentiability end to end (Table I): the displacement field of a sphere pressed into the cap at
+    a hidden position is the target; Adam on dL/dt of the indenter (etac_backward's pose gradients), starting 0.5 mm
+    off (sideways and in depth), finds the position again to 1e-3 mm although the contact set changes along the way.
+    ETAC_ACTIVE_PROPAGATE context: with the mask M_p of Eq. 2 a node's row jumps from the propagated value to
+    u^ = -delta n ~ 0 when it enters contact, so the loss is discontinuous in the pose and a descent stalls at the jumps
+    (measured on the same case: it ends 0.05-0.8 mm off); without the mask the field is continuous in delta."""
+    import torch
+    wl = W.config2(21, 4)
+    ind = wl.indenters.copy()
+    ind["type"][:, 1:] = 0                                                  # one sphere per env
+    ind["type"][:, 0] = 1
+    ind["param"][:, 0, 0] = 4.0
+    c = np.nonzero(wl.mesh.normal[:, 2] > 0.8)[0][[3, 17, 40, 71]]
+    t_star = (wl.mesh.pos[c] + wl.mesh.normal[c] * (4.0 - 0.9)).astype(np.float32)   # pressed 0.9 mm into node c
+    ind["pose"][:, 0, 0:3] = t_star
+    ind["pose"][:, 0, 3:7] = [0, 0, 0, 1]
+    eng = T.Etac(wl, precision="fp32", active_mode=T.ETAC_ACTIVE_PROPAGATE)
+    try:
+        stream = torch.cuda.current_stream().cuda_stream
+        target = eng.step(wl.n_envs, eng.upload(indenters=ind)).clone()
+        assert float(target.abs().max()) > 0.5
+        t = t_star.astype(np.float64) + np.asarray([[0.4, -0.3, 0.15], [-0.5, 0.2, 0.1], [0.3, 0.4, -0.2], [-0.2, -0.45, 0.25]])
+        err0 = np.linalg.norm(t - t_star, axis=1)
+        g_alpha = torch.empty(len(wl.alpha), device=eng.device)
+        g_pen = torch.empty((wl.n_envs, eng.N), device=eng.device)
+        g_ind = torch.empty((wl.n_envs, wl.max_indenters, 6), device=eng.device)
+        m1, m2, losses = np.zeros_like(t), np.zeros_like(t), []
+        for it in range(1, 201):
+            ind["pose"][:, 0, 0:3] = t.astype(np.float32)
+            dev = eng.upload(indenters=ind)
+            G = eng.step(wl.n_envs, dev) - target
+            losses.append(0.5 * float((G * G).sum()))
+            T.etac_backward(eng.ctx, stream, wl.n_envs, G.contiguous(), g_alpha, None, grad_penetration=g_pen,
+                            grad_indenter_pose=g_ind, **dev)
+            g = g_ind[:, 0, 0:3].cpu().numpy().astype(np.float64)
+            m1, m2 = 0.9 * m1 + 0.1 * g, 0.999 * m2 + 0.001 * g * g
+            t = t - 0.02 * (m1 / (1 - 0.9 ** it)) / (np.sqrt(m2 / (1 - 0.999 ** it)) + 1e-12)
+    finally:
+        eng.close()
+    err = np.linalg.norm(t - t_star, axis=1)
+    print(f"[pose recovery] |t - t*| {err0.round(3)} -> {err.round(4)} mm; loss {losses[0]:.4g} -> {losses[-1]:.4g}")
+    assert (err < 1e-3).all() and losses[-1] < 1e-6 * losses[0]
+
+
 @pytest.mark.parametrize("precision", ["fp32", "bf16"])
 def test_update_params_equals_a_fresh_context(precision):
     """etac_update_params (a gradient-descent step of Eq. 3 writes alpha and Phi back): the context then
