@@ -252,6 +252,9 @@ typedef struct {
      optional; ETAC_IN_INDENTERS mode only; need d_grad_penetration (read back by the kernel) and max_indenters <= 256.
      A row is (dL/dt[3], dL/dtheta[3]): t the pose's translation, theta a rotation applied on the LEFT in the world
      frame, R <- exp([theta]x) R (the torque about the body's own origin t, up to sign conventions of the caller).
+     Where the SDF has no gradient -- a node on the shape's medial axis: the centre of a sphere, the axis segment of a
+     capsule, a plane of equal distance to two faces inside a box, a cell face of a sampled grid -- the node's
+     contribution has the direction rounding gives it (a set of measure zero in pose space).
      A struct_size that ends before these two fields is accepted (no pose gradients). */
   float* d_grad_indenter_pose;        /* device [E x max_indenters x 6] fp32, overwritten, or NULL; 0 for empty slots */
   float* d_grad_patch_pose;           /* device [E x P x 6] fp32, overwritten, or NULL; 0 if d_patch_pose is NULL */
