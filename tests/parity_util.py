@@ -134,3 +134,66 @@ def self_contact_workload(mesh, caps, seed, n_envs, n_ind, precision="bf16", wei
     wl = W.Workload("self_contact", mesh, np.asarray([alpha], np.float32), weights or W.make_weights(3, seed), n_envs,
                     n_ind, ind, pose, precision, meta)
     return wl
+
+
+def random_case(seed):
+    """Seeded random workload for the randomised sweeps: 1-6 patches (caps and pads of 9-1400 nodes, sometimes a
+    2048-3300-node cap: the cluster-pair path), 1-260 envs, 1-3 indenter slots (sphere / box / capsule, a quarter
+    empty) each pressed 0.05-1.2 mm into a random node and shifted sideways off the shape's axis, with or without
+    per-patch rigid poses; random residual form, alpha per patch or shared, precision, path and active-row mode.
+    Returns (workload, resid_arch, precision, path, active_mode)."""
+    rng = np.random.default_rng(seed)
+    P = int(rng.integers(1, 7))
+    parts = []
+    for p in range(P):
+        kind = rng.integers(0, 3)
+        if kind == 0:
+            parts.append(W.fib_cap(float(rng.uniform(5, 12)), int(rng.integers(9, 700))))
+        elif kind == 1:
+            g1, g2 = int(rng.integers(3, 26)), int(rng.integers(3, 26))
+            parts.append(W.flat_pad(g1, g2, float(rng.uniform(0.6, 1.5))))
+        else:
+            big = rng.random() < 0.35
+            parts.append(W.fib_cap(float(rng.uniform(8, 14)), int(rng.integers(2048, 3300)) if big else int(rng.integers(128, 1400))))
+    mesh = W.assemble(parts)
+    E = int(rng.integers(1, 72)) if rng.random() < 0.7 else int(rng.integers(72, 260))
+    M = int(rng.integers(1, 4))
+    ind = W._blank_indenters(E, M)
+    off = np.asarray(mesh.patch_offset)
+    posed = bool(rng.integers(0, 2))
+    pose = None
+    if posed:
+        pose = np.zeros((E, P, 7), np.float32)
+        for e in range(E):
+            Rm = W.random_rotations(rng, P)
+            pose[e, :, 0:3] = np.stack([70.0 * np.arange(P), np.zeros(P), np.zeros(P)], 1) + rng.uniform(-5, 5, (P, 3))
+            pose[e, :, 3:7] = W.quat_from_matrix(Rm)
+    for e in range(E):
+        for k in range(M):
+            if rng.random() < 0.25:
+                continue
+            p = int(rng.integers(0, P))
+            c = np.asarray([int(rng.integers(off[p], off[p + 1]))])
+            itype = int(rng.integers(1, 4))
+            size = rng.uniform(1.5, 5.0, 1)
+            centre, q = W._press_on_node(mesh.pos, mesh.normal, c, None, size, rng.uniform(0.05, 1.2, 1), rng.uniform(0, 6.28, 1))
+            prm = [size[0], 0, 0]
+            if itype == W.IND_BOX: prm = [rng.uniform(1.5, 5), rng.uniform(1.5, 5), size[0]]
+            if itype == W.IND_CAPSULE: prm = [size[0] * 0.6, size[0] * 0.4, 0]
+            cen, qq = centre[0], np.asarray(q[0], np.float64)
+            cen = cen + O.quat_to_rot(qq) @ np.asarray([rng.uniform(0.05, 0.3), rng.uniform(0.05, 0.3), 0.0])   # no node on the shape's axis
+            if posed:
+                Rp = O.quat_to_rot(pose[e, p, 3:7].astype(np.float64))
+                Rk = O.quat_to_rot(qq)
+                cen = Rp @ cen + pose[e, p, 0:3]
+                qq = W.quat_from_matrix(Rp @ Rk)
+            ind["type"][e, k], ind["param"][e, k] = itype, prm
+            ind["pose"][e, k, 0:3], ind["pose"][e, k, 3:7] = cen, qq
+    arch = ["pernode", "pointnet", "none"][int(rng.integers(0, 3))]
+    weights = W.make_pointnet_weights(9, seed, std=0.15) if arch == "pointnet" else W.make_weights(9, seed, std=0.2)
+    alpha = np.asarray(rng.uniform(0.3, 0.9, P if rng.random() < 0.5 else 1), np.float32)
+    prec = "bf16" if rng.random() < 0.6 else "fp32"
+    wl = W.Workload(f"random{seed}", mesh, alpha, weights, E, M, ind, pose, prec)
+    path = T.ETAC_PATH_AUTO if prec == "fp32" else [T.ETAC_PATH_DENSE, T.ETAC_PATH_SPARSE][int(rng.integers(0, 2))]
+    mode = [T.ETAC_ACTIVE_PASSTHROUGH, T.ETAC_ACTIVE_PROPAGATE][int(rng.integers(0, 2))]
+    return wl, arch, prec, path, mode

@@ -12,7 +12,7 @@ import pytest
 
 from paper_2604_20295_b200 import etac as T
 from paper_2604_20295_b200 import workloads as W
-from parity_util import TOL, compare, run_gpu, run_oracle
+from parity_util import TOL, compare, random_case, run_gpu, run_oracle
 
 pytestmark = pytest.mark.gpu
 
@@ -714,6 +714,69 @@ def test_backward_pose_gradients_against_the_oracle(resid_arch):
             print(f"[backward pose {resid_arch}] {k} {part}: max|ref| {scale:.4g} max err {err:.3g} ({err / scale:.2e} rel)")
             assert scale > 1e-2 and err <= 2e-5 * scale, (k, part, err, scale)
     assert ((np.abs(ref["indenter"]).max(axis=2) > 0).sum(axis=0) >= 4).all()  # every indenter type is in contact in >= 4 of 5 envs
+
+
+@pytest.mark.parametrize("first_seed", [0, 40, 80])
+def test_randomised_parity_sweep(first_seed):
+    """40 seeded random workloads per parameter (parity_util.random_case: patch counts and sizes incl. the large-patch
+    path, env counts over several tiles, indenter types, poses, both forms of Phi or none, both precisions, dense and
+    gather paths, both active-row modes), two steps each on one context, against the oracle at the usual tolerances."""
+    for seed in range(first_seed, first_seed + 40):
+        wl, arch, prec, path, mode = random_case(seed)
+        resid = arch != "none"
+        gpu = run_gpu(wl, precision=prec, path=path, resid=resid, active_mode=mode, steps=2)
+        ref = run_oracle(wl, resid=resid, active_mode="propagate" if mode == T.ETAC_ACTIVE_PROPAGATE else "passthrough")
+        label = f"random{seed} sizes {np.diff(wl.mesh.patch_offset).tolist()} E {wl.n_envs} {arch} {prec} path {path} mode {mode}"
+        if np.abs(ref["U"]).max() == 0:
+            assert not gpu["U"].any(), label
+            continue
+        compare(gpu, ref, TOL[prec], label=label, delta_tol=1e-4)
+
+
+def test_randomised_backward_sweep():
+    """etac_backward incl. the pose gradients on the random workloads of modest size (<= 1500 nodes, <= 12 envs) among the
+    first 300 seeds, against the gradient oracle: 1e-4 of the largest entry of every tensor."""
+    import torch
+    from oracle import etac_oracle as O, etac_oracle_grad as OG
+    n = 0
+    for seed in range(300):
+        wl, arch, prec, path, mode = random_case(seed)
+        if wl.mesh.n_nodes > 1500 or wl.n_envs > 12:
+            continue
+        m = O.model_from_workload(wl, resid_arch=arch, active_mode="propagate" if mode == T.ETAC_ACTIVE_PROPAGATE else "passthrough")
+        U = O.step(m, indenters=wl.indenters, patch_pose=wl.patch_pose)["U"]
+        if np.abs(U).max() == 0:
+            continue
+        G = U - np.random.default_rng(seed).normal(0, 0.2, U.shape)
+        ref = dict(OG.backward(m, G, indenters=wl.indenters, patch_pose=wl.patch_pose))
+        ref.update(OG.pose_gradients(m, ref["delta"], wl.indenters, wl.patch_pose))
+        eng = T.Etac(wl, precision=prec, active_mode=mode, resid=arch != "none")
+        try:
+            dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+            d_G = torch.from_numpy(G.astype(np.float32)).to(eng.device)
+            g_alpha = torch.empty(len(wl.alpha), device=eng.device)
+            n_w = T.ETAC_GRAD_WEIGHTS_POINTNET_LEN if arch == "pointnet" else T.ETAC_GRAD_WEIGHTS_LEN
+            g_w = torch.empty(n_w, device=eng.device) if arch != "none" else None
+            g_pen = torch.empty((wl.n_envs, eng.N), device=eng.device)
+            g_ind = torch.empty((wl.n_envs, wl.max_indenters, 6), device=eng.device)
+            g_patch = torch.empty((wl.n_envs, eng.P, 6), device=eng.device)
+            T.etac_backward(eng.ctx, torch.cuda.current_stream().cuda_stream, wl.n_envs, d_G, g_alpha, g_w, grad_penetration=g_pen,
+                            grad_indenter_pose=g_ind, grad_patch_pose=g_patch, **dev)
+            torch.cuda.synchronize()
+            got = {"alpha": g_alpha.cpu().numpy(), "delta": g_pen.cpu().numpy(), "indenter": g_ind.cpu().numpy(), "patch": g_patch.cpu().numpy()}
+            if g_w is not None:
+                got.update(T.split_grad_weights(g_w.cpu().numpy()))
+        finally:
+            eng.close()
+        for k in ref:
+            scale = np.abs(ref[k]).max()
+            if scale < 1e-6:
+                assert np.abs(got[k]).max() < 1e-4, (seed, k)
+                continue
+            err = np.abs(got[k].astype(np.float64) - ref[k]).max() / scale
+            assert err < 1e-4, (seed, k, err, scale, arch, prec)
+        n += 1
+    assert n >= 15, n
 
 
 def test_pose_gradients_recover_an_indenter_pose_from_a_tactile_target():
