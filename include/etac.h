@@ -143,7 +143,10 @@ typedef struct {
 } etac_step_args;
 
 /* Enqueues S1-S4 for n_envs environments on cuda_stream (a cudaStream_t; NULL = default stream).
- * Output for a patch none of whose nodes is in contact in that environment is exactly 0. */
+ * Output for a patch none of whose nodes is in contact in that environment is exactly 0.
+ * Reproducibility: repeated steps of the same inputs give the same bits.  On a bf16 context an environment's result
+ * does not depend on the other environments of the batch; on an fp32 context it can differ in the last bits with
+ * n_envs (the gather kernel groups its sums by the size of the launch: 2e-7 of max|u| measured). */
 etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args);
 
 /* Options / introspection. */
@@ -223,7 +226,8 @@ etac_status etac_patches_from_adjacency(int32_t n_nodes, const int32_t* adj_rowp
  * Given the upstream gradient G = dL/dU of one step (same inputs as etac_step), returns dL/dalpha and
  * dL/d(weights of the per-node residual MLP).  Rows that Eq. (2) overwrites with u^ (the active nodes,
  * ETAC_ACTIVE_PASSTHROUGH) and rows of contact-free (env, patch) pairs carry no gradient to them.  Optionally
- * also dL/d(penetration); gradients with respect to poses are not computed.  Arithmetic: fp32 on the fp32 copies of
+ * also dL/d(penetration) and, chained through the SDF gradients, dL/d(indenter poses) and dL/d(patch poses) (see the
+ * last two fields of etac_backward_args).  Arithmetic: fp32 on the fp32 copies of
  * K and the weights, whatever the context's precision; sums over environments use fp32 atomics, so
  * repeated calls agree to rounding, not bit for bit.  With ETAC_RESID_POINTNET (the network of PAPER.md:L91-L99,
  * whose input is [P, N, U^]) Phi does not depend on alpha, the weight gradients are those of its five layers and
