@@ -144,9 +144,8 @@ typedef struct {
 
 /* Enqueues S1-S4 for n_envs environments on cuda_stream (a cudaStream_t; NULL = default stream).
  * Output for a patch none of whose nodes is in contact in that environment is exactly 0.
- * Reproducibility: repeated steps of the same inputs give the same bits.  On a bf16 context an environment's result
- * does not depend on the other environments of the batch; on an fp32 context it can differ in the last bits with
- * n_envs (the gather kernel groups its sums by the size of the launch: 2e-7 of max|u| measured). */
+ * Reproducibility: repeated steps of the same inputs give the same bits, and an environment's result does not depend
+ * on the other environments of the batch or on n_envs. */
 etac_status etac_step(etac_ctx* ctx, void* cuda_stream, const etac_step_args* args);
 
 /* Options / introspection. */

@@ -29,6 +29,7 @@ constexpr int kCtasPerSm = 3;            // 80 registers, 73 KB of shared memory
 constexpr int kGT = 2 * kGatherChunk;   // threads per CTA
 constexpr int kSub = 4, kSweep = kSub * kGT;  // nodes of a patch scanned per sweep: kSub per thread
 constexpr int kCache = 1024;             // entries of the cached active-node list
+constexpr int kMaxSeg = 64;              // sweeps of a patch whose list can be cached (patches of up to 65,536 nodes)
 constexpr int kDepth = 16;              // K loads in flight per thread in the gather
 constexpr int kHld = kGatherChunk + 4;  // row pitch of the [64][128] activation arrays (rows stay 16-byte aligned)
 struct GatherSmem {
@@ -47,6 +48,7 @@ struct GatherSmem {
   // (last: the one-chunk-per-item instantiation is launched without them)
   float cu[kCache][3];             // cached list of a patch's active nodes, shared by the chunks of an item
   int cj[kCache];
+  int seg[kMaxSeg + 1];            // first entry of every sweep's part of the cached list (+ end)
 };
 constexpr size_t kGatherSmemNoCache = offsetof(GatherSmem, cu);
 static_assert(sizeof(float) * (kSweep * 3 + kSweep) <= sizeof(float) * 64 * kHld, "sweep arrays inside H");
@@ -137,7 +139,7 @@ __global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m
   for (int64_t item = blockIdx.x; item < n_items; item += gridDim.x) {
    const int e = (int)(item / gpe);
    const int c0 = (int)(item - (int64_t)e * gpe) * cpg, c1 = min(c0 + cpg, m.n_chunks);
-   int cache_patch = -1, cache_total = -1;  // cache_total < 0: the list of cache_patch did not fit
+   int cache_patch = -1, cache_total = -1, cache_nseg = 0;  // cache_total < 0: the list of cache_patch did not fit
    for (int c = c0; c < c1; ++c) {
     const ChunkInfo ch = m.chunk[c];
     if (!m.flags[(int64_t)e * m.n_patches + ch.patch]) continue;  // S1 zero-filled this patch (uniform over the CTA)
@@ -151,12 +153,22 @@ __global__ void __launch_bounds__(kGT, kCtasPerSm) gather_fp32_kernel(DevModel m
     // ---- Omega U_a over the patch's active nodes in node order
     float ax = 0.f, ay = 0.f, az = 0.f;
     if (kShare && ch.patch != cache_patch && c + 1 < c1 && m.chunk[c + 1].patch == ch.patch) {  // more chunks of this patch follow
-      int total = 0;
-      for (int base = 0; base < pi.n; base += kSweep) total += compact_sweep(S, m.nrm4 + pi.off, pi.n, delta, base, S.cu, S.cj, total, kCache);
-      cache_patch = ch.patch, cache_total = total <= kCache ? total : -1;
+      // (the list is summed sweep by sweep, like the uncached form below: an environment's result then has the same
+      //  bits whichever form the size of the launch selects)
+      int total = 0, ns = 0;
+      for (int base = 0; base < pi.n; base += kSweep, ++ns) {
+        if (t == 0 && ns < kMaxSeg) S.seg[ns] = min(total, kCache);
+        total += compact_sweep(S, m.nrm4 + pi.off, pi.n, delta, base, S.cu, S.cj, total, kCache);
+      }
+      if (t == 0 && ns <= kMaxSeg) S.seg[ns] = min(total, kCache);
+      __syncthreads();
+      cache_patch = ch.patch, cache_total = (total <= kCache && ns <= kMaxSeg) ? total : -1, cache_nseg = ns;
     }
     if (kShare && ch.patch == cache_patch && cache_total >= 0) {
-      gather_list(S.cu, S.cj, cache_total, K, pi.n, li, half, ax, ay, az);
+      for (int sg = 0; sg < cache_nseg; ++sg) {
+        const int b0 = S.seg[sg];
+        gather_list(S.cu + b0, S.cj + b0, S.seg[sg + 1] - b0, K, pi.n, li, half, ax, ay, az);
+      }
     } else {
       for (int base = 0; base < pi.n; base += kSweep) {  // (sweep arrays inside H: the previous chunk's MLP is over)
         const int total = compact_sweep(S, m.nrm4 + pi.off, pi.n, delta, base, S.u, S.j, 0, kSweep);

@@ -733,6 +733,42 @@ def test_randomised_parity_sweep(first_seed):
         compare(gpu, ref, TOL[prec], label=label, delta_tol=1e-4)
 
 
+@pytest.mark.parametrize("seeds", [range(0, 25), (134, 163, 169)])
+def test_results_do_not_depend_on_batch_size_or_output_layout(seeds):
+    """On random workloads (parity_util.random_case; the three single seeds are fp32 contexts whose batch size switches
+    the gather kernel between shared and per-chunk active lists): the first E' < E environments stepped alone give the
+    bits they give inside the full batch, on a context with spare max_envs; the bf16 / strided outputs are the fp32
+    result rounded / moved, and the padding of the observation rows is untouched."""
+    import torch
+    for seed in seeds:
+        wl, arch, prec, path, mode = random_case(seed)
+        rng = np.random.default_rng(seed + 99)
+        E = wl.n_envs
+        E_run = int(rng.integers(1, E + 1))
+        eng = T.Etac(wl, precision=prec, active_mode=mode, resid=arch != "none", max_envs=E + int(rng.integers(0, 9)))
+        try:
+            T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+            dev = eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose)
+            stream = torch.cuda.current_stream().cuda_stream
+            full = eng.step(E, dev).clone()
+            part = eng.step(E_run, dev).clone()
+            assert torch.equal(part, full[:E_run]), (seed, prec, E, E_run, float((part - full[:E_run]).abs().max()))
+            N = eng.N
+            for dtype, code in ((torch.bfloat16, T.ETAC_OUT_BF16), (torch.float32, T.ETAC_OUT_F32)):
+                pf, pb = int(rng.integers(0, 9)), int(rng.integers(0, 9))
+                stride = pf + 3 * N + pb
+                obs = torch.full((E, stride), -7.0, dtype=dtype, device=eng.device)
+                out = obs.data_ptr() + pf * obs.element_size()
+                T.etac_step(eng.ctx, stream, eng.args(E, dev, out=out, out_env_stride=stride, out_dtype=code))
+                torch.cuda.synchronize()
+                got = obs.float()
+                assert bool((got[:, :pf] == -7.0).all()) and bool((got[:, pf + 3 * N:] == -7.0).all()), (seed, "padding")
+                want = full if dtype == torch.float32 else full.to(torch.bfloat16).float()
+                assert torch.equal(got[:, pf:pf + 3 * N].reshape(E, N, 3), want), (seed, str(dtype))
+        finally:
+            eng.close()
+
+
 def test_randomised_backward_sweep():
     """etac_backward incl. the pose gradients on the random workloads of modest size (<= 1500 nodes, <= 12 envs) among the
     first 300 seeds, against the gradient oracle: 1e-4 of the largest entry of every tensor."""
