@@ -769,6 +769,53 @@ def test_results_do_not_depend_on_batch_size_or_output_layout(seeds):
             eng.close()
 
 
+def test_randomised_penetration_sweep():
+    """Penetration input mode on 60 random workloads: random per-node penetrations with 0 / 0.2 / 2 / 20 / 90 % of the
+    nodes in contact (negatives clamp; sometimes an env without contact), against the oracle."""
+    for seed in range(60):
+        wl, arch, prec, path, mode = random_case(seed)
+        rng = np.random.default_rng(seed + 31)
+        E, N = min(wl.n_envs, 40), wl.mesh.n_nodes
+        frac = rng.choice([0.0, 0.002, 0.02, 0.2, 0.9])
+        pen = np.where(rng.random((E, N)) < frac, rng.uniform(0.0, 1.2, (E, N)), rng.uniform(-1.0, 0.0, (E, N))).astype(np.float32)
+        if rng.random() < 0.3:
+            pen[rng.integers(0, E)] = -0.5
+        resid = arch != "none"
+        gpu = run_gpu(wl, precision=prec, path=path, resid=resid, active_mode=mode, penetration=pen, n_envs=E)
+        ref = run_oracle(wl, resid=resid, active_mode="propagate" if mode == T.ETAC_ACTIVE_PROPAGATE else "passthrough", penetration=pen)
+        label = f"random{seed} sizes {np.diff(wl.mesh.patch_offset).tolist()} E {E} frac {frac} {arch} {prec} path {path} mode {mode}"
+        if np.abs(ref["U"]).max() == 0:
+            assert not gpu["U"].any(), label
+            continue
+        compare(gpu, ref, TOL[prec], label=label, delta_tol=1e-4)
+
+
+def test_randomised_workspace_reuse():
+    """60 random workloads: input set A, then set B (the envs in another order, 30 % of the indenters gone, fewer envs)
+    on ONE context gives the bits of B on a fresh context -- nothing of A survives in the per-step workspaces."""
+    import torch
+    for seed in range(60):
+        wl, arch, prec, path, mode = random_case(seed)
+        rng = np.random.default_rng(seed + 7)
+        E = wl.n_envs
+        perm = rng.permutation(E)
+        E_b = int(rng.integers(1, E + 1))
+        ind_b = wl.indenters[perm].copy()
+        ind_b["type"][rng.random(ind_b.shape) < 0.3] = 0
+        pose_b = None if wl.patch_pose is None else wl.patch_pose[perm].copy()
+
+        def run(first_a):
+            eng = T.Etac(wl, precision=prec, active_mode=mode, resid=arch != "none")
+            try:
+                T.etac_set_option(eng.ctx, T.ETAC_OPT_PATH, path)
+                if first_a:
+                    eng.step(E, eng.upload(indenters=wl.indenters, patch_pose=wl.patch_pose))
+                return eng.step(E_b, eng.upload(indenters=ind_b, patch_pose=pose_b)).clone()
+            finally:
+                eng.close()
+        assert torch.equal(run(False), run(True)), (seed, arch, prec, path, mode)
+
+
 def test_randomised_backward_sweep():
     """etac_backward incl. the pose gradients on the random workloads of modest size (<= 1500 nodes, <= 12 envs) among the
     first 300 seeds, against the gradient oracle: 1e-4 of the largest entry of every tensor."""
